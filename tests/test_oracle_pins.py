@@ -1,0 +1,371 @@
+"""Pins for the CPU oracle (oracle/rqa_oracle.cpp): everything here checks the oracle against something
+other than itself — hand-enumerated recurrence plots, closed forms, library order statistics, invariants,
+exact rational arithmetic, a statistical closed form.  CPU only (`-m "not gpu"`).
+
+Citations are PAPER.md lines (= /root/reference/PAPER.md) and DESIGN.md readings S1..S18.
+"""
+import math
+from fractions import Fraction
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from paper_2208_09136_b200 import workloads as wl
+
+GOLDEN = Path(__file__).resolve().parent / "golden" / "hand_cases.txt"
+NORMS = {"max": 0, "euclid": 1}
+
+
+# ------------------------------------------------------------------------------------ hand enumeration
+def _hand_cases():
+    cases = []
+    for line in GOLDEN.read_text().splitlines():
+        if not line.strip() or line.startswith("#"):
+            continue
+        name, y, m, tau, norm, rr, eps, C, hist, det = [f.strip() for f in line.split("|")]
+        e = np.float32(np.sqrt(np.float32(5.0))) if eps == "sqrt5" else np.float32(float(eps))
+        h = {int(a): int(b) for a, b in (t.split(":") for t in hist.split(","))}
+        num, den = det.split("/")
+        cases.append(pytest.param(np.array(y.split(), dtype=np.float32), int(m), int(tau), NORMS[norm], float(rr),
+                                  e, int(C), h, Fraction(int(num), int(den)), id=name))
+    return cases
+
+
+@pytest.mark.parametrize("y,m,tau,norm,rr,eps,C,hist,det", _hand_cases())
+def test_hand_enumerated(oracle, y, m, tau, norm, rr, eps, C, hist, det):
+    r = oracle.sweep(y, m, tau, [rr], norm, l_min=2)
+    P = oracle.n_pairs(len(y), m, tau)
+    assert r["eps"][0] == eps
+    assert int(r["count"][0]) == C
+    assert r["rr"][0] == C / P
+    got = {int(l): int(c) for l, c in enumerate(r["hist"][0]) if c}
+    assert got == hist
+    assert abs(r["det"][0] - float(det)) <= 1e-15
+    assert r["det_mean"] == r["det"][0]          # the average of one value is the value itself
+
+
+# ------------------------------------------------------------------------------------------ rank (S5)
+def test_rank_literal_fp64(oracle):
+    assert oracle.rank(0.07, 100) == 8      # 0.07*100 = 7.000000000000001 -> ceil = 8 (wart kept, reading S5)
+    assert oracle.rank(0.3, 10) == 3
+    assert oracle.rank(0.1, 3) == 1
+    assert oracle.rank(1e-12, 1000) == 1    # clamp below
+    assert oracle.rank(1.0, 4753) == 4753   # clamp above
+    P = 4999750003
+    for rr in wl.rr_log(20, 0.001, 0.2):
+        assert oracle.rank(rr, P) == math.ceil(rr * float(P))
+
+
+# ------------------------------------------------------------------------------- embedding
+@pytest.mark.parametrize("m,tau", [(1, 1), (3, 1), (4, 6), (5, 2)])
+def test_embed_is_delay_view(oracle, m, tau):
+    y = wl.gaussian(11, 64).astype(np.float32)
+    X = oracle.embed(y, m, tau)
+    ref = np.stack([y[c * tau: c * tau + len(y) - (m - 1) * tau] for c in range(m)], axis=1)
+    assert X.shape == ref.shape and np.array_equal(X, ref)
+
+
+# -------------------------------------------------------------- eps against a library order statistic
+def _numpy_condensed(y, m, tau, norm):
+    n = len(y) - (m - 1) * tau
+    X = np.stack([y[c * tau: c * tau + n] for c in range(m)], axis=1).astype(np.float32)
+    diff = X[:, None, :] - X[None, :, :]                       # fp32 subtraction, one rounding each
+    if norm == 0:
+        D = np.abs(diff).max(axis=2)
+    else:
+        sq = diff * diff
+        s = sq[:, :, 0]
+        for c in range(1, m):
+            s = s + sq[:, :, c]                                 # fixed order c = 0..m-1, fp32 each step
+        D = np.sqrt(s)
+    iu = np.triu_indices(n, 1)
+    return D[iu].astype(np.float32)
+
+
+@pytest.mark.parametrize("norm", [0, 1])
+@pytest.mark.parametrize("m,tau,N,seed", [(1, 1, 40, 1), (3, 1, 97, 2), (4, 6, 150, 3), (5, 2, 120, 4)])
+def test_eps_matches_numpy_partition(oracle, m, tau, N, seed, norm):
+    y = wl.gaussian(seed, N).astype(np.float32)
+    rr = np.array([0.003, 0.01, 0.05, 0.1, 0.25, 0.5, 0.99, 1.0])
+    eps, cnt, rrr = oracle.eps_for_rr(y, m, tau, rr, norm)
+    d = _numpy_condensed(y, m, tau, norm)
+    assert np.array_equal(np.sort(d), np.sort(oracle.distances(y, m, tau, norm)))
+    P = len(d)
+    for k, r_ in enumerate(rr):
+        r = min(max(math.ceil(r_ * float(P)), 1), P)
+        e = np.partition(d, r - 1)[r - 1]
+        assert eps[k] == e
+        assert int(cnt[k]) == int((d <= e).sum())
+        assert rrr[k] == int(cnt[k]) / P
+
+
+def test_eps_ties_and_duplicates(oracle):
+    # quantised series -> massive ties; several targets share one eps (reading S6)
+    y = (np.floor(wl.uniform01(5, 80) * 4)).astype(np.float32)
+    rr = np.array([0.05, 0.2, 0.21, 0.5, 0.9])
+    eps, cnt, _ = oracle.eps_for_rr(y, 2, 1, rr, 0)
+    d = _numpy_condensed(y, 2, 1, 0)
+    for k in range(len(rr)):
+        r = math.ceil(rr[k] * len(d))
+        assert eps[k] == np.sort(d)[r - 1]
+        assert int(cnt[k]) == int((d <= eps[k]).sum()) >= r
+    assert len(set(eps.tolist())) < len(rr)
+
+
+# ------------------------------------------------------------------------------ counting certificate
+@pytest.mark.parametrize("norm", [0, 1])
+def test_certificate_brackets_rank(oracle, norm):
+    y = wl.add_noise(wl.logistic_signal(300, 9), 1.0, 9)
+    rr = wl.rr_log(12, 0.001, 0.3)
+    eps, cnt, _ = oracle.eps_for_rr(y, 3, 1, rr, norm)
+    P = oracle.n_pairs(len(y), 3, 1)
+    lt, le = oracle.count_lt_le(y, 3, 1, eps, norm, threads=2)
+    for k in range(len(rr)):
+        r = oracle.rank(rr[k], P)
+        assert int(lt[k]) < r <= int(le[k])
+        assert int(le[k]) == int(cnt[k])
+    # a value that is not the order statistic must fail the certificate
+    lt2, le2 = oracle.count_lt_le(y, 3, 1, np.nextafter(eps, np.float32(np.inf)), norm, threads=1)
+    assert all(int(lt2[k]) >= oracle.rank(rr[k], P) for k in range(len(rr)))
+
+
+# ------------------------------------------------------------------------------------- closed forms
+@pytest.mark.parametrize("m,tau,N", [(1, 1, 50), (3, 2, 61), (4, 6, 120)])
+def test_ramp_closed_form(oracle, m, tau, N):
+    """y_i = i: d_ij = j - i for any (m, tau) under the max norm, so the sorted distances are (N'-1) ones,
+    (N'-2) twos, ...; eps_k = smallest o* with sum_{o<=o*}(N'-o) >= r_k; P_k(l) = 1 for l = N'-o*..N'-1."""
+    y = np.arange(N, dtype=np.float32)
+    n = N - (m - 1) * tau
+    P = n * (n - 1) // 2
+    rr = np.array([0.01, 0.1, 0.33, 0.5, 0.77, 1.0])
+    r = oracle.sweep(y, m, tau, rr, 0)
+    for k, q in enumerate(rr):
+        rank = min(max(math.ceil(q * float(P)), 1), P)
+        cum, ostar = 0, 0
+        while cum < rank:
+            ostar += 1
+            cum += n - ostar
+        assert r["eps"][k] == np.float32(ostar)
+        assert int(r["count"][k]) == cum
+        exp = np.zeros(n, dtype=np.uint64)
+        exp[n - ostar: n] = 1
+        assert np.array_equal(r["hist"][k], exp)
+
+
+def test_constant_series(oracle):
+    y = np.full(30, 2.5, dtype=np.float32)
+    r = oracle.sweep(y, 2, 3, [0.001, 0.5, 1.0], 0)
+    n = 27
+    assert np.all(r["eps"] == 0) and np.all(r["count"] == n * (n - 1) // 2)
+    exp = np.ones(n, dtype=np.uint64)
+    exp[0] = 0
+    for k in range(3):
+        assert np.array_equal(r["hist"][k], exp)      # one line per diagonal, lengths 1..N'-1
+
+
+def test_exactly_periodic_series(oracle):
+    """y_n = T[n mod q] with distinct table values: at eps = 0 a cell recurs iff o = 0 (mod q), so every
+    diagonal is all-or-nothing and P(N' - q t) = 1.  (The config-2 SNR=inf structure.)"""
+    T = np.array([0.0, 3.0, 1.0, 7.0, 4.0, 9.0, 2.0], dtype=np.float32)
+    q, N, m, tau = len(T), 100, 3, 2
+    y = T[np.arange(N) % q]
+    n = N - (m - 1) * tau
+    P = n * (n - 1) // 2
+    c0 = sum(n - q * t for t in range(1, n) if q * t < n)
+    rr_in = (c0 - 0.5) / P            # rank <= c0 -> eps = 0
+    rr_out = (c0 + 0.5) / P           # first rank beyond the zeros -> eps > 0
+    r = oracle.sweep(y, m, tau, [rr_in, rr_out], 0)
+    assert r["eps"][0] == 0 and int(r["count"][0]) == c0
+    exp = np.zeros(n, dtype=np.uint64)
+    for t in range(1, n):
+        if q * t < n:
+            exp[n - q * t] = 1
+    assert np.array_equal(r["hist"][0], exp)
+    assert r["det"][0] == 1.0
+    assert r["eps"][1] > 0
+
+
+def test_config2_sine_snr_inf_closed_form(oracle):
+    """SURVEY.md sec. 8(d), config 2 at SNR = inf: 39 fully recurrent diagonals o = 25..975, 18 798 zero
+    distances; targets 0.01-0.03 give eps = 0, C = 18 798, DET = 1; 0.04 is the first with eps > 0."""
+    w = wl.config2()
+    y = w.series[0]
+    r = oracle.sweep(y, w.m, w.tau, w.rr, w.norm)
+    assert w.n_points == 982 and w.n_pairs == 481671
+    for k in range(3):
+        assert r["eps"][k] == 0 and int(r["count"][k]) == 18798 and r["det"][k] == 1.0
+        nz = np.nonzero(r["hist"][k])[0]
+        assert sorted(nz.tolist()) == sorted(982 - 25 * t for t in range(1, 40))
+        assert np.all(r["hist"][k][nz] == 1)
+    assert r["eps"][3] > 0 and oracle.rank(w.rr[3], w.n_pairs) == 19267
+
+
+# ---------------------------------------------------------------------------------------- invariants
+@pytest.mark.parametrize("norm", [0, 1])
+@pytest.mark.parametrize("maker", ["noise", "logistic", "sine"])
+def test_invariants_sum_nesting_symmetry(oracle, maker, norm):
+    N, m, tau = 260, 3, 2
+    if maker == "noise":
+        y = wl.gaussian(21, N).astype(np.float32)
+    elif maker == "logistic":
+        y = wl.add_noise(wl.logistic_signal(N, 22), 3.0, 22)
+    else:
+        y = wl.add_noise(wl.sine_signal(N), 1.0, 23)
+    rr = wl.rr_log(9, 0.002, 0.4)
+    r = oracle.sweep(y, m, tau, rr, norm)
+    n = N - (m - 1) * tau
+    l = np.arange(n, dtype=np.uint64)
+    hist = r["hist"]
+    # sum_l l P_k(l) = C_k  ("RR can also be calculated from the histogram")
+    assert np.array_equal((hist * l).sum(axis=1), r["count"])
+    assert np.all(hist[:, 0] == 0)
+    # nesting: eps ascending -> C_k non-decreasing, sum_{l>=L} l P_k(l) non-decreasing in k for every L
+    assert np.all(np.diff(r["eps"]) >= 0) and np.all(np.diff(r["count"].astype(np.int64)) >= 0)
+    tail = np.cumsum((hist * l)[:, ::-1], axis=1)[:, ::-1].astype(np.int64)
+    assert np.all(np.diff(tail, axis=0) >= 0)
+    # symmetry: the lower triangle gives the identical histogram
+    assert np.array_equal(oracle.line_hist(y, m, tau, r["eps"], norm, lower=True), hist)
+    # the OpenMP split over diagonals changes nothing
+    assert np.array_equal(oracle.line_hist(y, m, tau, r["eps"], norm, threads=3), hist)
+
+
+def test_line_hist_brute_force_tiny(oracle):
+    """Independent run count on the explicit 0/1 matrix built with numpy (np.diagonal + split on zeros)."""
+    for seed in range(6):
+        N, m, tau = 24 + seed, 2, 1 + seed % 3
+        y = np.round(wl.gaussian(100 + seed, N) * 2).astype(np.float32)
+        n = N - (m - 1) * tau
+        eps = np.array([0.0, 1.0, 2.5], dtype=np.float32)
+        X = np.stack([y[c * tau: c * tau + n] for c in range(m)], axis=1)
+        D = np.abs(X[:, None, :] - X[None, :, :]).max(axis=2)
+        hist = oracle.line_hist(y, m, tau, eps, 0)
+        for k, e in enumerate(eps):
+            R = (D <= e).astype(np.int8)
+            exp = np.zeros(n, dtype=np.uint64)
+            for o in range(1, n):
+                s = "".join(map(str, np.diagonal(R, o)))
+                for run in s.split("0"):
+                    if run:
+                        exp[len(run)] += 1
+            assert np.array_equal(hist[k], exp)
+
+
+# ----------------------------------------------------------------------- statistical closed form (m = 1)
+def test_iid_uniform_det_closed_form(oracle):
+    """i.i.d. U(0,1), m = 1, max norm: a cell recurs with p = 2 eps - eps^2 and neighbouring cells on a
+    diagonal are independent, so a recurrent cell is isolated with probability (1-p)^2 and
+    DET (l_min = 2) ~ 1 - (1-p)^2.  Band: 3*(2 sigma_b) + 2/N', sigma_b binomial."""
+    N = 2000
+    for seed in (31, 32):
+        y = wl.uniform01(seed, N).astype(np.float32)
+        rr = np.array([0.05, 0.1, 0.2])
+        r = oracle.sweep(y, 1, 1, rr, 0)
+        for k in range(3):
+            e = float(r["eps"][k])
+            p = 2 * e - e * e
+            assert abs(p - rr[k]) < 0.01                 # eps really is the rr-quantile of |U1-U2|
+            q = (1 - p) ** 2
+            sigma_b = math.sqrt(q * (1 - q) / float(r["count"][k]))
+            assert abs(r["det"][k] - (1 - q)) <= 3 * (2 * sigma_b) + 2.0 / N
+
+
+# ------------------------------------------------------------------- Euclid: exact rational re-evaluation
+def _round_f32(x: Fraction) -> Fraction:
+    """Round an exact rational to the nearest binary32 value (ties to even), subnormals included."""
+    if x == 0:
+        return Fraction(0)
+    s = -1 if x < 0 else 1
+    a = abs(x)
+    e = math.floor(math.log2(a)) if a >= 1 else -math.ceil(math.log2(1 / a))
+    while Fraction(2) ** e > a:
+        e -= 1
+    while Fraction(2) ** (e + 1) <= a:
+        e += 1
+    q = max(e - 23, -149)                                  # exponent of the last place
+    scaled = a / (Fraction(2) ** q)
+    n = scaled.numerator // scaled.denominator
+    rem = scaled - n
+    if rem > Fraction(1, 2) or (rem == Fraction(1, 2) and n % 2 == 1):
+        n += 1
+    return s * n * (Fraction(2) ** q)
+
+
+def test_euclid_chain_is_exactly_rounded_fp32(oracle):
+    rng_vals = wl.gaussian(77, 400)
+    scales = [1.0, 1e-3, 1e-19, 3e-23, 1e10]               # 1e-19..3e-23: squares fall into the subnormals
+    m, tau = 3, 2
+    for sc in scales:
+        y = (rng_vals[:40] * sc).astype(np.float32)
+        got = oracle.distances(y, m, tau, 1)
+        n = len(y) - (m - 1) * tau
+        p = 0
+        for i in range(n):
+            for j in range(i + 1, n):
+                s = None
+                for c in range(m):
+                    t = _round_f32(Fraction(float(y[i + c * tau])) - Fraction(float(y[j + c * tau])))
+                    sq = _round_f32(t * t)
+                    s = sq if s is None else _round_f32(s + sq)
+                # correctly rounded sqrt of an fp32 value: fp64 sqrt then one rounding is safe (53 >= 2*24+2)
+                exp = np.float32(math.sqrt(float(s)))
+                assert got[p] == exp, (sc, i, j)
+                p += 1
+
+
+def test_max_norm_is_exact(oracle):
+    y = (wl.gaussian(78, 60) * 1e-20).astype(np.float32)
+    got = oracle.distances(y, 2, 3, 0)
+    n = len(y) - 3
+    p = 0
+    for i in range(n):
+        for j in range(i + 1, n):
+            e = max(_round_f32(abs(Fraction(float(y[i + c * 3])) - Fraction(float(y[j + c * 3])))) for c in range(2))
+            assert Fraction(float(got[p])) == e
+            p += 1
+
+
+# ------------------------------------------------------------------------------------- DET and mean
+def test_det_avg_integer_recompute(oracle):
+    y = wl.add_noise(wl.lorenz_signal(400), 1.0, 41)
+    rr = wl.rr_log(7, 0.005, 0.3)
+    r = oracle.sweep(y, 3, 3, rr, 0)
+    hist = r["hist"]
+    n = hist.shape[1]
+    for l_min in (1, 2, 3, 10, n - 1, n, n + 5):
+        det, mean = oracle.det_avg(hist, l_min)
+        acc = 0.0
+        for k in range(len(rr)):
+            num = sum(l * int(hist[k, l]) for l in range(max(l_min, 1), n))
+            den = sum(l * int(hist[k, l]) for l in range(1, n))
+            assert abs(det[k] - float(Fraction(num, den))) <= 1e-15
+            acc += det[k]
+        assert abs(mean - acc / len(rr)) <= 1e-15
+        if l_min == 1:
+            assert np.all(det == 1.0)
+        if l_min >= n:
+            assert np.all(det == 0.0)                      # reading S12
+
+
+def test_det_avg_empty_denominator(oracle):
+    hist = np.zeros((2, 10), dtype=np.uint64)
+    hist[1, 3] = 2
+    det, mean = oracle.det_avg(hist, 2)
+    assert det[0] == 0.0 and det[1] == 1.0 and mean == 0.5
+
+
+# ----------------------------------------------------------------------------------------- workloads
+def test_workloads_are_seeded_and_shaped():
+    a, b = wl.config1(), wl.config1()
+    assert np.array_equal(a.series, b.series) and a.series.dtype == np.float32
+    assert (a.batch, a.N, a.n_points, a.n_pairs, a.K) == (4, 100, 98, 4753, 10)
+    c2 = wl.config2()
+    assert (c2.batch, c2.N, c2.n_points, c2.n_pairs) == (5, 1000, 982, 481671)
+    assert np.allclose(wl.rr_log(20, 0.001, 0.2)[[0, -1]], [0.001, 0.2])
+    assert wl.rr_linear(10)[6] == 0.07
+    g = wl.gaussian(1, 200001)
+    assert abs(g.mean()) < 0.01 and abs(g.std() - 1) < 0.01
+    assert np.array_equal(wl.splitmix64(3, 5, offset=2), wl.splitmix64(3, 7)[2:])
+    y = wl.logistic_signal(500, 7)
+    assert y.min() > 0 and y.max() < 1
+    assert wl.fnv1a64(np.zeros(0, dtype=np.uint8)) == 0xCBF29CE484222325

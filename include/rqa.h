@@ -1,0 +1,160 @@
+/*
+ * rqa.h — C ABI of librqa.so: the data-parallel hot path of averaged recurrence quantification analysis
+ * (Panis, Adamek & Marwan, arXiv 2208.09136) on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are lines of the paper's text and the readings S1..S18 listed in DESIGN.md.
+ *
+ * The path (sec. 2, 3, 5):
+ *   rqa_embed       delay-coordinate embedding x_i[c] = y[i + c*tau]
+ *   rqa_eps_for_rr  thresholds eps_k that realise K target recurrence rates:          PAPER.md:78, Eq. 3 (:63)
+ *                   eps_k = the ceil(RR_k*P)-th smallest of the P = N'(N'-1)/2
+ *                   pairwise distances (exact order statistic, readings S4-S6)
+ *   rqa_line_hist   diagonal-line-length histograms P_k(l) of the recurrence plot     PAPER.md:69-72 (Eq. 4), :125
+ *                   R_ij = (d_ij <= eps_k), all K thresholds in one pass, upper
+ *                   triangle only, R never stored
+ *   rqa_det_avg     DET_k (Eq. 4) and its average over the K recurrence rates (Eq. 5)
+ *
+ * Conventions (BASELINE.json north_star):
+ *   - distances are fp32: maximum norm max_c |x_i[c]-x_j[c]|, or the Euclidean norm computed
+ *     as sqrtf(((t0*t0 + t1*t1) + ...)) in the order c = 0..m-1, every operation rounded to fp32, no FMA;
+ *   - recurrence means d <= eps (S1); the main diagonal is excluded and only pairs i<j are counted (S2);
+ *   - "N" of the paper is N' = N - (m-1)*tau embedded points everywhere (S3);
+ *   - runs that touch the border of the plot count with their truncated length (S8);
+ *   - counts are exact uint64; RR and DET are fp64 ratios of exact integers.
+ *
+ * Memory and ownership: every buffer is owned by the caller.  Pointers named d_* are DEVICE pointers,
+ * h_* are HOST pointers.  The library keeps no device allocation and no global state between calls.
+ * Every call enqueues its work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ * stream) and returns without synchronising; outputs are valid once the stream has been synchronised.
+ *
+ * Errors: a status code is returned, never an exception or an abort.  Argument errors are detected
+ * before anything is launched.  rqa_last_error() gives a thread-local detail string.  Conditions that can
+ * only be seen on the device (NaN/Inf in the series) are recorded in the workspace and reported by
+ * rqa_workspace_status().
+ *
+ * There is no CPU fallback: without a CUDA device every compute call returns RQA_ERR_CUDA.
+ */
+#ifndef RQA_H
+#define RQA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RQA_MAX_K 128 /* maximum number of thresholds per call */
+#define RQA_MAX_M 16  /* maximum embedding dimension */
+
+typedef enum {
+    RQA_OK = 0,
+    RQA_ERR_INVALID_ARG = 1,
+    RQA_ERR_NONFINITE_INPUT = 2,
+    RQA_ERR_WORKSPACE_TOO_SMALL = 3,
+    RQA_ERR_UNSUPPORTED = 4,
+    RQA_ERR_CUDA = 5
+} rqa_status;
+
+typedef enum { RQA_NORM_MAX = 0, RQA_NORM_EUCLID = 1 } rqa_norm;
+
+/*
+ * A batch of point sets, as a strided view of fp32 device memory:
+ *     x_i[c] of series b = data[b*batch_stride + i*point_stride + c*coord_stride],  0<=i<n_points, 0<=c<m.
+ * Delay view of raw series (what rqa_embed returns when d_X == NULL): point_stride = 1, coord_stride = tau.
+ * Materialised row-major X[batch][n_points][m]:                       point_stride = m, coord_stride = 1.
+ * All series of a batch share n_points, m and the strides.  Strides are in elements and must be >= 1.
+ */
+typedef struct rqa_points {
+    const float* data; /* device pointer */
+    int64_t n_points;  /* N' >= 2 */
+    int32_t m;         /* 1..RQA_MAX_M */
+    int32_t batch;     /* >= 1 */
+    int64_t point_stride;
+    int64_t coord_stride;
+    int64_t batch_stride;
+} rqa_points;
+
+const char* rqa_status_string(rqa_status s);
+const char* rqa_last_error(void);
+/* "major.minor sm_100a" build tag; never NULL. */
+const char* rqa_version(void);
+
+/*
+ * Bytes of device workspace that rqa_eps_for_rr / rqa_line_hist need for this shape (the larger of the two).
+ * The workspace is scratch: its contents need not survive between calls, except that rqa_workspace_status()
+ * reads the status block the last call wrote.  It must be 256-byte aligned.
+ */
+rqa_status rqa_workspace_bytes(const rqa_points* pts, int32_t K, size_t* bytes);
+
+/*
+ * Synchronises `stream`, then returns what the last call that used this workspace recorded on the device:
+ * RQA_OK, RQA_ERR_NONFINITE_INPUT (a NaN or Inf among the points; outputs are then undefined) or
+ * RQA_ERR_CUDA.
+ */
+rqa_status rqa_workspace_status(const void* d_ws, void* stream);
+
+/*
+ * Delay embedding (forward indexing, reading S7).  N' = N - (m-1)*tau must be >= 2.
+ *   d_series  [batch] series of N samples, series b at d_series + b*series_stride
+ *   d_X       NULL: nothing is copied, *view_out describes the strided delay view of d_series;
+ *             else: [batch][N'][m] row-major, written by the call, and *view_out describes it.
+ */
+rqa_status rqa_embed(const float* d_series, int64_t N, int32_t batch, int64_t series_stride, int32_t m,
+                     int64_t tau, float* d_X, rqa_points* view_out, void* stream);
+
+/*
+ * Thresholds for target recurrence rates (readings S4-S6).
+ *   h_rr            HOST array of K target rates, each in (0, 1], any order, duplicates allowed
+ *   d_eps           [batch][K] eps_k = the r_k-th smallest pairwise distance, r_k = ceil(rr_k * P) evaluated
+ *                   in fp64 and clamped to [1, P], P = N'(N'-1)/2 — in the caller's order of h_rr
+ *   d_count         [batch][K] C_k = #{i<j : d_ij <= eps_k}  (>= r_k when there are ties)
+ *   d_rr_realised   [batch][K] (double)C_k / (double)P
+ * 1 <= K <= RQA_MAX_K.
+ */
+rqa_status rqa_eps_for_rr(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps,
+                          uint64_t* d_count, double* d_rr_realised, void* d_ws, size_t ws_bytes, void* stream);
+
+/*
+ * Diagonal-line histograms at K thresholds.
+ *   d_eps   [batch][K] thresholds (device), any order, duplicates allowed, each finite and >= 0
+ *   d_hist  [batch][K][n_points] uint64, overwritten: d_hist[b][k][l] = number of maximal runs of exactly l
+ *           consecutive recurrent cells (d <= eps_k) along the diagonals j-i = 1..N'-1; [..][0] = 0.
+ * Invariant tying it to rqa_eps_for_rr: sum_l l*d_hist[b][k][l] == C_k.
+ */
+rqa_status rqa_line_hist(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
+                         void* d_ws, size_t ws_bytes, void* stream);
+
+/*
+ * DET_k = sum_{l>=l_min} l*P_k(l) / sum_{l>=1} l*P_k(l)  (Eq. 4; 0 if the denominator is 0) and
+ * mean_b = (1/K) * sum_{k=0}^{K-1} DET_k, summed left to right in fp64 (Eq. 5; reading S11).
+ *   d_hist      [batch][K][n_points] from rqa_line_hist
+ *   d_det       [batch][K]     d_det_mean  [batch]
+ */
+rqa_status rqa_det_avg(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
+                       double* d_det, double* d_det_mean, void* stream);
+
+/*
+ * The whole path for HOST buffers (what bench.py's `e2e` times): copies the series to the device workspace,
+ * runs rqa_embed (view) -> rqa_eps_for_rr -> rqa_line_hist -> rqa_det_avg on `stream`, copies the results
+ * back and synchronises the stream before returning.
+ *   h_series  [batch][N] fp32 (pinned memory gives asynchronous copies)
+ *   h_eps, h_count, h_rr_realised, h_det  [batch][K];  h_det_mean [batch];  h_hist [batch][K][N'] or NULL
+ *   d_ws      device workspace of at least rqa_sweep_workspace_bytes(...) bytes
+ */
+rqa_status rqa_sweep_workspace_bytes(int64_t N, int32_t batch, int32_t m, int64_t tau, int32_t K, size_t* bytes);
+rqa_status rqa_sweep_host(const float* h_series, int64_t N, int32_t batch, int32_t m, int64_t tau, rqa_norm norm,
+                          const double* h_rr, int32_t K, int64_t l_min, float* h_eps, uint64_t* h_count,
+                          double* h_rr_realised, double* h_det, double* h_det_mean, uint64_t* h_hist, void* d_ws,
+                          size_t ws_bytes, void* stream);
+
+/*
+ * Number of kernel launches the library has enqueued from this process so far (monotone counter; bench.py
+ * reports the difference over its timed region as `gpu_launches`).
+ */
+uint64_t rqa_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RQA_H */

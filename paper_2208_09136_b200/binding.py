@@ -1,0 +1,185 @@
+"""Thin ctypes binding over librqa.so (include/rqa.h).  Same names as the C ABI; argument marshalling only —
+every step of the path runs in the library's CUDA kernels.  PyTorch supplies device memory and streams.
+
+There is no fallback: if librqa.so is missing or cannot be loaded, load_library() raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+PKG = Path(__file__).resolve().parent
+LIB_PATH = PKG / "librqa.so"
+
+RQA_OK = 0
+RQA_ERR_INVALID_ARG = 1
+RQA_ERR_NONFINITE_INPUT = 2
+RQA_ERR_WORKSPACE_TOO_SMALL = 3
+RQA_ERR_UNSUPPORTED = 4
+RQA_ERR_CUDA = 5
+RQA_NORM_MAX = 0
+RQA_NORM_EUCLID = 1
+RQA_MAX_K = 128
+RQA_MAX_M = 16
+
+# every symbol include/rqa.h declares (tests check that the library exports them all)
+EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_bytes", "rqa_workspace_status",
+           "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
+           "rqa_sweep_host", "rqa_launch_count"]
+
+
+class RqaPoints(ctypes.Structure):
+    """struct rqa_points"""
+    _fields_ = [("data", ctypes.c_void_p), ("n_points", ctypes.c_int64), ("m", ctypes.c_int32),
+                ("batch", ctypes.c_int32), ("point_stride", ctypes.c_int64), ("coord_stride", ctypes.c_int64),
+                ("batch_stride", ctypes.c_int64)]
+
+
+class RqaError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{msg} (status {status})")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_2208_09136_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(str(LIB_PATH))
+    vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+    pts = ctypes.POINTER(RqaPoints)
+    lib.rqa_status_string.restype = ctypes.c_char_p
+    lib.rqa_status_string.argtypes = [ctypes.c_int]
+    lib.rqa_last_error.restype = ctypes.c_char_p
+    lib.rqa_version.restype = ctypes.c_char_p
+    lib.rqa_launch_count.restype = ctypes.c_uint64
+    lib.rqa_workspace_bytes.argtypes = [pts, i32, ctypes.POINTER(sz)]
+    lib.rqa_workspace_status.argtypes = [vp, vp]
+    lib.rqa_embed.argtypes = [vp, i64, i32, i64, i32, i64, vp, pts, vp]
+    lib.rqa_eps_for_rr.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, vp, vp, sz, vp]
+    lib.rqa_line_hist.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp]
+    lib.rqa_det_avg.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp]
+    lib.rqa_sweep_workspace_bytes.argtypes = [i64, i32, i32, i64, i32, ctypes.POINTER(sz)]
+    lib.rqa_sweep_host.argtypes = [vp, i64, i32, i32, i64, ctypes.c_int, vp, i32, i64, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    _lib = lib
+    return lib
+
+
+def _check(st: int):
+    if st != RQA_OK:
+        lib = load_library()
+        raise RqaError(st, f"{lib.rqa_status_string(st).decode()}: {lib.rqa_last_error().decode()}")
+
+
+def _stream(stream=None) -> int:
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _dev(t, dtype, what: str) -> int:
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{what} must be a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{what} must be a contiguous {dtype} tensor")
+    return t.data_ptr()
+
+
+def rqa_version() -> str:
+    return load_library().rqa_version().decode()
+
+
+def rqa_launch_count() -> int:
+    return int(load_library().rqa_launch_count())
+
+
+def rqa_workspace_bytes(pts: RqaPoints, K: int) -> int:
+    n = ctypes.c_size_t(0)
+    _check(load_library().rqa_workspace_bytes(ctypes.byref(pts), K, ctypes.byref(n)))
+    return int(n.value)
+
+
+def rqa_workspace_status(ws, stream=None) -> None:
+    """Synchronises the stream; raises RqaError (e.g. RQA_ERR_NONFINITE_INPUT) if the last call recorded one."""
+    import torch
+    _check(load_library().rqa_workspace_status(_dev(ws, torch.uint8, "ws"), _stream(stream)))
+
+
+def rqa_embed(series, m: int, tau: int, X=None, stream=None) -> RqaPoints:
+    """series: float32 CUDA tensor [batch][N] (or [N]).  Returns the rqa_points view (of `series` itself when
+    X is None, else of the materialised X[batch][N'][m] the call writes)."""
+    import torch
+    if series.dim() == 1:
+        series = series.unsqueeze(0)
+    p = _dev(series, torch.float32, "series")
+    batch, N = series.shape
+    view = RqaPoints()
+    xp = None if X is None else _dev(X, torch.float32, "X")
+    _check(load_library().rqa_embed(p, N, batch, N, m, tau, xp, ctypes.byref(view), _stream(stream)))
+    return view
+
+
+def rqa_eps_for_rr(pts: RqaPoints, norm: int, rr, eps, count, rr_realised, ws, stream=None) -> None:
+    """rr: host float64 array [K]; eps float32 / count int64(uint64 bits) / rr_realised float64 CUDA tensors
+    [batch][K]; ws: uint8 CUDA workspace."""
+    import torch
+    rr = np.ascontiguousarray(rr, dtype=np.float64)
+    K = len(rr)
+    _check(load_library().rqa_eps_for_rr(ctypes.byref(pts), norm, rr.ctypes.data, K, _dev(eps, torch.float32, "eps"),
+                                         _dev(count, torch.int64, "count"),
+                                         _dev(rr_realised, torch.float64, "rr_realised"),
+                                         _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream)))
+
+
+def rqa_line_hist(pts: RqaPoints, norm: int, eps, hist, ws, stream=None) -> None:
+    """eps float32 CUDA [batch][K]; hist int64 (uint64 bits) CUDA [batch][K][n_points]."""
+    import torch
+    K = eps.shape[-1]
+    _check(load_library().rqa_line_hist(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps"), K,
+                                        _dev(hist, torch.int64, "hist"), _dev(ws, torch.uint8, "ws"), ws.numel(),
+                                        _stream(stream)))
+
+
+def rqa_det_avg(hist, l_min: int, det, det_mean, stream=None) -> None:
+    """hist int64 CUDA [batch][K][n_points]; det float64 [batch][K]; det_mean float64 [batch]."""
+    import torch
+    batch, K, n = hist.shape
+    _check(load_library().rqa_det_avg(_dev(hist, torch.int64, "hist"), batch, K, n, l_min,
+                                      _dev(det, torch.float64, "det"), _dev(det_mean, torch.float64, "det_mean"),
+                                      _stream(stream)))
+
+
+def rqa_sweep_workspace_bytes(N: int, batch: int, m: int, tau: int, K: int) -> int:
+    n = ctypes.c_size_t(0)
+    _check(load_library().rqa_sweep_workspace_bytes(N, batch, m, tau, K, ctypes.byref(n)))
+    return int(n.value)
+
+
+def rqa_sweep_host(series, m: int, tau: int, norm: int, rr, l_min: int, eps, count, rr_realised, det, det_mean, hist,
+                   ws, stream=None) -> None:
+    """Host buffers in, host buffers out (CPU torch tensors, pinned for asynchronous copies); `ws` is a CUDA
+    uint8 workspace of rqa_sweep_workspace_bytes(...).  hist may be None."""
+    import torch
+    rr = np.ascontiguousarray(rr, dtype=np.float64)
+
+    def host(t, dtype, what):
+        if t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+            raise TypeError(f"{what} must be a contiguous CPU {dtype} tensor")
+        return t.data_ptr()
+
+    batch, N = series.shape
+    _check(load_library().rqa_sweep_host(
+        host(series, torch.float32, "series"), N, batch, m, tau, norm, rr.ctypes.data, len(rr), l_min,
+        host(eps, torch.float32, "eps"), host(count, torch.int64, "count"),
+        host(rr_realised, torch.float64, "rr_realised"), host(det, torch.float64, "det"),
+        host(det_mean, torch.float64, "det_mean"), None if hist is None else host(hist, torch.int64, "hist"),
+        _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream)))

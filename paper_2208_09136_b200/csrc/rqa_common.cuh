@@ -1,0 +1,126 @@
+// rqa_common.cuh — internal declarations shared by the translation units of librqa.so.
+// Not part of the public ABI (that is include/rqa.h) and not shared with the oracle.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+
+#include "rqa.h"
+
+namespace rqa {
+
+// ---------------------------------------------------------------------------------------------- errors
+void set_error(const char* fmt, ...);
+extern std::atomic<uint64_t> g_launches;
+
+#define RQA_CUDA_TRY(expr)                                                                         \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            rqa::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return RQA_ERR_CUDA;                                                                   \
+        }                                                                                          \
+    } while (0)
+
+// counts the launch and checks cudaGetLastError
+#define RQA_LAUNCH_CHECK()                                                                         \
+    do {                                                                                           \
+        rqa::g_launches.fetch_add(1, std::memory_order_relaxed);                                   \
+        cudaError_t e__ = cudaGetLastError();                                                      \
+        if (e__ != cudaSuccess) {                                                                  \
+            rqa::set_error("kernel launch failed: %s (%s:%d)", cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return RQA_ERR_CUDA;                                                                   \
+        }                                                                                          \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------ view
+// Device-side copy of rqa_points (x_i[c] of series b = data[b*bs + i*ps + c*cs]).
+struct View {
+    const float* data;
+    int64_t n;   // N'
+    int32_t m;
+    int32_t batch;
+    int64_t ps, cs, bs;
+};
+
+inline View make_view(const rqa_points& p) {
+    View v;
+    v.data = p.data;
+    v.n = p.n_points;
+    v.m = p.m;
+    v.batch = p.batch;
+    v.ps = p.point_stride;
+    v.cs = p.coord_stride;
+    v.bs = p.batch_stride;
+    return v;
+}
+
+inline uint64_t n_pairs(int64_t n) { return (uint64_t)n * (uint64_t)(n - 1) / 2; }
+
+rqa_status validate_points(const rqa_points* pts, const char* who);
+
+// ------------------------------------------------------------------------------------------- workspace
+// Status block at the start of every workspace (256 bytes reserved).
+struct WsStatus {
+    int32_t nonfinite;   // set to 1 by the finite check when a NaN/Inf is seen
+    int32_t internal;    // set to 1 on an internal inconsistency (should never happen)
+    int32_t pad[62];
+};
+static_assert(sizeof(WsStatus) == 256, "status block is 256 bytes");
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Simple bump allocator over the caller's workspace.
+struct Arena {
+    char* base;
+    size_t size, off;
+    Arena(void* p, size_t n) : base((char*)p), size(n), off(0) {}
+    template <typename T>
+    T* take(size_t count) {
+        size_t bytes = align_up(count * sizeof(T));
+        T* r = (T*)(base + off);
+        off += bytes;
+        return r;
+    }
+    bool ok() const { return off <= size; }
+};
+
+// ------------------------------------------------------------------------------------ internal launchers
+rqa_status launch_finite_check(const View& v, WsStatus* st, cudaStream_t s);
+
+size_t select_workspace_bytes(const View& v, int K);
+rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
+                      double* d_rr, Arena& ws, cudaStream_t s);
+
+size_t line_workspace_bytes(const View& v, int K);
+rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws,
+                         cudaStream_t s);
+
+// ---------------------------------------------------------------------------------------- device helpers
+#ifdef __CUDACC__
+// Distance between embedded points i and j of one series (yb = series base).  Max norm: PAPER.md:50.
+// Euclid: fixed order c = 0..m-1, every operation individually rounded (no FMA) — DESIGN.md reading S13.
+template <int NORM>
+__device__ __forceinline__ float point_distance(const float* __restrict__ yb, int64_t i, int64_t j, int m,
+                                                int64_t ps, int64_t cs) {
+    const float* a = yb + i * ps;
+    const float* b = yb + j * ps;
+    if (NORM == RQA_NORM_MAX) {
+        float d = 0.0f;
+        for (int c = 0; c < m; ++c) d = fmaxf(d, fabsf(__fsub_rn(a[c * cs], b[c * cs])));
+        return d;
+    } else {
+        float t = __fsub_rn(a[0], b[0]);
+        float s = __fmul_rn(t, t);
+        for (int c = 1; c < m; ++c) {
+            t = __fsub_rn(a[c * cs], b[c * cs]);
+            s = __fadd_rn(s, __fmul_rn(t, t));
+        }
+        return __fsqrt_rn(s);
+    }
+}
+#endif
+
+}  // namespace rqa

@@ -218,17 +218,18 @@ def config3(norm: int = NORM_MAX, N: int = 10000) -> Workload:
     return Workload(f"config3_lorenz_N{N}_{nm}", np.stack(rows), 3, 3, norm, rr_log(20, 0.001, 0.2), (2,), labels)
 
 
-def config4(N: int = 100000, which=None) -> Workload:
+def config4(N: int = 100000, which=None, realisation: int = 0) -> Workload:
     """Headline: N=1e5 logistic and Lorenz x at SNR in {1, 0.1}, plus white noise; m=3, tau=1, max; K=20 log.
     `which` selects a subset of the five series by index (0 logistic/1, 1 logistic/0.1, 2 lorenz/1,
-    3 lorenz/0.1, 4 white noise)."""
+    3 lorenz/0.1, 4 white noise); `realisation` picks the noise/initial-condition seeds (bench.py gives every
+    rank its own)."""
     specs = [(SIG_LOGISTIC, 1.0, 0), (SIG_LOGISTIC, 0.1, 1), (SIG_LORENZ, 1.0, 0), (SIG_LORENZ, 0.1, 1),
              (SIG_NOISE, 0.0, 0)]
     if which is not None:
         specs = [specs[i] for i in which]
     rows, labels = [], []
     for sig, snr, si in specs:
-        seed = make_seed(4, sig, si)
+        seed = make_seed(4, sig, si, realisation)
         if sig == SIG_LOGISTIC:
             rows.append(add_noise(logistic_signal(N, seed), snr, seed))
         elif sig == SIG_LORENZ:

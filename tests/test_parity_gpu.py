@@ -1,0 +1,292 @@
+"""Parity of the CUDA path (librqa.so through the thin binding) against the CPU oracle, element by element on
+the same seeded inputs.  Bar (BASELINE.json north_star): eps_k, C_k, realised RR_k and every P_k(l) bit-exact;
+DET_k and mean DET within 1e-12.  All tests here need a GPU (`-m gpu`) and call through the C ABI.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2208_09136_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+DET_TOL = 1e-12
+
+
+def gpu_sweep(rqa, series, m, tau, rr, norm=0, l_min=2):
+    import torch
+    s = torch.as_tensor(np.ascontiguousarray(series, dtype=np.float32)).cuda()
+    buf = rqa.averaged_rqa(s, m, tau, rr, norm, l_min)
+    torch.cuda.synchronize()
+    return {
+        "eps": buf.eps.cpu().numpy(),
+        "count": buf.count.cpu().numpy().view(np.uint64),
+        "rr": buf.rr.cpu().numpy(),
+        "hist": buf.hist.cpu().numpy().view(np.uint64),
+        "det": buf.det.cpu().numpy(),
+        "det_mean": buf.det_mean.cpu().numpy(),
+    }
+
+
+def assert_parity(oracle, g, series, m, tau, rr, norm=0, l_min=2, threads=0):
+    series = np.atleast_2d(series)
+    for b in range(series.shape[0]):
+        r = oracle.sweep(series[b], m, tau, rr, norm, l_min, threads=threads)
+        assert np.array_equal(g["eps"][b].view(np.uint32), r["eps"].view(np.uint32)), f"eps, series {b}"
+        assert np.array_equal(g["count"][b], r["count"]), f"count, series {b}"
+        assert np.array_equal(g["rr"][b], r["rr"]), f"realised rr, series {b}"
+        if not np.array_equal(g["hist"][b], r["hist"]):
+            bad = np.argwhere(g["hist"][b] != r["hist"])
+            k, l = bad[0]
+            raise AssertionError(f"hist, series {b}: {len(bad)} cells differ, first at k={k} l={l}: "
+                                 f"gpu {g['hist'][b][k, l]} oracle {r['hist'][k, l]}")
+        assert np.max(np.abs(g["det"][b] - r["det"])) <= DET_TOL
+        assert abs(g["det_mean"][b] - r["det_mean"]) <= DET_TOL
+
+
+# ---------------------------------------------------------------------------------------- BASELINE configs
+def test_config1_logistic_n100(rqa, oracle):
+    w = wl.config1()
+    g = gpu_sweep(rqa, w.series, w.m, w.tau, w.rr, w.norm)
+    assert_parity(oracle, g, w.series, w.m, w.tau, w.rr, w.norm)
+
+
+def test_config2_sine_batch_of_5(rqa, oracle):
+    w = wl.config2()
+    g = gpu_sweep(rqa, w.series, w.m, w.tau, w.rr, w.norm)
+    assert_parity(oracle, g, w.series, w.m, w.tau, w.rr, w.norm)
+    # closed form at SNR = inf: eps = 0, C = 18 798 for targets 0.01..0.03
+    assert np.all(g["eps"][0][:3] == 0) and np.all(g["count"][0][:3] == 18798)
+
+
+@pytest.mark.parametrize("norm", [0, 1])
+def test_config3_lorenz_n1e4(rqa, oracle, norm):
+    w = wl.config3(norm)
+    g = gpu_sweep(rqa, w.series, w.m, w.tau, w.rr, w.norm)
+    assert_parity(oracle, g, w.series, w.m, w.tau, w.rr, w.norm)
+
+
+def test_config5_shape_small_batch(rqa, oracle):
+    """config 5's shape (m=5, tau=2, K=32 log 0.0005..0.3, l_min in {2,3}) on a reduced batch the oracle finishes
+    in seconds: 3 signals x 2 SNRs x 1 seed at N = 3000."""
+    import torch
+    w = wl.config5(N=3000, n_snr=2, n_seeds=1)
+    s = torch.as_tensor(w.series).cuda()
+    for l_min in w.l_min:
+        buf = rqa.averaged_rqa(s, w.m, w.tau, w.rr, w.norm, l_min)
+        g = {"eps": buf.eps.cpu().numpy(), "count": buf.count.cpu().numpy().view(np.uint64), "rr": buf.rr.cpu().numpy(),
+             "hist": buf.hist.cpu().numpy().view(np.uint64), "det": buf.det.cpu().numpy(),
+             "det_mean": buf.det_mean.cpu().numpy()}
+        assert_parity(oracle, g, w.series, w.m, w.tau, w.rr, w.norm, l_min)
+
+
+# ----------------------------------------------------------------------------- ragged sizes, tiles, tails
+@pytest.mark.parametrize("norm", [0, 1])
+@pytest.mark.parametrize("N,m,tau", [(2, 1, 1), (3, 1, 1), (5, 2, 2), (33, 1, 1), (34, 3, 1), (130, 3, 1), (257, 2, 5),
+                                     (513, 3, 1), (700, 4, 6), (1025, 1, 1), (1500, 3, 3), (2100, 5, 2), (4099, 3, 1)])
+def test_ragged_sizes(rqa, oracle, N, m, tau, norm):
+    kind = N % 3
+    if kind == 0:
+        y = wl.gaussian(1000 + N, N).astype(np.float32)
+    elif kind == 1:
+        y = wl.add_noise(wl.logistic_signal(N, N), 2.0, N)
+    else:
+        y = wl.add_noise(wl.sine_signal(N), 0.5, N)
+    rr = np.array([0.5, 0.001, 0.02, 0.02, 0.11, 1.0, 0.3])       # unsorted, duplicate, rr = 1
+    g = gpu_sweep(rqa, y, m, tau, rr, norm)
+    assert_parity(oracle, g, y, m, tau, rr, norm)
+
+
+def test_batch_ragged(rqa, oracle):
+    ys = np.stack([wl.gaussian(50 + b, 777).astype(np.float32) * (b + 1) for b in range(7)])
+    rr = wl.rr_log(13, 0.002, 0.35)
+    g = gpu_sweep(rqa, ys, 3, 2, rr, 0)
+    assert_parity(oracle, g, ys, 3, 2, rr, 0)
+
+
+# ---------------------------------------------------------------------------------------- degenerate cases
+def test_hand_cases_on_gpu(rqa, oracle):
+    from test_oracle_pins import _hand_cases
+    for p in _hand_cases():
+        y, m, tau, norm, rr, eps, C, hist, det = p.values
+        g = gpu_sweep(rqa, y, m, tau, [rr], norm)
+        assert g["eps"][0, 0] == eps and int(g["count"][0, 0]) == C
+        got = {int(l): int(c) for l, c in enumerate(g["hist"][0, 0]) if c}
+        assert got == hist
+        assert abs(g["det"][0, 0] - float(det)) <= DET_TOL
+
+
+@pytest.mark.parametrize("N", [40, 900, 5000])
+def test_constant_and_quantised_series(rqa, oracle, N):
+    rr = np.array([0.001, 0.3, 1.0])
+    y = np.full(N, -1.25, dtype=np.float32)
+    g = gpu_sweep(rqa, y, 3, 1, rr, 0)
+    n = N - 2
+    assert np.all(g["eps"] == 0) and np.all(g["count"] == n * (n - 1) // 2)
+    exp = np.ones(n, dtype=np.uint64)
+    exp[0] = 0
+    assert all(np.array_equal(g["hist"][0, k], exp) for k in range(3))
+    if N <= 900:
+        yq = np.floor(wl.uniform01(N, N) * 3).astype(np.float32)      # massive ties
+        g = gpu_sweep(rqa, yq, 2, 1, rr, 0)
+        assert_parity(oracle, g, yq, 2, 1, rr, 0)
+
+
+@pytest.mark.parametrize("N,m,tau", [(3000, 3, 1), (20000, 4, 6)])
+def test_ramp_closed_form_large(rqa, N, m, tau):
+    """y_i = i: eps_k = o*, C_k = sum_{o<=o*}(N'-o), P_k(l) = 1 for l = N'-o*..N'-1 — needs no oracle, stresses very
+    long lines across many tiles."""
+    y = np.arange(N, dtype=np.float32)
+    n = N - (m - 1) * tau
+    P = n * (n - 1) // 2
+    rr = np.array([0.0005, 0.01, 0.1, 0.5, 0.9])
+    g = gpu_sweep(rqa, y, m, tau, rr, 0)
+    for k, q in enumerate(rr):
+        rank = min(max(math.ceil(q * float(P)), 1), P)
+        cum, ostar = 0, 0
+        while cum < rank:
+            ostar += 1
+            cum += n - ostar
+        assert g["eps"][0, k] == np.float32(ostar) and int(g["count"][0, k]) == cum
+        exp = np.zeros(n, dtype=np.uint64)
+        exp[n - ostar:] = 1
+        assert np.array_equal(g["hist"][0, k], exp)
+
+
+def test_max_k_and_k1(rqa, oracle):
+    y = wl.add_noise(wl.lorenz_signal(600), 1.0, 5)
+    rr = wl.rr_log(128, 0.0005, 0.9)
+    g = gpu_sweep(rqa, y, 3, 3, rr, 0)
+    assert_parity(oracle, g, y, 3, 3, rr, 0)
+    g1 = gpu_sweep(rqa, y, 3, 3, [0.07], 0)
+    assert_parity(oracle, g1, y, 3, 3, [0.07], 0)
+    assert g1["det_mean"][0] == g1["det"][0, 0]
+
+
+def test_tiny_scale_and_denormals(rqa, oracle):
+    y = (wl.gaussian(8, 500) * 1e-20).astype(np.float32)     # Euclid squares underflow into the subnormals
+    rr = wl.rr_log(6, 0.01, 0.5)
+    for norm in (0, 1):
+        g = gpu_sweep(rqa, y, 3, 1, rr, norm)
+        assert_parity(oracle, g, y, 3, 1, rr, norm)
+
+
+# ---------------------------------------------------------------------------- boundary behaviour on the GPU
+def test_materialised_points_equal_delay_view(rqa, oracle):
+    import torch
+    y = wl.add_noise(wl.sine_signal(900), 1.0, 3)
+    m, tau = 4, 6
+    rr = wl.rr_linear(10)
+    s = torch.as_tensor(y).cuda().unsqueeze(0)
+    n = len(y) - (m - 1) * tau
+    X = torch.empty((1, n, m), dtype=torch.float32, device="cuda")
+    view = rqa.rqa_embed(s, m, tau, X)
+    assert (view.point_stride, view.coord_stride, view.n_points) == (m, 1, n)
+    assert np.array_equal(X.cpu().numpy()[0], oracle.embed(y, m, tau))
+    K = len(rr)
+    eps = torch.empty((1, K), dtype=torch.float32, device="cuda")
+    cnt = torch.empty((1, K), dtype=torch.int64, device="cuda")
+    rrr = torch.empty((1, K), dtype=torch.float64, device="cuda")
+    hist = torch.empty((1, K, n), dtype=torch.int64, device="cuda")
+    ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
+    rqa.rqa_eps_for_rr(view, 0, rr, eps, cnt, rrr, ws)
+    rqa.rqa_line_hist(view, 0, eps, hist, ws)
+    rqa.rqa_workspace_status(ws)
+    r = oracle.sweep(y, m, tau, rr, 0)
+    assert np.array_equal(eps.cpu().numpy()[0], r["eps"])
+    assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], r["hist"])
+
+
+def test_line_hist_with_caller_thresholds(rqa, oracle):
+    """rqa_line_hist takes any thresholds (unsorted, duplicated, zero, huge), not only order statistics."""
+    import torch
+    y = wl.add_noise(wl.logistic_signal(1200, 4), 1.0, 4)
+    eps = np.array([0.3, 0.0, 0.05, 0.3, 10.0, 0.11], dtype=np.float32)
+    s = torch.as_tensor(y).cuda().unsqueeze(0)
+    view = rqa.rqa_embed(s, 3, 1)
+    n = int(view.n_points)
+    hist = torch.empty((1, len(eps), n), dtype=torch.int64, device="cuda")
+    ws = torch.empty(rqa.rqa_workspace_bytes(view, len(eps)), dtype=torch.uint8, device="cuda")
+    rqa.rqa_line_hist(view, 0, torch.as_tensor(eps).cuda().unsqueeze(0), hist, ws)
+    rqa.rqa_workspace_status(ws)
+    assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], oracle.line_hist(y, 3, 1, eps, 0))
+
+
+def test_nonfinite_input_is_reported(rqa):
+    import torch
+    y = wl.gaussian(2, 300).astype(np.float32)
+    y[123] = np.nan
+    with pytest.raises(rqa.RqaError) as e:
+        rqa.averaged_rqa(torch.as_tensor(y).cuda(), 3, 1, [0.1])
+    assert e.value.status == rqa.RQA_ERR_NONFINITE_INPUT
+
+
+def test_workspace_too_small_is_reported(rqa):
+    import torch
+    s = torch.zeros((1, 500), dtype=torch.float32, device="cuda")
+    view = rqa.rqa_embed(s, 3, 1)
+    K = 4
+    eps = torch.empty((1, K), dtype=torch.float32, device="cuda")
+    cnt = torch.empty((1, K), dtype=torch.int64, device="cuda")
+    rrr = torch.empty((1, K), dtype=torch.float64, device="cuda")
+    ws = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(rqa.RqaError) as e:
+        rqa.rqa_eps_for_rr(view, 0, [0.1] * K, eps, cnt, rrr, ws)
+    assert e.value.status == rqa.RQA_ERR_WORKSPACE_TOO_SMALL
+
+
+def test_det_avg_l_min_variants(rqa, oracle):
+    import torch
+    y = wl.add_noise(wl.lorenz_signal(800), 0.3, 6)
+    rr = wl.rr_log(9, 0.001, 0.3)
+    r = oracle.sweep(y, 3, 3, rr, 0)
+    hist = torch.as_tensor(r["hist"].view(np.int64)).cuda().unsqueeze(0)
+    n = r["hist"].shape[1]
+    for l_min in (1, 2, 3, 17, n - 1, n, n + 9):
+        det = torch.empty((1, len(rr)), dtype=torch.float64, device="cuda")
+        mean = torch.empty((1,), dtype=torch.float64, device="cuda")
+        rqa.rqa_det_avg(hist, l_min, det, mean)
+        od, om = oracle.det_avg(r["hist"], l_min)
+        assert np.max(np.abs(det.cpu().numpy()[0] - od)) <= DET_TOL and abs(float(mean[0]) - om) <= DET_TOL
+
+
+def test_sweep_host_matches_device_path(rqa, oracle):
+    import torch
+    w = wl.config2()
+    K, n = w.K, w.n_points
+    series = torch.as_tensor(w.series).pin_memory()
+    eps = torch.empty((w.batch, K), dtype=torch.float32).pin_memory()
+    cnt = torch.empty((w.batch, K), dtype=torch.int64).pin_memory()
+    rrr = torch.empty((w.batch, K), dtype=torch.float64).pin_memory()
+    det = torch.empty((w.batch, K), dtype=torch.float64).pin_memory()
+    mean = torch.empty((w.batch,), dtype=torch.float64).pin_memory()
+    hist = torch.empty((w.batch, K, n), dtype=torch.int64).pin_memory()
+    ws = torch.empty(rqa.rqa_sweep_workspace_bytes(w.N, w.batch, w.m, w.tau, K), dtype=torch.uint8, device="cuda")
+    rqa.rqa_sweep_host(series, w.m, w.tau, w.norm, w.rr, 2, eps, cnt, rrr, det, mean, hist, ws)
+    g = {"eps": eps.numpy(), "count": cnt.numpy().view(np.uint64), "rr": rrr.numpy(), "hist": hist.numpy().view(np.uint64),
+         "det": det.numpy(), "det_mean": mean.numpy()}
+    assert_parity(oracle, g, w.series, w.m, w.tau, w.rr, w.norm)
+
+
+# ------------------------------------------------------------------- full size, bench.py's launch configuration
+@pytest.mark.slow
+def test_config4_full_size_white_noise(rqa, oracle):
+    """N = 1e5, K = 20 (the headline workload, same call sequence as bench.py): the sorted distance array would be
+    20 GB, so eps_k is checked with the counting certificate #{d<eps} < r <= #{d<=eps} (oracle, O(1) memory), C_k with
+    #{d<=eps}, and the histograms with the invariant sum_l l*P_k(l) = C_k plus the oracle's own line histogram at the
+    three smallest thresholds."""
+    w = wl.config4(which=[4])
+    g = gpu_sweep(rqa, w.series, w.m, w.tau, w.rr, w.norm)
+    P = w.n_pairs
+    eps = g["eps"][0]
+    lt, le = oracle.count_lt_le(w.series[0], w.m, w.tau, eps, w.norm, threads=0)
+    for k in range(w.K):
+        r = oracle.rank(w.rr[k], P)
+        assert int(lt[k]) < r <= int(le[k]), f"k={k}: eps is not the rank-{r} order statistic"
+        assert int(g["count"][0, k]) == int(le[k])
+        assert g["rr"][0, k] == int(le[k]) / P
+    l = np.arange(w.n_points, dtype=np.uint64)
+    assert np.array_equal((g["hist"][0] * l).sum(axis=1), g["count"][0])
+    oh = oracle.line_hist(w.series[0], w.m, w.tau, eps[:3], w.norm, threads=0)
+    assert np.array_equal(g["hist"][0][:3], oh)

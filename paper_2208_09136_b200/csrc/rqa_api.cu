@@ -149,6 +149,7 @@ rqa_status rqa_workspace_status(const void* d_ws, void* stream) {
     RQA_CUDA_TRY(cudaMemcpyAsync(&h, d_ws, sizeof(h), cudaMemcpyDeviceToHost, s));
     RQA_CUDA_TRY(cudaStreamSynchronize(s));
     if (h.nonfinite) { set_error("non-finite value (NaN or Inf) among the input points"); return RQA_ERR_NONFINITE_INPUT; }
+    if (h.bad_eps) { set_error("rqa_line_hist: a threshold is NaN, Inf or negative"); return RQA_ERR_INVALID_ARG; }
     if (h.internal) { set_error("internal inconsistency recorded on the device"); return RQA_ERR_CUDA; }
     return RQA_OK;
 }

@@ -66,7 +66,8 @@ rqa_status validate_points(const rqa_points* pts, const char* who);
 struct WsStatus {
     int32_t nonfinite;   // set to 1 by the finite check when a NaN/Inf is seen
     int32_t internal;    // set to 1 on an internal inconsistency (should never happen)
-    int32_t pad[62];
+    int32_t bad_eps;     // set to 1 by rqa_line_hist when a threshold is NaN, Inf or negative
+    int32_t pad[61];
 };
 static_assert(sizeof(WsStatus) == 256, "status block is 256 bytes");
 

@@ -1,17 +1,567 @@
-// rqa_line.cu — rqa_line_hist: diagonal-line-length histograms P_k(l) at K thresholds
-// (Eq. 4 and the sentence under it; PAPER.md:125 upper triangle, R computed on the fly).
+// rqa_line.cu — rqa_line_hist: diagonal-line-length histograms P_k(l) at K thresholds in ONE pass over the
+// upper triangle (Eq. 4 and the sentence under it; upper triangle only, R_ij
+// computed on the fly, never stored).  Design notes: DESIGN.md "Kernel: diagonal scan".
 //
-// v0 (this file): one thread per diagonal, K run counters, global atomics.  Correct and simple; the fused
-// tiled kernel replaces it.
+// Work decomposition
+//   tile   = 256 adjacent diagonals (one per thread) x one chunk of <= 1023 positions; a thread walks its
+//            chunk of its diagonal sequentially, lanes of a warp read y[i] (broadcast) and y[i+o+lane]
+//            (consecutive) from two windows of the series staged in shared memory.
+//   cell   : distance d (sliding window over e_i = |y_i - y_{i+o}| for the max norm), then its LEVEL
+//            v = #{distinct thresholds < d} by one table lookup + one exact compare (thresholds are nested:
+//            the cell is recurrent at threshold j iff v <= j).
+//   runs   : the run length of every threshold is carried in packed fp16x2 registers (exact up to 2048):
+//            b = (v <= j) by HSET2.BF / HADD2.SAT on two thresholds at once, run = run*b + b by HFMA2.
+//   lines  : P_j(1), P_j(2), P_j(3) are NOT emitted line by line.  The kernel histograms the level of every
+//            cell and the window maxima of 2 and 3 consecutive levels (thread-private shared-memory columns, no
+//            conflicts); their prefix sums over the level are C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and
+//            Q3_j = sum_{l>=3} (l-2)*P_j(l), from which the finalize kernel solves P_j(1..3) exactly.
+//            Lines of length >= 4 that lie inside a chunk go to a shared-memory histogram (l < 256) or to
+//            global atomics (longer).  Runs touching a chunk border are written as (prefix, suffix) summaries
+//            and joined along each diagonal by the stitch kernel.
+#include <cuda_fp16.h>
+
 #include "rqa_common.cuh"
 
 namespace rqa {
 
 namespace {
 
+constexpr int LW = 256;          // diagonals per tile = threads per block
+constexpr int LMAX = 1023;       // longest chunk: run lengths stay exact in fp16 and 1024+run has ulp 1
+constexpr int NB = 4096;         // level look-up table buckets (one byte each)
+constexpr int LS = 256;          // lines shorter than this are counted in shared memory
+constexpr int GK = 32;           // thresholds per group (one scan launch per group of 32 sorted thresholds)
+constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
+constexpr unsigned FULL = 0xffffffffu;
+
+// Everything the scan needs to know about one group of <= 32 thresholds of one series.
+struct LineGroup {
+    int32_t J;            // number of distinct thresholds in the group, 1..32
+    int32_t multi;        // 1 if some table bucket holds two or more distinct thresholds (refine by a loop)
+    int32_t kcount;       // caller thresholds in this group
+    int32_t pad;
+    float scale;          // bucket(d) = bits(fmaf(min(d, dcap), scale, +0)) — a denormal-range FMA, exact rounding
+    float dcap;
+    float epsd[GK + 1];   // distinct thresholds ascending, epsd[J] = +inf
+    int32_t k_of[GK];     // sorted position -> caller's index k
+    int32_t j_of[GK];     // sorted position -> distinct index j
+    int32_t rep_k[GK];    // distinct index j -> the caller index whose histogram row accumulates the counts
+    uint8_t lut[NB];      // bucket -> 4 * #{distinct thresholds in lower buckets}
+};
+
+__device__ __forceinline__ uint32_t bucket_of(float d, float dcap, float scale) {
+    return __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
+}
+
+// One block per series: sort the K thresholds, split them into groups of 32, build each group's table.
+__global__ void __launch_bounds__(128) line_groups_kernel(const float* __restrict__ eps, int K, int NG,
+                                                          LineGroup* __restrict__ groups, WsStatus* status) {
+    const int b = blockIdx.x;
+    const float* e = eps + (int64_t)b * K;
+    __shared__ float s_sorted[RQA_MAX_K];
+    __shared__ int s_korder[RQA_MAX_K];
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) s_bad = 0;
+    __syncthreads();
+    for (int k = threadIdx.x; k < K; k += blockDim.x) {
+        float x = e[k];
+        if (!(x >= 0.0f) || isinf(x)) { s_bad = 1; x = 0.0f; }
+        int pos = 0;
+        for (int q = 0; q < K; ++q) {
+            float z = e[q];
+            if (!(z >= 0.0f) || isinf(z)) z = 0.0f;
+            pos += (z < x) || (z == x && q < k);
+        }
+        s_sorted[pos] = x;
+        s_korder[pos] = k;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && s_bad) atomicExch(&status->bad_eps, 1);
+    for (int g = 0; g < NG; ++g) {
+        LineGroup& G = groups[(int64_t)b * NG + g];
+        const int base = g * GK;
+        const int kc = min(GK, K - base);
+        __shared__ int s_J;
+        __shared__ float s_scale, s_dcap;
+        if (threadIdx.x == 0) {
+            int J = 0;
+            for (int q = 0; q < kc; ++q) {
+                float x = s_sorted[base + q];
+                if (q == 0 || x != s_sorted[base + q - 1]) { G.epsd[J] = x; G.rep_k[J] = s_korder[base + q]; ++J; }
+                G.k_of[q] = s_korder[base + q];
+                G.j_of[q] = J - 1;
+            }
+            for (int q = J; q <= GK; ++q) G.epsd[q] = __int_as_float(0x7f800000);
+            G.J = J;
+            G.kcount = kc;
+            G.pad = 0;
+            // bucket function: linear in d up to just above the largest threshold, NB-1 buckets wide
+            float emax = s_sorted[base + kc - 1];
+            float dcap = emax >= 3.0e38f ? 3.4028234e38f : nextafterf(emax, __int_as_float(0x7f800000));
+            double sc = ((double)NB - 1.5) * 1.401298464324817e-45 / (double)dcap;   // (NB-1.5) * 2^-149 / dcap
+            float scale = sc > 3.0e38 ? 3.0e38f : (float)sc;
+            while (scale > 0.0f && bucket_of(dcap, dcap, scale) > (uint32_t)(NB - 1)) scale = nextafterf(scale, 0.0f);
+            G.scale = scale;
+            G.dcap = dcap;
+            s_J = J; s_scale = scale; s_dcap = dcap;
+        }
+        __syncthreads();
+        const int J = s_J;
+        const float scale = s_scale, dcap = s_dcap;
+        int multi = 0;
+        for (int q = threadIdx.x; q < NB; q += blockDim.x) {
+            int below = 0, inside = 0;
+            for (int j = 0; j < J; ++j) {
+                uint32_t bj = bucket_of(G.epsd[j], dcap, scale);
+                below += bj < (uint32_t)q;
+                inside += bj == (uint32_t)q;
+            }
+            G.lut[q] = (uint8_t)(4 * below);
+            multi |= inside > 1;
+        }
+        multi = __syncthreads_or(multi);
+        if (threadIdx.x == 0) G.multi = multi;
+        __syncthreads();
+    }
+}
+
+// tile_start[ob] = number of tiles of the diagonal blocks before ob; diagonal block ob = diagonals
+// 1 + 256*ob .. 256 + 256*ob, its longest diagonal has n - 1 - 256*ob cells, cut into chunks of L.
+__global__ void __launch_bounds__(1024) tile_table_kernel(int64_t n, int L, int n_ob, uint32_t* __restrict__ tile_start) {
+    __shared__ uint32_t s_part[1024];
+    const int per = (n_ob + 1023) / 1024;
+    const int lo = threadIdx.x * per, hi = min(n_ob, lo + per);
+    uint32_t sum = 0;
+    for (int ob = lo; ob < hi; ++ob) sum += (uint32_t)((n - 1 - (int64_t)LW * ob + L - 1) / L);
+    s_part[threadIdx.x] = sum;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+        uint32_t t = threadIdx.x >= off ? s_part[threadIdx.x - off] : 0;
+        __syncthreads();
+        s_part[threadIdx.x] += t;
+        __syncthreads();
+    }
+    uint32_t run = s_part[threadIdx.x] - sum;
+    for (int ob = lo; ob < hi; ++ob) {
+        tile_start[ob] = run;
+        run += (uint32_t)((n - 1 - (int64_t)LW * ob + L - 1) / L);
+    }
+    if (threadIdx.x == 1023) tile_start[n_ob] = s_part[1023];
+}
+
+// ------------------------------------------------------------------------------------------ the scan
+// M > 0: compile-time (M, TAU), the distance is a sliding window over a register ring of S = (M-1)*TAU + 1
+// elements e_i = |y_i - y_{i+o}| (max norm) or (y_i - y_{i+o})^2 (Euclid).  M == 0: run-time (m, tau), the
+// distance is recomputed from the shared-memory windows for every cell.
+template <int M, int TAU>
+struct Span { static constexpr int S = M > 0 ? (M - 1) * TAU + 1 : 1; };
+
+// Shared-memory plan of the scan kernel (bytes); NP = threshold pairs carried per thread (J <= 2*NP).
+// The two series windows come last because their length depends on the run-time span (m-1)*tau.
+template <int NP>
+struct ScanSmem {
+    static constexpr int NLEV = 2 * NP + 1;                   // levels 0..2NP
+    static constexpr int off_lut = 0;
+    static constexpr int off_eps = off_lut + NB;
+    static constexpr int off_agg = off_eps + 4 * (GK + 4);
+    static constexpr int agg_row = 4 * (LW / 2);              // one level: 128 words, two 16-bit counters each
+    static constexpr int agg_one = NLEV * agg_row;            // one of the three histograms
+    static constexpr int off_sh = off_agg + 3 * agg_one;
+    static constexpr int off_ya = off_sh + 4 * 2 * NP * LS;
+};
+// i-side window: y[s-2 .. s-2+LA), j-side window: y[s-2+o0 .. s-2+o0+LB)
+__host__ __device__ inline int window_la(int L, int span) { return (L + 8 + 2 * span + 3) & ~3; }
+__host__ __device__ inline int window_lb(int L, int span) { return (L + 8 + 2 * span + LW + 3) & ~3; }
+
+struct ScanArgs {
+    View v;
+    int g, NG, K, L, n_ob;
+    const LineGroup* groups;
+    const uint32_t* tile_start;
+    unsigned long long* hist;   // [batch][K][n]
+    unsigned long long* agg;    // [batch][NG][3][GK+1]
+    uint16_t* pre;              // [batch][tiles][2*NP][LW]
+    uint32_t* suf;              // [batch][tiles][NP][LW]   raw fp16x2 run registers
+    uint32_t tiles;
+    int m, tau;                 // run-time embedding (used by the M == 0 variant)
+};
+
+template <int NORM, int M, int TAU, int NP>
+struct Scanner {
+    static constexpr int S = Span<M, TAU>::S;
+    using SM = ScanSmem<NP>;
+
+    // per-thread state
+    float ring[S];
+    uint32_t run[NP];           // fp16x2: run lengths of thresholds 2p (low half) and 2p+1 (high half)
+    uint32_t v1, v2;            // 4*level of the previous two cells
+    uint32_t w2a, w2b, w2c;     // max(level pairs) of the previous three cells (newest first)
+    uint32_t pm;                // 4 * running maximum level since the chunk start
+    // per-thread constants
+    const float* ya;
+    const float* yb;            // already offset by the thread's diagonal
+    const uint8_t* lut;
+    const char* eps;
+    char* agg;                  // thread's column of histogram 1, level 0
+    uint32_t* sh;
+    unsigned long long* grow;   // hist + b*K*n (rows indexed through rep)
+    const int* rep;
+    uint16_t* pre_out;
+    float scale, dcap;
+    uint32_t inc, J4;
+    int multi;
+    int m, tau;
+    int64_t n;
+
+    __device__ __forceinline__ float new_elem(int t) const {
+        float a = ya[t + 2 + S - 1], b = yb[t + 2 + S - 1];
+        float diff = __fsub_rn(a, b);
+        return NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
+    }
+    template <int R>
+    __device__ __forceinline__ float distance(int t) const {
+        if (M == 0) {                                         // run-time (m, tau): straight from the windows
+            float diff = __fsub_rn(ya[t + 2], yb[t + 2]);
+            float d = NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
+            for (int c = 1; c < m; ++c) {
+                diff = __fsub_rn(ya[t + 2 + c * tau], yb[t + 2 + c * tau]);
+                d = NORM == RQA_NORM_MAX ? fmaxf(d, fabsf(diff)) : __fadd_rn(d, __fmul_rn(diff, diff));
+            }
+            return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
+        }
+        float d = ring[R % S];
+#pragma unroll
+        for (int c = 1; c < M; ++c) {
+            float x = ring[(R + c * TAU) % S];
+            d = NORM == RQA_NORM_MAX ? fmaxf(d, x) : __fadd_rn(d, x);
+        }
+        return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
+    }
+    __device__ __forceinline__ uint32_t level4(float d) const {
+        uint32_t idx = __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
+        uint32_t q = lut[idx];
+        float er = *(const float*)(eps + q);
+        uint32_t v4 = q + (d > er ? 4u : 0u);
+        if (multi) {
+            while (d > *(const float*)(eps + v4)) v4 += 4;
+        }
+        return v4;
+    }
+
+    // Lines of length >= 4 that ended at the previous cell, for the levels [lo4, hi4) / 4 of this lane.
+    __device__ __forceinline__ void emit(unsigned mask, bool trig, uint32_t lo4, uint32_t hi4) {
+        uint32_t lm = 0;
+        if (trig && hi4 > lo4) lm = (0xffffffffu >> (32 - ((hi4 - lo4) >> 2))) << (lo4 >> 2);
+        uint32_t wm = __reduce_or_sync(mask, lm);
+        while (wm) {
+            const int j = __ffs(wm) - 1;
+            wm &= wm - 1;
+            uint32_t r = 0;
+            switch (j >> 1) {
+#define RQA_CASE(P) case P: if (P < NP) r = run[P < NP ? P : 0]; break;
+                RQA_CASE(0) RQA_CASE(1) RQA_CASE(2) RQA_CASE(3) RQA_CASE(4) RQA_CASE(5) RQA_CASE(6) RQA_CASE(7)
+                RQA_CASE(8) RQA_CASE(9) RQA_CASE(10) RQA_CASE(11) RQA_CASE(12) RQA_CASE(13) RQA_CASE(14) RQA_CASE(15)
+#undef RQA_CASE
+            }
+            if ((lm >> j) & 1u) {
+                __half2 h = *(__half2*)&r;
+                uint32_t l = (uint32_t)__half2int_rn((j & 1) ? __high2half(h) : __low2half(h));
+                if (l < (uint32_t)LS) atomicAdd(&sh[j * LS + l], 1u);
+                else atomicAdd(&grow[(int64_t)rep[j] * n + l], 1ull);
+            }
+        }
+    }
+
+    // One cell.  R = ring phase (static), t = position inside the chunk (t < 0: warm-up cells before the chunk),
+    // cnt = this lane's number of cells, GUARD = false in the part of the chunk where every lane is inside.
+    template <int R, bool GUARD>
+    __device__ __forceinline__ void cell(int t, int cnt, bool at_diag_start) {
+        if (M > 0) ring[(R + S - 1) % S] = new_elem(t);
+        bool live = true, warm = false;
+        if (GUARD) { live = t < cnt; warm = t < 0; }
+        unsigned mask = FULL;
+        if (GUARD) mask = __ballot_sync(FULL, live && !warm);
+        if (GUARD && warm) {
+            uint32_t v4 = at_diag_start ? J4 : level4(distance<R>(t));
+            v2 = v1; v1 = v4;
+            return;
+        }
+        if (GUARD && !live) return;
+        const float d = distance<R>(t);
+        const uint32_t v4 = level4(d);
+        // aggregates: level, max of 2, max of 3 consecutive levels (thread-private columns)
+        const uint32_t w2 = max(v4, v1), w3 = max(w2, v2);
+        atomicAdd((uint32_t*)(agg + v4 * (SM::agg_row / 4)), inc);
+        atomicAdd((uint32_t*)(agg + SM::agg_one + w2 * (SM::agg_row / 4)), inc);
+        atomicAdd((uint32_t*)(agg + 2 * SM::agg_one + w3 * (SM::agg_row / 4)), inc);
+        // lines of length >= 4 that end here: thresholds j with max(level of the 4 previous cells) <= j < level
+        const uint32_t w4p = max(w2a, w2c);
+        const bool trig = v4 > w4p;
+        if (__any_sync(mask, trig)) emit(mask, trig, w4p, min(v4, pm));
+        // prefix runs (recurrent since the chunk start) that end here have length t
+        if (v4 > pm) {
+            for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
+            pm = v4;
+        }
+        // run update for all thresholds, two per instruction
+        const uint32_t vvb = v4 * 0x00010001u + 0x64006400u;             // fp16x2 (1024 + 4v, 1024 + 4v)
+        const __half2 vv = *(const __half2*)&vvb;
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            __half2 bb;
+            if (p % 5 < 3) {                                              // HSET2.BF on the ALU pipe
+                const __half2 kk = __halves2half2(__ushort_as_half((unsigned short)(0x6400 + 8 * p)),
+                                                  __ushort_as_half((unsigned short)(0x6400 + 8 * p + 4)));
+                bb = __hle2(vv, kk);
+            } else {                                                      // HADD2.SAT on the FMA pipe
+                const __half2 kk = __halves2half2(__ushort_as_half((unsigned short)(0x6400 + 8 * p + 4)),
+                                                  __ushort_as_half((unsigned short)(0x6400 + 8 * p + 8)));
+                bb = __hadd2_sat(kk, __hneg2(vv));
+            }
+            __half2 r = *(__half2*)&run[p];
+            r = __hfma2(r, bb, bb);
+            run[p] = *(uint32_t*)&r;
+        }
+        v2 = v1; v1 = v4;
+        w2c = w2b; w2b = w2a; w2a = w2;
+    }
+
+    template <bool GUARD, int... R>
+    __device__ __forceinline__ void superstep(int t, int cnt, bool ds, std::integer_sequence<int, R...>) {
+        (cell<R, GUARD>(t + R, cnt, ds), ...);
+    }
+};
+
+template <int NORM, int M, int TAU, int NP>
+__global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanArgs a) {
+    using SC = Scanner<NORM, M, TAU, NP>;
+    using SM = typename SC::SM;
+    constexpr int S = SC::S;
+    extern __shared__ __align__(16) char smem[];
+    __shared__ int s_ob;
+    __shared__ int s_rep[GK];
+
+    const int tid = threadIdx.x;
+    const int b = blockIdx.y;
+    const uint32_t tile = blockIdx.x;
+    const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
+    // which diagonal block / chunk is this tile
+    for (int q = tid; q < a.n_ob; q += LW)
+        if (a.tile_start[q] <= tile && tile < a.tile_start[q + 1]) s_ob = q;
+    // stage the group's table and thresholds, clear the histograms
+    uint8_t* lut_s = (uint8_t*)(smem + SM::off_lut);
+    float* eps_s = (float*)(smem + SM::off_eps);
+    const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
+    const int LA = window_la(a.L, span), LB = window_lb(a.L, span);
+    float* ya_s = (float*)(smem + SM::off_ya);
+    float* yb_s = ya_s + LA;
+    uint32_t* agg_s = (uint32_t*)(smem + SM::off_agg);
+    uint32_t* sh_s = (uint32_t*)(smem + SM::off_sh);
+    for (int q = tid; q < NB / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)G.lut)[q];
+    if (tid <= GK) eps_s[tid] = G.epsd[tid];
+    if (tid < GK) s_rep[tid] = G.rep_k[tid];
+    for (int q = tid; q < 3 * SM::agg_one / 4; q += LW) agg_s[q] = 0;
+    for (int q = tid; q < 2 * NP * LS; q += LW) sh_s[q] = 0;
+    __syncthreads();
+    const int ob = s_ob;
+    const int c = (int)(tile - a.tile_start[ob]);
+    const int L = a.L;
+    const int64_t n = a.v.n;
+    const int64_t o0 = 1 + (int64_t)LW * ob;
+    const int64_t s = (int64_t)c * L;                       // chunk start along the diagonals
+    // the two windows of the series: y[s-2 + x] and y[s-2 + o0 + x]; the series has n + (M-1)*TAU samples
+    const float* y = a.v.data + (int64_t)b * a.v.bs;
+    const int64_t ny = n + span;
+    for (int x = tid; x < LA; x += LW) {
+        int64_t gi = s - 2 + x;
+        ya_s[x] = (gi >= 0 && gi < ny) ? y[gi] : 0.0f;
+    }
+    for (int x = tid; x < LB; x += LW) {
+        int64_t gi = s - 2 + o0 + x;
+        yb_s[x] = (gi >= 0 && gi < ny) ? y[gi] : 0.0f;
+    }
+    __syncthreads();
+
+    const int J = G.J;
+    const int64_t o = o0 + tid;
+    const int64_t len = n - o;                              // cells on this thread's diagonal (may be <= 0)
+    int cnt = (int)max((int64_t)0, min((int64_t)L, len - s));
+    const int cnt_hi = __shfl_sync(FULL, cnt, 0);           // the warp's longest lane (smallest o)
+    const int cnt_lo = __shfl_sync(FULL, cnt, 31);
+
+    SC sc;
+    sc.ya = ya_s;
+    sc.yb = yb_s + tid;
+    sc.lut = lut_s;
+    sc.eps = (const char*)eps_s;
+    sc.agg = (char*)agg_s + 4 * (tid & (LW / 2 - 1));
+    sc.sh = sh_s;
+    sc.grow = a.hist + (int64_t)b * a.K * n;
+    sc.rep = s_rep;
+    sc.pre_out = a.pre + (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
+    sc.scale = G.scale;
+    sc.dcap = G.dcap;
+    sc.inc = tid < LW / 2 ? 1u : 0x10000u;
+    sc.J4 = 4u * (uint32_t)J;
+    sc.multi = G.multi;
+    sc.m = a.m;
+    sc.tau = a.tau;
+    sc.n = n;
+    sc.v1 = sc.v2 = sc.J4;
+    sc.w2a = sc.w2b = sc.w2c = sc.J4;
+    sc.pm = 0;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) sc.run[p] = 0;
+
+    if (cnt_hi > 0) {
+        // ring holds e_{t}..e_{t+S-2} before cell t is processed; first cell is the warm-up cell t = -2
+#pragma unroll
+        for (int x = 0; x < (M > 0 ? S - 1 : 0); ++x) {
+            float diff = __fsub_rn(sc.ya[x], sc.yb[x]);
+            sc.ring[x] = NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
+        }
+        const bool ds = (s == 0);
+        constexpr int U = S >= 3 ? S : (S == 2 ? 4 : 4);     // cells per super-step, a multiple of S
+        using Seq = std::make_integer_sequence<int, U>;
+        int t = -2;
+        sc.template superstep<true>(t, cnt, ds, Seq{});      // warm-up cells and the first U-2 cells, guarded
+        t += U;
+        for (; t + U <= cnt_lo; t += U) sc.template superstep<false>(t, cnt, ds, Seq{});
+        for (; t < cnt_hi; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
+        if (cnt > 0) {
+            // runs alive at the end of the chunk, and prefix runs that never ended (the whole chunk)
+            uint32_t* suf_out = a.suf + (((int64_t)b * a.tiles + tile) * NP) * LW + tid;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) suf_out[p * LW] = sc.run[p];
+            for (uint32_t j4 = sc.pm; j4 < sc.J4; j4 += 4) sc.pre_out[(j4 >> 2) * LW] = (uint16_t)cnt;
+        }
+    }
+    __syncthreads();
+    // flush: aggregates (sum the 256 private columns of every level) and the short-line histogram
+    {
+        const int warp = tid >> 5, lane = tid & 31;
+        unsigned long long* ag = a.agg + ((int64_t)b * a.NG + a.g) * 3 * (GK + 1);
+        for (int row = warp; row < 3 * SM::NLEV; row += LW / 32) {
+            const int h = row / SM::NLEV, lev = row - h * SM::NLEV;
+            const uint32_t* r = agg_s + row * (LW / 2);
+            uint32_t sum = 0;
+            for (int q = lane; q < LW / 2; q += 32) { uint32_t w = r[q]; sum += (w & 0xffffu) + (w >> 16); }
+            for (int off = 16; off; off >>= 1) sum += __shfl_down_sync(FULL, sum, off);
+            if (lane == 0 && sum && lev <= J) atomicAdd(&ag[h * (GK + 1) + lev], (unsigned long long)sum);
+        }
+        for (int q = tid; q < J * LS; q += LW) {
+            uint32_t cnum = sh_s[q];
+            if (cnum) {
+                int j = q / LS, l = q - j * LS;
+                atomicAdd(&sc.grow[(int64_t)s_rep[j] * n + l], (unsigned long long)cnum);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------- stitching
+// One thread per (diagonal, distinct threshold): join the (prefix, suffix) summaries of consecutive chunks and
+// emit the lines of length >= 4 that touch a chunk border (including the two ends of the diagonal).
+struct StitchArgs {
+    int64_t n;
+    int g, NG, K, L, n_ob, NP;
+    const LineGroup* groups;
+    const uint32_t* tile_start;
+    unsigned long long* hist;
+    const uint16_t* pre;
+    const uint32_t* suf;
+    uint32_t tiles;
+};
+
+__global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
+    const int ob = blockIdx.x, j = blockIdx.y, b = blockIdx.z;
+    const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
+    if (j >= G.J) return;
+    const int tid = threadIdx.x;
+    const int64_t o = 1 + (int64_t)LW * ob + tid;
+    const int64_t len = a.n - o;
+    if (len <= 0) return;
+    unsigned long long* row = a.hist + ((int64_t)b * a.K + G.rep_k[j]) * a.n;
+    const uint32_t t0 = a.tile_start[ob];
+    const int nc = (int)((len + a.L - 1) / a.L);
+    uint32_t carry = 0;
+    for (int c = 0; c < nc; ++c) {
+        const uint32_t cntc = (uint32_t)min((int64_t)a.L, len - (int64_t)c * a.L);
+        const int64_t tile = (int64_t)b * a.tiles + t0 + c;
+        const uint32_t p = a.pre[(tile * (2 * a.NP) + j) * LW + tid];
+        if (p == cntc) {
+            carry += cntc;
+        } else {
+            const uint32_t tot = carry + p;
+            if (tot >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[tot], 1ull);
+            const uint32_t w = a.suf[(tile * a.NP + (j >> 1)) * LW + tid];
+            const __half2 h = *(const __half2*)&w;
+            carry = (uint32_t)__half2int_rn((j & 1) ? __high2half(h) : __low2half(h));
+        }
+    }
+    if (carry >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[carry], 1ull);
+}
+
+// ------------------------------------------------------------------------------------------ finalize
+// One block per (distinct threshold, series): P(1), P(2), P(3) from the aggregates and the explicit lines
+//   C  = sum_l l P(l),  Q2 = sum_{l>=2} (l-1) P(l),  Q3 = sum_{l>=3} (l-2) P(l)      (all exact integers)
+// then the rows of caller thresholds that share this value are copied from the representative row.
+__global__ void __launch_bounds__(256) line_finalize_kernel(int64_t n, int g, int NG, int K,
+                                                            const LineGroup* __restrict__ groups,
+                                                            const unsigned long long* __restrict__ agg,
+                                                            unsigned long long* __restrict__ hist, WsStatus* status) {
+    const int j = blockIdx.x, b = blockIdx.y;
+    const LineGroup& G = groups[(int64_t)b * NG + g];
+    if (j >= G.J) return;
+    unsigned long long* row = hist + ((int64_t)b * K + G.rep_k[j]) * n;
+    unsigned long long e0 = 0, c4 = 0;
+    for (int64_t l = LMIN_EXPLICIT + threadIdx.x; l < n; l += blockDim.x) {
+        unsigned long long h = row[l];
+        e0 += (unsigned long long)l * h;
+        c4 += h;
+    }
+    __shared__ unsigned long long s_e0[8], s_c4[8];
+    for (int off = 16; off; off >>= 1) {
+        e0 += __shfl_down_sync(FULL, e0, off);
+        c4 += __shfl_down_sync(FULL, c4, off);
+    }
+    if ((threadIdx.x & 31) == 0) { s_e0[threadIdx.x >> 5] = e0; s_c4[threadIdx.x >> 5] = c4; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        e0 = 0; c4 = 0;
+        for (int q = 0; q < 8; ++q) { e0 += s_e0[q]; c4 += s_c4[q]; }
+        const unsigned long long* ag = agg + ((int64_t)b * NG + g) * 3 * (GK + 1);
+        unsigned long long C = 0, Q2 = 0, Q3 = 0;
+        for (int u = 0; u <= j; ++u) { C += ag[u]; Q2 += ag[(GK + 1) + u]; Q3 += ag[2 * (GK + 1) + u]; }
+        const long long P3 = (long long)Q3 - (long long)(e0 - 2 * c4);
+        const long long P2 = (long long)Q2 - (long long)(e0 - c4) - 2 * P3;
+        const long long P1 = (long long)C - (long long)e0 - 3 * P3 - 2 * P2;
+        if (P1 < 0 || P2 < 0 || P3 < 0) atomicExch(&status->internal, 1);
+        if (n > 1) row[1] = (unsigned long long)P1;
+        if (n > 2) row[2] = (unsigned long long)P2;
+        if (n > 3) row[3] = (unsigned long long)P3;
+    }
+}
+
+__global__ void __launch_bounds__(256) line_copy_rows_kernel(int64_t n, int g, int NG, int K,
+                                                             const LineGroup* __restrict__ groups,
+                                                             unsigned long long* __restrict__ hist) {
+    const int q = blockIdx.y, b = blockIdx.z;
+    const LineGroup& G = groups[(int64_t)b * NG + g];
+    if (q >= G.kcount) return;
+    const int k = G.k_of[q], rep = G.rep_k[G.j_of[q]];
+    if (k == rep) return;
+    const unsigned long long* src = hist + ((int64_t)b * K + rep) * n;
+    unsigned long long* dst = hist + ((int64_t)b * K + k) * n;
+    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (int64_t)gridDim.x * blockDim.x) dst[l] = src[l];
+}
+
+// ------------------------------------------------------------ general strided views (materialised X)
+// One thread per diagonal, K run counters, global atomics.  Only used when the points are not a delay view of a
+// series (point_stride != 1) or the embedding window does not fit the scan kernel's shared-memory windows.
 template <int NORM>
-__global__ void __launch_bounds__(128) line_naive_kernel(View v, const float* __restrict__ eps, int K,
-                                                         unsigned long long* __restrict__ hist) {
+__global__ void __launch_bounds__(128) line_strided_kernel(View v, const float* __restrict__ eps, int K,
+                                                           unsigned long long* __restrict__ hist) {
     const int b = blockIdx.y;
     const int64_t o = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= v.n) return;
@@ -35,18 +585,122 @@ __global__ void __launch_bounds__(128) line_naive_kernel(View v, const float* __
         if (run[k]) atomicAdd(&h[(int64_t)k * v.n + run[k]], 1ull);
 }
 
+// ------------------------------------------------------------------------------------------ host side
+struct LinePlan {
+    bool scan;          // false: strided fallback
+    int L, n_ob, NG, NP, span;
+    uint32_t tiles;
+    size_t smem;
+};
+
+constexpr int MAX_SPAN = 4096;
+
+int pairs_for(int kg) { return kg <= 10 ? 5 : (kg <= 20 ? 10 : 16); }
+
+template <int NP>
+size_t scan_smem_bytes(int L, int span) {
+    return (size_t)ScanSmem<NP>::off_ya + 4 * ((size_t)window_la(L, span) + window_lb(L, span));
+}
+
+LinePlan make_plan(const View& v, int K) {
+    LinePlan p{};
+    p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
+    p.scan = v.ps == 1 && p.span <= MAX_SPAN;
+    p.NG = (K + GK - 1) / GK;
+    p.NP = pairs_for(std::min(K, GK));
+    // chunk length: aim at >= 8 waves of 3 blocks per SM over the whole batch, at most 1023 positions
+    const double cells = (double)n_pairs(v.n) * (double)v.batch;
+    int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
+    p.L = (int)std::max<int64_t>(32, std::min<int64_t>(LMAX, L));
+    p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
+    uint64_t tiles = 0;
+    for (int ob = 0; ob < p.n_ob; ++ob) tiles += (uint64_t)((v.n - 1 - (int64_t)LW * ob + p.L - 1) / p.L);
+    p.tiles = (uint32_t)tiles;
+    p.smem = p.NP == 5 ? scan_smem_bytes<5>(p.L, p.span) : (p.NP == 10 ? scan_smem_bytes<10>(p.L, p.span) : scan_smem_bytes<16>(p.L, p.span));
+    return p;
+}
+
+template <int NORM, int M, int TAU, int NP>
+rqa_status launch_scan(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
+    auto kern = line_scan_kernel<NORM, M, TAU, NP>;
+    RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
+    kern<<<dim3(p.tiles, (unsigned)batch), LW, p.smem, s>>>(a);
+    RQA_LAUNCH_CHECK();
+    return RQA_OK;
+}
+
+template <int NORM, int NP>
+rqa_status dispatch_embedding(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
+    if (a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, batch, s);
+    return launch_scan<NORM, 0, 0, NP>(a, p, batch, s);
+}
+
+template <int NORM>
+rqa_status dispatch_pairs(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
+    if (p.NP == 5) return dispatch_embedding<NORM, 5>(a, p, batch, s);
+    if (p.NP == 10) return dispatch_embedding<NORM, 10>(a, p, batch, s);
+    return dispatch_embedding<NORM, 16>(a, p, batch, s);
+}
+
 }  // namespace
 
-size_t line_workspace_bytes(const View&, int) { return 256; }
+size_t line_workspace_bytes(const View& v, int K) {
+    LinePlan p = make_plan(v, K);
+    if (!p.scan) return 256;
+    size_t bytes = 0;
+    bytes += align_up(sizeof(LineGroup) * (size_t)v.batch * p.NG);
+    bytes += align_up(sizeof(uint32_t) * ((size_t)p.n_ob + 1));
+    bytes += align_up(sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1));
+    bytes += align_up(sizeof(uint16_t) * (size_t)v.batch * p.tiles * 2 * p.NP * LW);
+    bytes += align_up(sizeof(uint32_t) * (size_t)v.batch * p.tiles * p.NP * LW);
+    return bytes;
+}
 
-rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena&, cudaStream_t s) {
+rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s) {
+    WsStatus* status = (WsStatus*)ws.base;
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * (size_t)v.batch * K * v.n, s));
-    dim3 grid((unsigned)((v.n - 1 + 127) / 128), (unsigned)v.batch);
-    if (norm == RQA_NORM_MAX)
-        line_naive_kernel<RQA_NORM_MAX><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
-    else
-        line_naive_kernel<RQA_NORM_EUCLID><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
+    LinePlan p = make_plan(v, K);
+    if (!p.scan) {
+        dim3 grid((unsigned)((v.n - 1 + 127) / 128), (unsigned)v.batch);
+        if (norm == RQA_NORM_MAX)
+            line_strided_kernel<RQA_NORM_MAX><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
+        else
+            line_strided_kernel<RQA_NORM_EUCLID><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
+        RQA_LAUNCH_CHECK();
+        return RQA_OK;
+    }
+    LineGroup* groups = ws.take<LineGroup>((size_t)v.batch * p.NG);
+    uint32_t* tile_start = ws.take<uint32_t>((size_t)p.n_ob + 1);
+    unsigned long long* agg = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * p.NG * 3 * (GK + 1));
+    uint16_t* pre = ws.take<uint16_t>((size_t)v.batch * p.tiles * 2 * p.NP * LW);
+    uint32_t* suf = ws.take<uint32_t>((size_t)v.batch * p.tiles * p.NP * LW);
+    if (!ws.ok()) { set_error("rqa_line_hist: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
+    RQA_CUDA_TRY(cudaMemsetAsync(agg, 0, sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1), s));
+    line_groups_kernel<<<v.batch, 128, 0, s>>>(d_eps, K, p.NG, groups, status);
     RQA_LAUNCH_CHECK();
+    tile_table_kernel<<<1, 1024, 0, s>>>(v.n, p.L, p.n_ob, tile_start);
+    RQA_LAUNCH_CHECK();
+    for (int g = 0; g < p.NG; ++g) {
+        ScanArgs a;
+        a.v = v; a.g = g; a.NG = p.NG; a.K = K; a.L = p.L; a.n_ob = p.n_ob;
+        a.groups = groups; a.tile_start = tile_start; a.hist = (unsigned long long*)d_hist; a.agg = agg;
+        a.pre = pre; a.suf = suf; a.tiles = p.tiles; a.m = v.m; a.tau = (int)v.cs;
+        rqa_status st = norm == RQA_NORM_MAX ? dispatch_pairs<RQA_NORM_MAX>(a, p, v.batch, s)
+                                             : dispatch_pairs<RQA_NORM_EUCLID>(a, p, v.batch, s);
+        if (st != RQA_OK) return st;
+        StitchArgs sa;
+        sa.n = v.n; sa.g = g; sa.NG = p.NG; sa.K = K; sa.L = p.L; sa.n_ob = p.n_ob; sa.NP = p.NP;
+        sa.groups = groups; sa.tile_start = tile_start; sa.hist = (unsigned long long*)d_hist; sa.pre = pre; sa.suf = suf;
+        sa.tiles = p.tiles;
+        line_stitch_kernel<<<dim3((unsigned)p.n_ob, (unsigned)(2 * p.NP), (unsigned)v.batch), LW, 0, s>>>(sa);
+        RQA_LAUNCH_CHECK();
+        line_finalize_kernel<<<dim3((unsigned)(2 * p.NP), (unsigned)v.batch), 256, 0, s>>>(v.n, g, p.NG, K, groups, agg,
+                                                                                         (unsigned long long*)d_hist, status);
+        RQA_LAUNCH_CHECK();
+        unsigned cb = (unsigned)std::min<int64_t>((v.n + 255) / 256, 64);
+        line_copy_rows_kernel<<<dim3(cb, GK, (unsigned)v.batch), 256, 0, s>>>(v.n, g, p.NG, K, groups, (unsigned long long*)d_hist);
+        RQA_LAUNCH_CHECK();
+    }
     return RQA_OK;
 }
 

@@ -154,6 +154,19 @@ rqa_status rqa_sweep_host(const float* h_series, int64_t N, int32_t batch, int32
  */
 uint64_t rqa_launch_count(void);
 
+/*
+ * Expert / testing knobs, process-wide, not thread-safe against concurrent calls; value 0 restores the automatic
+ * choice.  They change how a result is computed, never the result (every path of rqa_eps_for_rr is exact).
+ * Workspace sizes depend on them: set options before rqa_workspace_bytes.
+ *   "select_path"  rqa_eps_for_rr: 1 = materialise all distances (small P), 2 = sample-bracket + one counting pass,
+ *                  3 = four radix passes
+ *   "sample_size"  bracket path: number of sampled pair distances per series
+ *   "cand_cap"     bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
+ *   "line_chunk"   rqa_line_hist: chunk length along the diagonals, 1..1023
+ * Unknown names and negative values return RQA_ERR_INVALID_ARG.
+ */
+rqa_status rqa_set_option(const char* name, int64_t value);
+
 #ifdef __cplusplus
 }
 #endif

@@ -27,7 +27,7 @@ RQA_MAX_M = 16
 # every symbol include/rqa.h declares (tests check that the library exports them all)
 EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_bytes", "rqa_workspace_status",
            "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
-           "rqa_sweep_host", "rqa_launch_count"]
+           "rqa_sweep_host", "rqa_launch_count", "rqa_set_option"]
 
 
 class RqaPoints(ctypes.Structure):
@@ -69,6 +69,7 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_det_avg.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp]
     lib.rqa_sweep_workspace_bytes.argtypes = [i64, i32, i32, i64, i32, ctypes.POINTER(sz)]
     lib.rqa_sweep_host.argtypes = [vp, i64, i32, i32, i64, ctypes.c_int, vp, i32, i64, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.rqa_set_option.argtypes = [ctypes.c_char_p, i64]
     _lib = lib
     return lib
 
@@ -100,6 +101,11 @@ def rqa_version() -> str:
 
 def rqa_launch_count() -> int:
     return int(load_library().rqa_launch_count())
+
+
+def rqa_set_option(name: str, value: int) -> None:
+    """Expert / testing knob (include/rqa.h); 0 restores the automatic choice."""
+    _check(load_library().rqa_set_option(name.encode(), int(value)))
 
 
 def rqa_workspace_bytes(pts: RqaPoints, K: int) -> int:

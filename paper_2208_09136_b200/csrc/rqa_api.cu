@@ -12,6 +12,8 @@ namespace rqa {
 
 static thread_local char t_err[512] = "";
 std::atomic<uint64_t> g_launches{0};
+static Options g_options{0, 0, 0, 0};
+const Options& options() { return g_options; }
 
 void set_error(const char* fmt, ...) {
     va_list ap;
@@ -127,6 +129,26 @@ const char* rqa_status_string(rqa_status s) {
 const char* rqa_last_error(void) { return t_err; }
 const char* rqa_version(void) { return "0.1 sm_100a"; }
 uint64_t rqa_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+rqa_status rqa_set_option(const char* name, int64_t value) {
+    if (!name) { set_error("rqa_set_option: name is NULL"); return RQA_ERR_INVALID_ARG; }
+    if (value < 0) { set_error("rqa_set_option: value must be >= 0"); return RQA_ERR_INVALID_ARG; }
+    if (!strcmp(name, "select_path")) {
+        if (value > 3) { set_error("rqa_set_option: select_path is 0..3"); return RQA_ERR_INVALID_ARG; }
+        g_options.select_path = value;
+    } else if (!strcmp(name, "sample_size")) {
+        g_options.sample_size = value;
+    } else if (!strcmp(name, "cand_cap")) {
+        g_options.cand_cap = value;
+    } else if (!strcmp(name, "line_chunk")) {
+        if (value > 1023) { set_error("rqa_set_option: line_chunk is at most 1023"); return RQA_ERR_INVALID_ARG; }
+        g_options.line_chunk = value;
+    } else {
+        set_error("rqa_set_option: unknown option '%s'", name);
+        return RQA_ERR_INVALID_ARG;
+    }
+    return RQA_OK;
+}
 
 rqa_status rqa_workspace_bytes(const rqa_points* pts, int32_t K, size_t* bytes) {
     if (!bytes) { set_error("rqa_workspace_bytes: bytes is NULL"); return RQA_ERR_INVALID_ARG; }

@@ -35,6 +35,16 @@ extern std::atomic<uint64_t> g_launches;
         }                                                                                          \
     } while (0)
 
+// --------------------------------------------------------------------------------------------- options
+// Process-wide expert/testing knobs (rqa_set_option); 0 = automatic.
+struct Options {
+    int64_t select_path;   // 0 auto, 1 direct (materialise all distances), 2 bracket (sample + one counting pass), 3 radix
+    int64_t sample_size;   // bracket path: sample size S
+    int64_t cand_cap;      // bracket path: candidate capacity per series
+    int64_t line_chunk;    // diagonal scan: chunk length L (<= 1023)
+};
+const Options& options();
+
 // ------------------------------------------------------------------------------------------------ view
 // Device-side copy of rqa_points (x_i[c] of series b = data[b*bs + i*ps + c*cs]).
 struct View {

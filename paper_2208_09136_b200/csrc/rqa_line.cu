@@ -20,19 +20,15 @@
 //            and joined along each diagonal by the stitch kernel.
 #include <cuda_fp16.h>
 
-#include "rqa_common.cuh"
+#include "rqa_tiles.cuh"
 
 namespace rqa {
 
 namespace {
 
-constexpr int LW = 256;          // diagonals per tile = threads per block
 constexpr int LMAX = 1023;       // longest chunk: run lengths stay exact in fp16 and 1024+run has ulp 1
-constexpr int NB = 4096;         // level look-up table buckets (one byte each)
 constexpr int LS = 256;          // lines shorter than this are counted in shared memory
-constexpr int GK = 32;           // thresholds per group (one scan launch per group of 32 sorted thresholds)
 constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
-constexpr unsigned FULL = 0xffffffffu;
 
 // Everything the scan needs to know about one group of <= 32 thresholds of one series.
 struct LineGroup {
@@ -48,10 +44,6 @@ struct LineGroup {
     int32_t rep_k[GK];    // distinct index j -> the caller index whose histogram row accumulates the counts
     uint8_t lut[NB];      // bucket -> 4 * #{distinct thresholds in lower buckets}
 };
-
-__device__ __forceinline__ uint32_t bucket_of(float d, float dcap, float scale) {
-    return __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
-}
 
 // One block per series: sort the K thresholds, split them into groups of 32, build each group's table.
 __global__ void __launch_bounds__(128) line_groups_kernel(const float* __restrict__ eps, int K, int NG,
@@ -98,9 +90,7 @@ __global__ void __launch_bounds__(128) line_groups_kernel(const float* __restric
             // bucket function: linear in d up to just above the largest threshold, NB-1 buckets wide
             float emax = s_sorted[base + kc - 1];
             float dcap = emax >= 3.0e38f ? 3.4028234e38f : nextafterf(emax, __int_as_float(0x7f800000));
-            double sc = ((double)NB - 1.5) * 1.401298464324817e-45 / (double)dcap;   // (NB-1.5) * 2^-149 / dcap
-            float scale = sc > 3.0e38 ? 3.0e38f : (float)sc;
-            while (scale > 0.0f && bucket_of(dcap, dcap, scale) > (uint32_t)(NB - 1)) scale = nextafterf(scale, 0.0f);
+            float scale = bucket_scale(dcap);
             G.scale = scale;
             G.dcap = dcap;
             s_J = J; s_scale = scale; s_dcap = dcap;
@@ -150,12 +140,7 @@ __global__ void __launch_bounds__(1024) tile_table_kernel(int64_t n, int L, int 
 }
 
 // ------------------------------------------------------------------------------------------ the scan
-// M > 0: compile-time (M, TAU), the distance is a sliding window over a register ring of S = (M-1)*TAU + 1
-// elements e_i = |y_i - y_{i+o}| (max norm) or (y_i - y_{i+o})^2 (Euclid).  M == 0: run-time (m, tau), the
-// distance is recomputed from the shared-memory windows for every cell.
-template <int M, int TAU>
-struct Span { static constexpr int S = M > 0 ? (M - 1) * TAU + 1 : 1; };
-
+// Cell distances: CellDist (rqa_tiles.cuh) with two warm-up cells before the chunk.
 // Shared-memory plan of the scan kernel (bytes); NP = threshold pairs carried per thread (J <= 2*NP).
 // The two series windows come last because their length depends on the run-time span (m-1)*tau.
 template <int NP>
@@ -169,10 +154,6 @@ struct ScanSmem {
     static constexpr int off_sh = off_agg + 3 * agg_one;
     static constexpr int off_ya = off_sh + 4 * 2 * NP * LS;
 };
-// i-side window: y[s-2 .. s-2+LA), j-side window: y[s-2+o0 .. s-2+o0+LB)
-__host__ __device__ inline int window_la(int L, int span) { return (L + 8 + 2 * span + 3) & ~3; }
-__host__ __device__ inline int window_lb(int L, int span) { return (L + 8 + 2 * span + LW + 3) & ~3; }
-
 struct ScanArgs {
     View v;
     int g, NG, K, L, n_ob;
@@ -187,19 +168,17 @@ struct ScanArgs {
 };
 
 template <int NORM, int M, int TAU, int NP>
-struct Scanner {
-    static constexpr int S = Span<M, TAU>::S;
+struct Scanner : CellDist<NORM, M, TAU, 2> {
+    using CD = CellDist<NORM, M, TAU, 2>;
+    static constexpr int S = CD::S;
     using SM = ScanSmem<NP>;
 
     // per-thread state
-    float ring[S];
     uint32_t run[NP];           // fp16x2: run lengths of thresholds 2p (low half) and 2p+1 (high half)
     uint32_t v1, v2;            // 4*level of the previous two cells
     uint32_t w2a, w2b, w2c;     // max(level pairs) of the previous three cells (newest first)
     uint32_t pm;                // 4 * running maximum level since the chunk start
     // per-thread constants
-    const float* ya;
-    const float* yb;            // already offset by the thread's diagonal
     const uint8_t* lut;
     const char* eps;
     char* agg;                  // thread's column of histogram 1, level 0
@@ -210,33 +189,8 @@ struct Scanner {
     float scale, dcap;
     uint32_t inc, J4;
     int multi;
-    int m, tau;
     int64_t n;
 
-    __device__ __forceinline__ float new_elem(int t) const {
-        float a = ya[t + 2 + S - 1], b = yb[t + 2 + S - 1];
-        float diff = __fsub_rn(a, b);
-        return NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
-    }
-    template <int R>
-    __device__ __forceinline__ float distance(int t) const {
-        if (M == 0) {                                         // run-time (m, tau): straight from the windows
-            float diff = __fsub_rn(ya[t + 2], yb[t + 2]);
-            float d = NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
-            for (int c = 1; c < m; ++c) {
-                diff = __fsub_rn(ya[t + 2 + c * tau], yb[t + 2 + c * tau]);
-                d = NORM == RQA_NORM_MAX ? fmaxf(d, fabsf(diff)) : __fadd_rn(d, __fmul_rn(diff, diff));
-            }
-            return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
-        }
-        float d = ring[R % S];
-#pragma unroll
-        for (int c = 1; c < M; ++c) {
-            float x = ring[(R + c * TAU) % S];
-            d = NORM == RQA_NORM_MAX ? fmaxf(d, x) : __fadd_rn(d, x);
-        }
-        return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
-    }
     __device__ __forceinline__ uint32_t level4(float d) const {
         uint32_t idx = __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
         uint32_t q = lut[idx];
@@ -276,18 +230,18 @@ struct Scanner {
     // cnt = this lane's number of cells, GUARD = false in the part of the chunk where every lane is inside.
     template <int R, bool GUARD>
     __device__ __forceinline__ void cell(int t, int cnt, bool at_diag_start) {
-        if (M > 0) ring[(R + S - 1) % S] = new_elem(t);
+        CD::template push<R>(t);
         bool live = true, warm = false;
         if (GUARD) { live = t < cnt; warm = t < 0; }
         unsigned mask = FULL;
         if (GUARD) mask = __ballot_sync(FULL, live && !warm);
         if (GUARD && warm) {
-            uint32_t v4 = at_diag_start ? J4 : level4(distance<R>(t));
+            uint32_t v4 = at_diag_start ? J4 : level4(CD::template distance<R>(t));
             v2 = v1; v1 = v4;
             return;
         }
         if (GUARD && !live) return;
-        const float d = distance<R>(t);
+        const float d = CD::template distance<R>(t);
         const uint32_t v4 = level4(d);
         // aggregates: level, max of 2, max of 3 consecutive levels (thread-private columns)
         const uint32_t w2 = max(v4, v1), w3 = max(w2, v2);
@@ -346,13 +300,12 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     const uint32_t tile = blockIdx.x;
     const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
     // which diagonal block / chunk is this tile
-    for (int q = tid; q < a.n_ob; q += LW)
-        if (a.tile_start[q] <= tile && tile < a.tile_start[q + 1]) s_ob = q;
+    find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
     // stage the group's table and thresholds, clear the histograms
     uint8_t* lut_s = (uint8_t*)(smem + SM::off_lut);
     float* eps_s = (float*)(smem + SM::off_eps);
     const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
-    const int LA = window_la(a.L, span), LB = window_lb(a.L, span);
+    const int LA = window_la(a.L, span, 2), LB = window_lb(a.L, span, 2);
     float* ya_s = (float*)(smem + SM::off_ya);
     float* yb_s = ya_s + LA;
     uint32_t* agg_s = (uint32_t*)(smem + SM::off_agg);
@@ -372,14 +325,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     // the two windows of the series: y[s-2 + x] and y[s-2 + o0 + x]; the series has n + (M-1)*TAU samples
     const float* y = a.v.data + (int64_t)b * a.v.bs;
     const int64_t ny = n + span;
-    for (int x = tid; x < LA; x += LW) {
-        int64_t gi = s - 2 + x;
-        ya_s[x] = (gi >= 0 && gi < ny) ? y[gi] : 0.0f;
-    }
-    for (int x = tid; x < LB; x += LW) {
-        int64_t gi = s - 2 + o0 + x;
-        yb_s[x] = (gi >= 0 && gi < ny) ? y[gi] : 0.0f;
-    }
+    stage_windows(y, ny, s - 2, s - 2 + o0, ya_s, LA, yb_s, LB);
     __syncthreads();
 
     const int J = G.J;
@@ -414,12 +360,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     for (int p = 0; p < NP; ++p) sc.run[p] = 0;
 
     if (cnt_hi > 0) {
-        // ring holds e_{t}..e_{t+S-2} before cell t is processed; first cell is the warm-up cell t = -2
-#pragma unroll
-        for (int x = 0; x < (M > 0 ? S - 1 : 0); ++x) {
-            float diff = __fsub_rn(sc.ya[x], sc.yb[x]);
-            sc.ring[x] = NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
-        }
+        sc.prime(-2);                                         // first cell is the warm-up cell t = -2
         const bool ds = (s == 0);
         constexpr int U = S >= 3 ? S : (S == 2 ? 4 : 4);     // cells per super-step, a multiple of S
         using Seq = std::make_integer_sequence<int, U>;
@@ -593,13 +534,11 @@ struct LinePlan {
     size_t smem;
 };
 
-constexpr int MAX_SPAN = 4096;
-
 int pairs_for(int kg) { return kg <= 10 ? 5 : (kg <= 20 ? 10 : 16); }
 
 template <int NP>
 size_t scan_smem_bytes(int L, int span) {
-    return (size_t)ScanSmem<NP>::off_ya + 4 * ((size_t)window_la(L, span) + window_lb(L, span));
+    return (size_t)ScanSmem<NP>::off_ya + 4 * ((size_t)window_la(L, span, 2) + window_lb(L, span, 2));
 }
 
 LinePlan make_plan(const View& v, int K) {
@@ -612,6 +551,7 @@ LinePlan make_plan(const View& v, int K) {
     const double cells = (double)n_pairs(v.n) * (double)v.batch;
     int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
     p.L = (int)std::max<int64_t>(32, std::min<int64_t>(LMAX, L));
+    if (options().line_chunk > 0) p.L = (int)std::min<int64_t>(LMAX, options().line_chunk);
     p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
     uint64_t tiles = 0;
     for (int ob = 0; ob < p.n_ob; ++ob) tiles += (uint64_t)((v.n - 1 - (int64_t)LW * ob + p.L - 1) / p.L);
@@ -643,6 +583,12 @@ rqa_status dispatch_pairs(const ScanArgs& a, const LinePlan& p, int batch, cudaS
 }
 
 }  // namespace
+
+rqa_status launch_tile_table(int64_t n, int L, int n_ob, uint32_t* tile_start, cudaStream_t s) {
+    tile_table_kernel<<<1, 1024, 0, s>>>(n, L, n_ob, tile_start);
+    RQA_LAUNCH_CHECK();
+    return RQA_OK;
+}
 
 size_t line_workspace_bytes(const View& v, int K) {
     LinePlan p = make_plan(v, K);
@@ -678,8 +624,10 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     RQA_CUDA_TRY(cudaMemsetAsync(agg, 0, sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1), s));
     line_groups_kernel<<<v.batch, 128, 0, s>>>(d_eps, K, p.NG, groups, status);
     RQA_LAUNCH_CHECK();
-    tile_table_kernel<<<1, 1024, 0, s>>>(v.n, p.L, p.n_ob, tile_start);
-    RQA_LAUNCH_CHECK();
+    {
+        rqa_status st = launch_tile_table(v.n, p.L, p.n_ob, tile_start, s);
+        if (st != RQA_OK) return st;
+    }
     for (int g = 0; g < p.NG; ++g) {
         ScanArgs a;
         a.v = v; a.g = g; a.NG = p.NG; a.K = K; a.L = p.L; a.n_ob = p.n_ob;

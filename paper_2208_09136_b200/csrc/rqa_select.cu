@@ -1,35 +1,532 @@
 // rqa_select.cu — rqa_eps_for_rr: exact multi-target order statistics of the P = N'(N'-1)/2 pairwise
 // distances ("preselect RR and use the corresponding eps"; readings S4-S6).
 //
-// The N'^2 distance matrix is never stored: every pass recomputes d_ij tile by tile.
-// Non-negative fp32 values order like their uint32 bit patterns, so the select works on patterns.
+// The N'^2 distance matrix is never stored: distances are recomputed tile by tile.  Non-negative
+// fp32 values order like their uint32 bit patterns, so every select below works on patterns.
 //
-// v0 (this file, generic fallback): classic most-significant-digit radix select, 4 passes of 8 bits, all K
-// targets resolved in each pass; targets that share a prefix share one 256-bin histogram ("group").
-#include "rqa_common.cuh"
+// Three paths, all exact:
+//   DIRECT   (P <= 2^22)  all P distances are written to a scratch buffer once and a 4-pass multi-target radix
+//            select runs over the buffer.
+//   BRACKET  (delay views, the headline path)  ONE full pass over the triangle:
+//              1. a pseudo-random sample of S ~ 5.5 P^(2/3) pair distances is drawn and 2 sample order statistics
+//                 per target (rank S*q -/+ 4.5 sigma) are found by the buffer select: a bracket (lo_k, hi_k] that
+//                 holds the true eps_k with overwhelming probability;
+//              2. the counting pass visits every cell once (tiles, sliding-window distance, level table as in the
+//                 diagonal scan), counts the cells of every inter-boundary level exactly (thread-private
+//                 shared-memory columns, no conflicts) and appends the few cells inside brackets to a candidate list;
+//              3. the exact counts locate each target's rank inside its bracket — this is a proof, not a guess: if
+//                 a rank falls outside its bracket (or the candidate list overflows, e.g. massive ties) the series is
+//                 flagged and handled by RADIX — and the buffer select over the candidates gives eps_k and C_k.
+//   RADIX    (general strided views; fallback)  most-significant-digit radix select, 4 full passes of 8 bits, all K
+//            targets resolved in each pass; targets that share a prefix share one 256-bin histogram.
+#include <algorithm>
+#include <cmath>
+
+#include "rqa_tiles.cuh"
 
 namespace rqa {
 
 namespace {
 
-struct SelBatch {
-    int32_t G;                        // number of live groups (distinct prefixes)
+constexpr int BT = 64;                // targets per buffer-select call
+constexpr int NLEV_MAX = 2 * GK + 1;  // levels of the counting pass: 2 boundaries per bracket
+constexpr int WCAP = 256;             // candidates a warp buffers in shared memory before flushing
+constexpr double BRACKET_SIGMAS = 4.5;
+
+// ------------------------------------------------------------------------------------------ per-series state
+struct SelState {
+    int32_t fallback;                 // 1: the series is (re)done by the radix passes
     int32_t pad;
-    uint32_t gprefix[RQA_MAX_K];      // distinct prefixes, ascending (determined high bits, low bits zero)
-    int32_t group_of[RQA_MAX_K];      // target -> group
-    uint32_t prefix[RQA_MAX_K];       // target -> prefix
-    uint64_t resid[RQA_MAX_K];        // 1-based residual rank inside the prefix range
-    uint64_t below[RQA_MAX_K];        // number of distances strictly below the prefix range
+    unsigned long long ncand;         // candidates appended by the counting pass (may exceed the capacity)
+    unsigned long long level_count[NLEV_MAX + 1];
+};
+
+// state of one buffer select (<= BT targets) of one series
+struct BufSel {
+    int32_t G;                        // live groups (distinct prefixes)
+    int32_t T;
+    uint32_t gprefix[BT];             // distinct prefixes, ascending (determined high bits, low bits zero)
+    int32_t group_of[BT];
+    uint32_t prefix[BT];
+    unsigned long long resid[BT];     // 1-based residual rank inside the prefix range
+    unsigned long long below[BT];     // elements strictly below the prefix range
+    unsigned long long base[BT];      // added to (below + ties) for the final count
+    float out_val[BT];
+    unsigned long long out_cnt[BT];   // #{x <= out_val} within the buffer
+};
+
+struct Ranks64 {
+    unsigned long long r[BT];
+};
+
+// bracket boundaries of one group of <= GK targets of one series (the counting pass's level table)
+struct SelTable {
+    int32_t J;                        // boundaries in use (even), levels 0..J
+    int32_t pad;
+    float scale, dcap;
+    float beta[2 * GK + 4];           // ascending, beta[J..] = +inf
+    uint16_t lut[NB];                 // bucket -> #{boundaries in lower buckets}
+};
+
+struct SampleRanks {                  // per target of the group: sample ranks of the bracket ends (0 = open end)
+    unsigned long long lo[GK], hi[GK];
+    unsigned long long rank[GK];      // the target's rank among all P distances
+    int32_t kc;
+};
+
+// ------------------------------------------------------------------------------------------ small kernels
+__global__ void sel_init_kernel(SelState* ss, int force_fallback) {
+    SelState& s = ss[blockIdx.x];
+    if (threadIdx.x == 0) { s.fallback = force_fallback; s.pad = 0; s.ncand = 0; }
+    for (int q = threadIdx.x; q <= NLEV_MAX; q += blockDim.x) s.level_count[q] = 0;
+}
+
+__global__ void sel_group_reset_kernel(SelState* ss) {
+    SelState& s = ss[blockIdx.x];
+    if (threadIdx.x == 0) s.ncand = 0;
+    for (int q = threadIdx.x; q <= NLEV_MAX; q += blockDim.x) s.level_count[q] = 0;
+}
+
+__device__ __forceinline__ uint64_t mix64(uint64_t z) {
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+// S pseudo-random pairs i < j (uniform over the P pairs, with replacement) -> their distances.
+template <int NORM>
+__global__ void __launch_bounds__(256) sel_sample_kernel(View v, unsigned long long S, float* __restrict__ out) {
+    const int b = blockIdx.y;
+    const float* yb = v.data + (int64_t)b * v.bs;
+    float* o = out + (int64_t)b * S;
+    const uint32_t n = (uint32_t)v.n;
+    for (unsigned long long s = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; s < S;
+         s += (unsigned long long)gridDim.x * blockDim.x) {
+        uint64_t h = mix64((s + 1) * 0x9E3779B97F4A7C15ull + (uint64_t)b * 0xD1B54A32D192ED03ull);
+        uint32_t i = __umulhi((uint32_t)(h >> 32), n);
+        uint32_t j = __umulhi((uint32_t)h, n - 1);
+        if (j >= i) ++j;
+        uint32_t lo = min(i, j), hi = max(i, j);
+        o[s] = point_distance<NORM>(yb, lo, hi, v.m, v.ps, v.cs);
+    }
+}
+
+// All P distances, diagonal by diagonal (any strided view).
+template <int NORM>
+__global__ void __launch_bounds__(256) sel_direct_kernel(View v, unsigned long long P, float* __restrict__ out) {
+    const int b = blockIdx.y;
+    const float* yb = v.data + (int64_t)b * v.bs;
+    float* o = out + (int64_t)b * P;
+    const int64_t n = v.n;
+    for (int64_t row = blockIdx.x; row < n - 1; row += gridDim.x) {
+        // row i: pairs (i, i+1..n-1) stored at offset i*n - i(i+1)/2
+        const int64_t off = row * n - row * (row + 1) / 2 - row - 1;
+        for (int64_t j = row + 1 + threadIdx.x; j < n; j += blockDim.x)
+            o[off + j] = point_distance<NORM>(yb, row, j, v.m, v.ps, v.cs);
+    }
+}
+
+// ---------------------------------------------------------------------------------------- buffer select
+__device__ void bufsel_reset(BufSel& s, int T) {
+    s.G = 1;
+    s.T = T;
+    s.gprefix[0] = 0;
+}
+
+__global__ void bufsel_init_kernel(BufSel* st, Ranks64 ranks, int T) {
+    BufSel& s = st[blockIdx.x];
+    const int t = threadIdx.x;
+    if (t == 0) bufsel_reset(s, T);
+    if (t < T) {
+        s.group_of[t] = 0;
+        s.prefix[t] = 0;
+        s.resid[t] = ranks.r[t];
+        s.below[t] = 0;
+        s.base[t] = 0;
+    }
+}
+
+// One 8-bit pass over the buffer of series b: n = n_ptr ? min(*n_ptr of the series, cap) : cap.
+__global__ void __launch_bounds__(256) bufsel_pass_kernel(const float* __restrict__ buf, unsigned long long stride,
+                                                         unsigned long long cap, const SelState* __restrict__ ss,
+                                                         int use_ncand, int pass, const BufSel* __restrict__ st,
+                                                         unsigned long long* __restrict__ bins) {
+    extern __shared__ uint32_t sbins[];      // [G][256]
+    __shared__ uint32_t s_gprefix[BT];
+    const int b = blockIdx.y;
+    if (use_ncand && ss[b].fallback) return;
+    const BufSel& s = st[b];
+    const int G = s.G;
+    unsigned long long n = cap;
+    if (use_ncand) n = min(cap, ss[b].ncand);
+    for (int q = threadIdx.x; q < G * 256; q += blockDim.x) sbins[q] = 0;
+    for (int q = threadIdx.x; q < G; q += blockDim.x) s_gprefix[q] = s.gprefix[q];
+    __syncthreads();
+    const uint32_t* x = (const uint32_t*)buf + (unsigned long long)b * stride;
+    const int shift = 24 - 8 * pass;
+    const uint32_t himask = pass == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * pass));
+    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < n;
+         e += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t key = x[e];
+        const uint32_t hi = key & himask;
+        int lo = 0, hiq = G;                 // first group with gprefix >= hi
+        while (lo < hiq) {
+            int mid = (lo + hiq) >> 1;
+            if (s_gprefix[mid] < hi) lo = mid + 1; else hiq = mid;
+        }
+        if (lo < G && s_gprefix[lo] == hi) atomicAdd(&sbins[lo * 256 + ((key >> shift) & 255u)], 1u);
+    }
+    __syncthreads();
+    unsigned long long* gb = bins + (int64_t)b * BT * 256;
+    for (int q = threadIdx.x; q < G * 256; q += blockDim.x) {
+        uint32_t c = sbins[q];
+        if (c) atomicAdd(&gb[q], (unsigned long long)c);
+    }
+}
+
+// One block per series: every target picks its digit; then the groups are rebuilt and the bins cleared.
+__global__ void __launch_bounds__(256) bufsel_resolve_kernel(BufSel* st, unsigned long long* bins, int pass,
+                                                            const SelState* __restrict__ ss, int use_ncand) {
+    const int b = blockIdx.x;
+    if (use_ncand && ss[b].fallback) return;
+    BufSel& s = st[b];
+    const int T = s.T;
+    unsigned long long* gb = bins + (int64_t)b * BT * 256;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const int shift = 24 - 8 * pass;
+    __shared__ uint32_t s_prefix[BT];
+    __shared__ int s_first[BT];
+    for (int t = warp; t < T; t += nwarps) {
+        const unsigned long long* h = gb + s.group_of[t] * 256;
+        unsigned long long c[8], sum = 0;
+        for (int q = 0; q < 8; ++q) { c[q] = h[lane * 8 + q]; sum += c[q]; }
+        unsigned long long incl = sum;
+        for (int off = 1; off < 32; off <<= 1) {
+            unsigned long long u = __shfl_up_sync(FULL, incl, off);
+            if (lane >= off) incl += u;
+        }
+        const unsigned long long resid = s.resid[t];
+        unsigned ball = __ballot_sync(FULL, incl >= resid);
+        int src = ball ? (__ffs(ball) - 1) : 31;      // ball == 0 only if the rank exceeds the buffer (flagged elsewhere)
+        int digit = 255;
+        unsigned long long e = incl - sum, ties = 0;
+        if (lane == src) {
+            for (int q = 0; q < 8; ++q) {
+                if (e + c[q] >= resid) { digit = lane * 8 + q; ties = c[q]; break; }
+                e += c[q];
+            }
+        }
+        digit = __shfl_sync(FULL, digit, src);
+        e = __shfl_sync(FULL, e, src);
+        ties = __shfl_sync(FULL, ties, src);
+        if (lane == 0) {
+            uint32_t p = s.prefix[t] | ((uint32_t)digit << shift);
+            s.prefix[t] = p;
+            s_prefix[t] = p;
+            unsigned long long below = s.below[t] + e;
+            s.below[t] = below;
+            s.resid[t] = resid - e;
+            if (pass == 3) {
+                s.out_val[t] = __uint_as_float(p);
+                s.out_cnt[t] = below + ties;
+            }
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < T; t += blockDim.x) {
+        int first = 1;
+        for (int j = 0; j < t; ++j) first &= (s_prefix[j] != s_prefix[t]);
+        s_first[t] = first;
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < T; t += blockDim.x) {
+        int less = 0;
+        for (int j = 0; j < T; ++j) less += (s_first[j] && s_prefix[j] < s_prefix[t]);
+        s.group_of[t] = less;
+        if (s_first[t]) s.gprefix[less] = s_prefix[t];
+    }
+    if (threadIdx.x == 0) {
+        int G = 0;
+        for (int j = 0; j < T; ++j) G += s_first[j];
+        s.G = G;
+    }
+    for (int q = threadIdx.x; q < T * 256; q += blockDim.x) gb[q] = 0ull;
+}
+
+// ------------------------------------------------------------------------------- bracket table (per group)
+// From the 2*kc sample order statistics: brackets (lo_k, hi_k], merged where they overlap, as an ascending boundary
+// list beta[0..J) (J even; bracket g = level 2g+1 = (beta[2g], beta[2g+1]]) and its bucket table.
+__global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict__ st, SampleRanks sr,
+                                                       SelTable* __restrict__ tabs) {
+    const int b = blockIdx.x;
+    const BufSel& s = st[b];
+    SelTable& T = tabs[b];
+    __shared__ int s_J;
+    __shared__ float s_scale, s_dcap;
+    __shared__ float s_beta[2 * GK + 4];
+    const float INF = __int_as_float(0x7f800000);
+    if (threadIdx.x == 0) {
+        int J = 0;
+        for (int k = 0; k < sr.kc; ++k) {
+            float lo = sr.lo[k] ? s.out_val[2 * k] : -1.0f;          // open lower end: below every distance
+            float hi = sr.hi[k] ? s.out_val[2 * k + 1] : INF;        // open upper end
+            if (J > 0 && lo <= s_beta[J - 1]) {                      // overlaps the previous bracket: extend it
+                s_beta[J - 1] = fmaxf(s_beta[J - 1], hi);
+            } else {
+                s_beta[J++] = lo;
+                s_beta[J++] = hi;
+            }
+        }
+        for (int q = J; q < 2 * GK + 4; ++q) s_beta[q] = INF;
+        float fmaxb = 0.0f;                                          // largest finite boundary
+        for (int q = 0; q < J; ++q)
+            if (s_beta[q] < INF) fmaxb = fmaxf(fmaxb, s_beta[q]);
+        float dcap = fmaxb >= 3.0e38f ? 3.4028234e38f : nextafterf(fmaxb, INF);
+        if (!(dcap > 0.0f)) dcap = 1.0e-30f;
+        s_dcap = dcap;
+        s_scale = bucket_scale(dcap);
+        s_J = J;
+        T.J = J; T.pad = 0; T.scale = s_scale; T.dcap = dcap;
+    }
+    __syncthreads();
+    const int J = s_J;
+    for (int q = threadIdx.x; q < 2 * GK + 4; q += blockDim.x) T.beta[q] = s_beta[q];
+    for (int q = threadIdx.x; q < NB; q += blockDim.x) {
+        int below = 0;
+        for (int j = 0; j < J; ++j) {
+            const float x = s_beta[j];
+            // negative boundary: below every bucket; +inf: in the top bucket (never exceeded anyway)
+            below += x < 0.0f ? 1 : (bucket_of(x, s_dcap, s_scale) < (uint32_t)q);
+        }
+        T.lut[q] = (uint16_t)below;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ counting pass
+struct CountArgs {
+    View v;
+    int L, n_ob;
+    const uint32_t* tile_start;
+    const SelTable* tabs;
+    SelState* ss;
+    float* cand;                      // [batch][cap]
+    unsigned long long cap;
+    int m, tau;
+};
+
+struct CountSmem {
+    static constexpr int off_lut = 0;                                   // uint16[NB]
+    static constexpr int off_beta = off_lut + 2 * NB;                   // float[2*GK+4]
+    static constexpr int off_cand = off_beta + 4 * (2 * GK + 4);        // float[LW/32][WCAP]
+    static constexpr int off_cols = off_cand + 4 * (LW / 32) * WCAP;    // uint32[nlev][LW/2]
+    static constexpr int col_row = 4 * (LW / 2);
+};
+
+template <int NORM, int M, int TAU>
+struct Counter : CellDist<NORM, M, TAU, 0> {
+    using CD = CellDist<NORM, M, TAU, 0>;
+    const uint16_t* lut;
+    const float* beta;
+    char* cols;                       // this thread's column, level 0
+    float* wbuf;                      // this warp's candidate buffer
+    float* gcand;                     // the series' candidate list
+    unsigned long long* gncand;
+    unsigned long long cap;
+    float scale, dcap;
+    uint32_t inc, wcount, lane_lt;
+
+    __device__ __forceinline__ void flush_warp() {
+        // all lanes hold the same wcount; lane 0 reserves space in the series' candidate list
+        const int lane = threadIdx.x & 31;
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(gncand, (unsigned long long)wcount);
+        base = __shfl_sync(FULL, base, 0);
+        __syncwarp();
+        for (uint32_t q = lane; q < wcount; q += 32)
+            if (base + q < cap) gcand[base + q] = wbuf[q];
+        __syncwarp();
+        wcount = 0;
+    }
+
+    template <int R, bool GUARD>
+    __device__ __forceinline__ void cell(int t, int cnt) {
+        CD::template push<R>(t);
+        const bool live = !GUARD || t < cnt;
+        const float d = CD::template distance<R>(t);
+        uint32_t q = lut[bucket_of(d, dcap, scale)];
+        while (d > beta[q]) ++q;
+        if (live) atomicAdd((uint32_t*)(cols + q * CountSmem::col_row), inc);
+        const unsigned mc = __ballot_sync(FULL, live && (q & 1u));
+        if (mc) {
+            const uint32_t nc = __popc(mc);
+            if (wcount + nc > (uint32_t)WCAP) flush_warp();
+            if (live && (q & 1u)) wbuf[wcount + __popc(mc & lane_lt)] = d;
+            wcount += nc;
+        }
+    }
+    template <bool GUARD, int... R>
+    __device__ __forceinline__ void superstep(int t, int cnt, std::integer_sequence<int, R...>) {
+        (cell<R, GUARD>(t + R, cnt), ...);
+    }
+};
+
+template <int NORM, int M, int TAU>
+__global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev) {
+    using CT = Counter<NORM, M, TAU>;
+    constexpr int S = CT::S;
+    extern __shared__ __align__(16) char smem[];
+    __shared__ int s_ob;
+    const int tid = threadIdx.x, b = blockIdx.y;
+    if (a.ss[b].fallback) return;
+    const uint32_t tile = blockIdx.x;
+    const SelTable& T = a.tabs[b];
+    find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
+    uint16_t* lut_s = (uint16_t*)(smem + CountSmem::off_lut);
+    float* beta_s = (float*)(smem + CountSmem::off_beta);
+    float* cand_s = (float*)(smem + CountSmem::off_cand);
+    uint32_t* cols_s = (uint32_t*)(smem + CountSmem::off_cols);
+    const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
+    const int LA = window_la(a.L, span, 0), LB = window_lb(a.L, span, 0);
+    float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * CountSmem::col_row);
+    float* yb_s = ya_s + LA;
+    for (int q = tid; q < NB / 2; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)T.lut)[q];
+    if (tid < 2 * GK + 4) beta_s[tid] = T.beta[tid];
+    for (int q = tid; q < nlev * (LW / 2); q += LW) cols_s[q] = 0;
+    __syncthreads();
+    const int ob = s_ob;
+    const int c = (int)(tile - a.tile_start[ob]);
+    const int L = a.L;
+    const int64_t n = a.v.n;
+    const int64_t o0 = 1 + (int64_t)LW * ob;
+    const int64_t s = (int64_t)c * L;
+    const float* y = a.v.data + (int64_t)b * a.v.bs;
+    stage_windows(y, n + span, s, s + o0, ya_s, LA, yb_s, LB);
+    __syncthreads();
+
+    const int64_t len = n - (o0 + tid);
+    const int cnt = (int)max((int64_t)0, min((int64_t)L, len - s));
+    const int cnt_hi = __shfl_sync(FULL, cnt, 0);
+    const int cnt_lo = __shfl_sync(FULL, cnt, 31);
+
+    CT ct;
+    ct.ya = ya_s;
+    ct.yb = yb_s + tid;
+    ct.m = a.m;
+    ct.tau = a.tau;
+    ct.lut = lut_s;
+    ct.beta = beta_s;
+    ct.cols = (char*)cols_s + 4 * (tid & (LW / 2 - 1));
+    ct.wbuf = cand_s + (tid >> 5) * WCAP;
+    ct.gcand = a.cand + (unsigned long long)b * a.cap;
+    ct.gncand = &a.ss[b].ncand;
+    ct.cap = a.cap;
+    ct.scale = T.scale;
+    ct.dcap = T.dcap;
+    ct.inc = tid < LW / 2 ? 1u : 0x10000u;
+    ct.wcount = 0;
+    ct.lane_lt = (1u << (tid & 31)) - 1u;
+    if (cnt_hi > 0) {
+        ct.prime(0);
+        constexpr int U = S >= 3 ? S : 4;                     // cells per super-step, a multiple of S
+        using Seq = std::make_integer_sequence<int, U>;
+        int t = 0;
+        for (; t + U <= cnt_lo; t += U) ct.template superstep<false>(t, cnt, Seq{});
+        for (; t < cnt_hi; t += U) ct.template superstep<true>(t, cnt, Seq{});
+        if (ct.wcount) ct.flush_warp();
+    }
+    __syncthreads();
+    {
+        const int warp = tid >> 5, lane = tid & 31;
+        unsigned long long* lc = a.ss[b].level_count;
+        for (int row = warp; row < nlev; row += LW / 32) {
+            const uint32_t* r = cols_s + row * (LW / 2);
+            uint32_t sum = 0;
+            for (int q = lane; q < LW / 2; q += 32) { uint32_t w = r[q]; sum += (w & 0xffffu) + (w >> 16); }
+            for (int off = 16; off; off >>= 1) sum += __shfl_down_sync(FULL, sum, off);
+            if (lane == 0 && sum) atomicAdd(&lc[row], (unsigned long long)sum);
+        }
+    }
+}
+
+// One block per series: exact level counts -> each target's bracket and its rank among the candidates.
+__global__ void __launch_bounds__(64) sel_bracket_resolve_kernel(SelState* ss, const SelTable* __restrict__ tabs,
+                                                               SampleRanks sr, BufSel* st, unsigned long long cap) {
+    const int b = blockIdx.x;
+    SelState& s = ss[b];
+    if (s.fallback) return;
+    const SelTable& T = tabs[b];
+    BufSel& bs = st[b];
+    __shared__ unsigned long long s_cum[NLEV_MAX + 1], s_odd[NLEV_MAX + 1];
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) {
+        unsigned long long cum = 0, odd = 0;
+        for (int v = 0; v <= T.J; ++v) {
+            s_cum[v] = cum;                                   // cells in the levels below v
+            s_odd[v] = odd;                                   // candidates in the brackets below v
+            cum += s.level_count[v];
+            if (v & 1) odd += s.level_count[v];
+        }
+        s_cum[T.J + 1] = cum;
+        s_bad = (odd != s.ncand) || (s.ncand > cap);
+        bufsel_reset(bs, sr.kc);
+    }
+    __syncthreads();
+    const int t = threadIdx.x;
+    int bad = s_bad;
+    if (t < sr.kc) {
+        const unsigned long long r = sr.rank[t];
+        int v = 0;
+        while (v <= T.J && s_cum[v + 1] < r) ++v;             // first level whose cumulative count reaches r
+        if (v > T.J || !(v & 1)) {
+            bad = 1;                                          // the rank is not inside a bracket
+            v = 1;
+        }
+        bs.group_of[t] = 0;
+        bs.prefix[t] = 0;
+        bs.below[t] = 0;
+        bs.resid[t] = bad ? 1 : s_odd[v] + (r - s_cum[v]);
+        bs.base[t] = bad ? 0 : s_cum[v] - s_odd[v];
+    }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) s.fallback = 1;
+}
+
+struct TargetMap {
+    int32_t k_of[BT];                 // target of this call -> caller's index
+    int32_t T;
+};
+
+__global__ void sel_finish_kernel(const SelState* __restrict__ ss, const BufSel* __restrict__ st, TargetMap tm, int K,
+                                  unsigned long long P, int use_flag, float* __restrict__ eps,
+                                  unsigned long long* __restrict__ count, double* __restrict__ rr) {
+    const int b = blockIdx.x, t = threadIdx.x;
+    if (t >= tm.T || (use_flag && ss[b].fallback)) return;
+    const BufSel& s = st[b];
+    const int k = tm.k_of[t];
+    const unsigned long long c = s.base[t] + s.out_cnt[t];
+    eps[(int64_t)b * K + k] = s.out_val[t];
+    count[(int64_t)b * K + k] = c;
+    rr[(int64_t)b * K + k] = (double)c / (double)P;
+}
+
+// ------------------------------------------------------------------------------------------ radix passes
+struct SelBatch {
+    int32_t G;
+    int32_t pad;
+    uint32_t gprefix[RQA_MAX_K];
+    int32_t group_of[RQA_MAX_K];
+    uint32_t prefix[RQA_MAX_K];
+    uint64_t resid[RQA_MAX_K];
+    uint64_t below[RQA_MAX_K];
 };
 
 struct Ranks {
     uint64_t r[RQA_MAX_K];
 };
 
-constexpr int SEL_W = 128;            // diagonals per block (= threads)
+constexpr int SEL_W = 128;            // diagonals per tile (= threads)
 constexpr int SEL_L = 512;            // positions per tile
 
-__global__ void select_init_kernel(SelBatch* st, Ranks ranks, int K) {
+__global__ void radix_init_kernel(SelBatch* st, Ranks ranks, int K) {
     SelBatch& s = st[blockIdx.x];
     int k = threadIdx.x;
     if (k == 0) { s.G = 1; s.gprefix[0] = 0; }
@@ -41,29 +538,30 @@ __global__ void select_init_kernel(SelBatch* st, Ranks ranks, int K) {
     }
 }
 
-// One pass: digit histogram of the cells whose determined high bits match a live prefix.
-// grid = (o-blocks, chunks, batch); thread t walks diagonal o0+t over positions [i0, i0+L).
+// One pass: digit histogram of the cells whose determined high bits match a live prefix.  Persistent blocks walk
+// the tiles (128 diagonals x 512 positions) of the series that are flagged for the radix path.
 template <int NORM>
 __global__ void __launch_bounds__(SEL_W) radix_pass_kernel(View v, int pass, const SelBatch* __restrict__ st,
-                                                           unsigned long long* __restrict__ bins, int K) {
+                                                           unsigned long long* __restrict__ bins, int K,
+                                                           const SelState* __restrict__ ss) {
     extern __shared__ uint32_t sbins[];      // [G][256]
     __shared__ uint32_t s_gprefix[RQA_MAX_K];
-    const int b = blockIdx.z;
-    const int64_t o0 = 1 + (int64_t)blockIdx.x * SEL_W;
-    const int64_t i0 = (int64_t)blockIdx.y * SEL_L;
-    if (i0 >= v.n - o0) return;              // empty tile (beyond the hypotenuse)
+    const int b = blockIdx.y;
+    if (!ss[b].fallback) return;
     const SelBatch& s = st[b];
     const int G = s.G;
     for (int q = threadIdx.x; q < G * 256; q += blockDim.x) sbins[q] = 0;
     for (int q = threadIdx.x; q < G; q += blockDim.x) s_gprefix[q] = s.gprefix[q];
     __syncthreads();
-
     const float* yb = v.data + (int64_t)b * v.bs;
-    const int64_t o = o0 + threadIdx.x;
     const int shift = 24 - 8 * pass;
     const uint32_t himask = pass == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * pass));
-    if (o < v.n) {
-        int64_t iend = min(i0 + (int64_t)SEL_L, v.n - o);
+    const int64_t nx = (v.n - 1 + SEL_W - 1) / SEL_W, ny = (v.n - 1 + SEL_L - 1) / SEL_L;
+    for (int64_t tile = blockIdx.x; tile < nx * ny; tile += gridDim.x) {
+        const int64_t o = 1 + (tile % nx) * SEL_W + threadIdx.x;
+        const int64_t i0 = (tile / nx) * SEL_L;
+        if (o >= v.n) continue;
+        const int64_t iend = min(i0 + (int64_t)SEL_L, v.n - o);
         for (int64_t i = i0; i < iend; ++i) {
             float d = point_distance<NORM>(yb, i, i + o, v.m, v.ps, v.cs);
             uint32_t key = __float_as_uint(d);
@@ -84,12 +582,13 @@ __global__ void __launch_bounds__(SEL_W) radix_pass_kernel(View v, int pass, con
     }
 }
 
-// One block per series: every target picks its digit, then the groups are rebuilt and the bins cleared.
 __global__ void __launch_bounds__(256) radix_resolve_kernel(SelBatch* st, unsigned long long* bins, int K, int pass,
-                                                            unsigned long long P, float* __restrict__ eps,
+                                                            unsigned long long P, const SelState* __restrict__ ss,
+                                                            float* __restrict__ eps,
                                                             unsigned long long* __restrict__ count,
                                                             double* __restrict__ rr) {
     const int b = blockIdx.x;
+    if (!ss[b].fallback) return;
     SelBatch& s = st[b];
     unsigned long long* gb = bins + (int64_t)b * K * 256;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
@@ -103,11 +602,11 @@ __global__ void __launch_bounds__(256) radix_resolve_kernel(SelBatch* st, unsign
         for (int q = 0; q < 8; ++q) { c[q] = h[lane * 8 + q]; sum += c[q]; }
         unsigned long long incl = sum;
         for (int off = 1; off < 32; off <<= 1) {
-            unsigned long long t = __shfl_up_sync(0xffffffffu, incl, off);
+            unsigned long long t = __shfl_up_sync(FULL, incl, off);
             if (lane >= off) incl += t;
         }
         const unsigned long long resid = s.resid[k];
-        unsigned ball = __ballot_sync(0xffffffffu, incl >= resid);
+        unsigned ball = __ballot_sync(FULL, incl >= resid);
         int src = ball ? (__ffs(ball) - 1) : 31;      // ball == 0 cannot happen (resid <= group total)
         unsigned long long excl = incl - sum;
         int digit = 0;
@@ -118,9 +617,9 @@ __global__ void __launch_bounds__(256) radix_resolve_kernel(SelBatch* st, unsign
                 e += c[q];
             }
         }
-        digit = __shfl_sync(0xffffffffu, digit, src);
-        e = __shfl_sync(0xffffffffu, e, src);
-        ties = __shfl_sync(0xffffffffu, ties, src);
+        digit = __shfl_sync(FULL, digit, src);
+        e = __shfl_sync(FULL, e, src);
+        ties = __shfl_sync(FULL, ties, src);
         if (lane == 0) {
             uint32_t p = s.prefix[k] | ((uint32_t)digit << shift);
             s.prefix[k] = p;
@@ -158,31 +657,232 @@ __global__ void __launch_bounds__(256) radix_resolve_kernel(SelBatch* st, unsign
     for (int q = threadIdx.x; q < K * 256; q += blockDim.x) gb[q] = 0ull;
 }
 
+// ------------------------------------------------------------------------------------------ host side
+enum { PATH_AUTO = 0, PATH_DIRECT = 1, PATH_BRACKET = 2, PATH_RADIX = 3 };
+
+struct SelectPlan {
+    int path;
+    unsigned long long P, S, cap;     // pairs, sample size, candidate capacity per series
+    int L, n_ob;
+    uint32_t tiles;
+    int span;
+};
+
+SelectPlan make_select_plan(const View& v, int K) {
+    const Options& opt = options();
+    SelectPlan p{};
+    p.P = n_pairs(v.n);
+    p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
+    const bool tiled_ok = v.ps == 1 && p.span <= MAX_SPAN;
+    p.path = (int)opt.select_path;
+    if (p.path == PATH_AUTO) p.path = p.P <= (1ull << 22) ? PATH_DIRECT : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
+    if (p.path == PATH_BRACKET && !tiled_ok) p.path = PATH_RADIX;
+    if (p.path == PATH_DIRECT && p.P > (1ull << 28)) p.path = tiled_ok ? PATH_BRACKET : PATH_RADIX;
+    if (p.path == PATH_BRACKET) {
+        double s = 5.5 * std::pow((double)p.P, 2.0 / 3.0);
+        unsigned long long S = (unsigned long long)std::min(std::max(s, 65536.0), 268435456.0);
+        if (opt.sample_size > 0) S = (unsigned long long)opt.sample_size;
+        p.S = std::max<unsigned long long>(16, S);
+        // capacity: 1.5 x the worst-case expected bracket content of one group (<= GK targets), at most 6 % of P
+        const int kg = std::min(K, GK);
+        double frac = std::min(0.06, kg * (BRACKET_SIGMAS + 1.0) / std::sqrt((double)p.S));
+        unsigned long long cap = (unsigned long long)(1.5 * frac * (double)p.P) + 4096;
+        if (opt.cand_cap > 0) cap = (unsigned long long)opt.cand_cap;
+        p.cap = std::min(cap, p.P);
+        const double cells = (double)p.P * (double)v.batch;
+        int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
+        p.L = (int)std::max<int64_t>(32, std::min<int64_t>(2047, L));
+        p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
+        p.tiles = (uint32_t)count_tiles(v.n, p.L);
+    }
+    return p;
+}
+
+size_t count_smem_bytes(int nlev, int L, int span) {
+    return (size_t)CountSmem::off_cols + (size_t)nlev * CountSmem::col_row +
+           4 * ((size_t)window_la(L, span, 0) + window_lb(L, span, 0));
+}
+
+template <int NORM, int M, int TAU>
+rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int batch, cudaStream_t s) {
+    auto kern = sel_count_kernel<NORM, M, TAU>;
+    const size_t smem = count_smem_bytes(nlev, p.L, p.span);
+    RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev);
+    RQA_LAUNCH_CHECK();
+    return RQA_OK;
+}
+
+template <int NORM>
+rqa_status dispatch_count(const CountArgs& a, const SelectPlan& p, int nlev, int batch, cudaStream_t s) {
+    if (a.m == 3 && a.tau == 1) return launch_count<NORM, 3, 1>(a, p, nlev, batch, s);
+    return launch_count<NORM, 0, 0>(a, p, nlev, batch, s);
+}
+
+// 4 radix passes over a buffer for the <= BT targets whose state is already initialised in `st`.
+rqa_status run_bufsel(const float* buf, unsigned long long stride, unsigned long long cap, const SelState* ss,
+                      int use_ncand, BufSel* st, unsigned long long* bins, int T, int batch, cudaStream_t s) {
+    const size_t smem = (size_t)T * 256 * sizeof(uint32_t);
+    if (smem > 48 * 1024)
+        RQA_CUDA_TRY(cudaFuncSetAttribute(bufsel_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    unsigned blocks = (unsigned)std::max<unsigned long long>(1, std::min<unsigned long long>((cap + 2047) / 2048, 148 * 4));
+    for (int pass = 0; pass < 4; ++pass) {
+        bufsel_pass_kernel<<<dim3(blocks, (unsigned)batch), 256, smem, s>>>(buf, stride, cap, ss, use_ncand, pass, st, bins);
+        RQA_LAUNCH_CHECK();
+        bufsel_resolve_kernel<<<batch, 256, 0, s>>>(st, bins, pass, ss, use_ncand);
+        RQA_LAUNCH_CHECK();
+    }
+    return RQA_OK;
+}
+
+struct SelectWs {
+    SelState* ss;
+    BufSel* st;
+    unsigned long long* bins;         // [batch][BT][256]
+    SelTable* tabs;
+    uint32_t* tile_start;
+    float* sample;                    // [batch][S] (DIRECT: [batch][P])
+    float* cand;                      // [batch][cap]
+    SelBatch* rst;
+    unsigned long long* rbins;        // [batch][K][256]
+};
+
+SelectWs carve(Arena& ws, const View& v, int K, const SelectPlan& p) {
+    SelectWs w{};
+    w.ss = ws.take<SelState>(v.batch);
+    w.st = ws.take<BufSel>(v.batch);
+    w.bins = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * BT * 256);
+    w.rst = ws.take<SelBatch>(v.batch);
+    w.rbins = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * K * 256);
+    if (p.path == PATH_DIRECT) w.sample = ws.take<float>((size_t)v.batch * p.P);
+    if (p.path == PATH_BRACKET) {
+        w.tabs = ws.take<SelTable>(v.batch);
+        w.tile_start = ws.take<uint32_t>((size_t)p.n_ob + 1);
+        w.sample = ws.take<float>((size_t)v.batch * p.S);
+        w.cand = ws.take<float>((size_t)v.batch * p.cap);
+    }
+    return w;
+}
+
 }  // namespace
 
 size_t select_workspace_bytes(const View& v, int K) {
-    return align_up(sizeof(SelBatch) * (size_t)v.batch) + align_up(sizeof(uint64_t) * (size_t)v.batch * K * 256);
+    SelectPlan p = make_select_plan(v, K);
+    Arena a(nullptr, ~(size_t)0);
+    carve(a, v, K, p);
+    return a.off;
 }
 
 rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
                       double* d_rr, Arena& ws, cudaStream_t s) {
-    SelBatch* st = ws.take<SelBatch>(v.batch);
-    unsigned long long* bins = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * K * 256);
-    if (!ws.ok()) { set_error("run_select: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
+    const SelectPlan p = make_select_plan(v, K);
+    SelectWs w = carve(ws, v, K, p);
+    if (!ws.ok()) { set_error("rqa_eps_for_rr: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
+    const unsigned long long P = p.P;
+    unsigned long long* d_cnt = (unsigned long long*)d_count;
+
+    sel_init_kernel<<<v.batch, 128, 0, s>>>(w.ss, p.path == PATH_RADIX ? 1 : 0);
+    RQA_LAUNCH_CHECK();
+    RQA_CUDA_TRY(cudaMemsetAsync(w.bins, 0, sizeof(uint64_t) * (size_t)v.batch * BT * 256, s));
+
+    // targets sorted by rank (groups are contiguous in rank)
+    int order[RQA_MAX_K];
+    for (int k = 0; k < K; ++k) order[k] = k;
+    std::stable_sort(order, order + K, [&](int a, int b) { return h_rank[a] < h_rank[b]; });
+
+    if (p.path == PATH_DIRECT) {
+        unsigned blocks = (unsigned)std::min<int64_t>(v.n - 1, 148 * 8);
+        if (norm == RQA_NORM_MAX) sel_direct_kernel<RQA_NORM_MAX><<<dim3(blocks, v.batch), 256, 0, s>>>(v, P, w.sample);
+        else sel_direct_kernel<RQA_NORM_EUCLID><<<dim3(blocks, v.batch), 256, 0, s>>>(v, P, w.sample);
+        RQA_LAUNCH_CHECK();
+        for (int base = 0; base < K; base += BT) {
+            const int T = std::min(BT, K - base);
+            Ranks64 rk{};
+            TargetMap tm{};
+            tm.T = T;
+            for (int t = 0; t < T; ++t) { rk.r[t] = h_rank[order[base + t]]; tm.k_of[t] = order[base + t]; }
+            bufsel_init_kernel<<<v.batch, BT, 0, s>>>(w.st, rk, T);
+            RQA_LAUNCH_CHECK();
+            rqa_status st = run_bufsel(w.sample, P, P, w.ss, 0, w.st, w.bins, T, v.batch, s);
+            if (st != RQA_OK) return st;
+            sel_finish_kernel<<<v.batch, BT, 0, s>>>(w.ss, w.st, tm, K, P, 0, d_eps, d_cnt, d_rr);
+            RQA_LAUNCH_CHECK();
+        }
+        return RQA_OK;
+    }
+
+    if (p.path == PATH_BRACKET) {
+        const unsigned long long S = p.S;
+        {
+            unsigned blocks = (unsigned)std::min<unsigned long long>((S + 255) / 256, 148 * 16);
+            if (norm == RQA_NORM_MAX) sel_sample_kernel<RQA_NORM_MAX><<<dim3(blocks, v.batch), 256, 0, s>>>(v, S, w.sample);
+            else sel_sample_kernel<RQA_NORM_EUCLID><<<dim3(blocks, v.batch), 256, 0, s>>>(v, S, w.sample);
+            RQA_LAUNCH_CHECK();
+        }
+        rqa_status st = launch_tile_table(v.n, p.L, p.n_ob, w.tile_start, s);
+        if (st != RQA_OK) return st;
+        for (int base = 0; base < K; base += GK) {
+            const int kc = std::min(GK, K - base);
+            SampleRanks sr{};
+            Ranks64 rk{};
+            TargetMap tm{};
+            sr.kc = kc;
+            tm.T = kc;
+            for (int t = 0; t < kc; ++t) {
+                const unsigned long long r = h_rank[order[base + t]];
+                const double q = (double)r / (double)P;
+                const double mean = q * (double)S, sd = std::sqrt((double)S * q * (1.0 - q));
+                const double lo = std::floor(mean - BRACKET_SIGMAS * sd) - 1.0;
+                const double hi = std::ceil(mean + BRACKET_SIGMAS * sd) + 1.0;
+                sr.lo[t] = lo >= 1.0 ? (unsigned long long)lo : 0;
+                sr.hi[t] = hi <= (double)S ? (unsigned long long)hi : 0;
+                sr.rank[t] = r;
+                rk.r[2 * t] = sr.lo[t] ? sr.lo[t] : 1;
+                rk.r[2 * t + 1] = sr.hi[t] ? sr.hi[t] : S;
+                tm.k_of[t] = order[base + t];
+            }
+            if (base > 0) {
+                sel_group_reset_kernel<<<v.batch, 128, 0, s>>>(w.ss);
+                RQA_LAUNCH_CHECK();
+            }
+            bufsel_init_kernel<<<v.batch, BT, 0, s>>>(w.st, rk, 2 * kc);
+            RQA_LAUNCH_CHECK();
+            st = run_bufsel(w.sample, S, S, w.ss, 0, w.st, w.bins, 2 * kc, v.batch, s);
+            if (st != RQA_OK) return st;
+            sel_table_kernel<<<v.batch, 512, 0, s>>>(w.st, sr, w.tabs);
+            RQA_LAUNCH_CHECK();
+            CountArgs a;
+            a.v = v; a.L = p.L; a.n_ob = p.n_ob; a.tile_start = w.tile_start; a.tabs = w.tabs; a.ss = w.ss;
+            a.cand = w.cand; a.cap = p.cap; a.m = v.m; a.tau = (int)v.cs;
+            const int nlev = 2 * kc + 1;
+            st = norm == RQA_NORM_MAX ? dispatch_count<RQA_NORM_MAX>(a, p, nlev, v.batch, s)
+                                      : dispatch_count<RQA_NORM_EUCLID>(a, p, nlev, v.batch, s);
+            if (st != RQA_OK) return st;
+            sel_bracket_resolve_kernel<<<v.batch, 64, 0, s>>>(w.ss, w.tabs, sr, w.st, p.cap);
+            RQA_LAUNCH_CHECK();
+            st = run_bufsel(w.cand, p.cap, p.cap, w.ss, 1, w.st, w.bins, kc, v.batch, s);
+            if (st != RQA_OK) return st;
+            sel_finish_kernel<<<v.batch, BT, 0, s>>>(w.ss, w.st, tm, K, P, 1, d_eps, d_cnt, d_rr);
+            RQA_LAUNCH_CHECK();
+        }
+    }
+
+    // radix passes: the whole job on the RADIX path, otherwise only the series the bracket path flagged (blocks of
+    // other series return at once)
     Ranks ranks;
     for (int k = 0; k < K; ++k) ranks.r[k] = h_rank[k];
-    RQA_CUDA_TRY(cudaMemsetAsync(bins, 0, sizeof(uint64_t) * (size_t)v.batch * K * 256, s));
-    select_init_kernel<<<v.batch, RQA_MAX_K, 0, s>>>(st, ranks, K);
+    RQA_CUDA_TRY(cudaMemsetAsync(w.rbins, 0, sizeof(uint64_t) * (size_t)v.batch * K * 256, s));
+    radix_init_kernel<<<v.batch, RQA_MAX_K, 0, s>>>(w.rst, ranks, K);
     RQA_LAUNCH_CHECK();
     const size_t smem = (size_t)K * 256 * sizeof(uint32_t);
     auto kern = norm == RQA_NORM_MAX ? radix_pass_kernel<RQA_NORM_MAX> : radix_pass_kernel<RQA_NORM_EUCLID>;
     if (smem > 48 * 1024) RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 grid((unsigned)((v.n - 1 + SEL_W - 1) / SEL_W), (unsigned)((v.n - 1 + SEL_L - 1) / SEL_L), (unsigned)v.batch);
-    const unsigned long long P = n_pairs(v.n);
+    const int64_t tiles = ((v.n - 1 + SEL_W - 1) / SEL_W) * ((v.n - 1 + SEL_L - 1) / SEL_L);
+    dim3 grid((unsigned)std::min<int64_t>(tiles, 148 * 16), (unsigned)v.batch);
     for (int pass = 0; pass < 4; ++pass) {
-        kern<<<grid, SEL_W, smem, s>>>(v, pass, st, bins, K);
+        kern<<<grid, SEL_W, smem, s>>>(v, pass, w.rst, w.rbins, K, w.ss);
         RQA_LAUNCH_CHECK();
-        radix_resolve_kernel<<<v.batch, 256, 0, s>>>(st, bins, K, pass, P, d_eps, (unsigned long long*)d_count, d_rr);
+        radix_resolve_kernel<<<v.batch, 256, 0, s>>>(w.rst, w.rbins, K, pass, P, w.ss, d_eps, d_cnt, d_rr);
         RQA_LAUNCH_CHECK();
     }
     return RQA_OK;

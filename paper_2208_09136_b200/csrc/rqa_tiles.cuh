@@ -1,0 +1,127 @@
+// rqa_tiles.cuh — what the two full passes over the upper triangle share (the counting pass of rqa_eps_for_rr
+// in rqa_select.cu and the diagonal scan of rqa_line_hist in rqa_line.cu): the tiling of the triangle, the
+// staging of the two series windows in shared memory, the sliding-window cell distance and the bucket function
+// of the level tables.  Internal to librqa.so; nothing here is shared with the oracle.
+//
+// Tiling.  The recurrence plot's upper triangle (only j > i is visited, R_ij is computed on the
+// fly) is cut into diagonal blocks of LW = 256 adjacent diagonals o = j - i (one per thread), and every diagonal
+// block into chunks of L consecutive positions i.  A tile = (diagonal block, chunk).  The lanes of a warp sit on
+// 32 adjacent diagonals at the same position i, so y[i] is a shared-memory broadcast and y[i + o] is 32
+// consecutive words: no bank conflicts.
+//
+// Distance.  With the delay view x_i[c] = y[i + c*tau] the max-norm distance along a diagonal is a
+// sliding maximum over e_i = |y_i - y_{i+o}|, and the squared Euclidean distance a sliding sum in the
+// fixed order c = 0..m-1 (reading S13): one new element per cell, kept in a register ring.
+#pragma once
+
+#include <utility>
+
+#include "rqa_common.cuh"
+
+namespace rqa {
+
+constexpr int LW = 256;          // diagonals per tile = threads per block
+constexpr int NB = 4096;         // buckets of a level look-up table
+constexpr int GK = 32;           // thresholds (or brackets) per group = per full pass
+constexpr int MAX_SPAN = 4096;   // largest (m-1)*tau the tiled kernels stage in shared memory
+constexpr unsigned FULL = 0xffffffffu;
+
+// bucket(d) = bits(fmaf(min(d, dcap), scale, +0)): a denormal-range FMA, i.e. an exactly rounded, monotone map of
+// [0, dcap] onto the integers 0..NB-1 in one instruction (scale is chosen so that dcap*scale < NB * 2^-149).
+__device__ __forceinline__ uint32_t bucket_of(float d, float dcap, float scale) {
+    return __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
+}
+
+// Largest scale for which bucket_of(dcap) <= NB-1.
+__device__ inline float bucket_scale(float dcap) {
+    double sc = ((double)NB - 1.5) * 1.401298464324817e-45 / (double)dcap;   // (NB-1.5) * 2^-149 / dcap
+    float scale = sc > 3.0e38 ? 3.0e38f : (float)sc;
+    while (scale > 0.0f && bucket_of(dcap, dcap, scale) > (uint32_t)(NB - 1)) scale = nextafterf(scale, 0.0f);
+    return scale;
+}
+
+// tile_start[ob] = number of tiles in the diagonal blocks before ob (ob = 0..n_ob); diagonal block ob holds the
+// diagonals 1 + LW*ob .. LW + LW*ob, its longest diagonal has n - 1 - LW*ob cells, cut into chunks of L.
+rqa_status launch_tile_table(int64_t n, int L, int n_ob, uint32_t* tile_start, cudaStream_t s);
+
+inline uint64_t count_tiles(int64_t n, int L) {
+    uint64_t tiles = 0;
+    const int n_ob = (int)((n - 1 + LW - 1) / LW);
+    for (int ob = 0; ob < n_ob; ++ob) tiles += (uint64_t)((n - 1 - (int64_t)LW * ob + L - 1) / L);
+    return tiles;
+}
+
+#ifdef __CUDACC__
+// Which diagonal block does `tile` belong to?  (block-wide search; the caller syncs before reading *s_ob)
+__device__ __forceinline__ void find_diagonal_block(const uint32_t* __restrict__ tile_start, int n_ob, uint32_t tile,
+                                                    int* s_ob) {
+    for (int q = threadIdx.x; q < n_ob; q += LW)
+        if (tile_start[q] <= tile && tile < tile_start[q + 1]) *s_ob = q;
+}
+
+// Window lengths (floats) for a chunk of L positions, embedding span (m-1)*tau and W warm-up cells before the chunk:
+// i-side window y[s-W .. s-W+LA), j-side window y[s-W+o0 .. s-W+o0+LB).
+__host__ __device__ inline int window_la(int L, int span, int W) { return (L + W + 6 + 2 * span + 3) & ~3; }
+__host__ __device__ inline int window_lb(int L, int span, int W) { return (L + W + 6 + 2 * span + LW + 3) & ~3; }
+
+// Stage the two windows of series `y` (ny samples); samples outside the series read as 0 (their cells are never
+// counted).
+__device__ __forceinline__ void stage_windows(const float* __restrict__ y, int64_t ny, int64_t start_a, int64_t start_b,
+                                              float* ya_s, int LA, float* yb_s, int LB) {
+    for (int x = threadIdx.x; x < LA; x += LW) {
+        int64_t gi = start_a + x;
+        ya_s[x] = (gi >= 0 && gi < ny) ? y[gi] : 0.0f;
+    }
+    for (int x = threadIdx.x; x < LB; x += LW) {
+        int64_t gi = start_b + x;
+        yb_s[x] = (gi >= 0 && gi < ny) ? y[gi] : 0.0f;
+    }
+}
+
+// Cell distances along one diagonal from the staged windows.  W = warm-up cells before the chunk (cell t of the
+// chunk reads window index t + W).  M > 0: compile-time (M, TAU), sliding window over a register ring of
+// S = (M-1)*TAU + 1 elements.  M == 0: run-time (m, tau), recomputed from the windows for every cell.
+template <int NORM, int M, int TAU, int W>
+struct CellDist {
+    static constexpr int S = M > 0 ? (M - 1) * TAU + 1 : 1;
+    float ring[S];
+    const float* ya;
+    const float* yb;            // already offset by the thread's diagonal
+    int m, tau;
+
+    __device__ __forceinline__ float elem(int x) const {
+        float diff = __fsub_rn(ya[x], yb[x]);
+        return NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
+    }
+    // Before the first cell t_first (which must be processed at ring phase R = 0) the ring holds e_t .. e_{t+S-2}.
+    __device__ __forceinline__ void prime(int t_first) {
+#pragma unroll
+        for (int x = 0; x < (M > 0 ? S - 1 : 0); ++x) ring[x] = elem(t_first + W + x);
+    }
+    // R = ring phase of cell t (number of cells since t_first, mod S; static); pushes e_{t+S-1}
+    template <int R>
+    __device__ __forceinline__ void push(int t) {
+        if (M > 0) ring[(R + S - 1) % S] = elem(t + W + S - 1);
+    }
+    template <int R>
+    __device__ __forceinline__ float distance(int t) const {
+        if (M == 0) {
+            float d = elem(t + W);
+            for (int c = 1; c < m; ++c) {
+                float x = elem(t + W + c * tau);
+                d = NORM == RQA_NORM_MAX ? fmaxf(d, x) : __fadd_rn(d, x);
+            }
+            return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
+        }
+        float d = ring[R % S];
+#pragma unroll
+        for (int c = 1; c < M; ++c) {
+            float x = ring[(R + c * TAU) % S];
+            d = NORM == RQA_NORM_MAX ? fmaxf(d, x) : __fadd_rn(d, x);
+        }
+        return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
+    }
+};
+#endif
+
+}  // namespace rqa

@@ -101,6 +101,27 @@ def test_line_hist_det_embed_reject_bad_arguments(lib):
         (982, 4, 5, 1, 6, 1000)
 
 
+def test_set_option_validation(lib):
+    assert lib.rqa_set_option(b"select_path", 2) == B.RQA_OK
+    assert lib.rqa_set_option(b"select_path", 0) == B.RQA_OK
+    assert lib.rqa_set_option(b"select_path", 4) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_set_option(b"line_chunk", 1024) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_set_option(b"no_such_option", 1) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_set_option(None, 1) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_set_option(b"sample_size", -1) == B.RQA_ERR_INVALID_ARG
+    # workspace sizes follow the options: the bracket path needs the sample and candidate buffers
+    sz0, sz2 = ctypes.c_size_t(0), ctypes.c_size_t(0)
+    pts = _pts(n=5000, bs=5002)
+    assert lib.rqa_set_option(b"select_path", 3) == B.RQA_OK
+    assert lib.rqa_workspace_bytes(ctypes.byref(pts), 20, ctypes.byref(sz0)) == B.RQA_OK
+    assert lib.rqa_set_option(b"select_path", 2) == B.RQA_OK
+    assert lib.rqa_set_option(b"sample_size", 50_000_000) == B.RQA_OK
+    assert lib.rqa_workspace_bytes(ctypes.byref(pts), 20, ctypes.byref(sz2)) == B.RQA_OK
+    assert lib.rqa_set_option(b"select_path", 0) == B.RQA_OK
+    assert lib.rqa_set_option(b"sample_size", 0) == B.RQA_OK
+    assert sz2.value >= 4 * 50_000_000 > sz0.value
+
+
 def test_no_cpu_fallback_without_gpu(lib):
     """Without a CUDA device a compute call must fail loudly with RQA_ERR_CUDA, never silently succeed."""
     import torch

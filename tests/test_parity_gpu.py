@@ -290,3 +290,92 @@ def test_config4_full_size_white_noise(rqa, oracle):
     assert np.array_equal((g["hist"][0] * l).sum(axis=1), g["count"][0])
     oh = oracle.line_hist(w.series[0], w.m, w.tau, eps[:3], w.norm, threads=0)
     assert np.array_equal(g["hist"][0][:3], oh)
+
+
+# ------------------------------------------------------------------ every path of rqa_eps_for_rr is exact
+@pytest.fixture
+def options(rqa):
+    """Set expert knobs for one test and restore the automatic choices afterwards."""
+    names = ["select_path", "sample_size", "cand_cap", "line_chunk"]
+
+    def setter(**kw):
+        for k, v in kw.items():
+            rqa.rqa_set_option(k, v)
+    yield setter
+    for n in names:
+        rqa.rqa_set_option(n, 0)
+
+
+def _select_only(rqa, series, m, tau, rr, norm=0):
+    import torch
+    s = torch.as_tensor(np.ascontiguousarray(np.atleast_2d(series), dtype=np.float32)).cuda()
+    K = len(rr)
+    view = rqa.rqa_embed(s, m, tau)
+    eps = torch.empty((s.shape[0], K), dtype=torch.float32, device="cuda")
+    cnt = torch.empty((s.shape[0], K), dtype=torch.int64, device="cuda")
+    rrr = torch.empty((s.shape[0], K), dtype=torch.float64, device="cuda")
+    ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
+    rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
+    rqa.rqa_workspace_status(ws)
+    return eps.cpu().numpy(), cnt.cpu().numpy().view(np.uint64), rrr.cpu().numpy()
+
+
+def _assert_select(oracle, got, series, m, tau, rr, norm=0):
+    series = np.atleast_2d(series)
+    for b in range(series.shape[0]):
+        e, c, r = oracle.eps_for_rr(series[b], m, tau, rr, norm)
+        assert np.array_equal(got[0][b].view(np.uint32), e.view(np.uint32)), f"eps, series {b}"
+        assert np.array_equal(got[1][b], c), f"count, series {b}"
+        assert np.array_equal(got[2][b], r), f"rr, series {b}"
+
+
+@pytest.mark.parametrize("path", [1, 2, 3])
+@pytest.mark.parametrize("norm", [0, 1])
+def test_select_paths_agree_with_oracle(rqa, oracle, options, path, norm):
+    """direct / bracket / radix on the same inputs: a noisy Lorenz batch (m=3, tau=1: compiled-in embedding) and a
+    sine batch (m=4, tau=6: run-time embedding), unsorted RRs with duplicates and rr = 1."""
+    options(select_path=path)
+    rr = np.array([0.3, 0.0007, 0.02, 0.02, 0.11, 1.0, 0.5, 0.004])
+    ys = np.stack([wl.add_noise(wl.lorenz_signal(2500), snr, 40 + i) for i, snr in enumerate([math.inf, 1.0, 0.1])])
+    _assert_select(oracle, _select_only(rqa, ys, 3, 1, rr, norm), ys, 3, 1, rr, norm)
+    ys = np.stack([wl.add_noise(wl.sine_signal(1800), snr, 50 + i) for i, snr in enumerate([2.0, 0.2])])
+    _assert_select(oracle, _select_only(rqa, ys, 4, 6, rr, norm), ys, 4, 6, rr, norm)
+
+
+@pytest.mark.parametrize("S", [16, 300, 5000, 200000])
+def test_bracket_path_any_sample_size(rqa, oracle, options, S):
+    """Tiny samples give open or huge brackets, large ones narrow brackets: the result never depends on S."""
+    options(select_path=2, sample_size=S)
+    y = wl.add_noise(wl.logistic_signal(3001, 9), 0.5, 9)
+    rr = wl.rr_log(20, 0.001, 0.2)
+    _assert_select(oracle, _select_only(rqa, y, 3, 1, rr), y, 3, 1, rr)
+
+
+def test_bracket_path_overflow_and_ties_fall_back(rqa, oracle, options):
+    """A candidate list that is too small, and tie-heavy data whose brackets collapse, are both detected from the exact
+    counts and redone by the radix passes — per series, inside one batched call."""
+    rr = wl.rr_log(12, 0.002, 0.4)
+    noisy = wl.add_noise(wl.sine_signal(2600), 0.7, 3)
+    clean = wl.sine_signal(2600).astype(np.float32)                      # 25 distinct values: massive ties
+    quant = np.floor(wl.uniform01(5, 2600) * 4).astype(np.float32)
+    ys = np.stack([noisy, clean, quant])
+    options(select_path=2)
+    _assert_select(oracle, _select_only(rqa, ys, 2, 3, rr), ys, 2, 3, rr)
+    options(select_path=2, cand_cap=64)
+    _assert_select(oracle, _select_only(rqa, ys, 2, 3, rr), ys, 2, 3, rr)
+
+
+def test_bracket_path_many_targets(rqa, oracle, options):
+    """K = 128 targets = four groups of 32 brackets; K = 33 = a full group and a group of one."""
+    options(select_path=2)
+    y = wl.add_noise(wl.lorenz_signal(2200), 0.5, 21)
+    for K in (128, 33):
+        rr = wl.rr_log(K, 0.0005, 0.95)
+        _assert_select(oracle, _select_only(rqa, y, 3, 3, rr), y, 3, 3, rr)
+
+
+def test_config3_size_default_path_is_bracket(rqa, oracle):
+    """N = 1e4 (P = 5e7 > 2^22) takes the bracket path by default: one Lorenz series at each norm."""
+    w = wl.config3(0)
+    for norm in (0, 1):
+        _assert_select(oracle, _select_only(rqa, w.series[2], w.m, w.tau, w.rr, norm), w.series[2], w.m, w.tau, w.rr, norm)

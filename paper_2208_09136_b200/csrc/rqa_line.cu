@@ -27,8 +27,9 @@ namespace rqa {
 namespace {
 
 constexpr int LMAX = 1023;       // longest chunk: run lengths stay exact in fp16 and 1024+run has ulp 1
-constexpr int LS = 256;          // lines shorter than this are counted in shared memory
+constexpr int LS = 128;          // lines shorter than this are counted in shared memory
 constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
+constexpr int QCAP = 32;         // line-end records a warp collects before it emits them, one record per lane
 
 // Everything the scan needs to know about one group of <= 32 thresholds of one series.
 struct LineGroup {
@@ -152,7 +153,9 @@ struct ScanSmem {
     static constexpr int agg_row = 4 * (LW / 2);              // one level: 128 words, two 16-bit counters each
     static constexpr int agg_one = NLEV * agg_row;            // one of the three histograms
     static constexpr int off_sh = off_agg + 3 * agg_one;
-    static constexpr int off_ya = off_sh + 4 * 2 * NP * LS;
+    static constexpr int QS = (NP + 1) | 1;                   // words per queue record (odd: conflict-free spill)
+    static constexpr int off_q = off_sh + 4 * 2 * NP * LS;    // per warp QCAP records of (range, NP run registers)
+    static constexpr int off_ya = off_q + 4 * (LW / 32) * QCAP * QS;
 };
 struct ScanArgs {
     View v;
@@ -167,6 +170,27 @@ struct ScanArgs {
     int m, tau;                 // run-time embedding (used by the M == 0 variant)
 };
 
+// Emit the queued line ends of one warp: record r = (lo4 | hi4 << 8, run registers of the lane that queued it);
+// thresholds j in [lo4/4, hi4/4) each end a line whose length is the fp16 half j of the run registers.
+template <int QS>
+__device__ __forceinline__ void flush_queue(unsigned mask, uint32_t lane_lt, uint32_t q, uint32_t qn, uint32_t sh,
+                                            unsigned long long* grow, const int* rep, int64_t n) {
+    __syncwarp(mask);
+    const uint32_t my = __popc(mask & lane_lt), nl = __popc(mask);
+    for (uint32_t r = my; r < qn; r += nl) {
+        const uint32_t rec = q + 4 * QS * r;
+        const uint32_t w = lds_u32(rec);
+        const uint32_t hi = w >> 10;
+#pragma unroll 1
+        for (uint32_t j = (w & 0xffu) >> 2; j < hi; ++j) {
+            const uint32_t l = (uint32_t)__half2int_rn(__ushort_as_half((unsigned short)lds_u16(rec + 4 + 2 * j)));
+            if (l < (uint32_t)LS) red_u32(sh + 4 * (j * LS + l), 1u);
+            else atomicAdd(&grow[(int64_t)rep[j] * n + l], 1ull);
+        }
+    }
+    __syncwarp(mask);
+}
+
 template <int NORM, int M, int TAU, int NP>
 struct Scanner : CellDist<NORM, M, TAU, 2> {
     using CD = CellDist<NORM, M, TAU, 2>;
@@ -179,10 +203,9 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t w2a, w2b, w2c;     // max(level pairs) of the previous three cells (newest first)
     uint32_t pm;                // 4 * running maximum level since the chunk start
     // per-thread constants
-    const uint8_t* lut;
-    const char* eps;
-    char* agg;                  // thread's column of histogram 1, level 0
-    uint32_t* sh;
+    uint32_t lut, eps;          // shared-window addresses of the bucket table and the thresholds
+    uint32_t agg;               // ... of the thread's column of histogram 1, level 0
+    uint32_t sh;                // ... of the short-line histogram
     unsigned long long* grow;   // hist + b*K*n (rows indexed through rep)
     const int* rep;
     uint16_t* pre_out;
@@ -190,40 +213,40 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t inc, J4;
     int multi;
     int64_t n;
+    uint32_t q;                 // ... of this warp's queue of line-end records
+    uint32_t qn;                // records in the queue (warp-uniform among the live lanes)
+    uint32_t lane_lt;
 
     __device__ __forceinline__ uint32_t level4(float d) const {
         uint32_t idx = __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
-        uint32_t q = lut[idx];
-        float er = *(const float*)(eps + q);
+        uint32_t q = lds_u8(lut + idx);
+        float er = lds_f32(eps + q);
         uint32_t v4 = q + (d > er ? 4u : 0u);
         if (multi) {
-            while (d > *(const float*)(eps + v4)) v4 += 4;
+            while (d > lds_f32(eps + v4)) v4 += 4;
         }
         return v4;
     }
 
-    // Lines of length >= 4 that ended at the previous cell, for the levels [lo4, hi4) / 4 of this lane.
-    __device__ __forceinline__ void emit(unsigned mask, bool trig, uint32_t lo4, uint32_t hi4) {
-        uint32_t lm = 0;
-        if (trig && hi4 > lo4) lm = (0xffffffffu >> (32 - ((hi4 - lo4) >> 2))) << (lo4 >> 2);
-        uint32_t wm = __reduce_or_sync(mask, lm);
-        while (wm) {
-            const int j = __ffs(wm) - 1;
-            wm &= wm - 1;
-            uint32_t r = 0;
-            switch (j >> 1) {
-#define RQA_CASE(P) case P: if (P < NP) r = run[P < NP ? P : 0]; break;
-                RQA_CASE(0) RQA_CASE(1) RQA_CASE(2) RQA_CASE(3) RQA_CASE(4) RQA_CASE(5) RQA_CASE(6) RQA_CASE(7)
-                RQA_CASE(8) RQA_CASE(9) RQA_CASE(10) RQA_CASE(11) RQA_CASE(12) RQA_CASE(13) RQA_CASE(14) RQA_CASE(15)
-#undef RQA_CASE
-            }
-            if ((lm >> j) & 1u) {
-                __half2 h = *(__half2*)&r;
-                uint32_t l = (uint32_t)__half2int_rn((j & 1) ? __high2half(h) : __low2half(h));
-                if (l < (uint32_t)LS) atomicAdd(&sh[j * LS + l], 1u);
-                else atomicAdd(&grow[(int64_t)rep[j] * n + l], 1ull);
-            }
+    // Lines of length >= 4 that ended at the previous cell, for the levels [lo4, hi4) / 4 of this lane: the lane
+    // appends one record (its range and a copy of its run registers) to the warp's queue.  Emission proper happens
+    // when the queue is full, one record per lane (flush_queue), so the divergent per-threshold loop runs with all
+    // lanes busy instead of once per warp-cell.
+    __device__ __forceinline__ void enqueue(unsigned mask, bool want, uint32_t lo4, uint32_t hi4) {
+        const unsigned wm = __ballot_sync(mask, want);
+        if (wm == 0) return;
+        const uint32_t add = __popc(wm);
+        if (qn + add > (uint32_t)QCAP) {
+            flush_queue<SM::QS>(mask, lane_lt, q, qn, sh, grow, rep, n);
+            qn = 0;
         }
+        if (want) {
+            const uint32_t rec = q + 4 * SM::QS * (qn + __popc(wm & lane_lt));
+            sts_u32(rec, lo4 | (hi4 << 8));
+#pragma unroll
+            for (int p = 0; p < NP; ++p) sts_u32(rec + 4 + 4 * p, run[p]);
+        }
+        qn += add;
     }
 
     // One cell.  R = ring phase (static), t = position inside the chunk (t < 0: warm-up cells before the chunk),
@@ -245,17 +268,28 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         const uint32_t v4 = level4(d);
         // aggregates: level, max of 2, max of 3 consecutive levels (thread-private columns)
         const uint32_t w2 = max(v4, v1), w3 = max(w2, v2);
-        atomicAdd((uint32_t*)(agg + v4 * (SM::agg_row / 4)), inc);
-        atomicAdd((uint32_t*)(agg + SM::agg_one + w2 * (SM::agg_row / 4)), inc);
-        atomicAdd((uint32_t*)(agg + 2 * SM::agg_one + w3 * (SM::agg_row / 4)), inc);
-        // lines of length >= 4 that end here: thresholds j with max(level of the 4 previous cells) <= j < level
-        const uint32_t w4p = max(w2a, w2c);
-        const bool trig = v4 > w4p;
-        if (__any_sync(mask, trig)) emit(mask, trig, w4p, min(v4, pm));
+        red_u32(agg + v4 * (SM::agg_row / 4), inc);
+        red_u32(agg + SM::agg_one + w2 * (SM::agg_row / 4), inc);
+        red_u32(agg + 2 * SM::agg_one + w3 * (SM::agg_row / 4), inc);
+        // lines of length >= 4 that end here: thresholds j with max(level of the 4 previous cells) <= j < level;
         // prefix runs (recurrent since the chunk start) that end here have length t
-        if (v4 > pm) {
-            for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
-            pm = v4;
+        const uint32_t w4p = max(w2a, w2c);
+        const uint32_t hi4 = min(v4, pm);
+        if (GUARD) {
+            enqueue(mask, hi4 > w4p, w4p, hi4);
+            if (v4 > pm) {
+#pragma unroll 1
+                for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
+                pm = v4;
+            }
+        } else if (__any_sync(FULL, v4 > w4p)) {
+            // unguarded cells have t >= 4, so pm >= w4p: a new prefix maximum is also a trigger
+            enqueue(FULL, hi4 > w4p, w4p, hi4);
+            if (v4 > pm) {
+#pragma unroll 1
+                for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
+                pm = v4;
+            }
         }
         // run update for all thresholds, two per instruction
         const uint32_t vvb = v4 * 0x00010001u + 0x64006400u;             // fp16x2 (1024 + 4v, 1024 + 4v)
@@ -336,18 +370,18 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     const int cnt_lo = __shfl_sync(FULL, cnt, 31);
 
     SC sc;
-    sc.ya = ya_s;
-    sc.yb = yb_s + tid;
-    sc.lut = lut_s;
-    sc.eps = (const char*)eps_s;
-    sc.agg = (char*)agg_s + 4 * (tid & (LW / 2 - 1));
-    sc.sh = sh_s;
+    sc.ya = smem_addr(ya_s);
+    sc.yb = pin(smem_addr(yb_s) + 4 * tid);
+    sc.lut = smem_addr(lut_s);
+    sc.eps = smem_addr(eps_s);
+    sc.agg = pin(smem_addr(agg_s) + 4 * (tid & (LW / 2 - 1)));
+    sc.sh = smem_addr(sh_s);
     sc.grow = a.hist + (int64_t)b * a.K * n;
-    sc.rep = s_rep;
+    sc.rep = G.rep_k;                                       // global copy: only read for lines of length >= LS
     sc.pre_out = a.pre + (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
     sc.scale = G.scale;
     sc.dcap = G.dcap;
-    sc.inc = tid < LW / 2 ? 1u : 0x10000u;
+    sc.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
     sc.J4 = 4u * (uint32_t)J;
     sc.multi = G.multi;
     sc.m = a.m;
@@ -356,6 +390,9 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     sc.v1 = sc.v2 = sc.J4;
     sc.w2a = sc.w2b = sc.w2c = sc.J4;
     sc.pm = 0;
+    sc.q = pin(smem_addr(smem + SM::off_q) + 4 * (tid >> 5) * (QCAP * SM::QS));
+    sc.qn = 0;
+    sc.lane_lt = (1u << (tid & 31)) - 1u;
 #pragma unroll
     for (int p = 0; p < NP; ++p) sc.run[p] = 0;
 
@@ -365,10 +402,13 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
         constexpr int U = S >= 3 ? S : (S == 2 ? 4 : 4);     // cells per super-step, a multiple of S
         using Seq = std::make_integer_sequence<int, U>;
         int t = -2;
-        sc.template superstep<true>(t, cnt, ds, Seq{});      // warm-up cells and the first U-2 cells, guarded
-        t += U;
+        // warm-up cells and the first cells of the chunk, guarded (the unguarded cell needs t >= 4)
+        for (; t < 4; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
         for (; t + U <= cnt_lo; t += U) sc.template superstep<false>(t, cnt, ds, Seq{});
         for (; t < cnt_hi; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
+        // lane 0 sits on the warp's longest diagonal, so it took part in every enqueue
+        const uint32_t qn = __shfl_sync(FULL, sc.qn, 0);
+        if (qn) flush_queue<SM::QS>(FULL, sc.lane_lt, sc.q, qn, sc.sh, sc.grow, sc.rep, sc.n);
         if (cnt > 0) {
             // runs alive at the end of the chunk, and prefix runs that never ended (the whole chunk)
             uint32_t* suf_out = a.suf + (((int64_t)b * a.tiles + tile) * NP) * LW + tid;

@@ -325,9 +325,8 @@ struct CountSmem {
 template <int NORM, int M, int TAU>
 struct Counter : CellDist<NORM, M, TAU, 0> {
     using CD = CellDist<NORM, M, TAU, 0>;
-    const uint16_t* lut;
-    const float* beta;
-    char* cols;                       // this thread's column, level 0
+    uint32_t lut, beta;               // shared-window addresses of the bucket table and the boundaries
+    uint32_t cols;                    // ... of this thread's column, level 0
     float* wbuf;                      // this warp's candidate buffer
     float* gcand;                     // the series' candidate list
     unsigned long long* gncand;
@@ -353,9 +352,9 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
         CD::template push<R>(t);
         const bool live = !GUARD || t < cnt;
         const float d = CD::template distance<R>(t);
-        uint32_t q = lut[bucket_of(d, dcap, scale)];
-        while (d > beta[q]) ++q;
-        if (live) atomicAdd((uint32_t*)(cols + q * CountSmem::col_row), inc);
+        uint32_t q = lds_u16(lut + 2 * bucket_of(d, dcap, scale));
+        while (d > lds_f32(beta + 4 * q)) ++q;
+        if (live) red_u32(cols + q * CountSmem::col_row, inc);
         const unsigned mc = __ballot_sync(FULL, live && (q & 1u));
         if (mc) {
             const uint32_t nc = __popc(mc);
@@ -409,13 +408,13 @@ __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev)
     const int cnt_lo = __shfl_sync(FULL, cnt, 31);
 
     CT ct;
-    ct.ya = ya_s;
-    ct.yb = yb_s + tid;
+    ct.ya = smem_addr(ya_s);
+    ct.yb = pin(smem_addr(yb_s) + 4 * tid);
     ct.m = a.m;
     ct.tau = a.tau;
-    ct.lut = lut_s;
-    ct.beta = beta_s;
-    ct.cols = (char*)cols_s + 4 * (tid & (LW / 2 - 1));
+    ct.lut = smem_addr(lut_s);
+    ct.beta = smem_addr(beta_s);
+    ct.cols = pin(smem_addr(cols_s) + 4 * (tid & (LW / 2 - 1)));
     ct.wbuf = cand_s + (tid >> 5) * WCAP;
     ct.gcand = a.cand + (unsigned long long)b * a.cap;
     ct.gncand = &a.ss[b].ncand;

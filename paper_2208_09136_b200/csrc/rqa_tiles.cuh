@@ -52,6 +52,19 @@ inline uint64_t count_tiles(int64_t n, int L) {
 }
 
 #ifdef __CUDACC__
+// Shared-memory accesses of the tiled passes' inner loops go through 32-bit shared-window addresses and explicit .shared
+// instructions: with generic pointers the compiler re-derives the window base inside the loop when registers are tight.
+// pin(): an identity shuffle (call it with the whole warp converged).  ptxas lowers a shared symbol's address to
+// S2R SR_CgaCtaId + LEA and, being "cheap", rematerialises that per use inside the loop; a shuffle result is kept.
+__device__ __forceinline__ uint32_t pin(uint32_t x) { return __shfl_sync(0xffffffffu, x, threadIdx.x & 31); }
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return pin((uint32_t)__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ uint32_t lds_u8(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts_u32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void red_u32(uint32_t a, uint32_t v) { asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+
 // Which diagonal block does `tile` belong to?  (block-wide search; the caller syncs before reading *s_ob)
 __device__ __forceinline__ void find_diagonal_block(const uint32_t* __restrict__ tile_start, int n_ob, uint32_t tile,
                                                     int* s_ob) {
@@ -85,13 +98,14 @@ template <int NORM, int M, int TAU, int W>
 struct CellDist {
     static constexpr int S = M > 0 ? (M - 1) * TAU + 1 : 1;
     float ring[S];
-    const float* ya;
-    const float* yb;            // already offset by the thread's diagonal
+    uint32_t ya;                // shared-window address of the i-side window
+    uint32_t yb;                // ... of the j-side window, already offset by the thread's diagonal
     int m, tau;
 
     __device__ __forceinline__ float elem(int x) const {
-        float diff = __fsub_rn(ya[x], yb[x]);
-        return NORM == RQA_NORM_MAX ? fabsf(diff) : __fmul_rn(diff, diff);
+        // max norm: the signed difference is kept, |.| is an operand modifier of the maximum in distance()
+        float diff = __fsub_rn(lds_f32(ya + 4 * x), lds_f32(yb + 4 * x));
+        return NORM == RQA_NORM_MAX ? diff : __fmul_rn(diff, diff);
     }
     // Before the first cell t_first (which must be processed at ring phase R = 0) the ring holds e_t .. e_{t+S-2}.
     __device__ __forceinline__ void prime(int t_first) {
@@ -107,17 +121,19 @@ struct CellDist {
     __device__ __forceinline__ float distance(int t) const {
         if (M == 0) {
             float d = elem(t + W);
+            if (NORM == RQA_NORM_MAX) d = fabsf(d);
             for (int c = 1; c < m; ++c) {
                 float x = elem(t + W + c * tau);
-                d = NORM == RQA_NORM_MAX ? fmaxf(d, x) : __fadd_rn(d, x);
+                d = NORM == RQA_NORM_MAX ? fmaxf(d, fabsf(x)) : __fadd_rn(d, x);
             }
             return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
         }
         float d = ring[R % S];
+        if (NORM == RQA_NORM_MAX) d = fabsf(d);
 #pragma unroll
         for (int c = 1; c < M; ++c) {
             float x = ring[(R + c * TAU) % S];
-            d = NORM == RQA_NORM_MAX ? fmaxf(d, x) : __fadd_rn(d, x);
+            d = NORM == RQA_NORM_MAX ? fmaxf(d, fabsf(x)) : __fadd_rn(d, x);
         }
         return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);
     }

@@ -29,7 +29,8 @@ namespace {
 constexpr int LMAX = 1023;       // longest chunk: run lengths stay exact in fp16 and 1024+run has ulp 1
 constexpr int LS = 128;          // lines shorter than this are counted in shared memory
 constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
-constexpr int QCAP = 32;         // line-end records a warp collects before it emits them, one record per lane
+constexpr int QCAP = 48;         // capacity of a warp's queue of line-end records
+constexpr int QFLUSH = QCAP - 31;  // records that trigger emission (a cell adds at most 32), one record per lane
 
 // Everything the scan needs to know about one group of <= 32 thresholds of one series.
 struct LineGroup {
@@ -153,9 +154,10 @@ struct ScanSmem {
     static constexpr int agg_row = 4 * (LW / 2);              // one level: 128 words, two 16-bit counters each
     static constexpr int agg_one = NLEV * agg_row;            // one of the three histograms
     static constexpr int off_sh = off_agg + 3 * agg_one;
-    static constexpr int QS = (NP + 1) | 1;                   // words per queue record (odd: conflict-free spill)
-    static constexpr int off_q = off_sh + 4 * 2 * NP * LS;    // per warp QCAP records of (range, NP run registers)
-    static constexpr int off_ya = off_q + 4 * (LW / 32) * QCAP * QS;
+    static constexpr int QS = (NP + 1 + 3) & ~3;              // words per queue record (16-byte vector stores)
+    static constexpr int QWARP = 4 * (QCAP * QS + 4);         // bytes per warp: the record count, then QCAP records
+    static constexpr int off_q = off_sh + 4 * 2 * NP * LS;
+    static constexpr int off_ya = off_q + (LW / 32) * QWARP;
 };
 struct ScanArgs {
     View v;
@@ -175,10 +177,9 @@ struct ScanArgs {
 template <int QS>
 __device__ __forceinline__ void flush_queue(unsigned mask, uint32_t lane_lt, uint32_t q, uint32_t qn, uint32_t sh,
                                             unsigned long long* grow, const int* rep, int64_t n) {
-    __syncwarp(mask);
     const uint32_t my = __popc(mask & lane_lt), nl = __popc(mask);
     for (uint32_t r = my; r < qn; r += nl) {
-        const uint32_t rec = q + 4 * QS * r;
+        const uint32_t rec = q + 16 + 4 * QS * r;
         const uint32_t w = lds_u32(rec);
         const uint32_t hi = w >> 10;
 #pragma unroll 1
@@ -188,6 +189,8 @@ __device__ __forceinline__ void flush_queue(unsigned mask, uint32_t lane_lt, uin
             else atomicAdd(&grow[(int64_t)rep[j] * n + l], 1ull);
         }
     }
+    __syncwarp(mask);
+    if (my == 0) sts_u32(q, 0u);
     __syncwarp(mask);
 }
 
@@ -214,7 +217,6 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     int multi;
     int64_t n;
     uint32_t q;                 // ... of this warp's queue of line-end records
-    uint32_t qn;                // records in the queue (warp-uniform among the live lanes)
     uint32_t lane_lt;
 
     __device__ __forceinline__ uint32_t level4(float d) const {
@@ -228,25 +230,28 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         return v4;
     }
 
-    // Lines of length >= 4 that ended at the previous cell, for the levels [lo4, hi4) / 4 of this lane: the lane
-    // appends one record (its range and a copy of its run registers) to the warp's queue.  Emission proper happens
-    // when the queue is full, one record per lane (flush_queue), so the divergent per-threshold loop runs with all
-    // lanes busy instead of once per warp-cell.
-    __device__ __forceinline__ void enqueue(unsigned mask, bool want, uint32_t lo4, uint32_t hi4) {
-        const unsigned wm = __ballot_sync(mask, want);
-        if (wm == 0) return;
-        const uint32_t add = __popc(wm);
-        if (qn + add > (uint32_t)QCAP) {
-            flush_queue<SM::QS>(mask, lane_lt, q, qn, sh, grow, rep, n);
-            qn = 0;
-        }
-        if (want) {
-            const uint32_t rec = q + 4 * SM::QS * (qn + __popc(wm & lane_lt));
-            sts_u32(rec, lo4 | (hi4 << 8));
+    // Line ends at one cell (call with the lanes of `mask` converged, when some lane has one).  Lines of length >= 4
+    // that ended at the previous cell, for the thresholds [lo4, hi4) / 4 of this lane: the lane appends one record
+    // (its range and a copy of its run registers) to the warp's queue.  Emission proper happens once QFLUSH records
+    // are queued, one record per lane (flush_queue), so the divergent per-threshold loop runs with most lanes busy
+    // instead of once per warp-cell.  Prefix runs (recurrent since the chunk start) that end here have length t.
+    __device__ __forceinline__ void line_ends(unsigned mask, uint32_t lo4, uint32_t hi4, uint32_t v4, int t) {
+        if (hi4 > lo4) {
+            const uint32_t rec = q + 16 + 4 * SM::QS * atom_u32(q, 1u);
+            sts_v4(rec, lo4 | (hi4 << 8), run[0], NP > 1 ? run[NP > 1 ? 1 : 0] : 0u, NP > 2 ? run[NP > 2 ? 2 : 0] : 0u);
 #pragma unroll
-            for (int p = 0; p < NP; ++p) sts_u32(rec + 4 + 4 * p, run[p]);
+            for (int p = 3; p < NP; p += 4)
+                sts_v4(rec + 4 + 4 * p, run[p], p + 1 < NP ? run[p + 1 < NP ? p + 1 : 0] : 0u,
+                       p + 2 < NP ? run[p + 2 < NP ? p + 2 : 0] : 0u, p + 3 < NP ? run[p + 3 < NP ? p + 3 : 0] : 0u);
         }
-        qn += add;
+        if (v4 > pm) {
+#pragma unroll 1
+            for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
+            pm = v4;
+        }
+        __syncwarp(mask);
+        const uint32_t qn = lds_u32(q);
+        if (qn >= (uint32_t)QFLUSH) flush_queue<SM::QS>(mask, lane_lt, q, qn, sh, grow, rep, n);
     }
 
     // One cell.  R = ring phase (static), t = position inside the chunk (t < 0: warm-up cells before the chunk),
@@ -271,26 +276,11 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         red_u32(agg + v4 * (SM::agg_row / 4), inc);
         red_u32(agg + SM::agg_one + w2 * (SM::agg_row / 4), inc);
         red_u32(agg + 2 * SM::agg_one + w3 * (SM::agg_row / 4), inc);
-        // lines of length >= 4 that end here: thresholds j with max(level of the 4 previous cells) <= j < level;
-        // prefix runs (recurrent since the chunk start) that end here have length t
+        // lines of length >= 4 that end here: thresholds j with max(level of the 4 previous cells) <= j < level.
+        // Unguarded cells have t >= 4, so pm >= w4p: there a new prefix maximum is also such a line end.
         const uint32_t w4p = max(w2a, w2c);
         const uint32_t hi4 = min(v4, pm);
-        if (GUARD) {
-            enqueue(mask, hi4 > w4p, w4p, hi4);
-            if (v4 > pm) {
-#pragma unroll 1
-                for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
-                pm = v4;
-            }
-        } else if (__any_sync(FULL, v4 > w4p)) {
-            // unguarded cells have t >= 4, so pm >= w4p: a new prefix maximum is also a trigger
-            enqueue(FULL, hi4 > w4p, w4p, hi4);
-            if (v4 > pm) {
-#pragma unroll 1
-                for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
-                pm = v4;
-            }
-        }
+        if (__any_sync(mask, GUARD ? (hi4 > w4p || v4 > pm) : (v4 > w4p))) line_ends(mask, w4p, hi4, v4, t);
         // run update for all thresholds, two per instruction
         const uint32_t vvb = v4 * 0x00010001u + 0x64006400u;             // fp16x2 (1024 + 4v, 1024 + 4v)
         const __half2 vv = *(const __half2*)&vvb;
@@ -349,6 +339,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     if (tid < GK) s_rep[tid] = G.rep_k[tid];
     for (int q = tid; q < 3 * SM::agg_one / 4; q += LW) agg_s[q] = 0;
     for (int q = tid; q < 2 * NP * LS; q += LW) sh_s[q] = 0;
+    if (tid < LW / 32) *(uint32_t*)(smem + SM::off_q + tid * SM::QWARP) = 0;
     __syncthreads();
     const int ob = s_ob;
     const int c = (int)(tile - a.tile_start[ob]);
@@ -390,8 +381,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     sc.v1 = sc.v2 = sc.J4;
     sc.w2a = sc.w2b = sc.w2c = sc.J4;
     sc.pm = 0;
-    sc.q = pin(smem_addr(smem + SM::off_q) + 4 * (tid >> 5) * (QCAP * SM::QS));
-    sc.qn = 0;
+    sc.q = pin(smem_addr(smem + SM::off_q) + (tid >> 5) * SM::QWARP);
     sc.lane_lt = (1u << (tid & 31)) - 1u;
 #pragma unroll
     for (int p = 0; p < NP; ++p) sc.run[p] = 0;
@@ -406,8 +396,8 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
         for (; t < 4; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
         for (; t + U <= cnt_lo; t += U) sc.template superstep<false>(t, cnt, ds, Seq{});
         for (; t < cnt_hi; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
-        // lane 0 sits on the warp's longest diagonal, so it took part in every enqueue
-        const uint32_t qn = __shfl_sync(FULL, sc.qn, 0);
+        __syncwarp();
+        const uint32_t qn = lds_u32(sc.q);
         if (qn) flush_queue<SM::QS>(FULL, sc.lane_lt, sc.q, qn, sc.sh, sc.grow, sc.rep, sc.n);
         if (cnt > 0) {
             // runs alive at the end of the chunk, and prefix runs that never ended (the whole chunk)

@@ -9,16 +9,17 @@
 //   cell   : distance d (sliding window over e_i = |y_i - y_{i+o}| for the max norm), then its LEVEL
 //            v = #{distinct thresholds < d} by one table lookup + one exact compare (thresholds are nested:
 //            the cell is recurrent at threshold j iff v <= j).
-//   runs   : the run length of every threshold is carried in packed fp16x2 registers (exact up to 2048):
-//            b = (v <= j) by HSET2.BF / HADD2.SAT on two thresholds at once, run = run*b + b by HFMA2.
+//   runs   : thresholds are nested, so the runs of all thresholds along a diagonal form a monotone stack of
+//            (lowest threshold, start position); it changes only when the maximum level of the last 4 cells
+//            changes, and one popped entry is one line length for a whole RANGE of thresholds, counted in a
+//            difference array over the thresholds.  The work per cell does not depend on K.
 //   lines  : P_j(1), P_j(2), P_j(3) are NOT emitted line by line.  The kernel histograms the level of every
 //            cell and the window maxima of 2 and 3 consecutive levels (thread-private shared-memory columns, no
 //            conflicts); their prefix sums over the level are C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and
 //            Q3_j = sum_{l>=3} (l-2)*P_j(l), from which the finalize kernel solves P_j(1..3) exactly.
-//            Lines of length >= 4 that lie inside a chunk go to a shared-memory histogram (l < 256) or to
-//            global atomics (longer).  Runs touching a chunk border are written as (prefix, suffix) summaries
+//            Lines of length >= 4 that lie inside a chunk go to the shared-memory difference array (l < 128) or
+//            to global atomics (longer).  Runs touching a chunk border are written as (prefix, suffix) summaries
 //            and joined along each diagonal by the stitch kernel.
-#include <cuda_fp16.h>
 
 #include "rqa_tiles.cuh"
 
@@ -26,11 +27,9 @@ namespace rqa {
 
 namespace {
 
-constexpr int LMAX = 1023;       // longest chunk: run lengths stay exact in fp16 and 1024+run has ulp 1
+constexpr int LMAX = 1023;       // longest chunk: cell positions fit the 10 bits of a stack entry, counters 16 bits
 constexpr int LS = 128;          // lines shorter than this are counted in shared memory
 constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
-constexpr int QCAP = 48;         // capacity of a warp's queue of line-end records
-constexpr int QFLUSH = QCAP - 31;  // records that trigger emission (a cell adds at most 32), one record per lane
 
 // Everything the scan needs to know about one group of <= 32 thresholds of one series.
 struct LineGroup {
@@ -143,7 +142,7 @@ __global__ void __launch_bounds__(1024) tile_table_kernel(int64_t n, int L, int 
 
 // ------------------------------------------------------------------------------------------ the scan
 // Cell distances: CellDist (rqa_tiles.cuh) with two warm-up cells before the chunk.
-// Shared-memory plan of the scan kernel (bytes); NP = threshold pairs carried per thread (J <= 2*NP).
+// Shared-memory plan of the scan kernel (bytes); NP: the group has J <= 2*NP distinct thresholds.
 // The two series windows come last because their length depends on the run-time span (m-1)*tau.
 template <int NP>
 struct ScanSmem {
@@ -153,11 +152,10 @@ struct ScanSmem {
     static constexpr int off_agg = off_eps + 4 * (GK + 4);
     static constexpr int agg_row = 4 * (LW / 2);              // one level: 128 words, two 16-bit counters each
     static constexpr int agg_one = NLEV * agg_row;            // one of the three histograms
-    static constexpr int off_sh = off_agg + 3 * agg_one;
-    static constexpr int QS = (NP + 1 + 3) & ~3;              // words per queue record (16-byte vector stores)
-    static constexpr int QWARP = 4 * (QCAP * QS + 4);         // bytes per warp: the record count, then QCAP records
-    static constexpr int off_q = off_sh + 4 * 2 * NP * LS;
-    static constexpr int off_ya = off_q + (LW / 32) * QWARP;
+    static constexpr int off_sh = off_agg + 3 * agg_one;      // int32 D[NLEV][LS]: difference array over the thresholds
+    static constexpr int stk_row = 2 * LW;                    // one stack depth: a 16-bit entry per thread
+    static constexpr int off_stk = off_sh + 4 * NLEV * LS;    // uint16 stack[NLEV][LW]
+    static constexpr int off_ya = off_stk + NLEV * stk_row;
 };
 struct ScanArgs {
     View v;
@@ -166,34 +164,21 @@ struct ScanArgs {
     const uint32_t* tile_start;
     unsigned long long* hist;   // [batch][K][n]
     unsigned long long* agg;    // [batch][NG][3][GK+1]
-    uint16_t* pre;              // [batch][tiles][2*NP][LW]
-    uint32_t* suf;              // [batch][tiles][NP][LW]   raw fp16x2 run registers
+    uint16_t* pre;              // [batch][tiles][2*NP][LW]  prefix run of every threshold (recurrent since the chunk start)
+    uint16_t* suf;              // [batch][tiles][2*NP][LW]  run alive at the chunk end
     uint32_t tiles;
     int m, tau;                 // run-time embedding (used by the M == 0 variant)
 };
 
-// Emit the queued line ends of one warp: record r = (lo4 | hi4 << 8, run registers of the lane that queued it);
-// thresholds j in [lo4/4, hi4/4) each end a line whose length is the fp16 half j of the run registers.
-template <int QS>
-__device__ __forceinline__ void flush_queue(unsigned mask, uint32_t lane_lt, uint32_t q, uint32_t qn, uint32_t sh,
-                                            unsigned long long* grow, const int* rep, int64_t n) {
-    const uint32_t my = __popc(mask & lane_lt), nl = __popc(mask);
-    for (uint32_t r = my; r < qn; r += nl) {
-        const uint32_t rec = q + 16 + 4 * QS * r;
-        const uint32_t w = lds_u32(rec);
-        const uint32_t hi = w >> 10;
-#pragma unroll 1
-        for (uint32_t j = (w & 0xffu) >> 2; j < hi; ++j) {
-            const uint32_t l = (uint32_t)__half2int_rn(__ushort_as_half((unsigned short)lds_u16(rec + 4 + 2 * j)));
-            if (l < (uint32_t)LS) red_u32(sh + 4 * (j * LS + l), 1u);
-            else atomicAdd(&grow[(int64_t)rep[j] * n + l], 1ull);
-        }
-    }
-    __syncwarp(mask);
-    if (my == 0) sts_u32(q, 0u);
-    __syncwarp(mask);
-}
-
+// Run state of one diagonal.  Thresholds are nested, so after a cell of level v exactly the thresholds j >= v are
+// inside a run, and the start of that run does not increase with j: the runs of all thresholds form a monotone stack.
+// Only runs that matter for explicit emission are kept: thresholds j >= A = max(level of the last 4 cells) have a run
+// of >= 4 cells (shorter lines come from the aggregates).  Entry = (lo, start) covers the thresholds [lo, lo of the
+// entry below); the top entry (lo = A) lives in registers, the others in a per-thread shared-memory column as
+// uint16 (start << 6 | lo), bottom-most a sentinel with lo = J.  Cells before the chunk count as level 0, so the
+// initial entry (0, start 0) stands for "recurrent since the chunk start" (prefix runs; start 0 marks them).
+// Per cell the state changes only when A changes: a higher level pops the entries it ends (one line length for a
+// whole range of thresholds -> D[lo][len]++, D[hi][len]--), a lower A pushes one entry.  Cost independent of K.
 template <int NORM, int M, int TAU, int NP>
 struct Scanner : CellDist<NORM, M, TAU, 2> {
     using CD = CellDist<NORM, M, TAU, 2>;
@@ -201,14 +186,17 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     using SM = ScanSmem<NP>;
 
     // per-thread state
-    uint32_t run[NP];           // fp16x2: run lengths of thresholds 2p (low half) and 2p+1 (high half)
-    uint32_t v1, v2;            // 4*level of the previous two cells
-    uint32_t w2a, w2b, w2c;     // max(level pairs) of the previous three cells (newest first)
-    uint32_t pm;                // 4 * running maximum level since the chunk start
+    uint32_t v1, v2;            // 4*level of the previous two cells (real cells, also before the chunk)
+    uint32_t w2a, w2b;          // max(level pairs) of the previous two cells (newest first)
+    uint32_t xa, xb;            // the same with cells before the chunk at level 0 (only used for t < 4)
+    uint32_t A;                 // 4 * lowest threshold in the stack = lo of the top entry (J4: stack empty)
+    uint32_t ts;                // start of the top entry's run (cell index inside the chunk)
+    uint32_t sp;                // entries below the top (the sentinel not counted)
     // per-thread constants
     uint32_t lut, eps;          // shared-window addresses of the bucket table and the thresholds
     uint32_t agg;               // ... of the thread's column of histogram 1, level 0
-    uint32_t sh;                // ... of the short-line histogram
+    uint32_t sh;                // ... of the difference array D
+    uint32_t stk;               // ... of the thread's stack column, depth 0 (the sentinel)
     unsigned long long* grow;   // hist + b*K*n (rows indexed through rep)
     const int* rep;
     uint16_t* pre_out;
@@ -216,8 +204,6 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t inc, J4;
     int multi;
     int64_t n;
-    uint32_t q;                 // ... of this warp's queue of line-end records
-    uint32_t lane_lt;
 
     __device__ __forceinline__ uint32_t level4(float d) const {
         uint32_t idx = __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
@@ -230,34 +216,51 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         return v4;
     }
 
-    // Line ends at one cell (call with the lanes of `mask` converged, when some lane has one).  Lines of length >= 4
-    // that ended at the previous cell, for the thresholds [lo4, hi4) / 4 of this lane: the lane appends one record
-    // (its range and a copy of its run registers) to the warp's queue.  Emission proper happens once QFLUSH records
-    // are queued, one record per lane (flush_queue), so the divergent per-threshold loop runs with most lanes busy
-    // instead of once per warp-cell.  Prefix runs (recurrent since the chunk start) that end here have length t.
-    __device__ __forceinline__ void line_ends(unsigned mask, uint32_t lo4, uint32_t hi4, uint32_t v4, int t) {
-        if (hi4 > lo4) {
-            const uint32_t rec = q + 16 + 4 * SM::QS * atom_u32(q, 1u);
-            sts_v4(rec, lo4 | (hi4 << 8), run[0], NP > 1 ? run[NP > 1 ? 1 : 0] : 0u, NP > 2 ? run[NP > 2 ? 2 : 0] : 0u);
-#pragma unroll
-            for (int p = 3; p < NP; p += 4)
-                sts_v4(rec + 4 + 4 * p, run[p], p + 1 < NP ? run[p + 1 < NP ? p + 1 : 0] : 0u,
-                       p + 2 < NP ? run[p + 2 < NP ? p + 2 : 0] : 0u, p + 3 < NP ? run[p + 3 < NP ? p + 3 : 0] : 0u);
-        }
-        if (v4 > pm) {
+    // One run of `len` cells ended for the thresholds [lo4, hi4) / 4.  start == 0: it began at the chunk start.
+    __device__ __forceinline__ void ended(uint32_t lo4, uint32_t hi4, uint32_t start, uint32_t len) {
+        if (start == 0) {
 #pragma unroll 1
-            for (uint32_t j4 = pm; j4 < v4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)t;
-            pm = v4;
+            for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)len;
+        } else if (len < (uint32_t)LS) {
+            red_u32(sh + lo4 * LS + 4 * len, 1u);
+            red_u32(sh + hi4 * LS + 4 * len, 0xffffffffu);
+        } else {
+#pragma unroll 1
+            for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) atomicAdd(&grow[(int64_t)rep[j4 >> 2] * n + len], 1ull);
         }
-        __syncwarp(mask);
-        const uint32_t qn = lds_u32(q);
-        if (qn >= (uint32_t)QFLUSH) flush_queue<SM::QS>(mask, lane_lt, q, qn, sh, grow, rep, n);
+    }
+
+    // The cell at position t has level v4 > A: the runs of the thresholds [A, v4) ended at the previous cell.
+    __device__ __forceinline__ void pop_runs(uint32_t v4, uint32_t t) {
+        uint32_t lo = A, st = ts;
+#pragma unroll 1
+        for (;;) {
+            const uint32_t e = lds_u16(stk + sp * SM::stk_row);     // the entry below (sp == 0: the sentinel)
+            const uint32_t nlo = (e & 63u) << 2;
+            ended(lo, min(nlo, v4), st, t - st);
+            if (nlo > v4) { A = v4; ts = st; return; }             // the rest of this entry lives on
+            if (sp == 0) { A = J4; return; }                       // everything ended
+            lo = nlo; st = e >> 6; --sp;
+            if (lo == v4) { A = v4; ts = st; return; }
+        }
+    }
+
+    // A_new < A: the thresholds [A_new, A) have just completed 4 cells; their run started at t - 3.
+    __device__ __forceinline__ void push_run(uint32_t a_new, uint32_t t) {
+        if (A < J4) {
+            ++sp;
+            sts_u16(stk + sp * SM::stk_row, (A >> 2) | (ts << 6));
+        }
+        A = a_new;
+        ts = t - 3;
     }
 
     // One cell.  R = ring phase (static), t = position inside the chunk (t < 0: warm-up cells before the chunk),
-    // cnt = this lane's number of cells, GUARD = false in the part of the chunk where every lane is inside.
-    template <int R, bool GUARD>
+    // cnt = this lane's number of cells.  PHASE 0: the first cells of the chunk (t < 4, guarded), 1: the part of the
+    // chunk where every lane is inside (unguarded), 2: the tail (guarded).
+    template <int R, int PHASE>
     __device__ __forceinline__ void cell(int t, int cnt, bool at_diag_start) {
+        constexpr bool GUARD = PHASE != 1;
         CD::template push<R>(t);
         bool live = true, warm = false;
         if (GUARD) { live = t < cnt; warm = t < 0; }
@@ -276,37 +279,44 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         red_u32(agg + v4 * (SM::agg_row / 4), inc);
         red_u32(agg + SM::agg_one + w2 * (SM::agg_row / 4), inc);
         red_u32(agg + 2 * SM::agg_one + w3 * (SM::agg_row / 4), inc);
-        // lines of length >= 4 that end here: thresholds j with max(level of the 4 previous cells) <= j < level.
-        // Unguarded cells have t >= 4, so pm >= w4p: there a new prefix maximum is also such a line end.
-        const uint32_t w4p = max(w2a, w2c);
-        const uint32_t hi4 = min(v4, pm);
-        if (__any_sync(mask, GUARD ? (hi4 > w4p || v4 > pm) : (v4 > w4p))) line_ends(mask, w4p, hi4, v4, t);
-        // run update for all thresholds, two per instruction
-        const uint32_t vvb = v4 * 0x00010001u + 0x64006400u;             // fp16x2 (1024 + 4v, 1024 + 4v)
-        const __half2 vv = *(const __half2*)&vvb;
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-            __half2 bb;
-            if (p % 5 < 3) {                                              // HSET2.BF on the ALU pipe
-                const __half2 kk = __halves2half2(__ushort_as_half((unsigned short)(0x6400 + 8 * p)),
-                                                  __ushort_as_half((unsigned short)(0x6400 + 8 * p + 4)));
-                bb = __hle2(vv, kk);
-            } else {                                                      // HADD2.SAT on the FMA pipe
-                const __half2 kk = __halves2half2(__ushort_as_half((unsigned short)(0x6400 + 8 * p + 4)),
-                                                  __ushort_as_half((unsigned short)(0x6400 + 8 * p + 8)));
-                bb = __hadd2_sat(kk, __hneg2(vv));
-            }
-            __half2 r = *(__half2*)&run[p];
-            r = __hfma2(r, bb, bb);
-            run[p] = *(uint32_t*)&r;
+        // runs of >= 4 cells: A_new = max level of the last 4 cells of the chunk
+        uint32_t x2 = w2;
+        if (PHASE == 0 && t == 0) x2 = v4;
+        const uint32_t a_new = max(x2, PHASE == 0 ? xb : w2b);
+        if (__any_sync(mask, a_new != A)) {
+            if (v4 > A) pop_runs(v4, (uint32_t)t);
+            else if (a_new < A) push_run(a_new, (uint32_t)t);
         }
         v2 = v1; v1 = v4;
-        w2c = w2b; w2b = w2a; w2a = w2;
+        w2b = w2a; w2a = w2;
+        if (PHASE == 0) { xb = xa; xa = x2; }
     }
 
-    template <bool GUARD, int... R>
+    template <int PHASE, int... R>
     __device__ __forceinline__ void superstep(int t, int cnt, bool ds, std::integer_sequence<int, R...>) {
-        (cell<R, GUARD>(t + R, cnt, ds), ...);
+        (cell<R, PHASE>(t + R, cnt, ds), ...);
+    }
+
+    // End of the chunk (cnt > 0 cells): the prefix runs that never ended, and the run alive at the end for every
+    // threshold (from the stack for j >= A/4, else 0..3 cells from the last levels).
+    __device__ __forceinline__ void finish(uint32_t cnt, uint16_t* suf_out) {
+        const uint32_t w3 = max(w2a, w2b);
+#pragma unroll 1
+        for (uint32_t j4 = 0; j4 < min(A, J4); j4 += 4)
+            suf_out[(j4 >> 2) * LW] = (uint16_t)((v1 <= j4) + (w2a <= j4) + (w3 <= j4));
+        uint32_t lo = A, st = ts;
+#pragma unroll 1
+        while (lo < J4) {
+            const uint32_t e = lds_u16(stk + sp * SM::stk_row);
+            const uint32_t nlo = (e & 63u) << 2;
+#pragma unroll 1
+            for (uint32_t j4 = lo; j4 < nlo; j4 += 4) {
+                suf_out[(j4 >> 2) * LW] = (uint16_t)(cnt - st);
+                if (st == 0) pre_out[(j4 >> 2) * LW] = (uint16_t)cnt;
+            }
+            lo = nlo; st = e >> 6;
+            if (sp) --sp;
+        }
     }
 };
 
@@ -333,13 +343,15 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     float* ya_s = (float*)(smem + SM::off_ya);
     float* yb_s = ya_s + LA;
     uint32_t* agg_s = (uint32_t*)(smem + SM::off_agg);
-    uint32_t* sh_s = (uint32_t*)(smem + SM::off_sh);
+    int32_t* sh_s = (int32_t*)(smem + SM::off_sh);
+    uint16_t* stk_s = (uint16_t*)(smem + SM::off_stk);
+    const int J = G.J;
     for (int q = tid; q < NB / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)G.lut)[q];
     if (tid <= GK) eps_s[tid] = G.epsd[tid];
     if (tid < GK) s_rep[tid] = G.rep_k[tid];
     for (int q = tid; q < 3 * SM::agg_one / 4; q += LW) agg_s[q] = 0;
-    for (int q = tid; q < 2 * NP * LS; q += LW) sh_s[q] = 0;
-    if (tid < LW / 32) *(uint32_t*)(smem + SM::off_q + tid * SM::QWARP) = 0;
+    for (int q = tid; q < SM::NLEV * LS; q += LW) sh_s[q] = 0;
+    stk_s[tid] = (uint16_t)J;                                  // the sentinel below every stack
     __syncthreads();
     const int ob = s_ob;
     const int c = (int)(tile - a.tile_start[ob]);
@@ -353,7 +365,6 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     stage_windows(y, ny, s - 2, s - 2 + o0, ya_s, LA, yb_s, LB);
     __syncthreads();
 
-    const int J = G.J;
     const int64_t o = o0 + tid;
     const int64_t len = n - o;                              // cells on this thread's diagonal (may be <= 0)
     int cnt = (int)max((int64_t)0, min((int64_t)L, len - s));
@@ -367,9 +378,11 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     sc.eps = smem_addr(eps_s);
     sc.agg = pin(smem_addr(agg_s) + 4 * (tid & (LW / 2 - 1)));
     sc.sh = smem_addr(sh_s);
+    sc.stk = pin(smem_addr(stk_s) + 2 * tid);
     sc.grow = a.hist + (int64_t)b * a.K * n;
     sc.rep = G.rep_k;                                       // global copy: only read for lines of length >= LS
-    sc.pre_out = a.pre + (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
+    const int64_t out_row = (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
+    sc.pre_out = a.pre + out_row;
     sc.scale = G.scale;
     sc.dcap = G.dcap;
     sc.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
@@ -379,12 +392,9 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     sc.tau = a.tau;
     sc.n = n;
     sc.v1 = sc.v2 = sc.J4;
-    sc.w2a = sc.w2b = sc.w2c = sc.J4;
-    sc.pm = 0;
-    sc.q = pin(smem_addr(smem + SM::off_q) + (tid >> 5) * SM::QWARP);
-    sc.lane_lt = (1u << (tid & 31)) - 1u;
-#pragma unroll
-    for (int p = 0; p < NP; ++p) sc.run[p] = 0;
+    sc.w2a = sc.w2b = sc.J4;
+    sc.xa = sc.xb = 0;
+    sc.A = 0; sc.ts = 0; sc.sp = 0;                          // every threshold: recurrent since the chunk start
 
     if (cnt_hi > 0) {
         sc.prime(-2);                                         // first cell is the warm-up cell t = -2
@@ -392,23 +402,13 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
         constexpr int U = S >= 3 ? S : (S == 2 ? 4 : 4);     // cells per super-step, a multiple of S
         using Seq = std::make_integer_sequence<int, U>;
         int t = -2;
-        // warm-up cells and the first cells of the chunk, guarded (the unguarded cell needs t >= 4)
-        for (; t < 4; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
-        for (; t + U <= cnt_lo; t += U) sc.template superstep<false>(t, cnt, ds, Seq{});
-        for (; t < cnt_hi; t += U) sc.template superstep<true>(t, cnt, ds, Seq{});
-        __syncwarp();
-        const uint32_t qn = lds_u32(sc.q);
-        if (qn) flush_queue<SM::QS>(FULL, sc.lane_lt, sc.q, qn, sc.sh, sc.grow, sc.rep, sc.n);
-        if (cnt > 0) {
-            // runs alive at the end of the chunk, and prefix runs that never ended (the whole chunk)
-            uint32_t* suf_out = a.suf + (((int64_t)b * a.tiles + tile) * NP) * LW + tid;
-#pragma unroll
-            for (int p = 0; p < NP; ++p) suf_out[p * LW] = sc.run[p];
-            for (uint32_t j4 = sc.pm; j4 < sc.J4; j4 += 4) sc.pre_out[(j4 >> 2) * LW] = (uint16_t)cnt;
-        }
+        for (; t < 4; t += U) sc.template superstep<0>(t, cnt, ds, Seq{});   // warm-up cells and t < 4
+        for (; t + U <= cnt_lo; t += U) sc.template superstep<1>(t, cnt, ds, Seq{});
+        for (; t < cnt_hi; t += U) sc.template superstep<2>(t, cnt, ds, Seq{});
+        if (cnt > 0) sc.finish((uint32_t)cnt, a.suf + out_row);
     }
     __syncthreads();
-    // flush: aggregates (sum the 256 private columns of every level) and the short-line histogram
+    // flush: aggregates (sum the 256 private columns of every level) and the short lines (prefix sums of D over j)
     {
         const int warp = tid >> 5, lane = tid & 31;
         unsigned long long* ag = a.agg + ((int64_t)b * a.NG + a.g) * 3 * (GK + 1);
@@ -420,11 +420,11 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
             for (int off = 16; off; off >>= 1) sum += __shfl_down_sync(FULL, sum, off);
             if (lane == 0 && sum && lev <= J) atomicAdd(&ag[h * (GK + 1) + lev], (unsigned long long)sum);
         }
-        for (int q = tid; q < J * LS; q += LW) {
-            uint32_t cnum = sh_s[q];
-            if (cnum) {
-                int j = q / LS, l = q - j * LS;
-                atomicAdd(&sc.grow[(int64_t)s_rep[j] * n + l], (unsigned long long)cnum);
+        for (int l = tid; l < LS; l += LW) {
+            int32_t acc = 0;
+            for (int j = 0; j < J; ++j) {
+                acc += sh_s[j * LS + l];
+                if (acc) atomicAdd(&sc.grow[(int64_t)s_rep[j] * n + l], (unsigned long long)acc);
             }
         }
     }
@@ -440,7 +440,7 @@ struct StitchArgs {
     const uint32_t* tile_start;
     unsigned long long* hist;
     const uint16_t* pre;
-    const uint32_t* suf;
+    const uint16_t* suf;
     uint32_t tiles;
 };
 
@@ -465,9 +465,7 @@ __global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
         } else {
             const uint32_t tot = carry + p;
             if (tot >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[tot], 1ull);
-            const uint32_t w = a.suf[(tile * a.NP + (j >> 1)) * LW + tid];
-            const __half2 h = *(const __half2*)&w;
-            carry = (uint32_t)__half2int_rn((j & 1) ? __high2half(h) : __low2half(h));
+            carry = a.suf[(tile * (2 * a.NP) + j) * LW + tid];
         }
     }
     if (carry >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[carry], 1ull);
@@ -628,7 +626,7 @@ size_t line_workspace_bytes(const View& v, int K) {
     bytes += align_up(sizeof(uint32_t) * ((size_t)p.n_ob + 1));
     bytes += align_up(sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1));
     bytes += align_up(sizeof(uint16_t) * (size_t)v.batch * p.tiles * 2 * p.NP * LW);
-    bytes += align_up(sizeof(uint32_t) * (size_t)v.batch * p.tiles * p.NP * LW);
+    bytes += align_up(sizeof(uint16_t) * (size_t)v.batch * p.tiles * 2 * p.NP * LW);
     return bytes;
 }
 
@@ -649,7 +647,7 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     uint32_t* tile_start = ws.take<uint32_t>((size_t)p.n_ob + 1);
     unsigned long long* agg = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * p.NG * 3 * (GK + 1));
     uint16_t* pre = ws.take<uint16_t>((size_t)v.batch * p.tiles * 2 * p.NP * LW);
-    uint32_t* suf = ws.take<uint32_t>((size_t)v.batch * p.tiles * p.NP * LW);
+    uint16_t* suf = ws.take<uint16_t>((size_t)v.batch * p.tiles * 2 * p.NP * LW);
     if (!ws.ok()) { set_error("rqa_line_hist: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
     RQA_CUDA_TRY(cudaMemsetAsync(agg, 0, sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1), s));
     line_groups_kernel<<<v.batch, 128, 0, s>>>(d_eps, K, p.NG, groups, status);

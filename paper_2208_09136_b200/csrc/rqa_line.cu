@@ -179,7 +179,7 @@ struct ScanArgs {
 // initial entry (0, start 0) stands for "recurrent since the chunk start" (prefix runs; start 0 marks them).
 // Per cell the state changes only when A changes: a higher level pops the entries it ends (one line length for a
 // whole range of thresholds -> D[lo][len]++, D[hi][len]--), a lower A pushes one entry.  Cost independent of K.
-template <int NORM, int M, int TAU, int NP>
+template <int NORM, int M, int TAU, int NP, bool MULTI>
 struct Scanner : CellDist<NORM, M, TAU, 2> {
     using CD = CellDist<NORM, M, TAU, 2>;
     static constexpr int S = CD::S;
@@ -191,18 +191,18 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t xa, xb;            // the same with cells before the chunk at level 0 (only used for t < 4)
     uint32_t A;                 // 4 * lowest threshold in the stack = lo of the top entry (J4: stack empty)
     uint32_t ts;                // start of the top entry's run (cell index inside the chunk)
-    uint32_t sp;                // entries below the top (the sentinel not counted)
+    uint32_t top;               // shared-window address of the entry below the top (stk: the sentinel)
     // per-thread constants
     uint32_t lut, eps;          // shared-window addresses of the bucket table and the thresholds
     uint32_t agg;               // ... of the thread's column of histogram 1, level 0
     uint32_t sh;                // ... of the difference array D
     uint32_t stk;               // ... of the thread's stack column, depth 0 (the sentinel)
+    uint32_t ya_org;            // ... of the i-side window, index 0
     unsigned long long* grow;   // hist + b*K*n (rows indexed through rep)
     const int* rep;
     uint16_t* pre_out;
     float scale, dcap;
     uint32_t inc, J4;
-    int multi;
     int64_t n;
 
     __device__ __forceinline__ uint32_t level4(float d) const {
@@ -210,7 +210,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         uint32_t q = lds_u8(lut + idx);
         float er = lds_f32(eps + q);
         uint32_t v4 = q + (d > er ? 4u : 0u);
-        if (multi) {
+        if (MULTI) {                                           // some bucket holds two or more thresholds
             while (d > lds_f32(eps + v4)) v4 += 4;
         }
         return v4;
@@ -218,12 +218,13 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
 
     // One run of `len` cells ended for the thresholds [lo4, hi4) / 4.  start == 0: it began at the chunk start.
     __device__ __forceinline__ void ended(uint32_t lo4, uint32_t hi4, uint32_t start, uint32_t len) {
-        if (start == 0) {
+        if (start != 0 && len < (uint32_t)LS) {
+            const uint32_t col = sh + 4 * len;
+            red_u32(col + lo4 * LS, 1u);
+            red_u32(col + hi4 * LS, 0xffffffffu);
+        } else if (start == 0) {
 #pragma unroll 1
             for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)len;
-        } else if (len < (uint32_t)LS) {
-            red_u32(sh + lo4 * LS + 4 * len, 1u);
-            red_u32(sh + hi4 * LS + 4 * len, 0xffffffffu);
         } else {
 #pragma unroll 1
             for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) atomicAdd(&grow[(int64_t)rep[j4 >> 2] * n + len], 1ull);
@@ -232,47 +233,49 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
 
     // The cell at position t has level v4 > A: the runs of the thresholds [A, v4) ended at the previous cell.
     __device__ __forceinline__ void pop_runs(uint32_t v4, uint32_t t) {
-        uint32_t lo = A, st = ts;
+        uint32_t e = lds_u16(top);                             // the entry below the top (or the sentinel)
+        uint32_t nlo = (e << 2) & 0xfcu;
+        ended(A, min(nlo, v4), ts, t - ts);
+        A = v4;                                                // the rest of the entry lives on ...
+        if (nlo > v4) return;
 #pragma unroll 1
-        for (;;) {
-            const uint32_t e = lds_u16(stk + sp * SM::stk_row);     // the entry below (sp == 0: the sentinel)
-            const uint32_t nlo = (e & 63u) << 2;
-            ended(lo, min(nlo, v4), st, t - st);
-            if (nlo > v4) { A = v4; ts = st; return; }             // the rest of this entry lives on
-            if (sp == 0) { A = J4; return; }                       // everything ended
-            lo = nlo; st = e >> 6; --sp;
-            if (lo == v4) { A = v4; ts = st; return; }
+        while (top != stk) {                                   // ... unless it ended entirely: next entry
+            top -= SM::stk_row;
+            ts = e >> 6;
+            if (nlo == v4) return;
+            const uint32_t lo = nlo;
+            e = lds_u16(top);
+            nlo = (e << 2) & 0xfcu;
+            ended(lo, min(nlo, v4), ts, t - ts);
+            if (nlo > v4) return;
         }
+        A = J4;                                                // the sentinel is reached: everything ended
     }
 
     // A_new < A: the thresholds [A_new, A) have just completed 4 cells; their run started at t - 3.
     __device__ __forceinline__ void push_run(uint32_t a_new, uint32_t t) {
         if (A < J4) {
-            ++sp;
-            sts_u16(stk + sp * SM::stk_row, (A >> 2) | (ts << 6));
+            top += SM::stk_row;
+            sts_u16(top, (A >> 2) | (ts << 6));
         }
         A = a_new;
         ts = t - 3;
     }
 
-    // One cell.  R = ring phase (static), t = position inside the chunk (t < 0: warm-up cells before the chunk),
-    // cnt = this lane's number of cells.  PHASE 0: the first cells of the chunk (t < 4, guarded), 1: the part of the
-    // chunk where every lane is inside (unguarded), 2: the tail (guarded).
+    // One cell.  R = offset from the cursor = ring phase (static), t = position inside the chunk (t < 0: warm-up
+    // cells before the chunk), cnt = this lane's number of cells.  PHASE 0: the first cells of the chunk (t < 4,
+    // guarded), 1: the part of the chunk where every lane is inside (unguarded; t is not used), 2: the tail (guarded).
     template <int R, int PHASE>
     __device__ __forceinline__ void cell(int t, int cnt, bool at_diag_start) {
         constexpr bool GUARD = PHASE != 1;
-        CD::template push<R>(t);
-        bool live = true, warm = false;
-        if (GUARD) { live = t < cnt; warm = t < 0; }
-        unsigned mask = FULL;
-        if (GUARD) mask = __ballot_sync(FULL, live && !warm);
-        if (GUARD && warm) {
-            uint32_t v4 = at_diag_start ? J4 : level4(CD::template distance<R>(t));
+        CD::template push<R>();
+        if (GUARD && t < 0) {
+            uint32_t v4 = at_diag_start ? J4 : level4(CD::template distance<R>());
             v2 = v1; v1 = v4;
             return;
         }
-        if (GUARD && !live) return;
-        const float d = CD::template distance<R>(t);
+        if (GUARD && t >= cnt) return;
+        const float d = CD::template distance<R>();
         const uint32_t v4 = level4(d);
         // aggregates: level, max of 2, max of 3 consecutive levels (thread-private columns)
         const uint32_t w2 = max(v4, v1), w3 = max(w2, v2);
@@ -283,9 +286,10 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         uint32_t x2 = w2;
         if (PHASE == 0 && t == 0) x2 = v4;
         const uint32_t a_new = max(x2, PHASE == 0 ? xb : w2b);
-        if (__any_sync(mask, a_new != A)) {
-            if (v4 > A) pop_runs(v4, (uint32_t)t);
-            else if (a_new < A) push_run(a_new, (uint32_t)t);
+        if (a_new != A) {
+            const uint32_t tt = PHASE == 1 ? (uint32_t)(CD::position(ya_org) + R) : (uint32_t)t;
+            if (v4 > A) pop_runs(v4, tt);
+            else push_run(a_new, tt);
         }
         v2 = v1; v1 = v4;
         w2b = w2a; w2a = w2;
@@ -295,6 +299,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     template <int PHASE, int... R>
     __device__ __forceinline__ void superstep(int t, int cnt, bool ds, std::integer_sequence<int, R...>) {
         (cell<R, PHASE>(t + R, cnt, ds), ...);
+        CD::advance((int)sizeof...(R));
     }
 
     // End of the chunk (cnt > 0 cells): the prefix runs that never ended, and the run alive at the end for every
@@ -307,24 +312,40 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         uint32_t lo = A, st = ts;
 #pragma unroll 1
         while (lo < J4) {
-            const uint32_t e = lds_u16(stk + sp * SM::stk_row);
-            const uint32_t nlo = (e & 63u) << 2;
+            const uint32_t e = lds_u16(top);
+            const uint32_t nlo = (e << 2) & 0xfcu;
 #pragma unroll 1
             for (uint32_t j4 = lo; j4 < nlo; j4 += 4) {
                 suf_out[(j4 >> 2) * LW] = (uint16_t)(cnt - st);
                 if (st == 0) pre_out[(j4 >> 2) * LW] = (uint16_t)cnt;
             }
             lo = nlo; st = e >> 6;
-            if (sp) --sp;
+            if (top != stk) top -= SM::stk_row;
         }
     }
 };
 
+// The walk of one thread along its chunk.  Two instantiations (MULTI) so that the common case, every bucket of the
+// level table holding at most one threshold, carries no refinement loop; a block executes only one of them.
+template <int NORM, int M, int TAU, int NP, bool MULTI>
+__device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc, int cnt, int cnt_lo, int cnt_hi, bool ds,
+                                           uint32_t yb_org, uint16_t* suf_out) {
+    using SC = Scanner<NORM, M, TAU, NP, MULTI>;
+    constexpr int S = SC::S;
+    constexpr int U = S >= 3 ? S : 4;                        // cells per super-step, a multiple of S
+    using Seq = std::make_integer_sequence<int, U>;
+    int t = -2;                                               // first cell is the warm-up cell t = -2
+    sc.seek(sc.ya_org, yb_org, t);
+    sc.prime();
+    for (; t < 4; t += U) sc.template superstep<0>(t, cnt, ds, Seq{});   // warm-up cells and t < 4
+    for (; t + U <= cnt_lo; t += U) sc.template superstep<1>(t, cnt, ds, Seq{});
+    for (; t < cnt_hi; t += U) sc.template superstep<2>(t, cnt, ds, Seq{});
+    if (cnt > 0) sc.finish((uint32_t)cnt, suf_out);
+}
+
 template <int NORM, int M, int TAU, int NP>
 __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanArgs a) {
-    using SC = Scanner<NORM, M, TAU, NP>;
-    using SM = typename SC::SM;
-    constexpr int S = SC::S;
+    using SM = ScanSmem<NP>;
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;
     __shared__ int s_rep[GK];
@@ -370,42 +391,42 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
     int cnt = (int)max((int64_t)0, min((int64_t)L, len - s));
     const int cnt_hi = __shfl_sync(FULL, cnt, 0);           // the warp's longest lane (smallest o)
     const int cnt_lo = __shfl_sync(FULL, cnt, 31);
-
-    SC sc;
-    sc.ya = smem_addr(ya_s);
-    sc.yb = pin(smem_addr(yb_s) + 4 * tid);
-    sc.lut = smem_addr(lut_s);
-    sc.eps = smem_addr(eps_s);
-    sc.agg = pin(smem_addr(agg_s) + 4 * (tid & (LW / 2 - 1)));
-    sc.sh = smem_addr(sh_s);
-    sc.stk = pin(smem_addr(stk_s) + 2 * tid);
-    sc.grow = a.hist + (int64_t)b * a.K * n;
-    sc.rep = G.rep_k;                                       // global copy: only read for lines of length >= LS
-    const int64_t out_row = (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
-    sc.pre_out = a.pre + out_row;
-    sc.scale = G.scale;
-    sc.dcap = G.dcap;
-    sc.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
-    sc.J4 = 4u * (uint32_t)J;
-    sc.multi = G.multi;
-    sc.m = a.m;
-    sc.tau = a.tau;
-    sc.n = n;
-    sc.v1 = sc.v2 = sc.J4;
-    sc.w2a = sc.w2b = sc.J4;
-    sc.xa = sc.xb = 0;
-    sc.A = 0; sc.ts = 0; sc.sp = 0;                          // every threshold: recurrent since the chunk start
+    unsigned long long* grow = a.hist + (int64_t)b * a.K * n;
 
     if (cnt_hi > 0) {
-        sc.prime(-2);                                         // first cell is the warm-up cell t = -2
-        const bool ds = (s == 0);
-        constexpr int U = S >= 3 ? S : (S == 2 ? 4 : 4);     // cells per super-step, a multiple of S
-        using Seq = std::make_integer_sequence<int, U>;
-        int t = -2;
-        for (; t < 4; t += U) sc.template superstep<0>(t, cnt, ds, Seq{});   // warm-up cells and t < 4
-        for (; t + U <= cnt_lo; t += U) sc.template superstep<1>(t, cnt, ds, Seq{});
-        for (; t < cnt_hi; t += U) sc.template superstep<2>(t, cnt, ds, Seq{});
-        if (cnt > 0) sc.finish((uint32_t)cnt, a.suf + out_row);
+        const int64_t out_row = (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
+        const uint32_t yb_org = pin(smem_addr(yb_s) + 4 * tid);
+        auto setup = [&](auto& sc) {
+            sc.ya_org = smem_addr(ya_s);
+            sc.lut = smem_addr(lut_s);
+            sc.eps = smem_addr(eps_s);
+            sc.agg = pin(smem_addr(agg_s) + 4 * (tid & (LW / 2 - 1)));
+            sc.sh = smem_addr(sh_s);
+            sc.stk = pin(smem_addr(stk_s) + 2 * tid);
+            sc.grow = grow;
+            sc.rep = G.rep_k;                               // global copy: only read for lines of length >= LS
+            sc.pre_out = a.pre + out_row;
+            sc.scale = G.scale;
+            sc.dcap = G.dcap;
+            sc.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
+            sc.J4 = 4u * (uint32_t)J;
+            sc.m = a.m;
+            sc.tau = a.tau;
+            sc.n = n;
+            sc.v1 = sc.v2 = sc.J4;
+            sc.w2a = sc.w2b = sc.J4;
+            sc.xa = sc.xb = 0;
+            sc.A = 0; sc.ts = 0; sc.top = sc.stk;           // every threshold: recurrent since the chunk start
+        };
+        if (G.multi) {
+            Scanner<NORM, M, TAU, NP, true> sc;
+            setup(sc);
+            scan_chunk(sc, cnt, cnt_lo, cnt_hi, s == 0, yb_org, a.suf + out_row);
+        } else {
+            Scanner<NORM, M, TAU, NP, false> sc;
+            setup(sc);
+            scan_chunk(sc, cnt, cnt_lo, cnt_hi, s == 0, yb_org, a.suf + out_row);
+        }
     }
     __syncthreads();
     // flush: aggregates (sum the 256 private columns of every level) and the short lines (prefix sums of D over j)
@@ -424,7 +445,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
             int32_t acc = 0;
             for (int j = 0; j < J; ++j) {
                 acc += sh_s[j * LS + l];
-                if (acc) atomicAdd(&sc.grow[(int64_t)s_rep[j] * n + l], (unsigned long long)acc);
+                if (acc) atomicAdd(&grow[(int64_t)s_rep[j] * n + l], (unsigned long long)acc);
             }
         }
     }

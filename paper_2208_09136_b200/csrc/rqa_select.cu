@@ -349,9 +349,9 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
 
     template <int R, bool GUARD>
     __device__ __forceinline__ void cell(int t, int cnt) {
-        CD::template push<R>(t);
+        CD::template push<R>();
         const bool live = !GUARD || t < cnt;
-        const float d = CD::template distance<R>(t);
+        const float d = CD::template distance<R>();
         uint32_t q = lds_u16(lut + 2 * bucket_of(d, dcap, scale));
         while (d > lds_f32(beta + 4 * q)) ++q;
         if (live) red_u32(cols + q * CountSmem::col_row, inc);
@@ -408,8 +408,7 @@ __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev)
     const int cnt_lo = __shfl_sync(FULL, cnt, 31);
 
     CT ct;
-    ct.ya = smem_addr(ya_s);
-    ct.yb = pin(smem_addr(yb_s) + 4 * tid);
+    ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid), 0);
     ct.m = a.m;
     ct.tau = a.tau;
     ct.lut = smem_addr(lut_s);
@@ -425,12 +424,12 @@ __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev)
     ct.wcount = 0;
     ct.lane_lt = (1u << (tid & 31)) - 1u;
     if (cnt_hi > 0) {
-        ct.prime(0);
+        ct.prime();
         constexpr int U = S >= 3 ? S : 4;                     // cells per super-step, a multiple of S
         using Seq = std::make_integer_sequence<int, U>;
         int t = 0;
-        for (; t + U <= cnt_lo; t += U) ct.template superstep<false>(t, cnt, Seq{});
-        for (; t < cnt_hi; t += U) ct.template superstep<true>(t, cnt, Seq{});
+        for (; t + U <= cnt_lo; t += U) { ct.template superstep<false>(t, cnt, Seq{}); ct.advance(U); }
+        for (; t < cnt_hi; t += U) { ct.template superstep<true>(t, cnt, Seq{}); ct.advance(U); }
         if (ct.wcount) ct.flush_warp();
     }
     __syncthreads();

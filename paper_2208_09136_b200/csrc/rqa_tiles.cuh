@@ -97,36 +97,48 @@ __device__ __forceinline__ void stage_windows(const float* __restrict__ y, int64
 // Cell distances along one diagonal from the staged windows.  W = warm-up cells before the chunk (cell t of the
 // chunk reads window index t + W).  M > 0: compile-time (M, TAU), sliding window over a register ring of
 // S = (M-1)*TAU + 1 elements.  M == 0: run-time (m, tau), recomputed from the windows for every cell.
+// The two window addresses are CURSORS: they point at the element of the first cell of the current super-step
+// (seek / advance), so that every access inside a super-step is cursor + a compile-time offset.
 template <int NORM, int M, int TAU, int W>
 struct CellDist {
     static constexpr int S = M > 0 ? (M - 1) * TAU + 1 : 1;
     float ring[S];
-    uint32_t ya;                // shared-window address of the i-side window
+    uint32_t ya;                // shared-window address of the i-side window element of cell t0
     uint32_t yb;                // ... of the j-side window, already offset by the thread's diagonal
     int m, tau;
 
+    // ya_org, yb_org: addresses of window index 0 (cell -W); afterwards the cursors stand at cell t0
+    __device__ __forceinline__ void seek(uint32_t ya_org, uint32_t yb_org, int t0) {
+        ya = ya_org + 4 * (t0 + W);
+        yb = yb_org + 4 * (t0 + W);
+    }
+    __device__ __forceinline__ void advance(int cells) { ya += 4 * cells; yb += 4 * cells; }
+    // cell t0 of the current super-step, given the address of window index 0
+    __device__ __forceinline__ int position(uint32_t ya_org) const { return (int)((ya - ya_org) >> 2) - W; }
+
+    // element x cells after the cursor
     __device__ __forceinline__ float elem(int x) const {
         // max norm: the signed difference is kept, |.| is an operand modifier of the maximum in distance()
         float diff = __fsub_rn(lds_f32(ya + 4 * x), lds_f32(yb + 4 * x));
         return NORM == RQA_NORM_MAX ? diff : __fmul_rn(diff, diff);
     }
-    // Before the first cell t_first (which must be processed at ring phase R = 0) the ring holds e_t .. e_{t+S-2}.
-    __device__ __forceinline__ void prime(int t_first) {
+    // Before the first cell (cursor on it; it must be processed at ring phase R = 0) the ring holds e_t .. e_{t+S-2}.
+    __device__ __forceinline__ void prime() {
 #pragma unroll
-        for (int x = 0; x < (M > 0 ? S - 1 : 0); ++x) ring[x] = elem(t_first + W + x);
+        for (int x = 0; x < (M > 0 ? S - 1 : 0); ++x) ring[x] = elem(x);
     }
-    // R = ring phase of cell t (number of cells since t_first, mod S; static); pushes e_{t+S-1}
+    // R = offset of the cell from the cursor = its ring phase (static); pushes e_{t+S-1}
     template <int R>
-    __device__ __forceinline__ void push(int t) {
-        if (M > 0) ring[(R + S - 1) % S] = elem(t + W + S - 1);
+    __device__ __forceinline__ void push() {
+        if (M > 0) ring[(R + S - 1) % S] = elem(R + S - 1);
     }
     template <int R>
-    __device__ __forceinline__ float distance(int t) const {
+    __device__ __forceinline__ float distance() const {
         if (M == 0) {
-            float d = elem(t + W);
+            float d = elem(R);
             if (NORM == RQA_NORM_MAX) d = fabsf(d);
             for (int c = 1; c < m; ++c) {
-                float x = elem(t + W + c * tau);
+                float x = elem(R + c * tau);
                 d = NORM == RQA_NORM_MAX ? fmaxf(d, fabsf(x)) : __fadd_rn(d, x);
             }
             return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);

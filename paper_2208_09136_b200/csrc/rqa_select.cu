@@ -21,6 +21,7 @@
 //            targets resolved in each pass; targets that share a prefix share one 256-bin histogram.
 #include <algorithm>
 #include <cmath>
+#include <type_traits>
 
 #include "rqa_tiles.cuh"
 
@@ -31,6 +32,7 @@ namespace {
 constexpr int BT = 64;                // targets per buffer-select call
 constexpr int NLEV_MAX = 2 * GK + 1;  // levels of the counting pass: 2 boundaries per bracket
 constexpr int WCAP = 256;             // candidates a warp buffers in shared memory before flushing
+constexpr int NBS = 2 * NB;           // buckets of the counting pass' level table (one byte each)
 constexpr double BRACKET_SIGMAS = 4.5;
 
 // ------------------------------------------------------------------------------------------ per-series state
@@ -62,10 +64,10 @@ struct Ranks64 {
 // bracket boundaries of one group of <= GK targets of one series (the counting pass's level table)
 struct SelTable {
     int32_t J;                        // boundaries in use (even), levels 0..J
-    int32_t pad;
+    int32_t multi;                    // 1 if some bucket holds two or more boundaries (refine by a loop)
     float scale, dcap;
     float beta[2 * GK + 4];           // ascending, beta[J..] = +inf
-    uint16_t lut[NB];                 // bucket -> #{boundaries in lower buckets}
+    uint8_t lut[NBS];                 // bucket -> #{boundaries in lower buckets}
 };
 
 struct SampleRanks {                  // per target of the group: sample ranks of the bracket ends (0 = open end)
@@ -284,22 +286,29 @@ __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict
         float dcap = fmaxb >= 3.0e38f ? 3.4028234e38f : nextafterf(fmaxb, INF);
         if (!(dcap > 0.0f)) dcap = 1.0e-30f;
         s_dcap = dcap;
-        s_scale = bucket_scale(dcap);
+        s_scale = bucket_scale(dcap, NBS);
         s_J = J;
-        T.J = J; T.pad = 0; T.scale = s_scale; T.dcap = dcap;
+        T.J = J; T.scale = s_scale; T.dcap = dcap;
     }
     __syncthreads();
     const int J = s_J;
     for (int q = threadIdx.x; q < 2 * GK + 4; q += blockDim.x) T.beta[q] = s_beta[q];
-    for (int q = threadIdx.x; q < NB; q += blockDim.x) {
-        int below = 0;
+    int multi = 0;
+    for (int q = threadIdx.x; q < NBS; q += blockDim.x) {
+        int below = 0, inside = 0;
         for (int j = 0; j < J; ++j) {
             const float x = s_beta[j];
             // negative boundary: below every bucket; +inf: in the top bucket (never exceeded anyway)
-            below += x < 0.0f ? 1 : (bucket_of(x, s_dcap, s_scale) < (uint32_t)q);
+            const bool neg = x < 0.0f;
+            const uint32_t bj = neg ? 0u : bucket_of(x, s_dcap, s_scale);
+            below += neg ? 1 : (bj < (uint32_t)q);
+            inside += !neg && bj == (uint32_t)q;
         }
-        T.lut[q] = (uint16_t)below;
+        T.lut[q] = (uint8_t)below;
+        multi |= inside > 1;
     }
+    multi = __syncthreads_or(multi);
+    if (threadIdx.x == 0) T.multi = multi;
 }
 
 // ------------------------------------------------------------------------------------------ counting pass
@@ -315,14 +324,14 @@ struct CountArgs {
 };
 
 struct CountSmem {
-    static constexpr int off_lut = 0;                                   // uint16[NB]
-    static constexpr int off_beta = off_lut + 2 * NB;                   // float[2*GK+4]
+    static constexpr int off_lut = 0;                                   // uint8[NBS]
+    static constexpr int off_beta = off_lut + NBS;                      // float[2*GK+4]
     static constexpr int off_cand = off_beta + 4 * (2 * GK + 4);        // float[LW/32][WCAP]
     static constexpr int off_cols = off_cand + 4 * (LW / 32) * WCAP;    // uint32[nlev][LW/2]
     static constexpr int col_row = 4 * (LW / 2);
 };
 
-template <int NORM, int M, int TAU>
+template <int NORM, int M, int TAU, bool MULTI>
 struct Counter : CellDist<NORM, M, TAU, 0> {
     using CD = CellDist<NORM, M, TAU, 0>;
     uint32_t lut, beta;               // shared-window addresses of the bucket table and the boundaries
@@ -352,8 +361,11 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
         CD::template push<R>();
         const bool live = !GUARD || t < cnt;
         const float d = CD::template distance<R>();
-        uint32_t q = lds_u16(lut + 2 * bucket_of(d, dcap, scale));
-        while (d > lds_f32(beta + 4 * q)) ++q;
+        uint32_t q = lds_u8(lut + bucket_of(d, dcap, scale));
+        q += d > lds_f32(beta + 4 * q) ? 1u : 0u;
+        if (MULTI) {                                          // some bucket holds two or more boundaries
+            while (d > lds_f32(beta + 4 * q)) ++q;
+        }
         if (live) red_u32(cols + q * CountSmem::col_row, inc);
         const unsigned mc = __ballot_sync(FULL, live && (q & 1u));
         if (mc) {
@@ -371,8 +383,6 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
 
 template <int NORM, int M, int TAU>
 __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev) {
-    using CT = Counter<NORM, M, TAU>;
-    constexpr int S = CT::S;
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;
     const int tid = threadIdx.x, b = blockIdx.y;
@@ -380,7 +390,7 @@ __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev)
     const uint32_t tile = blockIdx.x;
     const SelTable& T = a.tabs[b];
     find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
-    uint16_t* lut_s = (uint16_t*)(smem + CountSmem::off_lut);
+    uint8_t* lut_s = (uint8_t*)(smem + CountSmem::off_lut);
     float* beta_s = (float*)(smem + CountSmem::off_beta);
     float* cand_s = (float*)(smem + CountSmem::off_cand);
     uint32_t* cols_s = (uint32_t*)(smem + CountSmem::off_cols);
@@ -388,7 +398,7 @@ __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev)
     const int LA = window_la(a.L, span, 0), LB = window_lb(a.L, span, 0);
     float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * CountSmem::col_row);
     float* yb_s = ya_s + LA;
-    for (int q = tid; q < NB / 2; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)T.lut)[q];
+    for (int q = tid; q < NBS / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)T.lut)[q];
     if (tid < 2 * GK + 4) beta_s[tid] = T.beta[tid];
     for (int q = tid; q < nlev * (LW / 2); q += LW) cols_s[q] = 0;
     __syncthreads();
@@ -407,30 +417,41 @@ __global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev)
     const int cnt_hi = __shfl_sync(FULL, cnt, 0);
     const int cnt_lo = __shfl_sync(FULL, cnt, 31);
 
-    CT ct;
-    ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid), 0);
-    ct.m = a.m;
-    ct.tau = a.tau;
-    ct.lut = smem_addr(lut_s);
-    ct.beta = smem_addr(beta_s);
-    ct.cols = pin(smem_addr(cols_s) + 4 * (tid & (LW / 2 - 1)));
-    ct.wbuf = cand_s + (tid >> 5) * WCAP;
-    ct.gcand = a.cand + (unsigned long long)b * a.cap;
-    ct.gncand = &a.ss[b].ncand;
-    ct.cap = a.cap;
-    ct.scale = T.scale;
-    ct.dcap = T.dcap;
-    ct.inc = tid < LW / 2 ? 1u : 0x10000u;
-    ct.wcount = 0;
-    ct.lane_lt = (1u << (tid & 31)) - 1u;
     if (cnt_hi > 0) {
-        ct.prime();
-        constexpr int U = S >= 3 ? S : 4;                     // cells per super-step, a multiple of S
-        using Seq = std::make_integer_sequence<int, U>;
-        int t = 0;
-        for (; t + U <= cnt_lo; t += U) { ct.template superstep<false>(t, cnt, Seq{}); ct.advance(U); }
-        for (; t < cnt_hi; t += U) { ct.template superstep<true>(t, cnt, Seq{}); ct.advance(U); }
-        if (ct.wcount) ct.flush_warp();
+        // two instantiations: the common case (no bucket with two boundaries) carries no refinement loop
+        auto walk = [&](auto& ct) {
+            using CT = std::remove_reference_t<decltype(ct)>;
+            constexpr int S = CT::S;
+            ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid), 0);
+            ct.m = a.m;
+            ct.tau = a.tau;
+            ct.lut = smem_addr(lut_s);
+            ct.beta = smem_addr(beta_s);
+            ct.cols = pin(smem_addr(cols_s) + 4 * (tid & (LW / 2 - 1)));
+            ct.wbuf = cand_s + (tid >> 5) * WCAP;
+            ct.gcand = a.cand + (unsigned long long)b * a.cap;
+            ct.gncand = &a.ss[b].ncand;
+            ct.cap = a.cap;
+            ct.scale = T.scale;
+            ct.dcap = T.dcap;
+            ct.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
+            ct.wcount = 0;
+            ct.lane_lt = (1u << (tid & 31)) - 1u;
+            ct.prime();
+            constexpr int U = S >= 3 ? S : 4;                 // cells per super-step, a multiple of S
+            using Seq = std::make_integer_sequence<int, U>;
+            int t = 0;
+            for (; t + U <= cnt_lo; t += U) { ct.template superstep<false>(t, cnt, Seq{}); ct.advance(U); }
+            for (; t < cnt_hi; t += U) { ct.template superstep<true>(t, cnt, Seq{}); ct.advance(U); }
+            if (ct.wcount) ct.flush_warp();
+        };
+        if (T.multi) {
+            Counter<NORM, M, TAU, true> ct;
+            walk(ct);
+        } else {
+            Counter<NORM, M, TAU, false> ct;
+            walk(ct);
+        }
     }
     __syncthreads();
     {

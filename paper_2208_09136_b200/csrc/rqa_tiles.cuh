@@ -32,11 +32,11 @@ __device__ __forceinline__ uint32_t bucket_of(float d, float dcap, float scale) 
     return __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
 }
 
-// Largest scale for which bucket_of(dcap) <= NB-1.
-__device__ inline float bucket_scale(float dcap) {
-    double sc = ((double)NB - 1.5) * 1.401298464324817e-45 / (double)dcap;   // (NB-1.5) * 2^-149 / dcap
+// Largest scale for which bucket_of(dcap) <= nb-1.
+__device__ inline float bucket_scale(float dcap, int nb = NB) {
+    double sc = ((double)nb - 1.5) * 1.401298464324817e-45 / (double)dcap;   // (nb-1.5) * 2^-149 / dcap
     float scale = sc > 3.0e38 ? 3.0e38f : (float)sc;
-    while (scale > 0.0f && bucket_of(dcap, dcap, scale) > (uint32_t)(NB - 1)) scale = nextafterf(scale, 0.0f);
+    while (scale > 0.0f && bucket_of(dcap, dcap, scale) > (uint32_t)(nb - 1)) scale = nextafterf(scale, 0.0f);
     return scale;
 }
 

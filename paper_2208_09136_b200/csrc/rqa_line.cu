@@ -403,7 +403,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
             sc.agg = pin(smem_addr(agg_s) + 4 * (tid & (LW / 2 - 1)));
             sc.sh = smem_addr(sh_s);
             sc.stk = pin(smem_addr(stk_s) + 2 * tid);
-            sc.grow = grow;
+            sc.grow = (unsigned long long*)pin64((unsigned long long)grow);   // kept in registers, not re-read per cell
             sc.rep = G.rep_k;                               // global copy: only read for lines of length >= LS
             sc.pre_out = a.pre + out_row;
             sc.scale = G.scale;
@@ -412,7 +412,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanA
             sc.J4 = 4u * (uint32_t)J;
             sc.m = a.m;
             sc.tau = a.tau;
-            sc.n = n;
+            sc.n = (int64_t)pin64((unsigned long long)n);
             sc.v1 = sc.v2 = sc.J4;
             sc.w2a = sc.w2b = sc.J4;
             sc.xa = sc.xb = 0;

@@ -57,6 +57,7 @@ inline uint64_t count_tiles(int64_t n, int L) {
 // pin(): an identity shuffle (call it with the whole warp converged).  ptxas lowers a shared symbol's address to
 // S2R SR_CgaCtaId + LEA and, being "cheap", rematerialises that per use inside the loop; a shuffle result is kept.
 __device__ __forceinline__ uint32_t pin(uint32_t x) { return __shfl_sync(0xffffffffu, x, threadIdx.x & 31); }
+__device__ __forceinline__ unsigned long long pin64(unsigned long long x) { return __shfl_sync(0xffffffffu, x, threadIdx.x & 31); }
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return pin((uint32_t)__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }

@@ -344,7 +344,7 @@ __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc,
 }
 
 template <int NORM, int M, int TAU, int NP>
-__global__ void __launch_bounds__(LW, (NP <= 10 ? 3 : 2)) line_scan_kernel(ScanArgs a) {
+__global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanArgs a) {
     using SM = ScanSmem<NP>;
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;

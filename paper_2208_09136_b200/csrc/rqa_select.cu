@@ -382,7 +382,7 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
 };
 
 template <int NORM, int M, int TAU>
-__global__ void __launch_bounds__(LW, 3) sel_count_kernel(CountArgs a, int nlev) {
+__global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev) {
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;
     const int tid = threadIdx.x, b = blockIdx.y;

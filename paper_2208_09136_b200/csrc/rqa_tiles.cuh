@@ -20,7 +20,7 @@
 
 namespace rqa {
 
-constexpr int LW = 256;          // diagonals per tile = threads per block
+constexpr int LW = 512;          // diagonals per tile = threads per block
 constexpr int NB = 4096;         // buckets of a level look-up table
 constexpr int GK = 32;           // thresholds (or brackets) per group = per full pass
 constexpr int MAX_SPAN = 4096;   // largest (m-1)*tau the tiled kernels stage in shared memory

@@ -14,8 +14,8 @@
 //            changes, and one popped entry is one line length for a whole RANGE of thresholds, counted in a
 //            difference array over the thresholds.  The work per cell does not depend on K.
 //   lines  : P_j(1), P_j(2), P_j(3) are NOT emitted line by line.  The kernel histograms the level of every
-//            cell and the window maxima of 2 and 3 consecutive levels (thread-private shared-memory columns, no
-//            conflicts); their prefix sums over the level are C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and
+//            cell and the window maxima of 2 and 3 consecutive levels (thread-private shared-memory words of three
+//            10-bit counters, no conflicts; a chunk has <= 1023 cells); their prefix sums over the level are C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and
 //            Q3_j = sum_{l>=3} (l-2)*P_j(l), from which the finalize kernel solves P_j(1..3) exactly.
 //            Lines of length >= 4 that lie inside a chunk go to the shared-memory difference array (l < 128) or
 //            to global atomics (longer).  Runs touching a chunk border are written as (prefix, suffix) summaries
@@ -30,6 +30,7 @@ namespace {
 constexpr int LMAX = 1023;       // longest chunk: cell positions fit the 10 bits of a stack entry, counters 16 bits
 constexpr int LS = 128;          // lines shorter than this are counted in shared memory
 constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
+constexpr int QCELLS = 24;       // cells between two drains of the per-thread event queues (= their capacity)
 
 // Everything the scan needs to know about one group of <= 32 thresholds of one series.
 struct LineGroup {
@@ -150,12 +151,12 @@ struct ScanSmem {
     static constexpr int off_lut = 0;
     static constexpr int off_eps = off_lut + NB;
     static constexpr int off_agg = off_eps + 4 * (GK + 4);
-    static constexpr int agg_row = 4 * (LW / 2);              // one level: 128 words, two 16-bit counters each
-    static constexpr int agg_one = NLEV * agg_row;            // one of the three histograms
-    static constexpr int off_sh = off_agg + 3 * agg_one;      // int32 D[NLEV][LS]: difference array over the thresholds
+    static constexpr int agg_row = 4 * LW;                    // one level: a word per thread = three 10-bit counters
+    static constexpr int off_sh = off_agg + NLEV * agg_row;   // int32 D[NLEV][LS]: difference array over the thresholds
     static constexpr int stk_row = 2 * LW;                    // one stack depth: a 16-bit entry per thread
     static constexpr int off_stk = off_sh + 4 * NLEV * LS;    // uint16 stack[NLEV][LW]
-    static constexpr int off_ya = off_stk + NLEV * stk_row;
+    static constexpr int off_q = off_stk + NLEV * stk_row;    // uint16 queue[QCELLS][LW]: deferred stack events
+    static constexpr int off_ya = off_q + QCELLS * stk_row;
 };
 struct ScanArgs {
     View v;
@@ -192,17 +193,21 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t A;                 // 4 * lowest threshold in the stack = lo of the top entry (J4: stack empty)
     uint32_t ts;                // start of the top entry's run (cell index inside the chunk)
     uint32_t top;               // shared-window address of the entry below the top (stk: the sentinel)
+    uint32_t aprev;             // phase 1: 4 * max level of the 4 cells before this one (A lags until the drain)
+    uint32_t qp;                // phase 1: shared-window address of the thread's next free queue slot
+    uint32_t trel8;             // phase 1: (cells since the last drain) << 8
     // per-thread constants
     uint32_t lut, eps;          // shared-window addresses of the bucket table and the thresholds
     uint32_t agg;               // ... of the thread's column of histogram 1, level 0
     uint32_t sh;                // ... of the difference array D
     uint32_t stk;               // ... of the thread's stack column, depth 0 (the sentinel)
+    uint32_t q0;                // ... of the thread's event queue, slot 0
     uint32_t ya_org;            // ... of the i-side window, index 0
     unsigned long long* grow;   // hist + b*K*n (rows indexed through rep)
     const int* rep;
     uint16_t* pre_out;
     float scale, dcap;
-    uint32_t inc, J4;
+    uint32_t J4;
     int64_t n;
 
     __device__ __forceinline__ uint32_t level4(float d) const {
@@ -279,27 +284,57 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         const uint32_t v4 = level4(d);
         // aggregates: level, max of 2, max of 3 consecutive levels (thread-private columns)
         const uint32_t w2 = max(v4, v1), w3 = max(w2, v2);
-        red_u32(agg + v4 * (SM::agg_row / 4), inc);
-        red_u32(agg + SM::agg_one + w2 * (SM::agg_row / 4), inc);
-        red_u32(agg + 2 * SM::agg_one + w3 * (SM::agg_row / 4), inc);
-        // runs of >= 4 cells: A_new = max level of the last 4 cells of the chunk
-        uint32_t x2 = w2;
-        if (PHASE == 0 && t == 0) x2 = v4;
-        const uint32_t a_new = max(x2, PHASE == 0 ? xb : w2b);
-        if (a_new != A) {
-            const uint32_t tt = PHASE == 1 ? (uint32_t)(CD::position(ya_org) + R) : (uint32_t)t;
-            if (v4 > A) pop_runs(v4, tt);
-            else push_run(a_new, tt);
+        red_u32(agg + v4 * (SM::agg_row / 4), 1u);
+        red_u32(agg + w2 * (SM::agg_row / 4), 1u << 10);
+        red_u32(agg + w3 * (SM::agg_row / 4), 1u << 20);
+        // runs of >= 4 cells: A_new = max level of the last 4 cells of the chunk.  The stack changes only when it
+        // differs from the previous cell's.  Phase 1 does not touch the stack: the thread notes (cell, A_new) in its
+        // queue and all lanes replay their queues together every QCELLS cells (drain), so that the divergent stack
+        // code runs with most lanes busy instead of for one or two lanes per warp-cell.
+        if (PHASE == 1) {
+            const uint32_t a_new = max(w2, w2b);
+            if (a_new != aprev) {
+                sts_u16(qp, a_new + trel8 + ((uint32_t)R << 8));
+                qp += SM::stk_row;
+            }
+            aprev = a_new;
+        } else {
+            uint32_t x2 = w2;
+            if (PHASE == 0 && t == 0) x2 = v4;
+            const uint32_t a_new = max(x2, PHASE == 0 ? xb : w2b);
+            if (a_new != A) {
+                if (v4 > A) pop_runs(v4, (uint32_t)t);
+                else push_run(a_new, (uint32_t)t);
+            }
+            if (PHASE == 0) { xb = xa; xa = x2; }
         }
         v2 = v1; v1 = v4;
         w2b = w2a; w2a = w2;
-        if (PHASE == 0) { xb = xa; xa = x2; }
+    }
+
+    // Replay the queued events of the window that started at cell win_t0 (call with the warp converged).
+    __device__ __forceinline__ void drain(uint32_t win_t0) {
+        const uint32_t nmax = __reduce_max_sync(FULL, qp - q0);
+        uint32_t rp = q0;
+#pragma unroll 1
+        for (uint32_t k = 0; k < nmax; k += SM::stk_row) {
+            if (rp < qp) {
+                const uint32_t rec = lds_u16(rp);
+                const uint32_t a_new = rec & 0xffu, t = win_t0 + (rec >> 8);
+                if (a_new > A) pop_runs(a_new, t);            // a higher level: A_new is that level
+                else push_run(a_new, t);
+                rp += SM::stk_row;
+            }
+        }
+        qp = q0;
+        trel8 = 0;
     }
 
     template <int PHASE, int... R>
     __device__ __forceinline__ void superstep(int t, int cnt, bool ds, std::integer_sequence<int, R...>) {
         (cell<R, PHASE>(t + R, cnt, ds), ...);
         CD::advance((int)sizeof...(R));
+        if (PHASE == 1) trel8 += (uint32_t)sizeof...(R) << 8;
     }
 
     // End of the chunk (cnt > 0 cells): the prefix runs that never ended, and the run alive at the end for every
@@ -338,7 +373,16 @@ __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc,
     sc.seek(sc.ya_org, yb_org, t);
     sc.prime();
     for (; t < 4; t += U) sc.template superstep<0>(t, cnt, ds, Seq{});   // warm-up cells and t < 4
-    for (; t + U <= cnt_lo; t += U) sc.template superstep<1>(t, cnt, ds, Seq{});
+    constexpr int SPW = QCELLS / U;                          // super-steps per drain window
+    sc.aprev = sc.A;
+    sc.qp = sc.q0;
+    sc.trel8 = 0;
+    while (t + U <= cnt_lo) {
+        const int t0w = t;
+#pragma unroll 1
+        for (int w = 0; w < SPW && t + U <= cnt_lo; ++w, t += U) sc.template superstep<1>(t, cnt, ds, Seq{});
+        sc.drain((uint32_t)t0w);
+    }
     for (; t < cnt_hi; t += U) sc.template superstep<2>(t, cnt, ds, Seq{});
     if (cnt > 0) sc.finish((uint32_t)cnt, suf_out);
 }
@@ -370,7 +414,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
     for (int q = tid; q < NB / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)G.lut)[q];
     if (tid <= GK) eps_s[tid] = G.epsd[tid];
     if (tid < GK) s_rep[tid] = G.rep_k[tid];
-    for (int q = tid; q < 3 * SM::agg_one / 4; q += LW) agg_s[q] = 0;
+    for (int q = tid; q < SM::NLEV * LW; q += LW) agg_s[q] = 0;
     for (int q = tid; q < SM::NLEV * LS; q += LW) sh_s[q] = 0;
     stk_s[tid] = (uint16_t)J;                                  // the sentinel below every stack
     __syncthreads();
@@ -400,15 +444,15 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
             sc.ya_org = smem_addr(ya_s);
             sc.lut = smem_addr(lut_s);
             sc.eps = smem_addr(eps_s);
-            sc.agg = pin(smem_addr(agg_s) + 4 * (tid & (LW / 2 - 1)));
+            sc.agg = pin(smem_addr(agg_s) + 4 * tid);
             sc.sh = smem_addr(sh_s);
             sc.stk = pin(smem_addr(stk_s) + 2 * tid);
+            sc.q0 = pin(smem_addr(smem + SM::off_q) + 2 * tid);
             sc.grow = (unsigned long long*)pin64((unsigned long long)grow);   // kept in registers, not re-read per cell
             sc.rep = G.rep_k;                               // global copy: only read for lines of length >= LS
             sc.pre_out = a.pre + out_row;
             sc.scale = G.scale;
             sc.dcap = G.dcap;
-            sc.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
             sc.J4 = 4u * (uint32_t)J;
             sc.m = a.m;
             sc.tau = a.tau;
@@ -433,13 +477,20 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
     {
         const int warp = tid >> 5, lane = tid & 31;
         unsigned long long* ag = a.agg + ((int64_t)b * a.NG + a.g) * 3 * (GK + 1);
-        for (int row = warp; row < 3 * SM::NLEV; row += LW / 32) {
-            const int h = row / SM::NLEV, lev = row - h * SM::NLEV;
-            const uint32_t* r = agg_s + row * (LW / 2);
-            uint32_t sum = 0;
-            for (int q = lane; q < LW / 2; q += 32) { uint32_t w = r[q]; sum += (w & 0xffffu) + (w >> 16); }
-            for (int off = 16; off; off >>= 1) sum += __shfl_down_sync(FULL, sum, off);
-            if (lane == 0 && sum && lev <= J) atomicAdd(&ag[h * (GK + 1) + lev], (unsigned long long)sum);
+        for (int lev = warp; lev <= J; lev += LW / 32) {
+            const uint32_t* r = agg_s + lev * LW;
+            uint32_t s1 = 0, s2 = 0, s3 = 0;
+            for (int q = lane; q < LW; q += 32) { uint32_t w = r[q]; s1 += w & 0x3ffu; s2 += (w >> 10) & 0x3ffu; s3 += w >> 20; }
+            for (int off = 16; off; off >>= 1) {
+                s1 += __shfl_down_sync(FULL, s1, off);
+                s2 += __shfl_down_sync(FULL, s2, off);
+                s3 += __shfl_down_sync(FULL, s3, off);
+            }
+            if (lane == 0) {
+                if (s1) atomicAdd(&ag[lev], (unsigned long long)s1);
+                if (s2) atomicAdd(&ag[(GK + 1) + lev], (unsigned long long)s2);
+                if (s3) atomicAdd(&ag[2 * (GK + 1) + lev], (unsigned long long)s3);
+            }
         }
         for (int l = tid; l < LS; l += LW) {
             int32_t acc = 0;

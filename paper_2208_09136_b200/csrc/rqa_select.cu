@@ -32,7 +32,7 @@ namespace {
 constexpr int BT = 64;                // targets per buffer-select call
 constexpr int NLEV_MAX = 2 * GK + 1;  // levels of the counting pass: 2 boundaries per bracket
 constexpr int WCAP = 256;             // candidates a warp buffers in shared memory before flushing
-constexpr int NBS = 2 * NB;           // buckets of the counting pass' level table (one byte each)
+constexpr int NBS = NB;               // buckets of the counting pass' level table (8 bytes each)
 constexpr double BRACKET_SIGMAS = 4.5;
 
 // ------------------------------------------------------------------------------------------ per-series state
@@ -67,7 +67,7 @@ struct SelTable {
     int32_t multi;                    // 1 if some bucket holds two or more boundaries (refine by a loop)
     float scale, dcap;
     float beta[2 * GK + 4];           // ascending, beta[J..] = +inf
-    uint8_t lut[NBS];                 // bucket -> #{boundaries in lower buckets}
+    uint2 lut[NBS];                   // bucket -> (bits of the first boundary not in a lower bucket, its index)
 };
 
 struct SampleRanks {                  // per target of the group: sample ranks of the bracket ends (0 = open end)
@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict
             below += neg ? 1 : (bj < (uint32_t)q);
             inside += !neg && bj == (uint32_t)q;
         }
-        T.lut[q] = (uint8_t)below;
+        T.lut[q] = make_uint2(__float_as_uint(s_beta[below]), (uint32_t)below);
         multi |= inside > 1;
     }
     multi = __syncthreads_or(multi);
@@ -324,8 +324,8 @@ struct CountArgs {
 };
 
 struct CountSmem {
-    static constexpr int off_lut = 0;                                   // uint8[NBS]
-    static constexpr int off_beta = off_lut + NBS;                      // float[2*GK+4]
+    static constexpr int off_lut = 0;                                   // uint2[NBS]
+    static constexpr int off_beta = off_lut + 8 * NBS;                  // float[2*GK+4]
     static constexpr int off_cand = off_beta + 4 * (2 * GK + 4);        // float[LW/32][WCAP]
     static constexpr int off_cols = off_cand + 4 * (LW / 32) * WCAP;    // uint32[nlev][LW/2]
     static constexpr int col_row = 4 * (LW / 2);
@@ -361,8 +361,10 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
         CD::template push<R>();
         const bool live = !GUARD || t < cnt;
         const float d = CD::template distance<R>();
-        uint32_t q = lds_u8(lut + bucket_of(d, dcap, scale));
-        q += d > lds_f32(beta + 4 * q) ? 1u : 0u;
+        float er;
+        uint32_t q;
+        lds_f32_u32(lut + 8 * bucket_of(d, dcap, scale), er, q);   // one load: the boundary to compare with, its index
+        q += d > er ? 1u : 0u;
         if (MULTI) {                                          // some bucket holds two or more boundaries
             while (d > lds_f32(beta + 4 * q)) ++q;
         }
@@ -390,7 +392,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev)
     const uint32_t tile = blockIdx.x;
     const SelTable& T = a.tabs[b];
     find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
-    uint8_t* lut_s = (uint8_t*)(smem + CountSmem::off_lut);
+    uint2* lut_s = (uint2*)(smem + CountSmem::off_lut);
     float* beta_s = (float*)(smem + CountSmem::off_beta);
     float* cand_s = (float*)(smem + CountSmem::off_cand);
     uint32_t* cols_s = (uint32_t*)(smem + CountSmem::off_cols);
@@ -398,7 +400,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev)
     const int LA = window_la(a.L, span, 0), LB = window_lb(a.L, span, 0);
     float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * CountSmem::col_row);
     float* yb_s = ya_s + LA;
-    for (int q = tid; q < NBS / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)T.lut)[q];
+    for (int q = tid; q < NBS; q += LW) lut_s[q] = T.lut[q];
     if (tid < 2 * GK + 4) beta_s[tid] = T.beta[tid];
     for (int q = tid; q < nlev * (LW / 2); q += LW) cols_s[q] = 0;
     __syncthreads();

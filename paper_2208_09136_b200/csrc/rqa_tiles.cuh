@@ -60,6 +60,7 @@ __device__ __forceinline__ uint32_t pin(uint32_t x) { return __shfl_sync(0xfffff
 __device__ __forceinline__ unsigned long long pin64(unsigned long long x) { return __shfl_sync(0xffffffffu, x, threadIdx.x & 31); }
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return pin((uint32_t)__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void lds_f32_u32(uint32_t a, float& x, uint32_t& y) { asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=f"(x), "=r"(y) : "r"(a)); }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ uint32_t lds_u16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ uint32_t lds_u8(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a)); return v; }

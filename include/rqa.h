@@ -13,6 +13,8 @@
  *                   R_ij = (d_ij <= eps_k), all K thresholds in one pass, upper
  *                   triangle only, R never stored
  *   rqa_det_avg     DET_k (Eq. 4) and its average over the K recurrence rates (Eq. 5)
+ * On top of it: rqa_det_prefix_avg (Eq. 5 for every cut-off), rqa_line_measures (L, L_max, RR from the
+ * histogram) and rqa_sorting_rate_host (Eq. 6).
  *
  * Conventions (BASELINE.json north_star):
  *   - distances are fp32: maximum norm max_c |x_i[c]-x_j[c]|, or the Euclidean norm computed
@@ -133,6 +135,35 @@ rqa_status rqa_line_hist(const rqa_points* pts, rqa_norm norm, const float* d_ep
  */
 rqa_status rqa_det_avg(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
                        double* d_det, double* d_det_mean, void* stream);
+
+/*
+ * Eq. 5 as a curve ("we test the averaging for RR* in [1, 2, 3, ..., 99]"): the averaged determinism
+ * for every cut-off, d_prefix[b][k] = (d_det[b][0] + ... + d_det[b][k]) / (k+1), summed left to right in fp64, in the
+ * caller's order of the recurrence rates (pass them ascending for the paper's curve).  d_prefix[b][0] = d_det[b][0]
+ * ("the average of one value is the value itself"); d_prefix[b][K-1] = rqa_det_avg's mean.
+ *   d_det     [batch][K] from rqa_det_avg        d_prefix  [batch][K]
+ */
+rqa_status rqa_det_prefix_avg(const double* d_det, int32_t batch, int32_t K, double* d_prefix, void* stream);
+
+/*
+ * The other measures the paper derives from the same histogram ("DET, L, L_max and RR"):
+ *   d_L        [batch][K] average diagonal line length  sum_{l>=l_min} l*P_k(l) / sum_{l>=l_min} P_k(l)  (0 if no line)
+ *   d_Lmax     [batch][K] longest diagonal line  max{ l : P_k(l) > 0 }  (0 if none)
+ *   d_rr_hist  [batch][K] recurrence rate from the histogram  sum_{l>=1} l*P_k(l) / P,  P = N'(N'-1)/2
+ * Any of the three outputs may be NULL.  Sums are exact uint64; the ratios one fp64 division.
+ */
+rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
+                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, void* stream);
+
+/*
+ * Sorting rate S (Eq. 6), the paper's evaluation score; plain host arithmetic on R*n numbers.
+ *   h_measure  HOST [R][n]: the measure (DET or averaged DET) of n series given in their natural order (y_j = j, the
+ *              order the measure is expected to increase in), for R realisations
+ *   h_S        HOST: (W - D) / W with D = sum_i sum_j |x_j - y_j|, x_j = place of series j when the n values of one
+ *              realisation are ordered ascending (equal values keep the given order), and W = R * sum_j |n+1-2j|
+ *              (= 500 for n = R = 10).  1 = perfectly sorted, 0 = reversed.
+ */
+rqa_status rqa_sorting_rate_host(const double* h_measure, int32_t R, int32_t n, double* h_S);
 
 /*
  * The whole path for HOST buffers (what bench.py's `e2e` times): copies the series to the device workspace,

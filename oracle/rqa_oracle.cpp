@@ -34,6 +34,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 #ifdef _OPENMP
@@ -251,6 +252,62 @@ int rqa_oracle_det_avg(const uint64_t* hist, int K, int64_t n_points, int64_t l_
         sum += det[k];
     }
     *det_mean = sum / (double)K;
+    return ORACLE_OK;
+}
+
+/* Eq. 5 for every cut-off RR* (the paper evaluates RR* = 1..99): prefix[k] = (1/(k+1)) sum_{i<=k} DET_i,
+ * summed left to right, in the order the rates were given.  prefix[0] = DET_0. */
+int rqa_oracle_det_prefix_avg(const double* det, int K, double* prefix) {
+    if (!det || !prefix || K < 1) return ORACLE_BAD_ARG;
+    double sum = 0.0;
+    for (int k = 0; k < K; ++k) {
+        sum += det[k];
+        prefix[k] = sum / (double)(k + 1);
+    }
+    return ORACLE_OK;
+}
+
+/* The other measures read off the histogram ("DET, L, L_max and RR"): average diagonal line length
+ * L_k = sum_{l>=l_min} l*P_k(l) / sum_{l>=l_min} P_k(l) (0 without lines), longest line L_max, and the recurrence rate
+ * sum_{l>=1} l*P_k(l) / P with P = N'(N'-1)/2 (reading S2: upper triangle, main diagonal excluded). */
+int rqa_oracle_line_measures(const uint64_t* hist, int K, int64_t n_points, int64_t l_min, double* L, uint64_t* Lmax,
+                             double* rr_hist) {
+    if (!hist || !L || !Lmax || !rr_hist || K < 1 || n_points < 2 || l_min < 1) return ORACLE_BAD_ARG;
+    const double P = (double)((uint64_t)n_points * (uint64_t)(n_points - 1) / 2);
+    for (int k = 0; k < K; ++k) {
+        uint64_t pts = 0, lpts = 0, lines = 0, lmax = 0;
+        for (int64_t l = 1; l < n_points; ++l) {
+            const uint64_t h = hist[(size_t)k * n_points + l];
+            pts += (uint64_t)l * h;
+            if (l >= l_min) { lpts += (uint64_t)l * h; lines += h; }
+            if (h) lmax = (uint64_t)l;
+        }
+        L[k] = lines ? (double)lpts / (double)lines : 0.0;
+        Lmax[k] = lmax;
+        rr_hist[k] = (double)pts / P;
+    }
+    return ORACLE_OK;
+}
+
+/* Sorting rate S (Eq. 6).  measure[i][j]: the measure of series j (series given in their natural
+ * order, y = [1..n]) in realisation i.  x_j = place of series j when the n values are ordered ascending (equal values
+ * keep their given order), z = y reversed.  S = (sum_i sum_j |z_j-y_j| - sum_i sum_j |x_j-y_j|) / sum_i sum_j |z_j-y_j|. */
+int rqa_oracle_sorting_rate(const double* measure, int R, int n, double* S) {
+    if (!measure || !S || R < 1 || n < 2) return ORACLE_BAD_ARG;
+    std::vector<int> order(n), x(n);
+    long long worst = 0, dep = 0;
+    for (int i = 0; i < R; ++i) {
+        const double* m = measure + (size_t)i * n;
+        for (int j = 0; j < n; ++j) order[j] = j;
+        std::stable_sort(order.begin(), order.end(), [m](int a, int b) { return m[a] < m[b]; });
+        for (int place = 0; place < n; ++place) x[order[place]] = place + 1;
+        for (int j = 0; j < n; ++j) {
+            const int y = j + 1, z = n - j;
+            worst += std::llabs((long long)z - y);
+            dep += std::llabs((long long)x[j] - y);
+        }
+    }
+    *S = (double)(worst - dep) / (double)worst;
     return ORACLE_OK;
 }
 

@@ -57,6 +57,9 @@ def _load():
     lib.rqa_oracle_count_lt_le.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, u64p, i32]
     lib.rqa_oracle_line_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i32]
     lib.rqa_oracle_det_avg.argtypes = [u64p, i32, i64, i64, f64p, f64p]
+    lib.rqa_oracle_det_prefix_avg.argtypes = [f64p, i32, f64p]
+    lib.rqa_oracle_line_measures.argtypes = [u64p, i32, i64, i64, f64p, u64p, f64p]
+    lib.rqa_oracle_sorting_rate.argtypes = [f64p, i32, i32, f64p]
     _lib = lib
     return lib
 
@@ -158,6 +161,36 @@ def det_avg(hist, l_min: int = 2):
     _check(_load().rqa_oracle_det_avg(_p(hist, ctypes.c_uint64), K, n, l_min, _p(det, ctypes.c_double),
                                       ctypes.byref(mean)), "det_avg")
     return det, float(mean.value)
+
+
+def det_prefix_avg(det) -> np.ndarray:
+    """Eq. 5 for every cut-off: prefix[k] = mean(det[0..k])."""
+    det = np.ascontiguousarray(det, dtype=np.float64)
+    out = np.empty_like(det)
+    _check(_load().rqa_oracle_det_prefix_avg(_p(det, ctypes.c_double), det.shape[0], _p(out, ctypes.c_double)),
+           "det_prefix_avg")
+    return out
+
+
+def line_measures(hist, l_min: int = 2):
+    """-> (L[K] float64, Lmax[K] uint64, rr_hist[K] float64)"""
+    hist = np.ascontiguousarray(hist, dtype=np.uint64)
+    K, n = hist.shape
+    L = np.empty(K, dtype=np.float64)
+    Lmax = np.empty(K, dtype=np.uint64)
+    rr = np.empty(K, dtype=np.float64)
+    _check(_load().rqa_oracle_line_measures(_p(hist, ctypes.c_uint64), K, n, l_min, _p(L, ctypes.c_double),
+                                            _p(Lmax, ctypes.c_uint64), _p(rr, ctypes.c_double)), "line_measures")
+    return L, Lmax, rr
+
+
+def sorting_rate(measure) -> float:
+    """Eq. 6: measure [R][n] (n series in natural order, R realisations) -> S in [.., 1]."""
+    a = np.ascontiguousarray(measure, dtype=np.float64)
+    S = np.zeros(1, dtype=np.float64)
+    _check(_load().rqa_oracle_sorting_rate(_p(a, ctypes.c_double), a.shape[0], a.shape[1], _p(S, ctypes.c_double)),
+           "sorting_rate")
+    return float(S[0])
 
 
 def sweep(y, m: int, tau: int, rr, norm: int = NORM_MAX, l_min: int = 2, threads: int = 1):

@@ -27,7 +27,8 @@ RQA_MAX_M = 16
 # every symbol include/rqa.h declares (tests check that the library exports them all)
 EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_bytes", "rqa_workspace_status",
            "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
-           "rqa_sweep_host", "rqa_launch_count", "rqa_set_option"]
+           "rqa_sweep_host", "rqa_launch_count", "rqa_set_option", "rqa_det_prefix_avg", "rqa_line_measures",
+           "rqa_sorting_rate_host"]
 
 
 class RqaPoints(ctypes.Structure):
@@ -70,6 +71,9 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_sweep_workspace_bytes.argtypes = [i64, i32, i32, i64, i32, ctypes.POINTER(sz)]
     lib.rqa_sweep_host.argtypes = [vp, i64, i32, i32, i64, ctypes.c_int, vp, i32, i64, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.rqa_set_option.argtypes = [ctypes.c_char_p, i64]
+    lib.rqa_det_prefix_avg.argtypes = [vp, i32, i32, vp, vp]
+    lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp, vp]
+    lib.rqa_sorting_rate_host.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double)]
     _lib = lib
     return lib
 
@@ -162,6 +166,36 @@ def rqa_det_avg(hist, l_min: int, det, det_mean, stream=None) -> None:
     _check(load_library().rqa_det_avg(_dev(hist, torch.int64, "hist"), batch, K, n, l_min,
                                       _dev(det, torch.float64, "det"), _dev(det_mean, torch.float64, "det_mean"),
                                       _stream(stream)))
+
+
+def rqa_det_prefix_avg(det, prefix, stream=None) -> None:
+    """det, prefix float64 CUDA [batch][K]: Eq. 5 for every cut-off."""
+    import torch
+    batch, K = det.shape
+    _check(load_library().rqa_det_prefix_avg(_dev(det, torch.float64, "det"), batch, K,
+                                             _dev(prefix, torch.float64, "prefix"), _stream(stream)))
+
+
+def rqa_line_measures(hist, l_min: int, L=None, Lmax=None, rr_hist=None, stream=None) -> None:
+    """hist int64 CUDA [batch][K][n_points]; L, rr_hist float64 [batch][K]; Lmax int64 [batch][K]; each may be None."""
+    import torch
+    batch, K, n = hist.shape
+    _check(load_library().rqa_line_measures(_dev(hist, torch.int64, "hist"), batch, K, n, l_min,
+                                            None if L is None else _dev(L, torch.float64, "L"),
+                                            None if Lmax is None else _dev(Lmax, torch.int64, "Lmax"),
+                                            None if rr_hist is None else _dev(rr_hist, torch.float64, "rr_hist"),
+                                            _stream(stream)))
+
+
+def rqa_sorting_rate_host(measure) -> float:
+    """measure: host array [R][n] of float64 (n series in their natural order, R realisations) -> S of Eq. 6."""
+    import numpy as np
+    a = np.ascontiguousarray(measure, dtype=np.float64)
+    if a.ndim != 2:
+        raise ValueError("measure must be [R][n]")
+    out = ctypes.c_double(0.0)
+    _check(load_library().rqa_sorting_rate_host(a.ctypes.data, a.shape[0], a.shape[1], ctypes.byref(out)))
+    return float(out.value)
 
 
 def rqa_sweep_workspace_bytes(N: int, batch: int, m: int, tau: int, K: int) -> int:

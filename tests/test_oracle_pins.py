@@ -369,3 +369,67 @@ def test_workloads_are_seeded_and_shaped():
     y = wl.logistic_signal(500, 7)
     assert y.min() > 0 and y.max() < 1
     assert wl.fnv1a64(np.zeros(0, dtype=np.uint8)) == 0xCBF29CE484222325
+
+
+# ---------------------------------------------------------------- rows f1/f2: Eq. 5 curve, L / L_max / RR, Eq. 6
+def test_det_prefix_avg_pins(oracle):
+    """Eq. 5 for every cut-off: the average of one value is the value itself, a hand
+    example, the last entry is the plain mean, and exact rational arithmetic on random input."""
+    assert oracle.det_prefix_avg([0.625]).tolist() == [0.625]
+    assert oracle.det_prefix_avg([0.5, 1.0, 0.0]).tolist() == [0.5, 0.75, 0.5]
+    rng = np.random.default_rng(5)
+    det = rng.random(99)
+    got = oracle.det_prefix_avg(det)
+    acc = Fraction(0)
+    for k in range(99):
+        acc += Fraction(float(det[k]))
+        assert abs(Fraction(float(got[k])) - acc / (k + 1)) < Fraction(1, 10**13)
+    hist = np.zeros((3, 12), dtype=np.uint64)
+    hist[0, 1], hist[0, 3] = 4, 1
+    hist[1, 2], hist[1, 5] = 2, 1
+    hist[2, 1] = 7
+    d, mean = oracle.det_avg(hist, 2)
+    assert oracle.det_prefix_avg(d)[-1] == pytest.approx(mean, abs=1e-15)
+
+
+def test_line_measures_hand_cases(oracle):
+    """L, L_max and RR from the histogram on two hand-enumerated recurrence plots of SURVEY.md 8c:
+    A (y=0,1,0,1,0,1, m=1, rr=0.4): P(2)=P(4)=1 -> L=3, L_max=4, RR=6/15.
+    E (y=0,2,1,4,0,2,1,4,3, m=2, tau=2, rr=0.5): P(1)=5,P(2)=2,P(3)=1,P(5)=1 -> L=(4+3+5)/4=3, L_max=5, RR=17/21."""
+    r = oracle.sweep(np.array([0, 1, 0, 1, 0, 1], dtype=np.float32), 1, 1, [0.4], oracle.NORM_MAX, 2)
+    L, Lmax, rr = oracle.line_measures(r["hist"], 2)
+    assert (L[0], int(Lmax[0]), rr[0]) == (3.0, 4, 6 / 15)
+    r = oracle.sweep(np.array([0, 2, 1, 4, 0, 2, 1, 4, 3], dtype=np.float32), 2, 2, [0.5], oracle.NORM_MAX, 2)
+    L, Lmax, rr = oracle.line_measures(r["hist"], 2)
+    assert (L[0], int(Lmax[0]), rr[0]) == (3.0, 5, 17 / 21)
+    assert rr[0] == r["rr"][0]                       # "RR can also be calculated from the histogram" (PAPER.md:125)
+    L1, _, _ = oracle.line_measures(r["hist"], 1)    # l_min = 1: all 9 lines, 17 points
+    assert L1[0] == 17 / 9
+    empty = np.zeros((1, 7), dtype=np.uint64)
+    L, Lmax, rr = oracle.line_measures(empty, 2)
+    assert (L[0], int(Lmax[0]), rr[0]) == (0.0, 0, 0.0)
+
+
+def test_sorting_rate_pins(oracle):
+    """Eq. 6: the worst case sums to 500 for 10 series x 10 realisations, so the
+    reversed order gives S = 0 and the natural order S = 1; one adjacent swap per realisation costs 2 of 50; and an
+    independent rank computation (numpy argsort) on every permutation of 4 series."""
+    import itertools
+    up = np.tile(np.arange(10, dtype=np.float64), (10, 1))
+    assert oracle.sorting_rate(up) == 1.0
+    assert oracle.sorting_rate(up[:, ::-1]) == 0.0
+    assert sum(abs(11 - 2 * j) for j in range(1, 11)) * 10 == 500
+    sw = up.copy()
+    sw[:, [0, 1]] = sw[:, [1, 0]]
+    assert oracle.sorting_rate(sw) == pytest.approx((500 - 20) / 500, abs=1e-15)
+    half = up.copy()
+    half[5:] = half[5:, ::-1]                        # five realisations sorted, five reversed
+    assert oracle.sorting_rate(half) == 0.5
+    for perm in itertools.permutations(range(4)):
+        m = np.array([perm], dtype=np.float64)
+        x = np.empty(4, dtype=int)
+        x[np.argsort(m[0], kind="stable")] = np.arange(1, 5)
+        dep = int(np.abs(x - np.arange(1, 5)).sum())
+        assert oracle.sorting_rate(m) == pytest.approx((8 - dep) / 8, abs=1e-15)
+    ties = np.array([[1.0, 1.0, 1.0]])               # equal values keep their given order: perfectly "sorted"
+    assert oracle.sorting_rate(ties) == 1.0

@@ -379,3 +379,43 @@ def test_config3_size_default_path_is_bracket(rqa, oracle):
     w = wl.config3(0)
     for norm in (0, 1):
         _assert_select(oracle, _select_only(rqa, w.series[2], w.m, w.tau, w.rr, norm), w.series[2], w.m, w.tau, w.rr, norm)
+
+
+# ------------------------------------------------------ rows f1/f2: the paper's own sweep, Eq. 5 curve, L/L_max/RR, Eq. 6
+def test_paper_sweep_k99_prefix_measures_sorting(rqa, oracle):
+    """The paper's experiment in miniature: K = 99 integer-percent recurrence rates, the averaged
+    determinism for every cut-off RR* (Eq. 5), L / L_max / RR from the same histograms, and the
+    sorting rate S (Eq. 6) of 5 noise levels x 3 realisations of a logistic-map series (N = 700; un-embedded as in
+    the paper, m = 1)."""
+    import torch
+    rr = wl.rr_linear(99)
+    snrs = [0.1, 0.3, 1.0, 3.0, 10.0]                           # natural order: DET is expected to increase
+    series = np.stack([wl.add_noise(wl.logistic_signal(700, seed=70 + r), snr, seed=700 + 10 * r + i)
+                       for r in range(3) for i, snr in enumerate(snrs)])
+    s = torch.as_tensor(series).cuda()
+    buf = rqa.averaged_rqa(s, 1, 1, rr, 0, 2)
+    batch, K = buf.det.shape
+    prefix = torch.empty_like(buf.det)
+    L = torch.empty_like(buf.det)
+    Lmax = torch.empty((batch, K), dtype=torch.int64, device=s.device)
+    rrh = torch.empty_like(buf.det)
+    rqa.rqa_det_prefix_avg(buf.det, prefix)
+    rqa.rqa_line_measures(buf.hist, 2, L, Lmax, rrh)
+    torch.cuda.synchronize()
+    g = {"eps": buf.eps.cpu().numpy(), "count": buf.count.cpu().numpy().view(np.uint64), "rr": buf.rr.cpu().numpy(),
+         "hist": buf.hist.cpu().numpy().view(np.uint64), "det": buf.det.cpu().numpy(), "det_mean": buf.det_mean.cpu().numpy()}
+    assert_parity(oracle, g, series, 1, 1, rr, 0, 2)
+    prefix, L, Lmax, rrh = prefix.cpu().numpy(), L.cpu().numpy(), Lmax.cpu().numpy().view(np.uint64), rrh.cpu().numpy()
+    for b in range(batch):
+        assert np.max(np.abs(prefix[b] - oracle.det_prefix_avg(g["det"][b]))) <= DET_TOL
+        oL, oLmax, orr = oracle.line_measures(g["hist"][b], 2)
+        assert np.max(np.abs(L[b] - oL)) <= DET_TOL and np.array_equal(Lmax[b], oLmax)
+        assert np.max(np.abs(rrh[b] - orr)) <= DET_TOL and np.array_equal(rrh[b], g["rr"][b])
+        assert prefix[b][0] == g["det"][b][0] and abs(prefix[b][-1] - g["det_mean"][b]) <= DET_TOL
+    for cut in (0, 39, 98):                                     # DET_1, the recommended RR* = 40 %, RR* = 99 %
+        m = prefix[:, cut].reshape(3, 5)
+        assert rqa.rqa_sorting_rate_host(m) == pytest.approx(oracle.sorting_rate(m), abs=1e-15)
+    # Partial output set and argument checking
+    rqa.rqa_line_measures(buf.hist, 2, None, Lmax=torch.empty((batch, K), dtype=torch.int64, device=s.device))
+    with pytest.raises(rqa.RqaError):
+        rqa.rqa_sorting_rate_host(np.zeros((1, 1)))

@@ -528,16 +528,30 @@ __global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
     const uint32_t t0 = a.tile_start[ob];
     const int nc = (int)((len + a.L - 1) / a.L);
     uint32_t carry = 0;
-    for (int c = 0; c < nc; ++c) {
-        const uint32_t cntc = (uint32_t)min((int64_t)a.L, len - (int64_t)c * a.L);
-        const int64_t tile = (int64_t)b * a.tiles + t0 + c;
-        const uint32_t p = a.pre[(tile * (2 * a.NP) + j) * LW + tid];
-        if (p == cntc) {
-            carry += cntc;
-        } else {
-            const uint32_t tot = carry + p;
-            if (tot >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[tot], 1ull);
-            carry = a.suf[(tile * (2 * a.NP) + j) * LW + tid];
+    // the summaries of SB chunks are loaded together (independent loads), then joined in order
+    constexpr int SB = 8;
+    const int64_t stride = (int64_t)(2 * a.NP) * LW;
+    const int64_t base = (((int64_t)b * a.tiles + t0) * (2 * a.NP) + j) * LW + tid;
+    for (int c0 = 0; c0 < nc; c0 += SB) {
+        uint32_t p[SB], sf[SB];
+#pragma unroll
+        for (int u = 0; u < SB; ++u) {
+            const bool in = c0 + u < nc;
+            p[u] = in ? a.pre[base + (int64_t)(c0 + u) * stride] : 0u;
+            sf[u] = in ? a.suf[base + (int64_t)(c0 + u) * stride] : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < SB; ++u) {
+            if (c0 + u < nc) {
+                const uint32_t cntc = (uint32_t)min((int64_t)a.L, len - (int64_t)(c0 + u) * a.L);
+                if (p[u] == cntc) {
+                    carry += cntc;
+                } else {
+                    const uint32_t tot = carry + p[u];
+                    if (tot >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[tot], 1ull);
+                    carry = sf[u];
+                }
+            }
         }
     }
     if (carry >= (uint32_t)LMIN_EXPLICIT) atomicAdd(&row[carry], 1ull);
@@ -547,7 +561,7 @@ __global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
 // One block per (distinct threshold, series): P(1), P(2), P(3) from the aggregates and the explicit lines
 //   C  = sum_l l P(l),  Q2 = sum_{l>=2} (l-1) P(l),  Q3 = sum_{l>=3} (l-2) P(l)      (all exact integers)
 // then the rows of caller thresholds that share this value are copied from the representative row.
-__global__ void __launch_bounds__(256) line_finalize_kernel(int64_t n, int g, int NG, int K,
+__global__ void __launch_bounds__(1024) line_finalize_kernel(int64_t n, int g, int NG, int K,
                                                             const LineGroup* __restrict__ groups,
                                                             const unsigned long long* __restrict__ agg,
                                                             unsigned long long* __restrict__ hist, WsStatus* status) {
@@ -556,12 +570,13 @@ __global__ void __launch_bounds__(256) line_finalize_kernel(int64_t n, int g, in
     if (j >= G.J) return;
     unsigned long long* row = hist + ((int64_t)b * K + G.rep_k[j]) * n;
     unsigned long long e0 = 0, c4 = 0;
+#pragma unroll 4
     for (int64_t l = LMIN_EXPLICIT + threadIdx.x; l < n; l += blockDim.x) {
         unsigned long long h = row[l];
         e0 += (unsigned long long)l * h;
         c4 += h;
     }
-    __shared__ unsigned long long s_e0[8], s_c4[8];
+    __shared__ unsigned long long s_e0[32], s_c4[32];
     for (int off = 16; off; off >>= 1) {
         e0 += __shfl_down_sync(FULL, e0, off);
         c4 += __shfl_down_sync(FULL, c4, off);
@@ -570,7 +585,7 @@ __global__ void __launch_bounds__(256) line_finalize_kernel(int64_t n, int g, in
     __syncthreads();
     if (threadIdx.x == 0) {
         e0 = 0; c4 = 0;
-        for (int q = 0; q < 8; ++q) { e0 += s_e0[q]; c4 += s_c4[q]; }
+        for (int q = 0; q < (int)(blockDim.x >> 5); ++q) { e0 += s_e0[q]; c4 += s_c4[q]; }
         const unsigned long long* ag = agg + ((int64_t)b * NG + g) * 3 * (GK + 1);
         unsigned long long C = 0, Q2 = 0, Q3 = 0;
         for (int u = 0; u <= j; ++u) { C += ag[u]; Q2 += ag[(GK + 1) + u]; Q3 += ag[2 * (GK + 1) + u]; }
@@ -742,7 +757,7 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
         sa.tiles = p.tiles;
         line_stitch_kernel<<<dim3((unsigned)p.n_ob, (unsigned)(2 * p.NP), (unsigned)v.batch), LW, 0, s>>>(sa);
         RQA_LAUNCH_CHECK();
-        line_finalize_kernel<<<dim3((unsigned)(2 * p.NP), (unsigned)v.batch), 256, 0, s>>>(v.n, g, p.NG, K, groups, agg,
+        line_finalize_kernel<<<dim3((unsigned)(2 * p.NP), (unsigned)v.batch), 1024, 0, s>>>(v.n, g, p.NG, K, groups, agg,
                                                                                          (unsigned long long*)d_hist, status);
         RQA_LAUNCH_CHECK();
         unsigned cb = (unsigned)std::min<int64_t>((v.n + 255) / 256, 64);

@@ -167,9 +167,7 @@ __global__ void __launch_bounds__(256) bufsel_pass_kernel(const float* __restric
     const uint32_t* x = (const uint32_t*)buf + (unsigned long long)b * stride;
     const int shift = 24 - 8 * pass;
     const uint32_t himask = pass == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * pass));
-    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < n;
-         e += (unsigned long long)gridDim.x * blockDim.x) {
-        const uint32_t key = x[e];
+    auto count_key = [&](uint32_t key) {
         const uint32_t hi = key & himask;
         int lo = 0, hiq = G;                 // first group with gprefix >= hi
         while (lo < hiq) {
@@ -177,7 +175,16 @@ __global__ void __launch_bounds__(256) bufsel_pass_kernel(const float* __restric
             if (s_gprefix[mid] < hi) lo = mid + 1; else hiq = mid;
         }
         if (lo < G && s_gprefix[lo] == hi) atomicAdd(&sbins[lo * 256 + ((key >> shift) & 255u)], 1u);
+    };
+    // four keys per load where the series' buffer is 16-byte aligned (more bytes in flight per thread), then the tail
+    const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long nthreads = (unsigned long long)gridDim.x * blockDim.x;
+    const unsigned long long nvec = (((uintptr_t)x & 15) == 0) ? n / 4 : 0;
+    for (unsigned long long e = tid; e < nvec; e += nthreads) {
+        const uint4 k4 = ((const uint4*)x)[e];
+        count_key(k4.x); count_key(k4.y); count_key(k4.z); count_key(k4.w);
     }
+    for (unsigned long long e = 4 * nvec + tid; e < n; e += nthreads) count_key(x[e]);
     __syncthreads();
     unsigned long long* gb = bins + (int64_t)b * BT * 256;
     for (int q = threadIdx.x; q < G * 256; q += blockDim.x) {

@@ -30,10 +30,13 @@ namespace rqa {
 namespace {
 
 constexpr int BT = 64;                // targets per buffer-select call
-constexpr int NLEV_MAX = 2 * GK + 1;  // levels of the counting pass: 2 boundaries per bracket
+constexpr int NCUT = 4 * GK + 4;       // boundary slots: 2 per bracket, 2 more when both ends carry massive ties
+constexpr int NLEV_MAX = 4 * GK + 1;  // levels of the counting pass
+constexpr int TIE_MASS = 2048;        // a bracket end seen this often in the sample gets a level of its own
 constexpr int WCAP = 256;             // candidates a warp buffers in shared memory before flushing
 constexpr int NBS = NB;               // buckets of the counting pass' level table (8 bytes each)
 constexpr double BRACKET_SIGMAS = 4.5;
+enum : uint8_t { LEVEL_OUT = 0, LEVEL_CAND = 1, LEVEL_POINT = 2 };
 
 // ------------------------------------------------------------------------------------------ per-series state
 struct SelState {
@@ -41,6 +44,9 @@ struct SelState {
     int32_t pad;
     unsigned long long ncand;         // candidates appended by the counting pass (may exceed the capacity)
     unsigned long long level_count[NLEV_MAX + 1];
+    int32_t is_point[GK];             // target t of the group fell into a LEVEL_POINT level:
+    float point_val[GK];              //   eps = that value,
+    unsigned long long point_cnt[GK]; //   C = #{d <= eps}
 };
 
 // state of one buffer select (<= BT targets) of one series
@@ -63,10 +69,13 @@ struct Ranks64 {
 
 // bracket boundaries of one group of <= GK targets of one series (the counting pass's level table)
 struct SelTable {
-    int32_t J;                        // boundaries in use (even), levels 0..J
+    int32_t J;                        // boundaries in use, levels 0..J
     int32_t multi;                    // 1 if some bucket holds two or more boundaries (refine by a loop)
+    int32_t heavy;                    // 1 if J > 2 * targets: counted by the second, wider launch of the counting pass
+    int32_t pad;
     float scale, dcap;
-    float beta[2 * GK + 4];           // ascending, beta[J..] = +inf
+    float beta[NCUT];           // ascending, beta[J..] = +inf
+    uint8_t kind[NCUT];         // LEVEL_* of level q = (beta[q-1], beta[q]]
     uint2 lut[NBS];                   // bucket -> (bits of the first boundary not in a lower bucket, its index)
 };
 
@@ -263,8 +272,14 @@ __global__ void __launch_bounds__(256) bufsel_resolve_kernel(BufSel* st, unsigne
 }
 
 // ------------------------------------------------------------------------------- bracket table (per group)
-// From the 2*kc sample order statistics: brackets (lo_k, hi_k], merged where they overlap, as an ascending boundary
-// list beta[0..J) (J even; bracket g = level 2g+1 = (beta[2g], beta[2g+1]]) and its bucket table.
+// From the 2*kc sample order statistics: brackets (lo_k, hi_k].  A collapsed bracket (lo == hi = v: the sample sees
+// massive ties at v) becomes the single-value interval (prev(v), v].  All bracket ends together are the ascending cut
+// list beta[0..J); level q = (beta[q-1], beta[q]] has a kind:
+//   LEVEL_CAND   inside a bracket: its cells are appended to the candidate list
+//   LEVEL_POINT  a single fp32 value: counted only — a rank that falls into it has eps = beta[q] exactly
+//   LEVEL_OUT    outside every bracket: counted only — a rank that falls into it is a miss (radix fallback)
+// The bucket table entry of a bucket holds the first cut not in a lower bucket, its index, and in the two top bits
+// whether that level and the next one are candidate levels (see Counter::cell).
 __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict__ st, SampleRanks sr,
                                                        SelTable* __restrict__ tabs) {
     const int b = blockIdx.x;
@@ -272,21 +287,47 @@ __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict
     SelTable& T = tabs[b];
     __shared__ int s_J;
     __shared__ float s_scale, s_dcap;
-    __shared__ float s_beta[2 * GK + 4];
+    __shared__ float s_beta[NCUT];
+    __shared__ uint8_t s_kind[NCUT];
     const float INF = __int_as_float(0x7f800000);
     if (threadIdx.x == 0) {
+        float blo[GK], bhi[GK];
         int J = 0;
         for (int k = 0; k < sr.kc; ++k) {
             float lo = sr.lo[k] ? s.out_val[2 * k] : -1.0f;          // open lower end: below every distance
             float hi = sr.hi[k] ? s.out_val[2 * k + 1] : INF;        // open upper end
-            if (J > 0 && lo <= s_beta[J - 1]) {                      // overlaps the previous bracket: extend it
-                s_beta[J - 1] = fmaxf(s_beta[J - 1], hi);
-            } else {
-                s_beta[J++] = lo;
-                s_beta[J++] = hi;
+            const bool collapsed = lo == hi;
+            if (collapsed) lo = nextafterf(hi, -INF);                // the single value hi (negative if hi == 0)
+            blo[k] = lo; bhi[k] = hi;
+            // an end that the sample holds TIE_MASS times or more is a value with massive ties: the cut just below
+            // it makes it a level of its own (counted, never appended to the candidates)
+            const bool mlo = !collapsed && sr.lo[k] && s.out_cnt[2 * k] - s.below[2 * k] >= (unsigned long long)TIE_MASS;
+            const bool mhi = !collapsed && sr.hi[k] && s.out_cnt[2 * k + 1] - s.below[2 * k + 1] >= (unsigned long long)TIE_MASS;
+            for (int e = 0; e < 4; ++e) {                            // insert the cuts, ascending, without duplicates
+                if ((e == 2 && !mlo) || (e == 3 && !mhi)) continue;
+                const float x = e == 0 ? lo : e == 1 ? hi : nextafterf(e == 2 ? lo : hi, -INF);
+                int pos = 0;
+                while (pos < J && s_beta[pos] < x) ++pos;
+                if (pos < J && s_beta[pos] == x) continue;
+                for (int q = J; q > pos; --q) s_beta[q] = s_beta[q - 1];
+                s_beta[pos] = x;
+                ++J;
             }
         }
-        for (int q = J; q < 2 * GK + 4; ++q) s_beta[q] = INF;
+        for (int q = J; q < NCUT; ++q) s_beta[q] = INF;
+        for (int q = 0; q < NCUT; ++q) {
+            uint8_t kind = LEVEL_OUT;
+            if (q >= 1 && q < J) {
+                const float c0 = s_beta[q - 1], c1 = s_beta[q];
+                if (c1 < INF && (c0 == nextafterf(c1, -INF) || (c1 == 0.0f && c0 < 0.0f))) {   // distances are >= 0
+                    kind = LEVEL_POINT;
+                } else {
+                    for (int k = 0; k < sr.kc; ++k)
+                        if (blo[k] <= c0 && c1 <= bhi[k]) kind = LEVEL_CAND;
+                }
+            }
+            s_kind[q] = kind;
+        }
         float fmaxb = 0.0f;                                          // largest finite boundary
         for (int q = 0; q < J; ++q)
             if (s_beta[q] < INF) fmaxb = fmaxf(fmaxb, s_beta[q]);
@@ -295,11 +336,11 @@ __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict
         s_dcap = dcap;
         s_scale = bucket_scale(dcap, NBS);
         s_J = J;
-        T.J = J; T.scale = s_scale; T.dcap = dcap;
+        T.J = J; T.scale = s_scale; T.dcap = dcap; T.heavy = J > 2 * sr.kc; T.pad = 0;
     }
     __syncthreads();
     const int J = s_J;
-    for (int q = threadIdx.x; q < 2 * GK + 4; q += blockDim.x) T.beta[q] = s_beta[q];
+    for (int q = threadIdx.x; q < NCUT; q += blockDim.x) { T.beta[q] = s_beta[q]; T.kind[q] = s_kind[q]; }
     int multi = 0;
     for (int q = threadIdx.x; q < NBS; q += blockDim.x) {
         int below = 0, inside = 0;
@@ -311,7 +352,8 @@ __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict
             below += neg ? 1 : (bj < (uint32_t)q);
             inside += !neg && bj == (uint32_t)q;
         }
-        T.lut[q] = make_uint2(__float_as_uint(s_beta[below]), (uint32_t)below);
+        const uint32_t f0 = s_kind[below] == LEVEL_CAND, f1 = s_kind[below + 1] == LEVEL_CAND;
+        T.lut[q] = make_uint2(__float_as_uint(s_beta[below]), (uint32_t)below | ((2u * f0 + (f0 != f1)) << 30));
         multi |= inside > 1;
     }
     multi = __syncthreads_or(multi);
@@ -333,7 +375,8 @@ struct CountArgs {
 struct CountSmem {
     static constexpr int off_lut = 0;                                   // uint2[NBS]
     static constexpr int off_beta = off_lut + 8 * NBS;                  // float[2*GK+4]
-    static constexpr int off_cand = off_beta + 4 * (2 * GK + 4);        // float[LW/32][WCAP]
+    static constexpr int off_kind = off_beta + 4 * (NCUT);        // uint8[2*GK+4]
+    static constexpr int off_cand = off_kind + (NCUT);            // float[LW/32][WCAP]
     static constexpr int off_cols = off_cand + 4 * (LW / 32) * WCAP;    // uint32[nlev][LW/2]
     static constexpr int col_row = 4 * (LW / 2);
 };
@@ -341,7 +384,7 @@ struct CountSmem {
 template <int NORM, int M, int TAU, bool MULTI>
 struct Counter : CellDist<NORM, M, TAU, 0> {
     using CD = CellDist<NORM, M, TAU, 0>;
-    uint32_t lut, beta;               // shared-window addresses of the bucket table and the boundaries
+    uint32_t lut, beta, kind;         // shared-window addresses of the bucket table, the boundaries, the level kinds
     uint32_t cols;                    // ... of this thread's column, level 0
     float* wbuf;                      // this warp's candidate buffer
     float* gcand;                     // the series' candidate list
@@ -371,16 +414,23 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
         float er;
         uint32_t q;
         lds_f32_u32(lut + 8 * bucket_of(d, dcap, scale), er, q);   // one load: the boundary to compare with, its index
-        q += d > er ? 1u : 0u;
+        // bits 30-31 of the entry say whether level q and level q+1 are candidate levels, encoded so that adding
+        // 1 << 30 together with the level increment leaves the answer in bit 31; the level's byte offset below is
+        // q * 2^10 modulo 2^32, which drops those bits.
+        q += d > er ? 0x40000001u : 0u;
+        bool cand = (int32_t)q < 0;
         if (MULTI) {                                          // some bucket holds two or more boundaries
+            q &= 0xffffu;
             while (d > lds_f32(beta + 4 * q)) ++q;
+            cand = lds_u8(kind + q) == LEVEL_CAND;
         }
+        static_assert(CountSmem::col_row == 1024 || CountSmem::col_row == 512, "level offset must shift bits 30-31 out");
         if (live) red_u32(cols + q * CountSmem::col_row, inc);
-        const unsigned mc = __ballot_sync(FULL, live && (q & 1u));
+        const unsigned mc = __ballot_sync(FULL, live && cand);
         if (mc) {
             const uint32_t nc = __popc(mc);
             if (wcount + nc > (uint32_t)WCAP) flush_warp();
-            if (live && (q & 1u)) wbuf[wcount + __popc(mc & lane_lt)] = d;
+            if (live && cand) wbuf[wcount + __popc(mc & lane_lt)] = d;
             wcount += nc;
         }
     }
@@ -391,13 +441,14 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
 };
 
 template <int NORM, int M, int TAU>
-__global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev) {
+__global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev, int heavy_pass) {
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;
     const int tid = threadIdx.x, b = blockIdx.y;
     if (a.ss[b].fallback) return;
     const uint32_t tile = blockIdx.x;
     const SelTable& T = a.tabs[b];
+    if (T.heavy != heavy_pass) return;                        // series with extra tie levels: the wider second launch
     find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
     uint2* lut_s = (uint2*)(smem + CountSmem::off_lut);
     float* beta_s = (float*)(smem + CountSmem::off_beta);
@@ -408,7 +459,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev)
     float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * CountSmem::col_row);
     float* yb_s = ya_s + LA;
     for (int q = tid; q < NBS; q += LW) lut_s[q] = T.lut[q];
-    if (tid < 2 * GK + 4) beta_s[tid] = T.beta[tid];
+    if (tid < NCUT) { beta_s[tid] = T.beta[tid]; ((uint8_t*)(smem + CountSmem::off_kind))[tid] = T.kind[tid]; }
     for (int q = tid; q < nlev * (LW / 2); q += LW) cols_s[q] = 0;
     __syncthreads();
     const int ob = s_ob;
@@ -436,6 +487,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev)
             ct.tau = a.tau;
             ct.lut = smem_addr(lut_s);
             ct.beta = smem_addr(beta_s);
+            ct.kind = smem_addr(smem + CountSmem::off_kind);
             ct.cols = pin(smem_addr(cols_s) + 4 * (tid & (LW / 2 - 1)));
             ct.wbuf = cand_s + (tid >> 5) * WCAP;
             ct.gcand = a.cand + (unsigned long long)b * a.cap;
@@ -476,7 +528,8 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev)
     }
 }
 
-// One block per series: exact level counts -> each target's bracket and its rank among the candidates.
+// One block per series: exact level counts -> each target's level.  A candidate level: its rank among the candidates
+// (the buffer select finishes it).  A single-value level: eps and C are known here.  Anything else: radix fallback.
 __global__ void __launch_bounds__(64) sel_bracket_resolve_kernel(SelState* ss, const SelTable* __restrict__ tabs,
                                                                SampleRanks sr, BufSel* st, unsigned long long cap) {
     const int b = blockIdx.x;
@@ -484,18 +537,18 @@ __global__ void __launch_bounds__(64) sel_bracket_resolve_kernel(SelState* ss, c
     if (s.fallback) return;
     const SelTable& T = tabs[b];
     BufSel& bs = st[b];
-    __shared__ unsigned long long s_cum[NLEV_MAX + 1], s_odd[NLEV_MAX + 1];
+    __shared__ unsigned long long s_cum[NLEV_MAX + 2], s_cnd[NLEV_MAX + 2];
     __shared__ int s_bad;
     if (threadIdx.x == 0) {
-        unsigned long long cum = 0, odd = 0;
+        unsigned long long cum = 0, cnd = 0;
         for (int v = 0; v <= T.J; ++v) {
             s_cum[v] = cum;                                   // cells in the levels below v
-            s_odd[v] = odd;                                   // candidates in the brackets below v
+            s_cnd[v] = cnd;                                   // candidates in the levels below v
             cum += s.level_count[v];
-            if (v & 1) odd += s.level_count[v];
+            if (T.kind[v] == LEVEL_CAND) cnd += s.level_count[v];
         }
         s_cum[T.J + 1] = cum;
-        s_bad = (odd != s.ncand) || (s.ncand > cap);
+        s_bad = (cnd != s.ncand) || (s.ncand > cap);
         bufsel_reset(bs, sr.kc);
     }
     __syncthreads();
@@ -505,15 +558,20 @@ __global__ void __launch_bounds__(64) sel_bracket_resolve_kernel(SelState* ss, c
         const unsigned long long r = sr.rank[t];
         int v = 0;
         while (v <= T.J && s_cum[v + 1] < r) ++v;             // first level whose cumulative count reaches r
-        if (v > T.J || !(v & 1)) {
-            bad = 1;                                          // the rank is not inside a bracket
-            v = 1;
+        const int kind = v <= T.J ? T.kind[v] : LEVEL_OUT;
+        const bool point = kind == LEVEL_POINT;
+        if (kind == LEVEL_OUT) bad = 1;                       // the rank is not inside a bracket
+        s.is_point[t] = point;
+        if (point) {
+            s.point_val[t] = T.beta[v];
+            s.point_cnt[t] = s_cum[v + 1];
         }
+        const bool sel = kind == LEVEL_CAND && !bad;          // otherwise the buffer select gets a harmless rank
         bs.group_of[t] = 0;
         bs.prefix[t] = 0;
         bs.below[t] = 0;
-        bs.resid[t] = bad ? 1 : s_odd[v] + (r - s_cum[v]);
-        bs.base[t] = bad ? 0 : s_cum[v] - s_odd[v];
+        bs.resid[t] = sel ? s_cnd[v] + (r - s_cum[v]) : 1;
+        bs.base[t] = sel ? s_cum[v] - s_cnd[v] : 0;
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) s.fallback = 1;
 }
@@ -530,8 +588,9 @@ __global__ void sel_finish_kernel(const SelState* __restrict__ ss, const BufSel*
     if (t >= tm.T || (use_flag && ss[b].fallback)) return;
     const BufSel& s = st[b];
     const int k = tm.k_of[t];
-    const unsigned long long c = s.base[t] + s.out_cnt[t];
-    eps[(int64_t)b * K + k] = s.out_val[t];
+    const bool point = use_flag && ss[b].is_point[t];
+    const unsigned long long c = point ? ss[b].point_cnt[t] : s.base[t] + s.out_cnt[t];
+    eps[(int64_t)b * K + k] = point ? ss[b].point_val[t] : s.out_val[t];
     count[(int64_t)b * K + k] = c;
     rr[(int64_t)b * K + k] = (double)c / (double)P;
 }
@@ -734,9 +793,14 @@ size_t count_smem_bytes(int nlev, int L, int span) {
 template <int NORM, int M, int TAU>
 rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int batch, cudaStream_t s) {
     auto kern = sel_count_kernel<NORM, M, TAU>;
-    const size_t smem = count_smem_bytes(nlev, p.L, p.span);
-    RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev);
+    // second launch: only the series whose table carries extra single-value levels (massive ties); its blocks
+    // of the other series return at once, and so do the first launch's blocks of those series
+    const int nlev_heavy = 2 * nlev - 1;
+    const size_t smem = count_smem_bytes(nlev, p.L, p.span), smem_heavy = count_smem_bytes(nlev_heavy, p.L, p.span);
+    RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_heavy));
+    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, 0);
+    RQA_LAUNCH_CHECK();
+    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem_heavy, s>>>(a, nlev_heavy, 1);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }

@@ -352,8 +352,9 @@ def test_bracket_path_any_sample_size(rqa, oracle, options, S):
 
 
 def test_bracket_path_overflow_and_ties_fall_back(rqa, oracle, options):
-    """A candidate list that is too small, and tie-heavy data whose brackets collapse, are both detected from the exact
-    counts and redone by the radix passes — per series, inside one batched call."""
+    """Tie-heavy data (collapsed brackets become single-value levels, bracket ends with massive ties get a level of
+    their own) and a candidate list that is too small (detected from the exact counts, redone by the radix passes)
+    — per series, inside one batched call."""
     rr = wl.rr_log(12, 0.002, 0.4)
     noisy = wl.add_noise(wl.sine_signal(2600), 0.7, 3)
     clean = wl.sine_signal(2600).astype(np.float32)                      # 25 distinct values: massive ties
@@ -363,6 +364,21 @@ def test_bracket_path_overflow_and_ties_fall_back(rqa, oracle, options):
     _assert_select(oracle, _select_only(rqa, ys, 2, 3, rr), ys, 2, 3, rr)
     options(select_path=2, cand_cap=64)
     _assert_select(oracle, _select_only(rqa, ys, 2, 3, rr), ys, 2, 3, rr)
+
+
+@pytest.mark.parametrize("S", [0, 3000, 400000])
+def test_bracket_path_tie_levels(rqa, oracle, options, S):
+    """Exactly periodic and coarsely quantised series (every distance value carries massive ties) at K = 32: the
+    single-value levels, the wider second counting launch and ordinary brackets side by side in one batch, at
+    sample sizes on both sides of the tie-mass threshold."""
+    options(select_path=2, sample_size=S)
+    rr = wl.rr_log(32, 0.0005, 0.6)
+    clean = wl.sine_signal(3400).astype(np.float32)
+    quant = np.round(wl.gaussian(11, 3400) * 2.0).astype(np.float32)    # about a dozen distinct values
+    mixed = (np.round(wl.gaussian(12, 3400) * 40.0) / 40.0).astype(np.float32)
+    noisy = wl.add_noise(wl.sine_signal(3400), 1.0, 4)
+    ys = np.stack([clean, quant, mixed, noisy])
+    _assert_select(oracle, _select_only(rqa, ys, 3, 1, rr), ys, 3, 1, rr)
 
 
 def test_bracket_path_many_targets(rqa, oracle, options):

@@ -686,7 +686,10 @@ rqa_status launch_scan(const ScanArgs& a, const LinePlan& p, int batch, cudaStre
 
 template <int NORM, int NP>
 rqa_status dispatch_embedding(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
+    // the embeddings of BASELINE.json's large configs get a register ring; any other (m, tau) recomputes per cell
     if (a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, batch, s);
+    if (a.m == 3 && a.tau == 3) return launch_scan<NORM, 3, 3, NP>(a, p, batch, s);
+    if (a.m == 5 && a.tau == 2) return launch_scan<NORM, 5, 2, NP>(a, p, batch, s);
     return launch_scan<NORM, 0, 0, NP>(a, p, batch, s);
 }
 

@@ -378,7 +378,9 @@ struct CountSmem {
     static constexpr int off_kind = off_beta + 4 * (NCUT);        // uint8[2*GK+4]
     static constexpr int off_cand = off_kind + (NCUT);            // float[LW/32][WCAP]
     static constexpr int off_cols = off_cand + 4 * (LW / 32) * WCAP;    // uint32[nlev][LW/2]
-    static constexpr int col_row = 4 * (LW / 2);
+    // per-thread level counters: `fields` threads share a word, 2 x 16 bits (chunks of <= 2047 cells) or, when the
+    // group has many levels, 3 x 10 bits (chunks of <= 1023 cells)
+    __host__ __device__ static constexpr int col_words(int fields) { return (LW + fields - 1) / fields; }
 };
 
 template <int NORM, int M, int TAU, bool MULTI>
@@ -386,6 +388,7 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
     using CD = CellDist<NORM, M, TAU, 0>;
     uint32_t lut, beta, kind;         // shared-window addresses of the bucket table, the boundaries, the level kinds
     uint32_t cols;                    // ... of this thread's column, level 0
+    uint32_t col_row;                 // bytes between the levels of a column
     float* wbuf;                      // this warp's candidate buffer
     float* gcand;                     // the series' candidate list
     unsigned long long* gncand;
@@ -424,8 +427,7 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
             while (d > lds_f32(beta + 4 * q)) ++q;
             cand = lds_u8(kind + q) == LEVEL_CAND;
         }
-        static_assert(CountSmem::col_row == 1024 || CountSmem::col_row == 512, "level offset must shift bits 30-31 out");
-        if (live) red_u32(cols + q * CountSmem::col_row, inc);
+        if (live) red_u32(cols + q * col_row, inc);         // col_row is a multiple of 4: bits 30-31 of q drop out
         const unsigned mc = __ballot_sync(FULL, live && cand);
         if (mc) {
             const uint32_t nc = __popc(mc);
@@ -441,7 +443,7 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
 };
 
 template <int NORM, int M, int TAU>
-__global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev, int heavy_pass) {
+__global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev, int fields, int heavy_pass) {
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;
     const int tid = threadIdx.x, b = blockIdx.y;
@@ -456,11 +458,12 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     uint32_t* cols_s = (uint32_t*)(smem + CountSmem::off_cols);
     const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
     const int LA = window_la(a.L, span, 0), LB = window_lb(a.L, span, 0);
-    float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * CountSmem::col_row);
+    const int col_words = CountSmem::col_words(fields), field_bits = fields == 2 ? 16 : 10;
+    float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * 4 * col_words);
     float* yb_s = ya_s + LA;
     for (int q = tid; q < NBS; q += LW) lut_s[q] = T.lut[q];
     if (tid < NCUT) { beta_s[tid] = T.beta[tid]; ((uint8_t*)(smem + CountSmem::off_kind))[tid] = T.kind[tid]; }
-    for (int q = tid; q < nlev * (LW / 2); q += LW) cols_s[q] = 0;
+    for (int q = tid; q < nlev * col_words; q += LW) cols_s[q] = 0;
     __syncthreads();
     const int ob = s_ob;
     const int c = (int)(tile - a.tile_start[ob]);
@@ -488,14 +491,15 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
             ct.lut = smem_addr(lut_s);
             ct.beta = smem_addr(beta_s);
             ct.kind = smem_addr(smem + CountSmem::off_kind);
-            ct.cols = pin(smem_addr(cols_s) + 4 * (tid & (LW / 2 - 1)));
+            ct.cols = pin(smem_addr(cols_s) + 4 * (tid % col_words));
+            ct.col_row = pin(4u * (uint32_t)col_words);
             ct.wbuf = cand_s + (tid >> 5) * WCAP;
             ct.gcand = a.cand + (unsigned long long)b * a.cap;
             ct.gncand = &a.ss[b].ncand;
             ct.cap = a.cap;
             ct.scale = T.scale;
             ct.dcap = T.dcap;
-            ct.inc = pin(tid < LW / 2 ? 1u : 0x10000u);
+            ct.inc = pin(1u << (field_bits * (tid / col_words)));
             ct.wcount = 0;
             ct.lane_lt = (1u << (tid & 31)) - 1u;
             ct.prime();
@@ -519,9 +523,13 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
         const int warp = tid >> 5, lane = tid & 31;
         unsigned long long* lc = a.ss[b].level_count;
         for (int row = warp; row < nlev; row += LW / 32) {
-            const uint32_t* r = cols_s + row * (LW / 2);
+            const uint32_t* r = cols_s + row * col_words;
             uint32_t sum = 0;
-            for (int q = lane; q < LW / 2; q += 32) { uint32_t w = r[q]; sum += (w & 0xffffu) + (w >> 16); }
+            const uint32_t fmask = (1u << field_bits) - 1u;
+            for (int q = lane; q < col_words; q += 32) {
+                uint32_t w = r[q];
+                sum += (w & fmask) + ((w >> field_bits) & fmask) + (fields == 3 ? w >> 20 : 0u);
+            }
             for (int off = 16; off; off >>= 1) sum += __shfl_down_sync(FULL, sum, off);
             if (lane == 0 && sum) atomicAdd(&lc[row], (unsigned long long)sum);
         }
@@ -753,6 +761,7 @@ struct SelectPlan {
     int L, n_ob;
     uint32_t tiles;
     int span;
+    int fields;                       // counting pass: threads per counter word (2 or 3)
 };
 
 SelectPlan make_select_plan(const View& v, int K) {
@@ -778,15 +787,17 @@ SelectPlan make_select_plan(const View& v, int K) {
         p.cap = std::min(cap, p.P);
         const double cells = (double)p.P * (double)v.batch;
         int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
-        p.L = (int)std::max<int64_t>(32, std::min<int64_t>(2047, L));
+        // more than 20 brackets per group: 10-bit counters (two blocks per SM still fit), so shorter chunks
+        p.fields = std::min(K, GK) > 20 ? 3 : 2;
+        p.L = (int)std::max<int64_t>(32, std::min<int64_t>(p.fields == 3 ? 1023 : 2047, L));
         p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
         p.tiles = (uint32_t)count_tiles(v.n, p.L);
     }
     return p;
 }
 
-size_t count_smem_bytes(int nlev, int L, int span) {
-    return (size_t)CountSmem::off_cols + (size_t)nlev * CountSmem::col_row +
+size_t count_smem_bytes(int nlev, int fields, int L, int span) {
+    return (size_t)CountSmem::off_cols + (size_t)nlev * 4 * CountSmem::col_words(fields) +
            4 * ((size_t)window_la(L, span, 0) + window_lb(L, span, 0));
 }
 
@@ -796,11 +807,11 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
     // second launch: only the series whose table carries extra single-value levels (massive ties); its blocks
     // of the other series return at once, and so do the first launch's blocks of those series
     const int nlev_heavy = 2 * nlev - 1;
-    const size_t smem = count_smem_bytes(nlev, p.L, p.span), smem_heavy = count_smem_bytes(nlev_heavy, p.L, p.span);
+    const size_t smem = count_smem_bytes(nlev, p.fields, p.L, p.span), smem_heavy = count_smem_bytes(nlev_heavy, p.fields, p.L, p.span);
     RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_heavy));
-    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, 0);
+    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, p.fields, 0);
     RQA_LAUNCH_CHECK();
-    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem_heavy, s>>>(a, nlev_heavy, 1);
+    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem_heavy, s>>>(a, nlev_heavy, p.fields, 1);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }
@@ -808,6 +819,8 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
 template <int NORM>
 rqa_status dispatch_count(const CountArgs& a, const SelectPlan& p, int nlev, int batch, cudaStream_t s) {
     if (a.m == 3 && a.tau == 1) return launch_count<NORM, 3, 1>(a, p, nlev, batch, s);
+    if (a.m == 3 && a.tau == 3) return launch_count<NORM, 3, 3>(a, p, nlev, batch, s);
+    if (a.m == 5 && a.tau == 2) return launch_count<NORM, 5, 2>(a, p, nlev, batch, s);
     return launch_count<NORM, 0, 0>(a, p, nlev, batch, s);
 }
 

@@ -21,7 +21,7 @@ LIB = PKG / "librqa.so"
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
     "-I", str(ROOT / "include"), "-I", str(CSRC),
 ]
 
@@ -42,10 +42,23 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
+    objdir = PKG / "build"
+    objdir.mkdir(exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+    # one nvcc per translation unit, side by side (the two big ones take about a minute each), then link
+    jobs = []
+    for src in sources():
+        obj = objdir / f"{src.stem}.{os.getpid()}.o"
+        jobs.append((obj, subprocess.Popen([nvcc, *NVCC_FLAGS, *extra, "-c", "-o", str(obj), str(src)])))
+    failed = [str(obj) for obj, proc in jobs if proc.wait() != 0]
+    if failed:
+        raise RuntimeError(f"nvcc failed for {failed}")
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", str(tmp), *map(str, sources())]
-    subprocess.run(cmd, check=True)
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(tmp), *[str(obj) for obj, _ in jobs]],
+                   check=True)
     os.replace(tmp, LIB)
+    for obj, _ in jobs:
+        obj.unlink(missing_ok=True)
     return LIB
 
 

@@ -271,11 +271,12 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     // cells before the chunk), cnt = this lane's number of cells.  PHASE 0: the first cells of the chunk (t < 4,
     // guarded), 1: the part of the chunk where every lane is inside (unguarded; t is not used), 2: the tail (guarded).
     template <int R, int PHASE>
-    __device__ __forceinline__ void cell(int t, int cnt, bool at_diag_start) {
+    __device__ __forceinline__ void cell(int t, int cnt, int first_real) {
         constexpr bool GUARD = PHASE != 1;
         CD::template push<R>();
         if (GUARD && t < 0) {
-            uint32_t v4 = at_diag_start ? J4 : level4(CD::template distance<R>());
+            // cells before the start of the diagonal do not exist: not recurrent at any threshold
+            uint32_t v4 = t < first_real ? J4 : level4(CD::template distance<R>());
             v2 = v1; v1 = v4;
             return;
         }
@@ -331,7 +332,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     }
 
     template <int PHASE, int... R>
-    __device__ __forceinline__ void superstep(int t, int cnt, bool ds, std::integer_sequence<int, R...>) {
+    __device__ __forceinline__ void superstep(int t, int cnt, int ds, std::integer_sequence<int, R...>) {
         (cell<R, PHASE>(t + R, cnt, ds), ...);
         CD::advance((int)sizeof...(R));
         if (PHASE == 1) trel8 += (uint32_t)sizeof...(R) << 8;
@@ -363,7 +364,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
 // The walk of one thread along its chunk.  Two instantiations (MULTI) so that the common case, every bucket of the
 // level table holding at most one threshold, carries no refinement loop; a block executes only one of them.
 template <int NORM, int M, int TAU, int NP, bool MULTI>
-__device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc, int cnt, int cnt_lo, int cnt_hi, bool ds,
+__device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc, int cnt, int cnt_lo, int cnt_hi, int ds,
                                            uint32_t yb_org, uint16_t* suf_out) {
     using SC = Scanner<NORM, M, TAU, NP, MULTI>;
     constexpr int S = SC::S;
@@ -462,14 +463,15 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
             sc.xa = sc.xb = 0;
             sc.A = 0; sc.ts = 0; sc.top = sc.stk;           // every threshold: recurrent since the chunk start
         };
+        const int first_real = -(int)min((int64_t)2, s);     // warm-up cells before it lie outside the plot
         if (G.multi) {
             Scanner<NORM, M, TAU, NP, true> sc;
             setup(sc);
-            scan_chunk(sc, cnt, cnt_lo, cnt_hi, s == 0, yb_org, a.suf + out_row);
+            scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org, a.suf + out_row);
         } else {
             Scanner<NORM, M, TAU, NP, false> sc;
             setup(sc);
-            scan_chunk(sc, cnt, cnt_lo, cnt_hi, s == 0, yb_org, a.suf + out_row);
+            scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org, a.suf + out_row);
         }
     }
     __syncthreads();

@@ -435,3 +435,18 @@ def test_paper_sweep_k99_prefix_measures_sorting(rqa, oracle):
     rqa.rqa_line_measures(buf.hist, 2, None, Lmax=torch.empty((batch, K), dtype=torch.int64, device=s.device))
     with pytest.raises(rqa.RqaError):
         rqa.rqa_sorting_rate_host(np.zeros((1, 1)))
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 4, 5, 7, 26, 100, 1023])
+def test_line_hist_any_chunk_length(rqa, oracle, options, L):
+    """The diagonal scan cuts every diagonal into chunks of L cells and joins the runs that cross chunk borders
+    afterwards.  Chunks shorter than the 4-cell window of the run stack, chunks that end inside a drain window, and
+    one chunk per diagonal must all give the oracle's histograms: a noisy sine (short and long lines), an exactly
+    periodic one (lines as long as the diagonals) and a quantised series, embedded and not."""
+    options(line_chunk=L)
+    rr = wl.rr_log(12, 0.002, 0.5)
+    ys = np.stack([wl.add_noise(wl.sine_signal(1300), 2.0, 8), wl.sine_signal(1300).astype(np.float32),
+                   np.round(wl.gaussian(13, 1300) * 3.0).astype(np.float32)])
+    for m, tau in ((3, 1), (1, 1), (2, 7)):
+        g = gpu_sweep(rqa, ys, m, tau, rr, 0)
+        assert_parity(oracle, g, ys, m, tau, rr, 0, threads=0)

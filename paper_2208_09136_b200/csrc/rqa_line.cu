@@ -3,7 +3,7 @@
 // computed on the fly, never stored).  Design notes: DESIGN.md "Kernel: diagonal scan".
 //
 // Work decomposition
-//   tile   = 256 adjacent diagonals (one per thread) x one chunk of <= 1023 positions; a thread walks its
+//   tile   = 512 adjacent diagonals (one per thread) x one chunk of <= 1023 positions; a thread walks its
 //            chunk of its diagonal sequentially, lanes of a warp read y[i] (broadcast) and y[i+o+lane]
 //            (consecutive) from two windows of the series staged in shared memory.
 //   cell   : distance d (sliding window over e_i = |y_i - y_{i+o}| for the max norm), then its LEVEL
@@ -12,11 +12,14 @@
 //   runs   : thresholds are nested, so the runs of all thresholds along a diagonal form a monotone stack of
 //            (lowest threshold, start position); it changes only when the maximum level of the last 4 cells
 //            changes, and one popped entry is one line length for a whole RANGE of thresholds, counted in a
-//            difference array over the thresholds.  The work per cell does not depend on K.
+//            difference array over the thresholds.  The work per cell does not depend on K.  In the bulk of a
+//            chunk a thread only notes the changes in a small queue; all lanes replay their queues together
+//            every 24 cells, so that the divergent stack code runs with most lanes busy.
 //   lines  : P_j(1), P_j(2), P_j(3) are NOT emitted line by line.  The kernel histograms the level of every
 //            cell and the window maxima of 2 and 3 consecutive levels (thread-private shared-memory words of three
-//            10-bit counters, no conflicts; a chunk has <= 1023 cells); their prefix sums over the level are C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and
-//            Q3_j = sum_{l>=3} (l-2)*P_j(l), from which the finalize kernel solves P_j(1..3) exactly.
+//            10-bit counters, no conflicts; a chunk has <= 1023 cells); their prefix sums over the level are
+//            C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and Q3_j = sum_{l>=3} (l-2)*P_j(l), from which the
+//            finalize kernel solves P_j(1..3) exactly.
 //            Lines of length >= 4 that lie inside a chunk go to the shared-memory difference array (l < 128) or
 //            to global atomics (longer).  Runs touching a chunk border are written as (prefix, suffix) summaries
 //            and joined along each diagonal by the stitch kernel.
@@ -27,7 +30,7 @@ namespace rqa {
 
 namespace {
 
-constexpr int LMAX = 1023;       // longest chunk: cell positions fit the 10 bits of a stack entry, counters 16 bits
+constexpr int LMAX = 1023;       // longest chunk: cell positions fit the 10 bits of a stack entry, counters 10 bits
 constexpr int LS = 128;          // lines shorter than this are counted in shared memory
 constexpr int LMIN_EXPLICIT = 4; // lines of length >= 4 are emitted one by one; 1..3 come from the aggregates
 constexpr int QCELLS = 24;       // cells between two drains of the per-thread event queues (= their capacity)

@@ -13,10 +13,13 @@
 //                 holds the true eps_k with overwhelming probability;
 //              2. the counting pass visits every cell once (tiles, sliding-window distance, level table as in the
 //                 diagonal scan), counts the cells of every inter-boundary level exactly (thread-private
-//                 shared-memory columns, no conflicts) and appends the few cells inside brackets to a candidate list;
-//              3. the exact counts locate each target's rank inside its bracket — this is a proof, not a guess: if
-//                 a rank falls outside its bracket (or the candidate list overflows, e.g. massive ties) the series is
-//                 flagged and handled by RADIX — and the buffer select over the candidates gives eps_k and C_k.
+//                 shared-memory counters, no conflicts) and appends the few cells inside brackets to a candidate
+//                 list.  Values with massive ties (a collapsed bracket, a bracket end the sample holds thousands of
+//                 times) get a single-value level of their own: counted, never appended;
+//              3. the exact counts locate each target's rank — this is a proof, not a guess: a single-value level
+//                 gives eps_k and C_k at once, a bracket gives the rank among the candidates and the buffer select
+//                 over them gives eps_k and C_k; if a rank falls outside every bracket (or the candidate list
+//                 overflows) the series is flagged and handled by RADIX.
 //   RADIX    (general strided views; fallback)  most-significant-digit radix select, 4 full passes of 8 bits, all K
 //            targets resolved in each pass; targets that share a prefix share one 256-bin histogram.
 #include <algorithm>

@@ -150,10 +150,13 @@ rqa_status rqa_det_prefix_avg(const double* d_det, int32_t batch, int32_t K, dou
  *   d_L        [batch][K] average diagonal line length  sum_{l>=l_min} l*P_k(l) / sum_{l>=l_min} P_k(l)  (0 if no line)
  *   d_Lmax     [batch][K] longest diagonal line  max{ l : P_k(l) > 0 }  (0 if none)
  *   d_rr_hist  [batch][K] recurrence rate from the histogram  sum_{l>=1} l*P_k(l) / P,  P = N'(N'-1)/2
- * Any of the three outputs may be NULL.  Sums are exact uint64; the ratios one fp64 division.
+ * and, as one of the "other RQA measures" the averaging applies to (not defined in the paper itself),
+ *   d_entr     [batch][K] Shannon entropy of the line-length distribution  -sum_{l>=l_min} p(l) ln p(l),
+ *              p(l) = P_k(l) / sum_{l>=l_min} P_k(l)  (0 if no line), computed as ln T - (1/T) sum P ln P in fp64.
+ * Any of the four outputs may be NULL.  Integer sums are exact uint64; L and RR are one fp64 division.
  */
 rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
-                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, void* stream);
+                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, double* d_entr, void* stream);
 
 /*
  * Sorting rate S (Eq. 6), the paper's evaluation score; plain host arithmetic on R*n numbers.

@@ -269,10 +269,12 @@ int rqa_oracle_det_prefix_avg(const double* det, int K, double* prefix) {
 
 /* The other measures read off the histogram ("DET, L, L_max and RR"): average diagonal line length
  * L_k = sum_{l>=l_min} l*P_k(l) / sum_{l>=l_min} P_k(l) (0 without lines), longest line L_max, and the recurrence rate
- * sum_{l>=1} l*P_k(l) / P with P = N'(N'-1)/2 (reading S2: upper triangle, main diagonal excluded). */
+ * sum_{l>=1} l*P_k(l) / P with P = N'(N'-1)/2 (reading S2: upper triangle, main diagonal excluded); and the Shannon
+ * entropy of the line-length distribution, ENTR_k = -sum_{l>=l_min} p(l) ln p(l), p(l) = P_k(l) / sum_{l>=l_min} P_k(l)
+ * (one of the "other RQA measures" of PAPER.md:86; the paper does not define it, this is the textbook definition). */
 int rqa_oracle_line_measures(const uint64_t* hist, int K, int64_t n_points, int64_t l_min, double* L, uint64_t* Lmax,
-                             double* rr_hist) {
-    if (!hist || !L || !Lmax || !rr_hist || K < 1 || n_points < 2 || l_min < 1) return ORACLE_BAD_ARG;
+                             double* rr_hist, double* entr) {
+    if (!hist || !L || !Lmax || !rr_hist || !entr || K < 1 || n_points < 2 || l_min < 1) return ORACLE_BAD_ARG;
     const double P = (double)((uint64_t)n_points * (uint64_t)(n_points - 1) / 2);
     for (int k = 0; k < K; ++k) {
         uint64_t pts = 0, lpts = 0, lines = 0, lmax = 0;
@@ -285,6 +287,13 @@ int rqa_oracle_line_measures(const uint64_t* hist, int K, int64_t n_points, int6
         L[k] = lines ? (double)lpts / (double)lines : 0.0;
         Lmax[k] = lmax;
         rr_hist[k] = (double)pts / P;
+        /* entropy of the line-length distribution, the definition written out: -sum p(l) ln p(l), l ascending */
+        double e = 0.0;
+        for (int64_t l = l_min; l < n_points && lines; ++l) {
+            const uint64_t h = hist[(size_t)k * n_points + l];
+            if (h) { const double pl = (double)h / (double)lines; e -= pl * std::log(pl); }
+        }
+        entr[k] = e;
     }
     return ORACLE_OK;
 }

@@ -58,7 +58,7 @@ def _load():
     lib.rqa_oracle_line_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i32]
     lib.rqa_oracle_det_avg.argtypes = [u64p, i32, i64, i64, f64p, f64p]
     lib.rqa_oracle_det_prefix_avg.argtypes = [f64p, i32, f64p]
-    lib.rqa_oracle_line_measures.argtypes = [u64p, i32, i64, i64, f64p, u64p, f64p]
+    lib.rqa_oracle_line_measures.argtypes = [u64p, i32, i64, i64, f64p, u64p, f64p, f64p]
     lib.rqa_oracle_sorting_rate.argtypes = [f64p, i32, i32, f64p]
     _lib = lib
     return lib
@@ -173,15 +173,17 @@ def det_prefix_avg(det) -> np.ndarray:
 
 
 def line_measures(hist, l_min: int = 2):
-    """-> (L[K] float64, Lmax[K] uint64, rr_hist[K] float64)"""
+    """-> (L[K] float64, Lmax[K] uint64, rr_hist[K] float64, entr[K] float64)"""
     hist = np.ascontiguousarray(hist, dtype=np.uint64)
     K, n = hist.shape
     L = np.empty(K, dtype=np.float64)
     Lmax = np.empty(K, dtype=np.uint64)
     rr = np.empty(K, dtype=np.float64)
+    entr = np.empty(K, dtype=np.float64)
     _check(_load().rqa_oracle_line_measures(_p(hist, ctypes.c_uint64), K, n, l_min, _p(L, ctypes.c_double),
-                                            _p(Lmax, ctypes.c_uint64), _p(rr, ctypes.c_double)), "line_measures")
-    return L, Lmax, rr
+                                            _p(Lmax, ctypes.c_uint64), _p(rr, ctypes.c_double),
+                                            _p(entr, ctypes.c_double)), "line_measures")
+    return L, Lmax, rr, entr
 
 
 def sorting_rate(measure) -> float:

@@ -72,7 +72,7 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_sweep_host.argtypes = [vp, i64, i32, i32, i64, ctypes.c_int, vp, i32, i64, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.rqa_set_option.argtypes = [ctypes.c_char_p, i64]
     lib.rqa_det_prefix_avg.argtypes = [vp, i32, i32, vp, vp]
-    lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp, vp]
+    lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp, vp, vp]
     lib.rqa_sorting_rate_host.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double)]
     _lib = lib
     return lib
@@ -176,14 +176,16 @@ def rqa_det_prefix_avg(det, prefix, stream=None) -> None:
                                              _dev(prefix, torch.float64, "prefix"), _stream(stream)))
 
 
-def rqa_line_measures(hist, l_min: int, L=None, Lmax=None, rr_hist=None, stream=None) -> None:
-    """hist int64 CUDA [batch][K][n_points]; L, rr_hist float64 [batch][K]; Lmax int64 [batch][K]; each may be None."""
+def rqa_line_measures(hist, l_min: int, L=None, Lmax=None, rr_hist=None, entr=None, stream=None) -> None:
+    """hist int64 CUDA [batch][K][n_points]; L, rr_hist, entr float64 [batch][K]; Lmax int64 [batch][K]; each may be
+    None."""
     import torch
     batch, K, n = hist.shape
     _check(load_library().rqa_line_measures(_dev(hist, torch.int64, "hist"), batch, K, n, l_min,
                                             None if L is None else _dev(L, torch.float64, "L"),
                                             None if Lmax is None else _dev(Lmax, torch.int64, "Lmax"),
                                             None if rr_hist is None else _dev(rr_hist, torch.float64, "rr_hist"),
+                                            None if entr is None else _dev(entr, torch.float64, "entr"),
                                             _stream(stream)))
 
 

@@ -1,6 +1,7 @@
 // rqa_measures.cu — the cheap reductions that sit on top of the line histograms:
 //   rqa_det_prefix_avg     Eq. 5 as a curve: the averaged determinism for every cut-off RR*
-//   rqa_line_measures      "the histogram is used for the calculation of (DET, L, L_max and RR)"
+//   rqa_line_measures      "the histogram is used for the calculation of (DET, L, L_max and RR)",
+//                          plus the entropy of the line-length distribution (one of the "other RQA measures")
 //   rqa_sorting_rate_host  Eq. 6, the paper's evaluation score (host arithmetic on a few numbers)
 #include "rqa_common.cuh"
 
@@ -21,35 +22,44 @@ __global__ void det_prefix_kernel(const double* __restrict__ det, int K, int bat
 // One block per (threshold, series): exact uint64 sums over the histogram row.
 __global__ void __launch_bounds__(256) line_measures_kernel(const uint64_t* __restrict__ hist, int K, int64_t n, int64_t l_min,
                                                             double* __restrict__ L, uint64_t* __restrict__ Lmax,
-                                                            double* __restrict__ rr) {
+                                                            double* __restrict__ rr, double* __restrict__ entr) {
     const int k = blockIdx.x, b = blockIdx.y;
     const uint64_t* row = hist + ((int64_t)b * K + k) * n;
     unsigned long long pts = 0, lpts = 0, lines = 0, lmax = 0;
+    double hlogh = 0.0;                                      // sum h ln h: ENTR = ln T - (1/T) sum h ln h, T = #lines
     for (int64_t l = 1 + threadIdx.x; l < n; l += blockDim.x) {
         const unsigned long long h = row[l];
         pts += (unsigned long long)l * h;
-        if (l >= l_min) { lpts += (unsigned long long)l * h; lines += h; }
+        if (l >= l_min) {
+            lpts += (unsigned long long)l * h;
+            lines += h;
+            if (entr && h > 1) hlogh += (double)h * log((double)h);
+        }
         if (h) lmax = (unsigned long long)l;                 // l increases along the loop
     }
     __shared__ unsigned long long s[4][8];
+    __shared__ double s_e[8];
     for (int off = 16; off; off >>= 1) {
         pts += __shfl_down_sync(0xffffffffu, pts, off);
         lpts += __shfl_down_sync(0xffffffffu, lpts, off);
         lines += __shfl_down_sync(0xffffffffu, lines, off);
         lmax = max(lmax, __shfl_down_sync(0xffffffffu, lmax, off));
+        hlogh += __shfl_down_sync(0xffffffffu, hlogh, off);
     }
     if ((threadIdx.x & 31) == 0) {
         const int w = threadIdx.x >> 5;
-        s[0][w] = pts; s[1][w] = lpts; s[2][w] = lines; s[3][w] = lmax;
+        s[0][w] = pts; s[1][w] = lpts; s[2][w] = lines; s[3][w] = lmax; s_e[w] = hlogh;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
         pts = lpts = lines = lmax = 0;
-        for (int w = 0; w < 8; ++w) { pts += s[0][w]; lpts += s[1][w]; lines += s[2][w]; lmax = max(lmax, s[3][w]); }
+        hlogh = 0.0;
+        for (int w = 0; w < 8; ++w) { pts += s[0][w]; lpts += s[1][w]; lines += s[2][w]; lmax = max(lmax, s[3][w]); hlogh += s_e[w]; }
         const int64_t o = (int64_t)b * K + k;
         if (L) L[o] = lines ? (double)lpts / (double)lines : 0.0;
         if (Lmax) Lmax[o] = lmax;
         if (rr) rr[o] = (double)pts / (double)((unsigned long long)n * (unsigned long long)(n - 1) / 2);
+        if (entr) entr[o] = lines ? log((double)lines) - hlogh / (double)lines : 0.0;
     }
 }
 
@@ -69,10 +79,10 @@ rqa_status rqa_det_prefix_avg(const double* d_det, int32_t batch, int32_t K, dou
 }
 
 rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
-                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, void* stream) {
+                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, double* d_entr, void* stream) {
     if (!d_hist) { set_error("rqa_line_measures: d_hist is NULL"); return RQA_ERR_INVALID_ARG; }
     if (batch < 1 || K < 1 || K > RQA_MAX_K || n_points < 2 || l_min < 1) { set_error("rqa_line_measures: need batch >= 1, 1 <= K <= %d, n_points >= 2, l_min >= 1", RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
-    line_measures_kernel<<<dim3(K, batch), 256, 0, (cudaStream_t)stream>>>(d_hist, K, n_points, l_min, d_L, d_Lmax, d_rr_hist);
+    line_measures_kernel<<<dim3(K, batch), 256, 0, (cudaStream_t)stream>>>(d_hist, K, n_points, l_min, d_L, d_Lmax, d_rr_hist, d_entr);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }

@@ -397,17 +397,24 @@ def test_line_measures_hand_cases(oracle):
     A (y=0,1,0,1,0,1, m=1, rr=0.4): P(2)=P(4)=1 -> L=3, L_max=4, RR=6/15.
     E (y=0,2,1,4,0,2,1,4,3, m=2, tau=2, rr=0.5): P(1)=5,P(2)=2,P(3)=1,P(5)=1 -> L=(4+3+5)/4=3, L_max=5, RR=17/21."""
     r = oracle.sweep(np.array([0, 1, 0, 1, 0, 1], dtype=np.float32), 1, 1, [0.4], oracle.NORM_MAX, 2)
-    L, Lmax, rr = oracle.line_measures(r["hist"], 2)
+    L, Lmax, rr, entr = oracle.line_measures(r["hist"], 2)
     assert (L[0], int(Lmax[0]), rr[0]) == (3.0, 4, 6 / 15)
+    assert entr[0] == pytest.approx(math.log(2.0), abs=1e-15)          # two lines of different length: p = 1/2, 1/2
     r = oracle.sweep(np.array([0, 2, 1, 4, 0, 2, 1, 4, 3], dtype=np.float32), 2, 2, [0.5], oracle.NORM_MAX, 2)
-    L, Lmax, rr = oracle.line_measures(r["hist"], 2)
+    L, Lmax, rr, entr = oracle.line_measures(r["hist"], 2)
     assert (L[0], int(Lmax[0]), rr[0]) == (3.0, 5, 17 / 21)
+    assert entr[0] == pytest.approx(1.5 * math.log(2.0), abs=1e-15)    # p = 1/2, 1/4, 1/4
     assert rr[0] == r["rr"][0]                       # "RR can also be calculated from the histogram" (PAPER.md:125)
-    L1, _, _ = oracle.line_measures(r["hist"], 1)    # l_min = 1: all 9 lines, 17 points
+    L1, _, _, e1 = oracle.line_measures(r["hist"], 1)    # l_min = 1: all 9 lines, 17 points
     assert L1[0] == 17 / 9
+    p = np.array([5, 2, 1, 1]) / 9.0
+    assert e1[0] == pytest.approx(float(-(p * np.log(p)).sum()), abs=1e-15)
     empty = np.zeros((1, 7), dtype=np.uint64)
-    L, Lmax, rr = oracle.line_measures(empty, 2)
-    assert (L[0], int(Lmax[0]), rr[0]) == (0.0, 0, 0.0)
+    L, Lmax, rr, entr = oracle.line_measures(empty, 2)
+    assert (L[0], int(Lmax[0]), rr[0], entr[0]) == (0.0, 0, 0.0, 0.0)
+    single = np.zeros((1, 7), dtype=np.uint64)
+    single[0, 3] = 11                                 # one line length only: no uncertainty
+    assert oracle.line_measures(single, 2)[3][0] == 0.0
 
 
 def test_sorting_rate_pins(oracle):

@@ -415,16 +415,19 @@ def test_paper_sweep_k99_prefix_measures_sorting(rqa, oracle):
     L = torch.empty_like(buf.det)
     Lmax = torch.empty((batch, K), dtype=torch.int64, device=s.device)
     rrh = torch.empty_like(buf.det)
+    entr = torch.empty_like(buf.det)
     rqa.rqa_det_prefix_avg(buf.det, prefix)
-    rqa.rqa_line_measures(buf.hist, 2, L, Lmax, rrh)
+    rqa.rqa_line_measures(buf.hist, 2, L, Lmax, rrh, entr)
     torch.cuda.synchronize()
     g = {"eps": buf.eps.cpu().numpy(), "count": buf.count.cpu().numpy().view(np.uint64), "rr": buf.rr.cpu().numpy(),
          "hist": buf.hist.cpu().numpy().view(np.uint64), "det": buf.det.cpu().numpy(), "det_mean": buf.det_mean.cpu().numpy()}
     assert_parity(oracle, g, series, 1, 1, rr, 0, 2)
     prefix, L, Lmax, rrh = prefix.cpu().numpy(), L.cpu().numpy(), Lmax.cpu().numpy().view(np.uint64), rrh.cpu().numpy()
+    entr = entr.cpu().numpy()
     for b in range(batch):
         assert np.max(np.abs(prefix[b] - oracle.det_prefix_avg(g["det"][b]))) <= DET_TOL
-        oL, oLmax, orr = oracle.line_measures(g["hist"][b], 2)
+        oL, oLmax, orr, oentr = oracle.line_measures(g["hist"][b], 2)
+        assert np.max(np.abs(entr[b] - oentr)) <= 1e-11       # a different summation order and another libm's log
         assert np.max(np.abs(L[b] - oL)) <= DET_TOL and np.array_equal(Lmax[b], oLmax)
         assert np.max(np.abs(rrh[b] - orr)) <= DET_TOL and np.array_equal(rrh[b], g["rr"][b])
         assert prefix[b][0] == g["det"][b][0] and abs(prefix[b][-1] - g["det_mean"][b]) <= DET_TOL

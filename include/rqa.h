@@ -123,6 +123,8 @@ rqa_status rqa_eps_for_rr(const rqa_points* pts, rqa_norm norm, const double* h_
  *   d_hist  [batch][K][n_points] uint64, overwritten: d_hist[b][k][l] = number of maximal runs of exactly l
  *           consecutive recurrent cells (d <= eps_k) along the diagonals j-i = 1..N'-1; [..][0] = 0.
  * Invariant tying it to rqa_eps_for_rr: sum_l l*d_hist[b][k][l] == C_k.
+ * The strict Heaviside of the paper's Eq. 2 (H(0) = 0, recurrence means d < eps) needs no other kernel:
+ * fp32 distances are discrete, so d < eps is d <= nextafterf(eps, -inf) for eps > 0; pass those thresholds.
  */
 rqa_status rqa_line_hist(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
                          void* d_ws, size_t ws_bytes, void* stream);

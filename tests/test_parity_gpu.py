@@ -213,6 +213,40 @@ def test_line_hist_with_caller_thresholds(rqa, oracle):
     assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], oracle.line_hist(y, 3, 1, eps, 0))
 
 
+def test_strict_heaviside_by_previous_float(rqa):
+    """The paper's Eq. 2 has H(0) = 0, i.e. recurrence means d < eps (reading S1 fixes d <= eps for the
+    order statistics).  fp32 distances are discrete, so d < eps is d <= the float just below eps: rqa_line_hist with
+    nextafter(eps, -inf) gives the strict plot.  Checked against a brute-force numpy recurrence plot with a strict
+    compare, at thresholds that ARE distances of the series (where the two conventions differ)."""
+    import torch
+    y = np.round(wl.add_noise(wl.logistic_signal(400, 6), 2.0, 6) * 8.0).astype(np.float32) / 8.0   # ties on purpose
+    m, tau = 2, 3
+    n = len(y) - (m - 1) * tau
+    X = np.stack([y[c * tau:c * tau + n] for c in range(m)], axis=1)
+    D = np.abs(X[:, None, :] - X[None, :, :]).max(axis=2)
+    eps = np.array([0.125, 0.5, 1.0, 0.375], dtype=np.float32)
+    assert all((D == e).any() for e in eps)
+    want = np.zeros((len(eps), n), dtype=np.uint64)
+    for k, e in enumerate(eps):
+        R = D < e
+        for o in range(1, n):
+            run = 0
+            for v in np.append(np.diagonal(R, o), False):
+                if v:
+                    run += 1
+                elif run:
+                    want[k, run] += 1
+                    run = 0
+    s = torch.as_tensor(y).cuda().unsqueeze(0)
+    view = rqa.rqa_embed(s, m, tau)
+    hist = torch.empty((1, len(eps), n), dtype=torch.int64, device="cuda")
+    ws = torch.empty(rqa.rqa_workspace_bytes(view, len(eps)), dtype=torch.uint8, device="cuda")
+    below = np.nextafter(eps, np.float32(-np.inf)).astype(np.float32)
+    rqa.rqa_line_hist(view, 0, torch.as_tensor(below).cuda().unsqueeze(0), hist, ws)
+    rqa.rqa_workspace_status(ws)
+    assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], want)
+
+
 def test_nonfinite_input_is_reported(rqa):
     import torch
     y = wl.gaussian(2, 300).astype(np.float32)

@@ -408,7 +408,8 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
     uint8_t* lut_s = (uint8_t*)(smem + SM::off_lut);
     float* eps_s = (float*)(smem + SM::off_eps);
     const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
-    const int LA = window_la(a.L, span, 2), LB = window_lb(a.L, span, 2);
+    const int ps = M > 0 ? 1 : (int)a.v.ps;
+    const int LA = window_la(a.L, span, 2, ps), LB = window_lb(a.L, span, 2, ps);
     float* ya_s = (float*)(smem + SM::off_ya);
     float* yb_s = ya_s + LA;
     uint32_t* agg_s = (uint32_t*)(smem + SM::off_agg);
@@ -428,10 +429,10 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
     const int64_t n = a.v.n;
     const int64_t o0 = 1 + (int64_t)LW * ob;
     const int64_t s = (int64_t)c * L;                       // chunk start along the diagonals
-    // the two windows of the series: y[s-2 + x] and y[s-2 + o0 + x]; the series has n + (M-1)*TAU samples
+    // the two windows: the floats of the points s-2.. and s-2+o0..; the n points span (n-1)*ps + span + 1 floats
     const float* y = a.v.data + (int64_t)b * a.v.bs;
-    const int64_t ny = n + span;
-    stage_windows(y, ny, s - 2, s - 2 + o0, ya_s, LA, yb_s, LB);
+    const int64_t ny = (n - 1) * ps + span + 1;
+    stage_windows(y, ny, (s - 2) * ps, (s - 2 + o0) * ps, ya_s, LA, yb_s, LB);
     __syncthreads();
 
     const int64_t o = o0 + tid;
@@ -443,7 +444,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
 
     if (cnt_hi > 0) {
         const int64_t out_row = (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
-        const uint32_t yb_org = pin(smem_addr(yb_s) + 4 * tid);
+        const uint32_t yb_org = pin(smem_addr(yb_s) + 4 * tid * ps);
         auto setup = [&](auto& sc) {
             sc.ya_org = smem_addr(ya_s);
             sc.lut = smem_addr(lut_s);
@@ -460,6 +461,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
             sc.J4 = 4u * (uint32_t)J;
             sc.m = a.m;
             sc.tau = a.tau;
+            sc.ps = ps;
             sc.n = (int64_t)pin64((unsigned long long)n);
             sc.v1 = sc.v2 = sc.J4;
             sc.w2a = sc.w2b = sc.J4;
@@ -657,26 +659,34 @@ struct LinePlan {
 int pairs_for(int kg) { return kg <= 10 ? 5 : (kg <= 20 ? 10 : 16); }
 
 template <int NP>
-size_t scan_smem_bytes(int L, int span) {
-    return (size_t)ScanSmem<NP>::off_ya + 4 * ((size_t)window_la(L, span, 2) + window_lb(L, span, 2));
+size_t scan_smem_bytes(int L, int span, int ps) {
+    return (size_t)ScanSmem<NP>::off_ya + 4 * ((size_t)window_la(L, span, 2, ps) + window_lb(L, span, 2, ps));
 }
+size_t scan_smem_bytes(int NP, int L, int span, int ps) {
+    return NP == 5 ? scan_smem_bytes<5>(L, span, ps) : (NP == 10 ? scan_smem_bytes<10>(L, span, ps) : scan_smem_bytes<16>(L, span, ps));
+}
+constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of sm_100a, minus the static part
 
 LinePlan make_plan(const View& v, int K) {
     LinePlan p{};
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
-    p.scan = v.ps == 1 && p.span <= MAX_SPAN;
     p.NG = (K + GK - 1) / GK;
     p.NP = pairs_for(std::min(K, GK));
+    const int ps = (int)std::min<int64_t>(v.ps, 1 << 20);
+    // tiled scan: delay views, and materialised points (point stride > 1) whose windows fit the shared memory
+    p.scan = p.span <= MAX_SPAN && scan_smem_bytes(p.NP, 32, p.span, ps) <= SMEM_PER_BLOCK_MAX;
     // chunk length: aim at >= 8 waves of 3 blocks per SM over the whole batch, at most 1023 positions
     const double cells = (double)n_pairs(v.n) * (double)v.batch;
     int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
     p.L = (int)std::max<int64_t>(32, std::min<int64_t>(LMAX, L));
     if (options().line_chunk > 0) p.L = (int)std::min<int64_t>(LMAX, options().line_chunk);
+    // wide points: the two windows hold (2L + 512) points, so the chunk shrinks until they fit (one block per SM then)
+    while (p.scan && p.L > 32 && scan_smem_bytes(p.NP, p.L, p.span, ps) > SMEM_PER_BLOCK_MAX) p.L = std::max(32, p.L / 2);
     p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
     uint64_t tiles = 0;
     for (int ob = 0; ob < p.n_ob; ++ob) tiles += (uint64_t)((v.n - 1 - (int64_t)LW * ob + p.L - 1) / p.L);
     p.tiles = (uint32_t)tiles;
-    p.smem = p.NP == 5 ? scan_smem_bytes<5>(p.L, p.span) : (p.NP == 10 ? scan_smem_bytes<10>(p.L, p.span) : scan_smem_bytes<16>(p.L, p.span));
+    p.smem = scan_smem_bytes(p.NP, p.L, p.span, ps);
     return p;
 }
 
@@ -692,9 +702,10 @@ rqa_status launch_scan(const ScanArgs& a, const LinePlan& p, int batch, cudaStre
 template <int NORM, int NP>
 rqa_status dispatch_embedding(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
     // the embeddings of BASELINE.json's large configs get a register ring; any other (m, tau) recomputes per cell
-    if (a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, batch, s);
-    if (a.m == 3 && a.tau == 3) return launch_scan<NORM, 3, 3, NP>(a, p, batch, s);
-    if (a.m == 5 && a.tau == 2) return launch_scan<NORM, 5, 2, NP>(a, p, batch, s);
+    const bool delay = a.v.ps == 1;
+    if (delay && a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, batch, s);
+    if (delay && a.m == 3 && a.tau == 3) return launch_scan<NORM, 3, 3, NP>(a, p, batch, s);
+    if (delay && a.m == 5 && a.tau == 2) return launch_scan<NORM, 5, 2, NP>(a, p, batch, s);
     return launch_scan<NORM, 0, 0, NP>(a, p, batch, s);
 }
 

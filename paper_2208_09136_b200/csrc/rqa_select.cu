@@ -460,7 +460,8 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     float* cand_s = (float*)(smem + CountSmem::off_cand);
     uint32_t* cols_s = (uint32_t*)(smem + CountSmem::off_cols);
     const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
-    const int LA = window_la(a.L, span, 0), LB = window_lb(a.L, span, 0);
+    const int ps = M > 0 ? 1 : (int)a.v.ps;
+    const int LA = window_la(a.L, span, 0, ps), LB = window_lb(a.L, span, 0, ps);
     const int col_words = CountSmem::col_words(fields), field_bits = fields == 2 ? 16 : 10;
     float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * 4 * col_words);
     float* yb_s = ya_s + LA;
@@ -475,7 +476,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     const int64_t o0 = 1 + (int64_t)LW * ob;
     const int64_t s = (int64_t)c * L;
     const float* y = a.v.data + (int64_t)b * a.v.bs;
-    stage_windows(y, n + span, s, s + o0, ya_s, LA, yb_s, LB);
+    stage_windows(y, (n - 1) * ps + span + 1, s * ps, (s + o0) * ps, ya_s, LA, yb_s, LB);
     __syncthreads();
 
     const int64_t len = n - (o0 + tid);
@@ -488,9 +489,10 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
         auto walk = [&](auto& ct) {
             using CT = std::remove_reference_t<decltype(ct)>;
             constexpr int S = CT::S;
-            ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid), 0);
             ct.m = a.m;
             ct.tau = a.tau;
+            ct.ps = ps;
+            ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid * ps), 0);
             ct.lut = smem_addr(lut_s);
             ct.beta = smem_addr(beta_s);
             ct.kind = smem_addr(smem + CountSmem::off_kind);
@@ -765,14 +767,24 @@ struct SelectPlan {
     uint32_t tiles;
     int span;
     int fields;                       // counting pass: threads per counter word (2 or 3)
+    int ps;                           // point stride in floats
 };
+
+size_t count_smem_bytes(int nlev, int fields, int L, int span, int ps) {
+    return (size_t)CountSmem::off_cols + (size_t)nlev * 4 * CountSmem::col_words(fields) +
+           4 * ((size_t)window_la(L, span, 0, ps) + window_lb(L, span, 0, ps));
+}
+constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of sm_100a, minus the static part
 
 SelectPlan make_select_plan(const View& v, int K) {
     const Options& opt = options();
     SelectPlan p{};
     p.P = n_pairs(v.n);
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
-    const bool tiled_ok = v.ps == 1 && p.span <= MAX_SPAN;
+    p.ps = (int)std::min<int64_t>(v.ps, 1 << 20);
+    // tiled counting pass: delay views, and materialised points whose windows fit beside the widest level table
+    const int nlev_max = 2 * (2 * std::min(K, GK) + 1) - 1;
+    const bool tiled_ok = p.span <= MAX_SPAN && count_smem_bytes(nlev_max, 3, 32, p.span, p.ps) <= SMEM_PER_BLOCK_MAX;
     p.path = (int)opt.select_path;
     if (p.path == PATH_AUTO) p.path = p.P <= (1ull << 22) ? PATH_DIRECT : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
     if (p.path == PATH_BRACKET && !tiled_ok) p.path = PATH_RADIX;
@@ -793,15 +805,11 @@ SelectPlan make_select_plan(const View& v, int K) {
         // more than 20 brackets per group: 10-bit counters (two blocks per SM still fit), so shorter chunks
         p.fields = std::min(K, GK) > 20 ? 3 : 2;
         p.L = (int)std::max<int64_t>(32, std::min<int64_t>(p.fields == 3 ? 1023 : 2047, L));
+        while (p.L > 32 && count_smem_bytes(nlev_max, p.fields, p.L, p.span, p.ps) > SMEM_PER_BLOCK_MAX) p.L = std::max(32, p.L / 2);
         p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
         p.tiles = (uint32_t)count_tiles(v.n, p.L);
     }
     return p;
-}
-
-size_t count_smem_bytes(int nlev, int fields, int L, int span) {
-    return (size_t)CountSmem::off_cols + (size_t)nlev * 4 * CountSmem::col_words(fields) +
-           4 * ((size_t)window_la(L, span, 0) + window_lb(L, span, 0));
 }
 
 template <int NORM, int M, int TAU>
@@ -810,7 +818,7 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
     // second launch: only the series whose table carries extra single-value levels (massive ties); its blocks
     // of the other series return at once, and so do the first launch's blocks of those series
     const int nlev_heavy = 2 * nlev - 1;
-    const size_t smem = count_smem_bytes(nlev, p.fields, p.L, p.span), smem_heavy = count_smem_bytes(nlev_heavy, p.fields, p.L, p.span);
+    const size_t smem = count_smem_bytes(nlev, p.fields, p.L, p.span, p.ps), smem_heavy = count_smem_bytes(nlev_heavy, p.fields, p.L, p.span, p.ps);
     RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_heavy));
     kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, p.fields, 0);
     RQA_LAUNCH_CHECK();
@@ -821,9 +829,10 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
 
 template <int NORM>
 rqa_status dispatch_count(const CountArgs& a, const SelectPlan& p, int nlev, int batch, cudaStream_t s) {
-    if (a.m == 3 && a.tau == 1) return launch_count<NORM, 3, 1>(a, p, nlev, batch, s);
-    if (a.m == 3 && a.tau == 3) return launch_count<NORM, 3, 3>(a, p, nlev, batch, s);
-    if (a.m == 5 && a.tau == 2) return launch_count<NORM, 5, 2>(a, p, nlev, batch, s);
+    const bool delay = p.ps == 1;
+    if (delay && a.m == 3 && a.tau == 1) return launch_count<NORM, 3, 1>(a, p, nlev, batch, s);
+    if (delay && a.m == 3 && a.tau == 3) return launch_count<NORM, 3, 3>(a, p, nlev, batch, s);
+    if (delay && a.m == 5 && a.tau == 2) return launch_count<NORM, 5, 2>(a, p, nlev, batch, s);
     return launch_count<NORM, 0, 0>(a, p, nlev, batch, s);
 }
 

@@ -79,8 +79,9 @@ __device__ __forceinline__ void find_diagonal_block(const uint32_t* __restrict__
 
 // Window lengths (floats) for a chunk of L positions, embedding span (m-1)*tau and W warm-up cells before the chunk:
 // i-side window y[s-W .. s-W+LA), j-side window y[s-W+o0 .. s-W+o0+LB).
-__host__ __device__ inline int window_la(int L, int span, int W) { return (L + W + 6 + 2 * span + 3) & ~3; }
-__host__ __device__ inline int window_lb(int L, int span, int W) { return (L + W + 6 + 2 * span + LW + 3) & ~3; }
+// ps = point stride in floats (1 for a delay view, m for materialised row-major points); span = (m-1) * coord stride.
+__host__ __device__ inline int window_la(int L, int span, int W, int ps = 1) { return ((L + W + 6) * ps + 2 * span + 3) & ~3; }
+__host__ __device__ inline int window_lb(int L, int span, int W, int ps = 1) { return ((L + W + 6 + LW) * ps + 2 * span + 3) & ~3; }
 
 // Stage the two windows of series `y` (ny samples); samples outside the series read as 0 (their cells are never
 // counted).
@@ -107,16 +108,16 @@ struct CellDist {
     float ring[S];
     uint32_t ya;                // shared-window address of the i-side window element of cell t0
     uint32_t yb;                // ... of the j-side window, already offset by the thread's diagonal
-    int m, tau;
+    int m, tau;                 // M == 0: run-time dimension and coordinate stride (floats)
+    int ps;                     // M == 0: point stride (floats); the register-ring variants are delay views, stride 1
 
+    __device__ __forceinline__ int pstride() const { return M > 0 ? 1 : ps; }
     // ya_org, yb_org: addresses of window index 0 (cell -W); afterwards the cursors stand at cell t0
     __device__ __forceinline__ void seek(uint32_t ya_org, uint32_t yb_org, int t0) {
-        ya = ya_org + 4 * (t0 + W);
-        yb = yb_org + 4 * (t0 + W);
+        ya = ya_org + 4 * (t0 + W) * pstride();
+        yb = yb_org + 4 * (t0 + W) * pstride();
     }
-    __device__ __forceinline__ void advance(int cells) { ya += 4 * cells; yb += 4 * cells; }
-    // cell t0 of the current super-step, given the address of window index 0
-    __device__ __forceinline__ int position(uint32_t ya_org) const { return (int)((ya - ya_org) >> 2) - W; }
+    __device__ __forceinline__ void advance(int cells) { ya += 4 * cells * pstride(); yb += 4 * cells * pstride(); }
 
     // element x cells after the cursor
     __device__ __forceinline__ float elem(int x) const {
@@ -137,10 +138,10 @@ struct CellDist {
     template <int R>
     __device__ __forceinline__ float distance() const {
         if (M == 0) {
-            float d = elem(R);
+            float d = elem(R * ps);
             if (NORM == RQA_NORM_MAX) d = fabsf(d);
             for (int c = 1; c < m; ++c) {
-                float x = elem(R + c * tau);
+                float x = elem(R * ps + c * tau);
                 d = NORM == RQA_NORM_MAX ? fmaxf(d, fabsf(x)) : __fadd_rn(d, x);
             }
             return NORM == RQA_NORM_MAX ? d : __fsqrt_rn(d);

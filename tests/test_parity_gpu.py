@@ -173,29 +173,34 @@ def test_tiny_scale_and_denormals(rqa, oracle):
 
 
 # ---------------------------------------------------------------------------- boundary behaviour on the GPU
-def test_materialised_points_equal_delay_view(rqa, oracle):
+@pytest.mark.parametrize("N,m,tau,norm,batch", [(900, 4, 6, 0, 1), (3300, 3, 2, 0, 2), (3300, 3, 2, 1, 1), (3100, 7, 1, 0, 1),
+                                                (3050, 16, 3, 1, 1), (1200, 1, 1, 0, 1)])
+def test_materialised_points_equal_delay_view(rqa, oracle, N, m, tau, norm, batch):
+    """Row-major points X[n][m] (point stride m) take the tiled kernels too — the counting pass of the bracket path
+    above P = 2^22 and the diagonal scan — and give the results of the delay view they were embedded from."""
     import torch
-    y = wl.add_noise(wl.sine_signal(900), 1.0, 3)
-    m, tau = 4, 6
+    ys = np.stack([wl.add_noise(wl.sine_signal(N), 1.0, 3 + b) for b in range(batch)])
     rr = wl.rr_linear(10)
-    s = torch.as_tensor(y).cuda().unsqueeze(0)
-    n = len(y) - (m - 1) * tau
-    X = torch.empty((1, n, m), dtype=torch.float32, device="cuda")
+    s = torch.as_tensor(ys).cuda()
+    n = N - (m - 1) * tau
+    X = torch.empty((batch, n, m), dtype=torch.float32, device="cuda")
     view = rqa.rqa_embed(s, m, tau, X)
     assert (view.point_stride, view.coord_stride, view.n_points) == (m, 1, n)
-    assert np.array_equal(X.cpu().numpy()[0], oracle.embed(y, m, tau))
+    assert np.array_equal(X.cpu().numpy()[0], oracle.embed(ys[0], m, tau))
     K = len(rr)
-    eps = torch.empty((1, K), dtype=torch.float32, device="cuda")
-    cnt = torch.empty((1, K), dtype=torch.int64, device="cuda")
-    rrr = torch.empty((1, K), dtype=torch.float64, device="cuda")
-    hist = torch.empty((1, K, n), dtype=torch.int64, device="cuda")
+    eps = torch.empty((batch, K), dtype=torch.float32, device="cuda")
+    cnt = torch.empty((batch, K), dtype=torch.int64, device="cuda")
+    rrr = torch.empty((batch, K), dtype=torch.float64, device="cuda")
+    hist = torch.empty((batch, K, n), dtype=torch.int64, device="cuda")
     ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
-    rqa.rqa_eps_for_rr(view, 0, rr, eps, cnt, rrr, ws)
-    rqa.rqa_line_hist(view, 0, eps, hist, ws)
+    rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
+    rqa.rqa_line_hist(view, norm, eps, hist, ws)
     rqa.rqa_workspace_status(ws)
-    r = oracle.sweep(y, m, tau, rr, 0)
-    assert np.array_equal(eps.cpu().numpy()[0], r["eps"])
-    assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], r["hist"])
+    for b in range(batch):
+        r = oracle.sweep(ys[b], m, tau, rr, norm, threads=0)
+        assert np.array_equal(eps.cpu().numpy()[b], r["eps"])
+        assert np.array_equal(cnt.cpu().numpy().view(np.uint64)[b], r["count"])
+        assert np.array_equal(hist.cpu().numpy().view(np.uint64)[b], r["hist"])
 
 
 def test_line_hist_with_caller_thresholds(rqa, oracle):

@@ -29,6 +29,7 @@ rqa_status validate_points(const rqa_points* p, const char* who) {
     if (p->n_points > (int64_t)1 << 24) { set_error("%s: n_points = %lld > 2^24 unsupported", who, (long long)p->n_points); return RQA_ERR_UNSUPPORTED; }
     if (p->m < 1 || p->m > RQA_MAX_M) { set_error("%s: m = %d outside 1..%d", who, p->m, RQA_MAX_M); return RQA_ERR_INVALID_ARG; }
     if (p->batch < 1) { set_error("%s: batch = %d < 1", who, p->batch); return RQA_ERR_INVALID_ARG; }
+    if (p->batch > 65535) { set_error("%s: batch = %d > 65535 unsupported (one grid row per series)", who, p->batch); return RQA_ERR_UNSUPPORTED; }
     if (p->point_stride < 1 || p->coord_stride < 1 || p->batch_stride < 0) { set_error("%s: strides must be >= 1", who); return RQA_ERR_INVALID_ARG; }
     if (p->batch > 1 && p->batch_stride < 1) { set_error("%s: batch_stride must be >= 1 when batch > 1", who); return RQA_ERR_INVALID_ARG; }
     return RQA_OK;

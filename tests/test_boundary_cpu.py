@@ -57,6 +57,13 @@ def test_workspace_bytes_and_validation(lib):
     assert lib.rqa_workspace_bytes(ctypes.byref(_pts()), 129, ctypes.byref(sz)) == B.RQA_ERR_INVALID_ARG
     assert lib.rqa_workspace_bytes(ctypes.byref(_pts(n=(1 << 24) + 1)), 4, ctypes.byref(sz)) == B.RQA_ERR_UNSUPPORTED
     assert b"n_points" in lib.rqa_last_error()
+    assert lib.rqa_workspace_bytes(ctypes.byref(_pts(batch=65536)), 4, ctypes.byref(sz)) == B.RQA_ERR_UNSUPPORTED
+    assert lib.rqa_workspace_bytes(ctypes.byref(_pts(batch=65535)), 4, ctypes.byref(sz)) == B.RQA_OK
+    # materialised points: wide points still get a (larger) workspace; sizes grow with the batch
+    a, b2 = ctypes.c_size_t(0), ctypes.c_size_t(0)
+    assert lib.rqa_workspace_bytes(ctypes.byref(_pts(n=5000, m=16, ps=16, cs=1, bs=80000)), 20, ctypes.byref(a)) == B.RQA_OK
+    assert lib.rqa_workspace_bytes(ctypes.byref(_pts(n=5000, m=16, ps=16, cs=1, bs=80000, batch=3)), 20, ctypes.byref(b2)) == B.RQA_OK
+    assert b2.value > a.value > 256
     sw = ctypes.c_size_t(0)
     assert lib.rqa_sweep_workspace_bytes(1000, 5, 4, 6, 10, ctypes.byref(sw)) == B.RQA_OK
     assert sw.value > 5 * 10 * 982 * 8

@@ -508,7 +508,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
             ct.wcount = 0;
             ct.lane_lt = (1u << (tid & 31)) - 1u;
             ct.prime();
-            constexpr int U = S >= 3 ? S : 4;                 // cells per super-step, a multiple of S
+            constexpr int U = S == 3 ? 6 : (S > 3 ? S : 4);   // cells per super-step, a multiple of S
             using Seq = std::make_integer_sequence<int, U>;
             int t = 0;
             for (; t + U <= cnt_lo; t += U) { ct.template superstep<false>(t, cnt, Seq{}); ct.advance(U); }

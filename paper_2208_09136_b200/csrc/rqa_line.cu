@@ -372,6 +372,7 @@ __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc,
     using SC = Scanner<NORM, M, TAU, NP, MULTI>;
     constexpr int S = SC::S;
     constexpr int U = S == 3 ? 12 : (S > 3 ? S : 4);          // cells per super-step, a multiple of S
+    static_assert(U + 2 <= WSLACK && U <= QCELLS, "window slack and queue capacity cover one super-step");
     using Seq = std::make_integer_sequence<int, U>;
     int t = -2;                                               // first cell is the warm-up cell t = -2
     sc.seek(sc.ya_org, yb_org, t);

@@ -80,8 +80,11 @@ __device__ __forceinline__ void find_diagonal_block(const uint32_t* __restrict__
 // Window lengths (floats) for a chunk of L positions, embedding span (m-1)*tau and W warm-up cells before the chunk:
 // i-side window y[s-W .. s-W+LA), j-side window y[s-W+o0 .. s-W+o0+LB).
 // ps = point stride in floats (1 for a delay view, m for materialised row-major points); span = (m-1) * coord stride.
-__host__ __device__ inline int window_la(int L, int span, int W, int ps = 1) { return ((L + W + 6) * ps + 2 * span + 3) & ~3; }
-__host__ __device__ inline int window_lb(int L, int span, int W, int ps = 1) { return ((L + W + 6 + LW) * ps + 2 * span + 3) & ~3; }
+// WSLACK: the last super-step of a chunk starts before cell L and touches up to U - 1 cells plus S - 1 ring elements
+// beyond it (U <= 12 cells per super-step, S - 1 <= span), loaded before the guards look at them.
+constexpr int WSLACK = 16;
+__host__ __device__ inline int window_la(int L, int span, int W, int ps = 1) { return ((L + W + WSLACK) * ps + 2 * span + 3) & ~3; }
+__host__ __device__ inline int window_lb(int L, int span, int W, int ps = 1) { return ((L + W + WSLACK + LW) * ps + 2 * span + 3) & ~3; }
 
 // Stage the two windows of series `y` (ny samples); samples outside the series read as 0 (their cells are never
 // counted).

@@ -43,8 +43,8 @@ def line_scan_lane_instr_per_cell(m: int, K: int) -> int:
 
 
 # DRAM bytes of ONE line_scan_kernel launch over one N=1e5, K=20 series (dram__bytes_read.sum + dram__bytes_write.sum of
-# the ncu --set full capture in profiles/r1j_ncu_line_scan.md); the bench launch covers `batch` series.
-NCU_LINE_SCAN_DRAM_BYTES_PER_SERIES = 342.1e6
+# the ncu --set full capture in profiles/r1k_ncu_line_scan.md); the bench launch covers `batch` series.
+NCU_LINE_SCAN_DRAM_BYTES_PER_SERIES = 341.5e6
 
 
 def measured_peaks():
@@ -246,7 +246,7 @@ def run_ours(args):
     roofline = {"bound": "alu", "kernel": "rqa_line_hist (diagonal scan)", "achieved": achieved / 1e12, "peak": peak_lane / 1e12,
                 "unit": "Tlane-instr/s", "frac": achieved / peak_lane,
                 "traffic": (NCU_LINE_SCAN_DRAM_BYTES_PER_SERIES * w.batch) if (w.N == 100000 and K == 20) else None,
-                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1j_ncu_line_scan.md, x batch)",
+                "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1k_ncu_line_scan.md, x batch)",
                 "peak_source": f"148 SM x 128 lanes/clk x {sm_max_mhz:.0f} MHz ({peak_kind} sm_max_mhz)",
                 "algorithmic_lane_instr_per_cell": line_scan_lane_instr_per_cell(w.m, K),
                 "avg_launch_ms": line_ms}

@@ -126,7 +126,8 @@ def rqa_workspace_status(ws, stream=None) -> None:
 
 def rqa_embed(series, m: int, tau: int, X=None, stream=None) -> RqaPoints:
     """series: float32 CUDA tensor [batch][N] (or [N]).  Returns the rqa_points view (of `series` itself when
-    X is None, else of the materialised X[batch][N'][m] the call writes)."""
+    X is None, else of the materialised X[batch][N'][m] the call writes).  The returned view holds a reference to
+    the tensor it points into."""
     import torch
     if series.dim() == 1:
         series = series.unsqueeze(0)
@@ -135,6 +136,7 @@ def rqa_embed(series, m: int, tau: int, X=None, stream=None) -> RqaPoints:
     view = RqaPoints()
     xp = None if X is None else _dev(X, torch.float32, "X")
     _check(load_library().rqa_embed(p, N, batch, N, m, tau, xp, ctypes.byref(view), _stream(stream)))
+    view._owner = series if X is None else X                 # the view points into this tensor: keep it alive
     return view
 
 

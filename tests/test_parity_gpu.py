@@ -492,3 +492,57 @@ def test_line_hist_any_chunk_length(rqa, oracle, options, L):
     for m, tau in ((3, 1), (1, 1), (2, 7)):
         g = gpu_sweep(rqa, ys, m, tau, rr, 0)
         assert_parity(oracle, g, ys, m, tau, rr, 0, threads=0)
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_random_configurations(rqa, oracle, options, seed):
+    """Seeded random sweeps (40 per seed): series kind (noise, logistic, sine, quantised, ramp, denormal scale, constant),
+    N, m, tau, K, norm, batch, l_min, delay view or materialised points, and the expert knobs (select path, sample
+    size, candidate capacity, chunk length) all drawn at random; everything compared with the oracle."""
+    import torch
+    rng = np.random.default_rng(seed)
+
+    def series(kind, N, s):
+        if kind == 0:
+            return wl.gaussian(s, N).astype(np.float32)
+        if kind == 1:
+            return wl.add_noise(wl.logistic_signal(N, s), float(rng.choice([0.1, 1.0, 10.0])), s)
+        if kind == 2:
+            return wl.add_noise(wl.sine_signal(N, int(rng.integers(3, 40))), float(rng.choice([0.3, 3.0, np.inf])), s)
+        if kind == 3:
+            return np.round(wl.gaussian(s, N) * float(rng.choice([1.0, 4.0, 30.0]))).astype(np.float32)
+        if kind == 4:
+            return np.arange(N, dtype=np.float32) * float(rng.choice([1.0, 0.25]))
+        if kind == 5:
+            return (wl.gaussian(s, N) * 1e-20).astype(np.float32)
+        return np.full(N, 3.5, dtype=np.float32)
+
+    for case in range(40):
+        m, tau = [(1, 1), (2, 1), (3, 1), (3, 3), (5, 2), (4, 6), (7, 2), (2, 11)][int(rng.integers(8))]
+        N = int((m - 1) * tau + 2 + rng.integers(0, int(rng.choice([8, 60, 700, 3400]))))
+        batch, K, norm = int(rng.choice([1, 1, 2, 3])), int(rng.choice([1, 2, 5, 12, 20, 33, 70])), int(rng.integers(2))
+        rr = rng.random(K) ** 2 * 0.999 + 0.001
+        if rng.random() < 0.2:
+            rr[rng.integers(K)] = 1.0
+        l_min = int(rng.choice([1, 2, 2, 3, 5]))
+        ys = np.stack([series(int(rng.integers(7)), N, 1000 * case + b) for b in range(batch)])
+        options(select_path=int(rng.choice([0, 0, 1, 2, 3])), sample_size=int(rng.choice([0, 0, 50, 4000])),
+                line_chunk=int(rng.choice([0, 0, 0, 1, 2, 3, 6, 13, 64, 500])), cand_cap=int(rng.choice([0, 0, 0, 200])))
+        s = torch.as_tensor(ys).cuda()
+        n = N - (m - 1) * tau
+        X = torch.empty((batch, n, m), dtype=torch.float32, device="cuda") if rng.random() < 0.25 else None
+        view = rqa.rqa_embed(s, m, tau, X)                   # X stays referenced: the view points into it
+        eps = torch.empty((batch, K), dtype=torch.float32, device="cuda")
+        cnt = torch.empty((batch, K), dtype=torch.int64, device="cuda")
+        rrr = torch.empty((batch, K), dtype=torch.float64, device="cuda")
+        hist = torch.empty((batch, K, n), dtype=torch.int64, device="cuda")
+        det = torch.empty((batch, K), dtype=torch.float64, device="cuda")
+        mean = torch.empty((batch,), dtype=torch.float64, device="cuda")
+        ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
+        rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
+        rqa.rqa_line_hist(view, norm, eps, hist, ws)
+        rqa.rqa_det_avg(hist, l_min, det, mean)
+        rqa.rqa_workspace_status(ws)
+        g = {"eps": eps.cpu().numpy(), "count": cnt.cpu().numpy().view(np.uint64), "rr": rrr.cpu().numpy(),
+             "hist": hist.cpu().numpy().view(np.uint64), "det": det.cpu().numpy(), "det_mean": mean.cpu().numpy()}
+        assert_parity(oracle, g, ys, m, tau, rr, norm, l_min, threads=0)

@@ -66,6 +66,9 @@ typedef enum { RQA_NORM_MAX = 0, RQA_NORM_EUCLID = 1 } rqa_norm;
  * Delay view of raw series (what rqa_embed returns when d_X == NULL): point_stride = 1, coord_stride = tau.
  * Materialised row-major X[batch][n_points][m]:                       point_stride = m, coord_stride = 1.
  * All series of a batch share n_points, m and the strides.  Strides are in elements and must be >= 1.
+ * theiler = w > 1 excludes the diagonals j - i < w as well (temporally correlated neighbours; the paper uses none,
+ * reading S9): every "P" below is then P_w = (N'-w)(N'-w+1)/2, the number of pairs with j - i >= w, and lines are
+ * counted on the diagonals j - i = w..N'-1.  w <= N'-1.
  */
 typedef struct rqa_points {
     const float* data; /* device pointer */
@@ -75,6 +78,7 @@ typedef struct rqa_points {
     int64_t point_stride;
     int64_t coord_stride;
     int64_t batch_stride;
+    int64_t theiler;   /* Theiler window w: only pairs with j - i >= w are counted; 0 or 1 = the main diagonal only */
 } rqa_points;
 
 const char* rqa_status_string(rqa_status s);
@@ -151,14 +155,16 @@ rqa_status rqa_det_prefix_avg(const double* d_det, int32_t batch, int32_t K, dou
  * The other measures the paper derives from the same histogram ("DET, L, L_max and RR"):
  *   d_L        [batch][K] average diagonal line length  sum_{l>=l_min} l*P_k(l) / sum_{l>=l_min} P_k(l)  (0 if no line)
  *   d_Lmax     [batch][K] longest diagonal line  max{ l : P_k(l) > 0 }  (0 if none)
- *   d_rr_hist  [batch][K] recurrence rate from the histogram  sum_{l>=1} l*P_k(l) / P,  P = N'(N'-1)/2
+ *   d_rr_hist  [batch][K] recurrence rate from the histogram  sum_{l>=1} l*P_k(l) / P,  P = N'(N'-1)/2 (or P_w for the
+ *              Theiler window `theiler` the histogram was built with; 0 or 1 = none)
  * and, as one of the "other RQA measures" the averaging applies to (not defined in the paper itself),
  *   d_entr     [batch][K] Shannon entropy of the line-length distribution  -sum_{l>=l_min} p(l) ln p(l),
  *              p(l) = P_k(l) / sum_{l>=l_min} P_k(l)  (0 if no line), computed as ln T - (1/T) sum P ln P in fp64.
  * Any of the four outputs may be NULL.  Integer sums are exact uint64; L and RR are one fp64 division.
  */
 rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
-                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, double* d_entr, void* stream);
+                             int64_t theiler, double* d_L, uint64_t* d_Lmax, double* d_rr_hist, double* d_entr,
+                             void* stream);
 
 /*
  * Sorting rate S (Eq. 6), the paper's evaluation score; plain host arithmetic on R*n numbers.

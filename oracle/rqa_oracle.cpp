@@ -102,15 +102,26 @@ int rqa_oracle_embed(const float* y, int64_t N, int m, int64_t tau, float* X) {
     return ORACLE_OK;
 }
 
-/* All P = N'(N'-1)/2 distances of the pairs i<j, in row-major order of (i,j).  PAPER.md:47-50. */
-int rqa_oracle_distances(const float* y, int64_t N, int m, int64_t tau, int norm, float* out) {
-    if (!y || !out || m < 1 || tau < 1) return ORACLE_BAD_ARG;
+/* Pairs counted with a Theiler window w >= 1 (w = 1: only the main diagonal is excluded, reading S9): the
+ * pairs i<j with j - i >= w, P_w = (N'-w)(N'-w+1)/2 of them. */
+static uint64_t pairs_with_window(int64_t Np, int64_t w) {
+    return (uint64_t)(Np - w) * (uint64_t)(Np - w + 1) / 2;
+}
+
+/* All distances of the pairs i<j with j - i >= theiler, in row-major order of (i,j).  PAPER.md:47-50. */
+static int distances_w(const float* y, int64_t N, int m, int64_t tau, int norm, int64_t theiler, float* out) {
+    if (!y || !out || m < 1 || tau < 1 || theiler < 1) return ORACLE_BAD_ARG;
     int64_t Np = embedded_points(N, m, tau);
-    if (Np < 2) return ORACLE_BAD_ARG;
+    if (Np < 2 || theiler > Np - 1) return ORACLE_BAD_ARG;
     int64_t p = 0;
     for (int64_t i = 0; i < Np; ++i)
-        for (int64_t j = i + 1; j < Np; ++j) out[p++] = distance(y, i, j, m, tau, norm);
+        for (int64_t j = i + theiler; j < Np; ++j) out[p++] = distance(y, i, j, m, tau, norm);
     return ORACLE_OK;
+}
+
+/* All P = N'(N'-1)/2 distances of the pairs i<j, in row-major order of (i,j).  PAPER.md:47-50. */
+int rqa_oracle_distances(const float* y, int64_t N, int m, int64_t tau, int norm, float* out) {
+    return distances_w(y, N, m, tau, norm, 1, out);
 }
 
 /* Rank of the order statistic for a target recurrence rate: the literal fp64 expression
@@ -125,16 +136,16 @@ uint64_t rqa_oracle_rank(double rr, uint64_t P) {
 /* eps_k = the r_k-th smallest distance (1-based), C_k = #{d <= eps_k}, realised RR_k = C_k / P.
  * Full enumeration + std::sort (4*P bytes).  PAPER.md:78 + readings S4-S6. */
 int rqa_oracle_eps_for_rr(const float* y, int64_t N, int m, int64_t tau, int norm, const double* rr, int K,
-                          float* eps, uint64_t* count, double* rr_realised) {
-    if (!y || !rr || !eps || !count || !rr_realised || m < 1 || tau < 1 || K < 1) return ORACLE_BAD_ARG;
+                          float* eps, uint64_t* count, double* rr_realised, int64_t theiler) {
+    if (!y || !rr || !eps || !count || !rr_realised || m < 1 || tau < 1 || K < 1 || theiler < 1) return ORACLE_BAD_ARG;
     int64_t Np = embedded_points(N, m, tau);
-    if (Np < 2) return ORACLE_BAD_ARG;
+    if (Np < 2 || theiler > Np - 1) return ORACLE_BAD_ARG;
     if (!all_finite(y, N)) return ORACLE_NONFINITE;
     for (int k = 0; k < K; ++k)
         if (!(rr[k] > 0.0) || !(rr[k] <= 1.0)) return ORACLE_BAD_ARG;
-    uint64_t P = (uint64_t)Np * (uint64_t)(Np - 1) / 2;
+    uint64_t P = pairs_with_window(Np, theiler);
     std::vector<float> d((size_t)P);
-    int st = rqa_oracle_distances(y, N, m, tau, norm, d.data());
+    int st = distances_w(y, N, m, tau, norm, theiler, d.data());
     if (st != ORACLE_OK) return st;
     std::sort(d.begin(), d.end());
     for (int k = 0; k < K; ++k) {
@@ -194,13 +205,14 @@ int rqa_oracle_count_lt_le(const float* y, int64_t N, int m, int64_t tau, int no
  * S8); the main diagonal is excluded (S2).  hist[k][0] = 0.
  *   lower != 0 scans the lower triangle instead (cells (i+o, i)); by the symmetry of R
  *   the result must be identical — used only as a pin.
+ *   theiler = w > 1 scans the diagonals o = w..N'-1 only (a Theiler window; the paper uses none).
  *   threads: 1 = the literal serial loop; >1 (or 0 = all) splits the diagonals over OpenMP threads with
  *   private histograms that are summed.  PAPER.md:69-72, 125. */
 int rqa_oracle_line_hist(const float* y, int64_t N, int m, int64_t tau, int norm, const float* eps, int K,
-                         uint64_t* hist, int lower, int threads) {
-    if (!y || !eps || !hist || m < 1 || tau < 1 || K < 1) return ORACLE_BAD_ARG;
+                         uint64_t* hist, int lower, int threads, int64_t theiler) {
+    if (!y || !eps || !hist || m < 1 || tau < 1 || K < 1 || theiler < 1) return ORACLE_BAD_ARG;
     int64_t Np = embedded_points(N, m, tau);
-    if (Np < 2) return ORACLE_BAD_ARG;
+    if (Np < 2 || theiler > Np - 1) return ORACLE_BAD_ARG;
     int nt = pick_threads(threads);
     std::memset(hist, 0, sizeof(uint64_t) * (size_t)K * (size_t)Np);
     std::vector<uint64_t> priv;
@@ -210,7 +222,7 @@ int rqa_oracle_line_hist(const float* y, int64_t N, int m, int64_t tau, int norm
 #ifdef _OPENMP
 #pragma omp parallel for schedule(dynamic, 8) num_threads(nt) if (nt > 1)
 #endif
-        for (int64_t o = 1; o < Np; ++o) {
+        for (int64_t o = theiler; o < Np; ++o) {              /* theiler = 1: every diagonal but the main one */
             uint64_t* h = hist + (size_t)k * Np;
 #ifdef _OPENMP
             if (nt > 1) h = priv.data() + ((size_t)omp_get_thread_num() * K + k) * (size_t)Np;
@@ -273,9 +285,11 @@ int rqa_oracle_det_prefix_avg(const double* det, int K, double* prefix) {
  * entropy of the line-length distribution, ENTR_k = -sum_{l>=l_min} p(l) ln p(l), p(l) = P_k(l) / sum_{l>=l_min} P_k(l)
  * (one of the "other RQA measures" of PAPER.md:86; the paper does not define it, this is the textbook definition). */
 int rqa_oracle_line_measures(const uint64_t* hist, int K, int64_t n_points, int64_t l_min, double* L, uint64_t* Lmax,
-                             double* rr_hist, double* entr) {
-    if (!hist || !L || !Lmax || !rr_hist || !entr || K < 1 || n_points < 2 || l_min < 1) return ORACLE_BAD_ARG;
-    const double P = (double)((uint64_t)n_points * (uint64_t)(n_points - 1) / 2);
+                             double* rr_hist, double* entr, int64_t theiler) {
+    if (!hist || !L || !Lmax || !rr_hist || !entr || K < 1 || n_points < 2 || l_min < 1 || theiler < 1 ||
+        theiler > n_points - 1)
+        return ORACLE_BAD_ARG;
+    const double P = (double)pairs_with_window(n_points, theiler);
     for (int k = 0; k < K; ++k) {
         uint64_t pts = 0, lpts = 0, lines = 0, lmax = 0;
         for (int64_t l = 1; l < n_points; ++l) {

@@ -53,12 +53,12 @@ def _load():
     lib.rqa_oracle_distances.argtypes = [f32p, i64, i32, i64, i32, f32p]
     lib.rqa_oracle_rank.argtypes = [ctypes.c_double, ctypes.c_uint64]
     lib.rqa_oracle_rank.restype = ctypes.c_uint64
-    lib.rqa_oracle_eps_for_rr.argtypes = [f32p, i64, i32, i64, i32, f64p, i32, f32p, u64p, f64p]
+    lib.rqa_oracle_eps_for_rr.argtypes = [f32p, i64, i32, i64, i32, f64p, i32, f32p, u64p, f64p, i64]
     lib.rqa_oracle_count_lt_le.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, u64p, i32]
-    lib.rqa_oracle_line_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i32]
+    lib.rqa_oracle_line_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i32, i64]
     lib.rqa_oracle_det_avg.argtypes = [u64p, i32, i64, i64, f64p, f64p]
     lib.rqa_oracle_det_prefix_avg.argtypes = [f64p, i32, f64p]
-    lib.rqa_oracle_line_measures.argtypes = [u64p, i32, i64, i64, f64p, u64p, f64p, f64p]
+    lib.rqa_oracle_line_measures.argtypes = [u64p, i32, i64, i64, f64p, u64p, f64p, f64p, i64]
     lib.rqa_oracle_sorting_rate.argtypes = [f64p, i32, i32, f64p]
     _lib = lib
     return lib
@@ -113,8 +113,8 @@ def rank(rr: float, P: int) -> int:
     return int(_load().rqa_oracle_rank(float(rr), int(P)))
 
 
-def eps_for_rr(y, m: int, tau: int, rr, norm: int = NORM_MAX):
-    """-> (eps[K] float32, count[K] uint64, rr_realised[K] float64)"""
+def eps_for_rr(y, m: int, tau: int, rr, norm: int = NORM_MAX, theiler: int = 1):
+    """-> (eps[K] float32, count[K] uint64, rr_realised[K] float64); theiler = w > 1: pairs with j - i >= w only"""
     y = _series(y)
     rr = np.ascontiguousarray(rr, dtype=np.float64)
     K = len(rr)
@@ -123,7 +123,7 @@ def eps_for_rr(y, m: int, tau: int, rr, norm: int = NORM_MAX):
     rrr = np.empty(K, dtype=np.float64)
     _check(_load().rqa_oracle_eps_for_rr(_p(y, ctypes.c_float), len(y), m, tau, norm, _p(rr, ctypes.c_double), K,
                                          _p(eps, ctypes.c_float), _p(cnt, ctypes.c_uint64),
-                                         _p(rrr, ctypes.c_double)), "eps_for_rr")
+                                         _p(rrr, ctypes.c_double), max(1, theiler)), "eps_for_rr")
     return eps, cnt, rrr
 
 
@@ -140,15 +140,17 @@ def count_lt_le(y, m: int, tau: int, eps, norm: int = NORM_MAX, threads: int = 0
     return lt, le
 
 
-def line_hist(y, m: int, tau: int, eps, norm: int = NORM_MAX, lower: bool = False, threads: int = 1) -> np.ndarray:
-    """-> hist[K][N'] uint64"""
+def line_hist(y, m: int, tau: int, eps, norm: int = NORM_MAX, lower: bool = False, threads: int = 1,
+              theiler: int = 1) -> np.ndarray:
+    """-> hist[K][N'] uint64 (theiler = w > 1: only the diagonals j - i >= w)"""
     y = _series(y)
     eps = np.ascontiguousarray(eps, dtype=np.float32)
     K = len(eps)
     n = n_embedded(len(y), m, tau)
     hist = np.empty((K, n), dtype=np.uint64)
     _check(_load().rqa_oracle_line_hist(_p(y, ctypes.c_float), len(y), m, tau, norm, _p(eps, ctypes.c_float), K,
-                                        _p(hist, ctypes.c_uint64), 1 if lower else 0, threads), "line_hist")
+                                        _p(hist, ctypes.c_uint64), 1 if lower else 0, threads, max(1, theiler)),
+           "line_hist")
     return hist
 
 
@@ -172,7 +174,7 @@ def det_prefix_avg(det) -> np.ndarray:
     return out
 
 
-def line_measures(hist, l_min: int = 2):
+def line_measures(hist, l_min: int = 2, theiler: int = 1):
     """-> (L[K] float64, Lmax[K] uint64, rr_hist[K] float64, entr[K] float64)"""
     hist = np.ascontiguousarray(hist, dtype=np.uint64)
     K, n = hist.shape
@@ -182,7 +184,7 @@ def line_measures(hist, l_min: int = 2):
     entr = np.empty(K, dtype=np.float64)
     _check(_load().rqa_oracle_line_measures(_p(hist, ctypes.c_uint64), K, n, l_min, _p(L, ctypes.c_double),
                                             _p(Lmax, ctypes.c_uint64), _p(rr, ctypes.c_double),
-                                            _p(entr, ctypes.c_double)), "line_measures")
+                                            _p(entr, ctypes.c_double), max(1, theiler)), "line_measures")
     return L, Lmax, rr, entr
 
 
@@ -195,9 +197,9 @@ def sorting_rate(measure) -> float:
     return float(S[0])
 
 
-def sweep(y, m: int, tau: int, rr, norm: int = NORM_MAX, l_min: int = 2, threads: int = 1):
+def sweep(y, m: int, tau: int, rr, norm: int = NORM_MAX, l_min: int = 2, threads: int = 1, theiler: int = 1):
     """The whole hot path on one series: eps -> hist -> DET.  Returns a dict."""
-    eps, cnt, rrr = eps_for_rr(y, m, tau, rr, norm)
-    hist = line_hist(y, m, tau, eps, norm, threads=threads)
+    eps, cnt, rrr = eps_for_rr(y, m, tau, rr, norm, theiler)
+    hist = line_hist(y, m, tau, eps, norm, threads=threads, theiler=theiler)
     det, mean = det_avg(hist, l_min)
     return {"eps": eps, "count": cnt, "rr": rrr, "hist": hist, "det": det, "det_mean": mean}

@@ -35,7 +35,7 @@ class RqaPoints(ctypes.Structure):
     """struct rqa_points"""
     _fields_ = [("data", ctypes.c_void_p), ("n_points", ctypes.c_int64), ("m", ctypes.c_int32),
                 ("batch", ctypes.c_int32), ("point_stride", ctypes.c_int64), ("coord_stride", ctypes.c_int64),
-                ("batch_stride", ctypes.c_int64)]
+                ("batch_stride", ctypes.c_int64), ("theiler", ctypes.c_int64)]
 
 
 class RqaError(RuntimeError):
@@ -72,7 +72,7 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_sweep_host.argtypes = [vp, i64, i32, i32, i64, ctypes.c_int, vp, i32, i64, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.rqa_set_option.argtypes = [ctypes.c_char_p, i64]
     lib.rqa_det_prefix_avg.argtypes = [vp, i32, i32, vp, vp]
-    lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp, vp, vp]
+    lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp, vp]
     lib.rqa_sorting_rate_host.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double)]
     _lib = lib
     return lib
@@ -124,7 +124,7 @@ def rqa_workspace_status(ws, stream=None) -> None:
     _check(load_library().rqa_workspace_status(_dev(ws, torch.uint8, "ws"), _stream(stream)))
 
 
-def rqa_embed(series, m: int, tau: int, X=None, stream=None) -> RqaPoints:
+def rqa_embed(series, m: int, tau: int, X=None, stream=None, theiler: int = 0) -> RqaPoints:
     """series: float32 CUDA tensor [batch][N] (or [N]).  Returns the rqa_points view (of `series` itself when
     X is None, else of the materialised X[batch][N'][m] the call writes).  The returned view holds a reference to
     the tensor it points into."""
@@ -137,6 +137,7 @@ def rqa_embed(series, m: int, tau: int, X=None, stream=None) -> RqaPoints:
     xp = None if X is None else _dev(X, torch.float32, "X")
     _check(load_library().rqa_embed(p, N, batch, N, m, tau, xp, ctypes.byref(view), _stream(stream)))
     view._owner = series if X is None else X                 # the view points into this tensor: keep it alive
+    view.theiler = theiler                                   # a field of the view, not an argument of rqa_embed
     return view
 
 
@@ -178,12 +179,12 @@ def rqa_det_prefix_avg(det, prefix, stream=None) -> None:
                                              _dev(prefix, torch.float64, "prefix"), _stream(stream)))
 
 
-def rqa_line_measures(hist, l_min: int, L=None, Lmax=None, rr_hist=None, entr=None, stream=None) -> None:
+def rqa_line_measures(hist, l_min: int, L=None, Lmax=None, rr_hist=None, entr=None, stream=None, theiler: int = 0) -> None:
     """hist int64 CUDA [batch][K][n_points]; L, rr_hist, entr float64 [batch][K]; Lmax int64 [batch][K]; each may be
     None."""
     import torch
     batch, K, n = hist.shape
-    _check(load_library().rqa_line_measures(_dev(hist, torch.int64, "hist"), batch, K, n, l_min,
+    _check(load_library().rqa_line_measures(_dev(hist, torch.int64, "hist"), batch, K, n, l_min, theiler,
                                             None if L is None else _dev(L, torch.float64, "L"),
                                             None if Lmax is None else _dev(Lmax, torch.int64, "Lmax"),
                                             None if rr_hist is None else _dev(rr_hist, torch.float64, "rr_hist"),

@@ -32,6 +32,7 @@ rqa_status validate_points(const rqa_points* p, const char* who) {
     if (p->batch > 65535) { set_error("%s: batch = %d > 65535 unsupported (one grid row per series)", who, p->batch); return RQA_ERR_UNSUPPORTED; }
     if (p->point_stride < 1 || p->coord_stride < 1 || p->batch_stride < 0) { set_error("%s: strides must be >= 1", who); return RQA_ERR_INVALID_ARG; }
     if (p->batch > 1 && p->batch_stride < 1) { set_error("%s: batch_stride must be >= 1 when batch > 1", who); return RQA_ERR_INVALID_ARG; }
+    if (p->theiler < 0 || p->theiler > p->n_points - 1) { set_error("%s: theiler = %lld outside 0..n_points-1", who, (long long)p->theiler); return RQA_ERR_INVALID_ARG; }
     return RQA_OK;
 }
 
@@ -185,7 +186,7 @@ rqa_status rqa_embed(const float* d_series, int64_t N, int32_t batch, int64_t se
     int64_t n = N - (int64_t)(m - 1) * tau;
     if (n < 2) { set_error("rqa_embed: N' = N - (m-1)*tau = %lld < 2", (long long)n); return RQA_ERR_INVALID_ARG; }
     rqa_points v;
-    v.n_points = n; v.m = m; v.batch = batch;
+    v.n_points = n; v.m = m; v.batch = batch; v.theiler = 0;
     if (!d_X) {
         v.data = d_series; v.point_stride = 1; v.coord_stride = tau; v.batch_stride = series_stride;
     } else {
@@ -208,7 +209,7 @@ rqa_status rqa_eps_for_rr(const rqa_points* pts, rqa_norm norm, const double* h_
     if (!h_rr || !d_eps || !d_count || !d_rr_realised || !d_ws) { set_error("rqa_eps_for_rr: NULL argument"); return RQA_ERR_INVALID_ARG; }
     if (((uintptr_t)d_ws & 255) != 0) { set_error("rqa_eps_for_rr: workspace must be 256-byte aligned"); return RQA_ERR_INVALID_ARG; }
     View v = make_view(*pts);
-    uint64_t P = n_pairs(v.n);
+    uint64_t P = n_pairs(v);
     uint64_t rank[RQA_MAX_K];
     for (int k = 0; k < K; ++k) {
         double rr = h_rr[k];
@@ -285,7 +286,7 @@ rqa_status rqa_sweep_workspace_bytes(int64_t N, int32_t batch, int32_t m, int64_
     if (m < 1 || m > RQA_MAX_M || tau < 1 || batch < 1 || N - (int64_t)(m - 1) * tau < 2) { set_error("rqa_sweep_workspace_bytes: bad shape"); return RQA_ERR_INVALID_ARG; }
     rqa_points p;
     p.data = nullptr; p.n_points = N - (int64_t)(m - 1) * tau; p.m = m; p.batch = batch;
-    p.point_stride = 1; p.coord_stride = tau; p.batch_stride = N;
+    p.point_stride = 1; p.coord_stride = tau; p.batch_stride = N; p.theiler = 0;
     size_t inner = 0;
     rqa_status st = rqa_workspace_bytes(&p, K, &inner);
     if (st != RQA_OK) return st;
@@ -306,6 +307,7 @@ rqa_status rqa_sweep_host(const float* h_series, int64_t N, int32_t batch, int32
     int64_t n = N - (int64_t)(m - 1) * tau;
     rqa_points p;
     p.data = nullptr; p.n_points = n; p.m = m; p.batch = batch; p.point_stride = 1; p.coord_stride = tau; p.batch_stride = N;
+    p.theiler = 0;
     size_t inner = 0;
     rqa_workspace_bytes(&p, K, &inner);
     inner = align_up(inner);

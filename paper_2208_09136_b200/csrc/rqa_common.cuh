@@ -53,6 +53,7 @@ struct View {
     int32_t m;
     int32_t batch;
     int64_t ps, cs, bs;
+    int64_t w;   // first diagonal counted (Theiler window), >= 1
 };
 
 inline View make_view(const rqa_points& p) {
@@ -64,10 +65,14 @@ inline View make_view(const rqa_points& p) {
     v.ps = p.point_stride;
     v.cs = p.coord_stride;
     v.bs = p.batch_stride;
+    v.w = p.theiler > 1 ? p.theiler : 1;
     return v;
 }
 
 inline uint64_t n_pairs(int64_t n) { return (uint64_t)n * (uint64_t)(n - 1) / 2; }
+// With a Theiler window w the diagonals w..n-1 are counted: the same triangle as for n_diag = n - w + 1 points.
+inline int64_t n_diag(const View& v) { return v.n - v.w + 1; }
+inline uint64_t n_pairs(const View& v) { return n_pairs(n_diag(v)); }
 
 rqa_status validate_points(const rqa_points* pts, const char* who);
 

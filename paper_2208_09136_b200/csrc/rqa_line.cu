@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
     const int c = (int)(tile - a.tile_start[ob]);
     const int L = a.L;
     const int64_t n = a.v.n;
-    const int64_t o0 = 1 + (int64_t)LW * ob;
+    const int64_t o0 = a.v.w + (int64_t)LW * ob;            // w = 1, or the Theiler window
     const int64_t s = (int64_t)c * L;                       // chunk start along the diagonals
     // the two windows: the floats of the points s-2.. and s-2+o0..; the n points span (n-1)*ps + span + 1 floats
     const float* y = a.v.data + (int64_t)b * a.v.bs;
@@ -514,7 +514,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
 // One thread per (diagonal, distinct threshold): join the (prefix, suffix) summaries of consecutive chunks and
 // emit the lines of length >= 4 that touch a chunk border (including the two ends of the diagonal).
 struct StitchArgs {
-    int64_t n;
+    int64_t n, w;
     int g, NG, K, L, n_ob, NP;
     const LineGroup* groups;
     const uint32_t* tile_start;
@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
     const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
     if (j >= G.J) return;
     const int tid = threadIdx.x;
-    const int64_t o = 1 + (int64_t)LW * ob + tid;
+    const int64_t o = a.w + (int64_t)LW * ob + tid;
     const int64_t len = a.n - o;
     if (len <= 0) return;
     unsigned long long* row = a.hist + ((int64_t)b * a.K + G.rep_k[j]) * a.n;
@@ -627,7 +627,7 @@ template <int NORM>
 __global__ void __launch_bounds__(128) line_strided_kernel(View v, const float* __restrict__ eps, int K,
                                                            unsigned long long* __restrict__ hist) {
     const int b = blockIdx.y;
-    const int64_t o = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t o = v.w + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= v.n) return;
     const float* yb = v.data + (int64_t)b * v.bs;
     const float* e = eps + (int64_t)b * K;
@@ -677,15 +677,16 @@ LinePlan make_plan(const View& v, int K) {
     // tiled scan: delay views, and materialised points (point stride > 1) whose windows fit the shared memory
     p.scan = p.span <= MAX_SPAN && scan_smem_bytes(p.NP, 32, p.span, ps) <= SMEM_PER_BLOCK_MAX;
     // chunk length: aim at >= 8 waves of 3 blocks per SM over the whole batch, at most 1023 positions
-    const double cells = (double)n_pairs(v.n) * (double)v.batch;
+    const double cells = (double)n_pairs(v) * (double)v.batch;
     int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
     p.L = (int)std::max<int64_t>(32, std::min<int64_t>(LMAX, L));
     if (options().line_chunk > 0) p.L = (int)std::min<int64_t>(LMAX, options().line_chunk);
     // wide points: the two windows hold (2L + 512) points, so the chunk shrinks until they fit (one block per SM then)
     while (p.scan && p.L > 32 && scan_smem_bytes(p.NP, p.L, p.span, ps) > SMEM_PER_BLOCK_MAX) p.L = std::max(32, p.L / 2);
-    p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
+    const int64_t nd = n_diag(v);                              // the triangle of the counted diagonals w..n-1
+    p.n_ob = (int)((nd - 1 + LW - 1) / LW);
     uint64_t tiles = 0;
-    for (int ob = 0; ob < p.n_ob; ++ob) tiles += (uint64_t)((v.n - 1 - (int64_t)LW * ob + p.L - 1) / p.L);
+    for (int ob = 0; ob < p.n_ob; ++ob) tiles += (uint64_t)((nd - 1 - (int64_t)LW * ob + p.L - 1) / p.L);
     p.tiles = (uint32_t)tiles;
     p.smem = scan_smem_bytes(p.NP, p.L, p.span, ps);
     return p;
@@ -742,7 +743,7 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * (size_t)v.batch * K * v.n, s));
     LinePlan p = make_plan(v, K);
     if (!p.scan) {
-        dim3 grid((unsigned)((v.n - 1 + 127) / 128), (unsigned)v.batch);
+        dim3 grid((unsigned)((v.n - v.w + 127) / 128), (unsigned)v.batch);
         if (norm == RQA_NORM_MAX)
             line_strided_kernel<RQA_NORM_MAX><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
         else
@@ -760,7 +761,7 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     line_groups_kernel<<<v.batch, 128, 0, s>>>(d_eps, K, p.NG, groups, status);
     RQA_LAUNCH_CHECK();
     {
-        rqa_status st = launch_tile_table(v.n, p.L, p.n_ob, tile_start, s);
+        rqa_status st = launch_tile_table(n_diag(v), p.L, p.n_ob, tile_start, s);
         if (st != RQA_OK) return st;
     }
     for (int g = 0; g < p.NG; ++g) {
@@ -772,7 +773,7 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
                                              : dispatch_pairs<RQA_NORM_EUCLID>(a, p, v.batch, s);
         if (st != RQA_OK) return st;
         StitchArgs sa;
-        sa.n = v.n; sa.g = g; sa.NG = p.NG; sa.K = K; sa.L = p.L; sa.n_ob = p.n_ob; sa.NP = p.NP;
+        sa.n = v.n; sa.w = v.w; sa.g = g; sa.NG = p.NG; sa.K = K; sa.L = p.L; sa.n_ob = p.n_ob; sa.NP = p.NP;
         sa.groups = groups; sa.tile_start = tile_start; sa.hist = (unsigned long long*)d_hist; sa.pre = pre; sa.suf = suf;
         sa.tiles = p.tiles;
         line_stitch_kernel<<<dim3((unsigned)p.n_ob, (unsigned)(2 * p.NP), (unsigned)v.batch), LW, 0, s>>>(sa);

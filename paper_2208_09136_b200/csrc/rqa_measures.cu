@@ -21,6 +21,7 @@ __global__ void det_prefix_kernel(const double* __restrict__ det, int K, int bat
 
 // One block per (threshold, series): exact uint64 sums over the histogram row.
 __global__ void __launch_bounds__(256) line_measures_kernel(const uint64_t* __restrict__ hist, int K, int64_t n, int64_t l_min,
+                                                            int64_t w,
                                                             double* __restrict__ L, uint64_t* __restrict__ Lmax,
                                                             double* __restrict__ rr, double* __restrict__ entr) {
     const int k = blockIdx.x, b = blockIdx.y;
@@ -58,7 +59,7 @@ __global__ void __launch_bounds__(256) line_measures_kernel(const uint64_t* __re
         const int64_t o = (int64_t)b * K + k;
         if (L) L[o] = lines ? (double)lpts / (double)lines : 0.0;
         if (Lmax) Lmax[o] = lmax;
-        if (rr) rr[o] = (double)pts / (double)((unsigned long long)n * (unsigned long long)(n - 1) / 2);
+        if (rr) rr[o] = (double)pts / (double)((unsigned long long)(n - w) * (unsigned long long)(n - w + 1) / 2);
         if (entr) entr[o] = lines ? log((double)lines) - hlogh / (double)lines : 0.0;
     }
 }
@@ -79,10 +80,12 @@ rqa_status rqa_det_prefix_avg(const double* d_det, int32_t batch, int32_t K, dou
 }
 
 rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,
-                             double* d_L, uint64_t* d_Lmax, double* d_rr_hist, double* d_entr, void* stream) {
+                             int64_t theiler, double* d_L, uint64_t* d_Lmax, double* d_rr_hist, double* d_entr,
+                             void* stream) {
     if (!d_hist) { set_error("rqa_line_measures: d_hist is NULL"); return RQA_ERR_INVALID_ARG; }
-    if (batch < 1 || K < 1 || K > RQA_MAX_K || n_points < 2 || l_min < 1) { set_error("rqa_line_measures: need batch >= 1, 1 <= K <= %d, n_points >= 2, l_min >= 1", RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
-    line_measures_kernel<<<dim3(K, batch), 256, 0, (cudaStream_t)stream>>>(d_hist, K, n_points, l_min, d_L, d_Lmax, d_rr_hist, d_entr);
+    if (batch < 1 || K < 1 || K > RQA_MAX_K || n_points < 2 || l_min < 1 || theiler < 0 || theiler > n_points - 1) { set_error("rqa_line_measures: need batch >= 1, 1 <= K <= %d, n_points >= 2, l_min >= 1, 0 <= theiler <= n_points-1", RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
+    line_measures_kernel<<<dim3(K, batch), 256, 0, (cudaStream_t)stream>>>(d_hist, K, n_points, l_min, theiler > 1 ? theiler : 1, d_L,
+                                                                          d_Lmax, d_rr_hist, d_entr);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }

@@ -117,10 +117,25 @@ __global__ void __launch_bounds__(256) sel_sample_kernel(View v, unsigned long l
     for (unsigned long long s = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; s < S;
          s += (unsigned long long)gridDim.x * blockDim.x) {
         uint64_t h = mix64((s + 1) * 0x9E3779B97F4A7C15ull + (uint64_t)b * 0xD1B54A32D192ED03ull);
-        uint32_t i = __umulhi((uint32_t)(h >> 32), n);
-        uint32_t j = __umulhi((uint32_t)h, n - 1);
-        if (j >= i) ++j;
-        uint32_t lo = min(i, j), hi = max(i, j);
+        uint32_t lo, hi;
+        if (v.w <= 1) {
+            uint32_t i = __umulhi((uint32_t)(h >> 32), n);
+            uint32_t j = __umulhi((uint32_t)h, n - 1);
+            if (j >= i) ++j;
+            lo = min(i, j); hi = max(i, j);
+        } else {
+            // Theiler window: pair number r, uniform in [0, P_w), in the row-major order of sel_direct_kernel: row i
+            // holds the D - i pairs (i, i+w..n-1), D = n - w rows, C(i) = i*D - i(i-1)/2 pairs before it
+            const uint64_t D = (uint64_t)(v.n - v.w), Pw = D * (D + 1) / 2;
+            const uint64_t r = __umul64hi(h, Pw);
+            const double t = 2.0 * (double)D + 1.0;
+            int64_t i = (int64_t)((t - sqrt(t * t - 8.0 * (double)r)) * 0.5);
+            i = max((int64_t)0, min((int64_t)D - 1, i));
+            while (i > 0 && (uint64_t)i * D - (uint64_t)i * (uint64_t)(i - 1) / 2 > r) --i;
+            while ((uint64_t)(i + 1) * D - (uint64_t)(i + 1) * (uint64_t)i / 2 <= r) ++i;
+            lo = (uint32_t)i;
+            hi = (uint32_t)(i + v.w + (int64_t)(r - ((uint64_t)i * D - (uint64_t)i * (uint64_t)(i - 1) / 2)));
+        }
         o[s] = point_distance<NORM>(yb, lo, hi, v.m, v.ps, v.cs);
     }
 }
@@ -131,11 +146,11 @@ __global__ void __launch_bounds__(256) sel_direct_kernel(View v, unsigned long l
     const int b = blockIdx.y;
     const float* yb = v.data + (int64_t)b * v.bs;
     float* o = out + (int64_t)b * P;
-    const int64_t n = v.n;
-    for (int64_t row = blockIdx.x; row < n - 1; row += gridDim.x) {
-        // row i: pairs (i, i+1..n-1) stored at offset i*n - i(i+1)/2
-        const int64_t off = row * n - row * (row + 1) / 2 - row - 1;
-        for (int64_t j = row + 1 + threadIdx.x; j < n; j += blockDim.x)
+    const int64_t n = v.n, D = v.n - v.w;
+    for (int64_t row = blockIdx.x; row < D; row += gridDim.x) {
+        // row i: the D - i pairs (i, i+w..n-1) stored from offset i*D - i(i-1)/2
+        const int64_t off = row * D - row * (row - 1) / 2 - (row + v.w);
+        for (int64_t j = row + v.w + threadIdx.x; j < n; j += blockDim.x)
             o[off + j] = point_distance<NORM>(yb, row, j, v.m, v.ps, v.cs);
     }
 }
@@ -473,7 +488,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     const int c = (int)(tile - a.tile_start[ob]);
     const int L = a.L;
     const int64_t n = a.v.n;
-    const int64_t o0 = 1 + (int64_t)LW * ob;
+    const int64_t o0 = a.v.w + (int64_t)LW * ob;
     const int64_t s = (int64_t)c * L;
     const float* y = a.v.data + (int64_t)b * a.v.bs;
     stage_windows(y, (n - 1) * ps + span + 1, s * ps, (s + o0) * ps, ya_s, LA, yb_s, LB);
@@ -656,9 +671,9 @@ __global__ void __launch_bounds__(SEL_W) radix_pass_kernel(View v, int pass, con
     const float* yb = v.data + (int64_t)b * v.bs;
     const int shift = 24 - 8 * pass;
     const uint32_t himask = pass == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * pass));
-    const int64_t nx = (v.n - 1 + SEL_W - 1) / SEL_W, ny = (v.n - 1 + SEL_L - 1) / SEL_L;
+    const int64_t nx = (v.n - v.w + SEL_W - 1) / SEL_W, ny = (v.n - v.w + SEL_L - 1) / SEL_L;
     for (int64_t tile = blockIdx.x; tile < nx * ny; tile += gridDim.x) {
-        const int64_t o = 1 + (tile % nx) * SEL_W + threadIdx.x;
+        const int64_t o = v.w + (tile % nx) * SEL_W + threadIdx.x;
         const int64_t i0 = (tile / nx) * SEL_L;
         if (o >= v.n) continue;
         const int64_t iend = min(i0 + (int64_t)SEL_L, v.n - o);
@@ -779,7 +794,7 @@ constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of s
 SelectPlan make_select_plan(const View& v, int K) {
     const Options& opt = options();
     SelectPlan p{};
-    p.P = n_pairs(v.n);
+    p.P = n_pairs(v);
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
     p.ps = (int)std::min<int64_t>(v.ps, 1 << 20);
     // tiled counting pass: delay views, and materialised points whose windows fit beside the widest level table
@@ -806,8 +821,8 @@ SelectPlan make_select_plan(const View& v, int K) {
         p.fields = std::min(K, GK) > 20 ? 3 : 2;
         p.L = (int)std::max<int64_t>(32, std::min<int64_t>(p.fields == 3 ? 1023 : 2047, L));
         while (p.L > 32 && count_smem_bytes(nlev_max, p.fields, p.L, p.span, p.ps) > SMEM_PER_BLOCK_MAX) p.L = std::max(32, p.L / 2);
-        p.n_ob = (int)((v.n - 1 + LW - 1) / LW);
-        p.tiles = (uint32_t)count_tiles(v.n, p.L);
+        p.n_ob = (int)((n_diag(v) - 1 + LW - 1) / LW);
+        p.tiles = (uint32_t)count_tiles(n_diag(v), p.L);
     }
     return p;
 }
@@ -908,7 +923,7 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
     std::stable_sort(order, order + K, [&](int a, int b) { return h_rank[a] < h_rank[b]; });
 
     if (p.path == PATH_DIRECT) {
-        unsigned blocks = (unsigned)std::min<int64_t>(v.n - 1, 148 * 8);
+        unsigned blocks = (unsigned)std::min<int64_t>(v.n - v.w, 148 * 8);
         if (norm == RQA_NORM_MAX) sel_direct_kernel<RQA_NORM_MAX><<<dim3(blocks, v.batch), 256, 0, s>>>(v, P, w.sample);
         else sel_direct_kernel<RQA_NORM_EUCLID><<<dim3(blocks, v.batch), 256, 0, s>>>(v, P, w.sample);
         RQA_LAUNCH_CHECK();
@@ -936,7 +951,7 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
             else sel_sample_kernel<RQA_NORM_EUCLID><<<dim3(blocks, v.batch), 256, 0, s>>>(v, S, w.sample);
             RQA_LAUNCH_CHECK();
         }
-        rqa_status st = launch_tile_table(v.n, p.L, p.n_ob, w.tile_start, s);
+        rqa_status st = launch_tile_table(n_diag(v), p.L, p.n_ob, w.tile_start, s);
         if (st != RQA_OK) return st;
         for (int base = 0; base < K; base += GK) {
             const int kc = std::min(GK, K - base);
@@ -994,7 +1009,7 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
     const size_t smem = (size_t)K * 256 * sizeof(uint32_t);
     auto kern = norm == RQA_NORM_MAX ? radix_pass_kernel<RQA_NORM_MAX> : radix_pass_kernel<RQA_NORM_EUCLID>;
     if (smem > 48 * 1024) RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int64_t tiles = ((v.n - 1 + SEL_W - 1) / SEL_W) * ((v.n - 1 + SEL_L - 1) / SEL_L);
+    const int64_t tiles = ((v.n - v.w + SEL_W - 1) / SEL_W) * ((v.n - v.w + SEL_L - 1) / SEL_L);
     dim3 grid((unsigned)std::min<int64_t>(tiles, 148 * 16), (unsigned)v.batch);
     for (int pass = 0; pass < 4; ++pass) {
         kern<<<grid, SEL_W, smem, s>>>(v, pass, w.rst, w.rbins, K, w.ss);

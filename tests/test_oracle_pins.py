@@ -440,3 +440,41 @@ def test_sorting_rate_pins(oracle):
         assert oracle.sorting_rate(m) == pytest.approx((8 - dep) / 8, abs=1e-15)
     ties = np.array([[1.0, 1.0, 1.0]])               # equal values keep their given order: perfectly "sorted"
     assert oracle.sorting_rate(ties) == 1.0
+
+
+@pytest.mark.parametrize("w", [1, 2, 7, 58])
+def test_theiler_window_brute_force(oracle, w):
+    """Theiler window (row f3; the paper uses none, reading S9): only pairs with j - i >= w.  An independent numpy
+    brute force on the full distance matrix: the order statistic over the selected pairs, and the run lengths along
+    the diagonals w..N'-1.  w = 1 is the default path; w = N'-1 leaves the single pair (0, N'-1)."""
+    y = wl.add_noise(wl.sine_signal(64, 9), 1.5, 31)
+    m, tau = 2, 3
+    n = len(y) - (m - 1) * tau
+    if w == 58:
+        w = n - 1
+    X = np.stack([y[c * tau:c * tau + n] for c in range(m)], axis=1)
+    D = np.abs(X[:, None, :] - X[None, :, :]).max(axis=2).astype(np.float32)
+    sel = np.sort(np.concatenate([np.diagonal(D, o) for o in range(w, n)]))
+    P = len(sel)
+    assert P == (n - w) * (n - w + 1) // 2
+    rr = np.array([0.05, 0.3, 1.0])
+    eps, cnt, rrr = oracle.eps_for_rr(y, m, tau, rr, oracle.NORM_MAX, theiler=w)
+    for k in range(3):
+        r = min(P, max(1, math.ceil(rr[k] * P)))
+        assert eps[k] == sel[r - 1] and cnt[k] == int((sel <= eps[k]).sum()) and rrr[k] == cnt[k] / P
+    hist = oracle.line_hist(y, m, tau, eps, oracle.NORM_MAX, theiler=w)
+    want = np.zeros_like(hist)
+    for k in range(3):
+        for o in range(w, n):
+            run = 0
+            for v in np.append(np.diagonal(D, o) <= eps[k], False):
+                if v:
+                    run += 1
+                elif run:
+                    want[k, run] += 1
+                    run = 0
+    assert np.array_equal(hist, want)
+    assert np.array_equal((hist * np.arange(n, dtype=np.uint64)).sum(axis=1), cnt)
+    assert np.array_equal(oracle.line_measures(hist, 2, theiler=w)[2], rrr)      # RR from the histogram, over P_w
+    if w == 1:
+        assert np.array_equal(hist, oracle.line_hist(y, m, tau, eps, oracle.NORM_MAX))

@@ -546,3 +546,41 @@ def test_random_configurations(rqa, oracle, options, seed):
         g = {"eps": eps.cpu().numpy(), "count": cnt.cpu().numpy().view(np.uint64), "rr": rrr.cpu().numpy(),
              "hist": hist.cpu().numpy().view(np.uint64), "det": det.cpu().numpy(), "det_mean": mean.cpu().numpy()}
         assert_parity(oracle, g, ys, m, tau, rr, norm, l_min, threads=0)
+
+
+@pytest.mark.parametrize("path", [0, 1, 2, 3])
+def test_theiler_window(rqa, oracle, options, path):
+    """Theiler window w (rqa_points.theiler): thresholds over the pairs with j - i >= w and lines on the diagonals
+    w..N'-1, on every select path, for delay views and materialised points, several chunk lengths, windows from 2
+    to N'-1 (a single pair)."""
+    import torch
+    rr = np.array([0.004, 0.05, 0.2, 0.2, 0.7, 1.0])
+    ys = np.stack([wl.add_noise(wl.lorenz_signal(3100), 2.0, 5), wl.sine_signal(3100).astype(np.float32)])
+    for (m, tau, w, chunk, mat) in [(3, 1, 2, 0, False), (3, 1, 37, 5, False), (3, 3, 700, 0, False), (2, 4, 3095, 0, False),
+                                    (4, 2, 12, 64, True), (1, 1, 513, 1, False)]:
+        options(select_path=path, line_chunk=chunk)
+        s = torch.as_tensor(ys).cuda()
+        n = ys.shape[1] - (m - 1) * tau
+        X = torch.empty((2, n, m), dtype=torch.float32, device="cuda") if mat else None
+        view = rqa.rqa_embed(s, m, tau, X, theiler=w)
+        K = len(rr)
+        eps = torch.empty((2, K), dtype=torch.float32, device="cuda")
+        cnt = torch.empty((2, K), dtype=torch.int64, device="cuda")
+        rrr = torch.empty((2, K), dtype=torch.float64, device="cuda")
+        hist = torch.empty((2, K, n), dtype=torch.int64, device="cuda")
+        ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
+        rqa.rqa_eps_for_rr(view, 0, rr, eps, cnt, rrr, ws)
+        rqa.rqa_line_hist(view, 0, eps, hist, ws)
+        rqa.rqa_workspace_status(ws)
+        rrh = torch.empty_like(rrr)
+        rqa.rqa_line_measures(hist, 2, rr_hist=rrh, theiler=w)
+        assert torch.equal(rrh, rrr)                          # RR from the histogram, over the same P_w
+        for b in range(2):
+            r = oracle.sweep(ys[b], m, tau, rr, 0, 2, threads=0, theiler=w)
+            assert np.array_equal(eps[b].cpu().numpy(), r["eps"]), (m, tau, w)
+            assert np.array_equal(cnt[b].cpu().numpy().view(np.uint64), r["count"]), (m, tau, w)
+            assert np.array_equal(rrr[b].cpu().numpy(), r["rr"]), (m, tau, w)
+            assert np.array_equal(hist[b].cpu().numpy().view(np.uint64), r["hist"]), (m, tau, w, chunk)
+    with pytest.raises(rqa.RqaError):
+        bad = rqa.rqa_embed(torch.zeros(50, device="cuda"), 1, 1, theiler=50)
+        rqa.rqa_workspace_bytes(bad, 3)

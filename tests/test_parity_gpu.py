@@ -29,10 +29,10 @@ def gpu_sweep(rqa, series, m, tau, rr, norm=0, l_min=2):
     }
 
 
-def assert_parity(oracle, g, series, m, tau, rr, norm=0, l_min=2, threads=0):
+def assert_parity(oracle, g, series, m, tau, rr, norm=0, l_min=2, threads=0, theiler=1):
     series = np.atleast_2d(series)
     for b in range(series.shape[0]):
-        r = oracle.sweep(series[b], m, tau, rr, norm, l_min, threads=threads)
+        r = oracle.sweep(series[b], m, tau, rr, norm, l_min, threads=threads, theiler=theiler)
         assert np.array_equal(g["eps"][b].view(np.uint32), r["eps"].view(np.uint32)), f"eps, series {b}"
         assert np.array_equal(g["count"][b], r["count"]), f"count, series {b}"
         assert np.array_equal(g["rr"][b], r["rr"]), f"realised rr, series {b}"
@@ -497,7 +497,7 @@ def test_line_hist_any_chunk_length(rqa, oracle, options, L):
 @pytest.mark.parametrize("seed", [11, 12, 13])
 def test_random_configurations(rqa, oracle, options, seed):
     """Seeded random sweeps (40 per seed): series kind (noise, logistic, sine, quantised, ramp, denormal scale, constant),
-    N, m, tau, K, norm, batch, l_min, delay view or materialised points, and the expert knobs (select path, sample
+    N, m, tau, K, norm, batch, l_min, Theiler window, delay view or materialised points, and the expert knobs (select path, sample
     size, candidate capacity, chunk length) all drawn at random; everything compared with the oracle."""
     import torch
     rng = np.random.default_rng(seed)
@@ -531,7 +531,8 @@ def test_random_configurations(rqa, oracle, options, seed):
         s = torch.as_tensor(ys).cuda()
         n = N - (m - 1) * tau
         X = torch.empty((batch, n, m), dtype=torch.float32, device="cuda") if rng.random() < 0.25 else None
-        view = rqa.rqa_embed(s, m, tau, X)                   # X stays referenced: the view points into it
+        w = min(n - 1, int(rng.choice([0, 0, 0, 1, 2, 3, int(rng.integers(1, n)), n - 1])))      # Theiler window
+        view = rqa.rqa_embed(s, m, tau, X, theiler=w)        # X stays referenced: the view points into it
         eps = torch.empty((batch, K), dtype=torch.float32, device="cuda")
         cnt = torch.empty((batch, K), dtype=torch.int64, device="cuda")
         rrr = torch.empty((batch, K), dtype=torch.float64, device="cuda")
@@ -545,7 +546,7 @@ def test_random_configurations(rqa, oracle, options, seed):
         rqa.rqa_workspace_status(ws)
         g = {"eps": eps.cpu().numpy(), "count": cnt.cpu().numpy().view(np.uint64), "rr": rrr.cpu().numpy(),
              "hist": hist.cpu().numpy().view(np.uint64), "det": det.cpu().numpy(), "det_mean": mean.cpu().numpy()}
-        assert_parity(oracle, g, ys, m, tau, rr, norm, l_min, threads=0)
+        assert_parity(oracle, g, ys, m, tau, rr, norm, l_min, threads=0, theiler=w)
 
 
 @pytest.mark.parametrize("path", [0, 1, 2, 3])

@@ -41,7 +41,7 @@ struct LineGroup {
     int32_t multi;        // 1 if some table bucket holds two or more distinct thresholds (refine by a loop)
     int32_t kcount;       // caller thresholds in this group
     int32_t pad;
-    float scale;          // bucket(d) = bits(fmaf(min(d, dcap), scale, +0)) — a denormal-range FMA, exact rounding
+    float scale;          // bucket(d) = bucket_of(d, dcap, scale) (rqa_tiles.cuh): one FMA, exact rounding
     float dcap;
     float epsd[GK + 1];   // distinct thresholds ascending, epsd[J] = +inf
     int32_t k_of[GK];     // sorted position -> caller's index k
@@ -200,7 +200,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t qp;                // phase 1: shared-window address of the thread's next free queue slot
     uint32_t trel8;             // phase 1: (cells since the last drain) << 8
     // per-thread constants
-    uint32_t lut, eps;          // shared-window addresses of the bucket table and the thresholds
+    uint32_t lut, eps;          // shared-window addresses of the bucket table (biased, see level4) and the thresholds
     uint32_t agg;               // ... of the thread's column of histogram 1, level 0
     uint32_t sh;                // ... of the difference array D
     uint32_t stk;               // ... of the thread's stack column, depth 0 (the sentinel)
@@ -214,8 +214,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     int64_t n;
 
     __device__ __forceinline__ uint32_t level4(float d) const {
-        uint32_t idx = __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
-        uint32_t q = lds_u8(lut + idx);
+        uint32_t q = lds_u8(lut + bucket_bits(d, dcap, scale));   // lut is biased by -BUCKET_MAGIC_BITS
         float er = lds_f32(eps + q);
         uint32_t v4 = q + (d > er ? 4u : 0u);
         if (MULTI) {                                           // some bucket holds two or more thresholds
@@ -448,7 +447,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
         const uint32_t yb_org = pin(smem_addr(yb_s) + 4 * tid * ps);
         auto setup = [&](auto& sc) {
             sc.ya_org = smem_addr(ya_s);
-            sc.lut = smem_addr(lut_s);
+            sc.lut = pin(smem_addr(lut_s) - BUCKET_MAGIC_BITS);   // indexed with bucket_bits()
             sc.eps = smem_addr(eps_s);
             sc.agg = pin(smem_addr(agg_s) + 4 * tid);
             sc.sh = smem_addr(sh_s);

@@ -434,7 +434,7 @@ struct Counter : CellDist<NORM, M, TAU, 0> {
         const float d = CD::template distance<R>();
         float er;
         uint32_t q;
-        lds_f32_u32(lut + 8 * bucket_of(d, dcap, scale), er, q);   // one load: the boundary to compare with, its index
+        lds_f32_u32(lut + 8 * bucket_bits(d, dcap, scale), er, q);   // one load: the boundary to compare with, its index
         // bits 30-31 of the entry say whether level q and level q+1 are candidate levels, encoded so that adding
         // 1 << 30 together with the level increment leaves the answer in bit 31; the level's byte offset below is
         // q * 2^10 modulo 2^32, which drops those bits.
@@ -508,7 +508,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
             ct.tau = a.tau;
             ct.ps = ps;
             ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid * ps), 0);
-            ct.lut = smem_addr(lut_s);
+            ct.lut = pin(smem_addr(lut_s) - 8u * BUCKET_MAGIC_BITS);   // indexed with 8 * bucket_bits()
             ct.beta = smem_addr(beta_s);
             ct.kind = smem_addr(smem + CountSmem::off_kind);
             ct.cols = pin(smem_addr(cols_s) + 4 * (tid % col_words));

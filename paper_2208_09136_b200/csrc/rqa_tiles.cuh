@@ -26,15 +26,22 @@ constexpr int GK = 32;           // thresholds (or brackets) per group = per ful
 constexpr int MAX_SPAN = 4096;   // largest (m-1)*tau the tiled kernels stage in shared memory
 constexpr unsigned FULL = 0xffffffffu;
 
-// bucket(d) = bits(fmaf(min(d, dcap), scale, +0)): a denormal-range FMA, i.e. an exactly rounded, monotone map of
-// [0, dcap] onto the integers 0..NB-1 in one instruction (scale is chosen so that dcap*scale < NB * 2^-149).
+// bucket(d) = bits(fmaf(min(d, dcap), scale, 2^23)) - bits(2^23): adding 2^23 leaves round(d * scale) in the low
+// mantissa bits, i.e. an exactly rounded, monotone map of [0, dcap] onto the integers 0..nb-1 in one FMA, for
+// thresholds of any magnitude (scale = (nb - 1.5) / dcap is an ordinary float).  The subtraction folds into the table's
+// base address.
+constexpr uint32_t BUCKET_MAGIC_BITS = 0x4B000000u;              // bits of 8388608.0f = 2^23
+__device__ __forceinline__ uint32_t bucket_bits(float d, float dcap, float scale) {      // bucket + BUCKET_MAGIC_BITS
+    return __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 8388608.0f));
+}
 __device__ __forceinline__ uint32_t bucket_of(float d, float dcap, float scale) {
-    return __float_as_uint(__fmaf_rn(fminf(d, dcap), scale, 0.0f));
+    return bucket_bits(d, dcap, scale) - BUCKET_MAGIC_BITS;
 }
 
-// Largest scale for which bucket_of(dcap) <= nb-1.
+// Largest scale for which bucket_of(dcap) <= nb-1 (nb <= 2^22).  Denormal-small dcap: the scale saturates, every
+// distance falls into the lowest buckets and the tables' refinement loops do the work.
 __device__ inline float bucket_scale(float dcap, int nb = NB) {
-    double sc = ((double)nb - 1.5) * 1.401298464324817e-45 / (double)dcap;   // (nb-1.5) * 2^-149 / dcap
+    double sc = ((double)nb - 1.5) / (double)dcap;
     float scale = sc > 3.0e38 ? 3.0e38f : (float)sc;
     while (scale > 0.0f && bucket_of(dcap, dcap, scale) > (uint32_t)(nb - 1)) scale = nextafterf(scale, 0.0f);
     return scale;

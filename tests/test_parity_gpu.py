@@ -172,6 +172,18 @@ def test_tiny_scale_and_denormals(rqa, oracle):
         assert_parity(oracle, g, y, 3, 1, rr, norm)
 
 
+@pytest.mark.parametrize("scale", [1e-42, 1e-30, 3e7, 1e30])
+def test_any_magnitude(rqa, oracle, scale):
+    """The level tables bucket distances with one FMA whose scale is an ordinary float: series of any magnitude —
+    from the subnormals to 1e30 (Euclid squares would overflow beyond) — take the same tiled kernels (bracket path:
+    P > 2^22) and give the oracle's results."""
+    y = (wl.add_noise(wl.lorenz_signal(3200), 3.0, 2).astype(np.float64) * scale).astype(np.float32)
+    rr = wl.rr_log(20, 0.001, 0.2)
+    for norm in ((0,) if scale > 1e18 or scale < 1e-18 else (0, 1)):
+        g = gpu_sweep(rqa, y, 3, 1, rr, norm)
+        assert_parity(oracle, g, y, 3, 1, rr, norm, threads=0)
+
+
 # ---------------------------------------------------------------------------- boundary behaviour on the GPU
 @pytest.mark.parametrize("N,m,tau,norm,batch", [(900, 4, 6, 0, 1), (3300, 3, 2, 0, 2), (3300, 3, 2, 1, 1), (3100, 7, 1, 0, 1),
                                                 (3050, 16, 3, 1, 1), (1200, 1, 1, 0, 1)])

@@ -22,12 +22,12 @@ class SweepBuffers:
     ws: object
 
     @staticmethod
-    def allocate(series, m: int, tau: int, K: int):
+    def allocate(series, m: int, tau: int, K: int, theiler: int = 0):
         import torch
         if series.dim() == 1:
             series = series.unsqueeze(0)
         batch, N = series.shape
-        view = B.rqa_embed(series, m, tau)
+        view = B.rqa_embed(series, m, tau, theiler=theiler)
         n = int(view.n_points)
         dev = series.device
         return SweepBuffers(
@@ -43,16 +43,17 @@ class SweepBuffers:
 
 
 def averaged_rqa(series, m: int, tau: int, rr, norm: int = B.RQA_NORM_MAX, l_min: int = 2, buffers: SweepBuffers = None,
-                 check: bool = True):
+                 check: bool = True, theiler: int = 0):
     """series: float32 CUDA tensor [batch][N] or [N].  Runs rqa_embed (view) -> rqa_eps_for_rr -> rqa_line_hist ->
     rqa_det_avg on the current stream and returns the SweepBuffers holding the results (device tensors).
-    With check=True the stream is synchronised and device-side errors (non-finite input) are raised."""
+    With check=True the stream is synchronised and device-side errors (non-finite input) are raised.
+    theiler = w > 1: only pairs with j - i >= w (rqa_points.theiler); buffers must have been allocated for the same w."""
     rr = np.ascontiguousarray(rr, dtype=np.float64)
     if series.dim() == 1:
         series = series.unsqueeze(0)
-    buf = buffers if buffers is not None else SweepBuffers.allocate(series, m, tau, len(rr))
+    buf = buffers if buffers is not None else SweepBuffers.allocate(series, m, tau, len(rr), theiler)
     if buffers is not None:
-        buf.view = B.rqa_embed(series, m, tau)
+        buf.view = B.rqa_embed(series, m, tau, theiler=theiler)
     B.rqa_eps_for_rr(buf.view, norm, rr, buf.eps, buf.count, buf.rr, buf.ws)
     B.rqa_line_hist(buf.view, norm, buf.eps, buf.hist, buf.ws)
     B.rqa_det_avg(buf.hist, l_min, buf.det, buf.det_mean)

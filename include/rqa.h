@@ -25,7 +25,8 @@
  *   - counts are exact uint64; RR and DET are fp64 ratios of exact integers.
  *
  * Memory and ownership: every buffer is owned by the caller.  Pointers named d_* are DEVICE pointers,
- * h_* are HOST pointers.  The library keeps no device allocation and no global state between calls.
+ * h_* are HOST pointers.  The library keeps no device allocation and no global state between calls (the only
+ * process-wide datum is the monotone launch counter behind rqa_launch_count()).
  * Every call enqueues its work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
  * stream) and returns without synchronising; outputs are valid once the stream has been synchronised.
  *
@@ -197,17 +198,51 @@ rqa_status rqa_sweep_host(const float* h_series, int64_t N, int32_t batch, int32
 uint64_t rqa_launch_count(void);
 
 /*
- * Expert / testing knobs, process-wide, not thread-safe against concurrent calls; value 0 restores the automatic
- * choice.  They change how a result is computed, never the result (every path of rqa_eps_for_rr is exact).
- * Workspace sizes depend on them: set options before rqa_workspace_bytes.
- *   "select_path"  rqa_eps_for_rr: 1 = materialise all distances (small P), 2 = sample-bracket + one counting pass,
- *                  3 = four radix passes
- *   "sample_size"  bracket path: number of sampled pair distances per series
- *   "cand_cap"     bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
- *   "line_chunk"   rqa_line_hist: chunk length along the diagonals, 1..1023
- * Unknown names and negative values return RQA_ERR_INVALID_ARG.
+ * Per-call options (expert / testing knobs and the multi-GPU split).  The library keeps NO global state: the plain
+ * calls above are the `_opt` calls below with opt = NULL (every field 0 = automatic).  Options change how a result is
+ * computed, never the result (every path of rqa_eps_for_rr is exact).  Workspace sizes depend on them: pass the same
+ * options to rqa_workspace_bytes_opt and to the call that uses the workspace.
+ *   select_path   rqa_eps_for_rr: 0 automatic, 1 = materialise all distances (small P), 2 = sample-bracket + one
+ *                 counting pass, 3 = four radix passes
+ *   sample_size   bracket path: number of sampled pair distances per series
+ *   cand_cap      bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
+ *   line_chunk    rqa_line_hist: chunk length along the diagonals, 1..1023
+ *   line_segment  rqa_line_hist: consecutive chunks of one diagonal block that a block walks with the run state
+ *                 carried in place (only segment borders are joined by the stitch kernel), >= 1
+ *   line_buffers  rqa_line_hist: 1 = one set of series windows per block, staged by plain loads; 2 = two sets, the next
+ *                 chunk's windows fetched by bulk asynchronous copies while the current chunk is scanned
+ *   part_index, part_count
+ *                 split of ONE call over part_count processes (one GPU each): this process visits
+ *                 only its share of the tiles of the triangle (diagonal blocks part_index, part_index + part_count,
+ *                 ...), and every exact integer counter that must be summed over the parts before the next step can
+ *                 use it (level counts and digit bins of rqa_eps_for_rr; line aggregates and the histogram of
+ *                 rqa_line_hist) is handed to `reduce`.  After the call every part holds the complete, identical
+ *                 outputs.  part_count <= 1: the whole job, `reduce` is not called.
+ *   reduce        int reduce(ctx, d_counters, n, stream): sum the n uint64 device counters at d_counters element-wise
+ *                 over all parts, in place, ordered on `stream` (e.g. ncclAllReduce(ncclUint64, ncclSum), or
+ *                 torch.distributed.all_reduce on a tensor wrapping the pointer); return 0 on success.  Every part
+ *                 makes the same sequence of reduce calls with the same n.
  */
-rqa_status rqa_set_option(const char* name, int64_t value);
+typedef int (*rqa_reduce_fn)(void* ctx, uint64_t* d_counters, size_t n, void* stream);
+typedef struct rqa_options {
+    int32_t select_path;
+    int32_t line_chunk;
+    int32_t line_segment;
+    int32_t part_index;
+    int32_t part_count;
+    int32_t line_buffers;
+    int64_t sample_size;
+    int64_t cand_cap;
+    rqa_reduce_fn reduce;
+    void* reduce_ctx;
+} rqa_options;
+
+rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_options* opt, size_t* bytes);
+rqa_status rqa_eps_for_rr_opt(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps,
+                              uint64_t* d_count, double* d_rr_realised, void* d_ws, size_t ws_bytes, void* stream,
+                              const rqa_options* opt);
+rqa_status rqa_line_hist_opt(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
+                             void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt);
 
 #ifdef __cplusplus
 }

@@ -25,7 +25,8 @@
  * Pins (tests/test_oracle_pins.py, `-m "not gpu"`): hand-enumerated recurrence plots
  * (tests/golden/hand_cases.txt), closed forms for ramp / constant / exactly periodic series, numpy
  * order statistics, the counting certificate, sum_l l*P(l) = C, nesting, triangle symmetry, the i.i.d.
- * uniform-noise closed form DET ~ 1-(1-p)^2, exact-rational re-evaluation of the Euclidean chain.
+ * uniform-noise closed form DET ~ 1-(1-p)^2, exact-rational re-evaluation of the Euclidean chain; vertical lines:
+ * hand-enumerated plots, numpy run-length brute force on the full matrix, sum_v v*P(v) = 2C, ramp closed form.
  * Nothing here is "parity unpinned".
  *
  * The only parallel construct is an optional OpenMP `parallel for` over diagonals / rows whose
@@ -243,6 +244,72 @@ int rqa_oracle_line_hist(const float* y, int64_t N, int m, int64_t tau, int norm
     if (nt > 1)
         for (int t = 0; t < nt; ++t)
             for (size_t q = 0; q < (size_t)K * (size_t)Np; ++q) hist[q] += priv[(size_t)t * K * Np + q];
+    return ORACLE_OK;
+}
+
+/* Vertical-line histogram ("other RQA measures"; the paper defines no vertical-line measure itself —
+ * DESIGN.md reading S19 fixes the convention).  The FULL symmetric N' x N' recurrence matrix is walked
+ * column by column: in column j the cell (i, j) is recurrent iff |i - j| >= theiler (theiler = 1: only the main
+ * diagonal is excluded, readings S2/S9) and d(x_i, x_j) <= eps_k.  vhist[k][v] = number of maximal runs of exactly v
+ * recurrent cells along i; the excluded band splits a column in two; runs touching the border of the plot or the band
+ * count with their truncated length (as S8).  vhist is [K][N'] uint64, vhist[k][0] = 0.  Every recurrent cell of the
+ * upper triangle is visited twice (as (i,j) and as (j,i)), so sum_v v*vhist[k][v] = 2*C_k.
+ *   threads: 1 = the literal serial loop; >1 (0 = all) splits the columns over OpenMP threads (private histograms). */
+int rqa_oracle_vert_hist(const float* y, int64_t N, int m, int64_t tau, int norm, const float* eps, int K,
+                         uint64_t* vhist, int threads, int64_t theiler) {
+    if (!y || !eps || !vhist || m < 1 || tau < 1 || K < 1 || theiler < 1) return ORACLE_BAD_ARG;
+    int64_t Np = embedded_points(N, m, tau);
+    if (Np < 2 || theiler > Np - 1) return ORACLE_BAD_ARG;
+    int nt = pick_threads(threads);
+    std::memset(vhist, 0, sizeof(uint64_t) * (size_t)K * (size_t)Np);
+    std::vector<uint64_t> priv;
+    if (nt > 1) priv.assign((size_t)nt * (size_t)K * (size_t)Np, 0);
+    for (int k = 0; k < K; ++k) {
+        const float e = eps[k];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 8) num_threads(nt) if (nt > 1)
+#endif
+        for (int64_t j = 0; j < Np; ++j) {                     /* column j */
+            uint64_t* h = vhist + (size_t)k * Np;
+#ifdef _OPENMP
+            if (nt > 1) h = priv.data() + ((size_t)omp_get_thread_num() * K + k) * (size_t)Np;
+#endif
+            int64_t run = 0;
+            for (int64_t i = 0; i < Np; ++i) {                 /* down the column */
+                const int64_t gap = i > j ? i - j : j - i;
+                const bool rec = gap >= theiler && distance(y, i, j, m, tau, norm) <= e;
+                if (rec) {
+                    ++run;
+                } else {
+                    if (run > 0) h[run] += 1;
+                    run = 0;
+                }
+            }
+            if (run > 0) h[run] += 1;
+        }
+    }
+    if (nt > 1)
+        for (int t = 0; t < nt; ++t)
+            for (size_t q = 0; q < (size_t)K * (size_t)Np; ++q) vhist[q] += priv[(size_t)t * K * Np + q];
+    return ORACLE_OK;
+}
+
+/* Laminarity and trapping time from the vertical-line histogram (textbook definitions, Marwan et al. 2007 — the
+ * paper's ref. [2], which PAPER.md:86 points to; not written out in the paper):
+ *   LAM_k = sum_{v>=v_min} v*P_k(v) / sum_{v>=1} v*P_k(v),   TT_k = sum_{v>=v_min} v*P_k(v) / sum_{v>=v_min} P_k(v)
+ * (0 where the denominator is empty).  Integer sums exact in uint64, one fp64 divide each. */
+int rqa_oracle_lam_tt(const uint64_t* vhist, int K, int64_t n_points, int64_t v_min, double* lam, double* tt) {
+    if (!vhist || !lam || !tt || K < 1 || n_points < 2 || v_min < 1) return ORACLE_BAD_ARG;
+    for (int k = 0; k < K; ++k) {
+        uint64_t all = 0, num = 0, lines = 0;
+        for (int64_t v = 1; v < n_points; ++v) {
+            const uint64_t h = vhist[(size_t)k * n_points + v];
+            all += (uint64_t)v * h;
+            if (v >= v_min) { num += (uint64_t)v * h; lines += h; }
+        }
+        lam[k] = all ? (double)num / (double)all : 0.0;
+        tt[k] = lines ? (double)num / (double)lines : 0.0;
+    }
     return ORACLE_OK;
 }
 

@@ -56,6 +56,8 @@ def _load():
     lib.rqa_oracle_eps_for_rr.argtypes = [f32p, i64, i32, i64, i32, f64p, i32, f32p, u64p, f64p, i64]
     lib.rqa_oracle_count_lt_le.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, u64p, i32]
     lib.rqa_oracle_line_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i32, i64]
+    lib.rqa_oracle_vert_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i64]
+    lib.rqa_oracle_lam_tt.argtypes = [u64p, i32, i64, i64, f64p, f64p]
     lib.rqa_oracle_det_avg.argtypes = [u64p, i32, i64, i64, f64p, f64p]
     lib.rqa_oracle_det_prefix_avg.argtypes = [f64p, i32, f64p]
     lib.rqa_oracle_line_measures.argtypes = [u64p, i32, i64, i64, f64p, u64p, f64p, f64p, i64]
@@ -152,6 +154,29 @@ def line_hist(y, m: int, tau: int, eps, norm: int = NORM_MAX, lower: bool = Fals
                                         _p(hist, ctypes.c_uint64), 1 if lower else 0, threads, max(1, theiler)),
            "line_hist")
     return hist
+
+
+def vert_hist(y, m: int, tau: int, eps, norm: int = NORM_MAX, threads: int = 1, theiler: int = 1) -> np.ndarray:
+    """-> vhist[K][N'] uint64: vertical-line lengths over the columns of the full symmetric matrix (reading S19)"""
+    y = _series(y)
+    eps = np.ascontiguousarray(eps, dtype=np.float32)
+    K = len(eps)
+    n = n_embedded(len(y), m, tau)
+    vhist = np.empty((K, n), dtype=np.uint64)
+    _check(_load().rqa_oracle_vert_hist(_p(y, ctypes.c_float), len(y), m, tau, norm, _p(eps, ctypes.c_float), K,
+                                        _p(vhist, ctypes.c_uint64), threads, max(1, theiler)), "vert_hist")
+    return vhist
+
+
+def lam_tt(vhist, v_min: int = 2):
+    """-> (LAM[K], TT[K]) float64 from the vertical-line histogram"""
+    vhist = np.ascontiguousarray(vhist, dtype=np.uint64)
+    K, n = vhist.shape
+    lam = np.empty(K, dtype=np.float64)
+    tt = np.empty(K, dtype=np.float64)
+    _check(_load().rqa_oracle_lam_tt(_p(vhist, ctypes.c_uint64), K, n, v_min, _p(lam, ctypes.c_double),
+                                     _p(tt, ctypes.c_double)), "lam_tt")
+    return lam, tt
 
 
 def det_avg(hist, l_min: int = 2):

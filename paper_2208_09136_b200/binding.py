@@ -27,8 +27,8 @@ RQA_MAX_M = 16
 # every symbol include/rqa.h declares (tests check that the library exports them all)
 EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_bytes", "rqa_workspace_status",
            "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
-           "rqa_sweep_host", "rqa_launch_count", "rqa_set_option", "rqa_det_prefix_avg", "rqa_line_measures",
-           "rqa_sorting_rate_host"]
+           "rqa_sweep_host", "rqa_launch_count", "rqa_workspace_bytes_opt", "rqa_eps_for_rr_opt", "rqa_line_hist_opt",
+           "rqa_det_prefix_avg", "rqa_line_measures", "rqa_sorting_rate_host"]
 
 
 class RqaPoints(ctypes.Structure):
@@ -36,6 +36,42 @@ class RqaPoints(ctypes.Structure):
     _fields_ = [("data", ctypes.c_void_p), ("n_points", ctypes.c_int64), ("m", ctypes.c_int32),
                 ("batch", ctypes.c_int32), ("point_stride", ctypes.c_int64), ("coord_stride", ctypes.c_int64),
                 ("batch_stride", ctypes.c_int64), ("theiler", ctypes.c_int64)]
+
+
+REDUCE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+
+
+class RqaOptions(ctypes.Structure):
+    """struct rqa_options (per call; every field 0 = automatic)"""
+    _fields_ = [("select_path", ctypes.c_int32), ("line_chunk", ctypes.c_int32), ("line_segment", ctypes.c_int32),
+                ("part_index", ctypes.c_int32), ("part_count", ctypes.c_int32), ("line_buffers", ctypes.c_int32),
+                ("sample_size", ctypes.c_int64), ("cand_cap", ctypes.c_int64), ("reduce", REDUCE_FN),
+                ("reduce_ctx", ctypes.c_void_p)]
+
+
+def make_options(select_path=0, line_chunk=0, line_segment=0, line_buffers=0, sample_size=0, cand_cap=0, part_index=0,
+                 part_count=0, reduce=None) -> RqaOptions:
+    """reduce: a Python callable (d_ptr: int, n: int, stream: int) -> None that sums n uint64 device counters over the
+    parts of a split call (see parts.py); kept alive by the returned struct."""
+    o = RqaOptions()
+    o.select_path, o.line_chunk, o.line_segment, o.line_buffers = select_path, line_chunk, line_segment, line_buffers
+    o.sample_size, o.cand_cap, o.part_index, o.part_count = sample_size, cand_cap, part_index, part_count
+    if reduce is not None:
+        def _cb(ctx, ptr, n, stream):
+            try:
+                reduce(int(ptr or 0), int(n), int(stream or 0))
+                return 0
+            except Exception:                                # never let an exception cross the C ABI
+                import traceback
+                traceback.print_exc()
+                return 1
+        o._cb = REDUCE_FN(_cb)
+        o.reduce = o._cb
+    return o
+
+
+def _opt(options):
+    return None if options is None else ctypes.byref(options)
 
 
 class RqaError(RuntimeError):
@@ -70,7 +106,10 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_det_avg.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp]
     lib.rqa_sweep_workspace_bytes.argtypes = [i64, i32, i32, i64, i32, ctypes.POINTER(sz)]
     lib.rqa_sweep_host.argtypes = [vp, i64, i32, i32, i64, ctypes.c_int, vp, i32, i64, vp, vp, vp, vp, vp, vp, vp, sz, vp]
-    lib.rqa_set_option.argtypes = [ctypes.c_char_p, i64]
+    opt = ctypes.POINTER(RqaOptions)
+    lib.rqa_workspace_bytes_opt.argtypes = [pts, i32, opt, ctypes.POINTER(sz)]
+    lib.rqa_eps_for_rr_opt.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, vp, vp, sz, vp, opt]
+    lib.rqa_line_hist_opt.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp, opt]
     lib.rqa_det_prefix_avg.argtypes = [vp, i32, i32, vp, vp]
     lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp, vp]
     lib.rqa_sorting_rate_host.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double)]
@@ -90,12 +129,18 @@ def _stream(stream=None) -> int:
     return int(s.cuda_stream)
 
 
-def _dev(t, dtype, what: str) -> int:
+def _dev(t, dtype, what: str, numel: int = None) -> int:
+    """Device pointer of a contiguous CUDA tensor of the given dtype on the current device (and, when `numel` is given,
+    of exactly that many elements: a wrong shape would otherwise be a silent out-of-bounds device write)."""
     import torch
     if not isinstance(t, torch.Tensor) or not t.is_cuda:
         raise TypeError(f"{what} must be a CUDA tensor")
     if t.dtype != dtype or not t.is_contiguous():
         raise TypeError(f"{what} must be a contiguous {dtype} tensor")
+    if t.device.index != torch.cuda.current_device():
+        raise ValueError(f"{what} lives on {t.device}, the current device is cuda:{torch.cuda.current_device()}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{what} has {t.numel()} elements, expected {numel}")
     return t.data_ptr()
 
 
@@ -107,14 +152,9 @@ def rqa_launch_count() -> int:
     return int(load_library().rqa_launch_count())
 
 
-def rqa_set_option(name: str, value: int) -> None:
-    """Expert / testing knob (include/rqa.h); 0 restores the automatic choice."""
-    _check(load_library().rqa_set_option(name.encode(), int(value)))
-
-
-def rqa_workspace_bytes(pts: RqaPoints, K: int) -> int:
+def rqa_workspace_bytes(pts: RqaPoints, K: int, options: RqaOptions = None) -> int:
     n = ctypes.c_size_t(0)
-    _check(load_library().rqa_workspace_bytes(ctypes.byref(pts), K, ctypes.byref(n)))
+    _check(load_library().rqa_workspace_bytes_opt(ctypes.byref(pts), K, _opt(options), ctypes.byref(n)))
     return int(n.value)
 
 
@@ -134,32 +174,35 @@ def rqa_embed(series, m: int, tau: int, X=None, stream=None, theiler: int = 0) -
     p = _dev(series, torch.float32, "series")
     batch, N = series.shape
     view = RqaPoints()
-    xp = None if X is None else _dev(X, torch.float32, "X")
+    xp = None if X is None else _dev(X, torch.float32, "X", batch * (N - (m - 1) * tau) * m)
     _check(load_library().rqa_embed(p, N, batch, N, m, tau, xp, ctypes.byref(view), _stream(stream)))
     view._owner = series if X is None else X                 # the view points into this tensor: keep it alive
     view.theiler = theiler                                   # a field of the view, not an argument of rqa_embed
     return view
 
 
-def rqa_eps_for_rr(pts: RqaPoints, norm: int, rr, eps, count, rr_realised, ws, stream=None) -> None:
+def rqa_eps_for_rr(pts: RqaPoints, norm: int, rr, eps, count, rr_realised, ws, stream=None,
+                   options: RqaOptions = None) -> None:
     """rr: host float64 array [K]; eps float32 / count int64(uint64 bits) / rr_realised float64 CUDA tensors
     [batch][K]; ws: uint8 CUDA workspace."""
     import torch
     rr = np.ascontiguousarray(rr, dtype=np.float64)
     K = len(rr)
-    _check(load_library().rqa_eps_for_rr(ctypes.byref(pts), norm, rr.ctypes.data, K, _dev(eps, torch.float32, "eps"),
-                                         _dev(count, torch.int64, "count"),
-                                         _dev(rr_realised, torch.float64, "rr_realised"),
-                                         _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream)))
+    bk = int(pts.batch) * K
+    _check(load_library().rqa_eps_for_rr_opt(ctypes.byref(pts), norm, rr.ctypes.data, K,
+                                             _dev(eps, torch.float32, "eps", bk), _dev(count, torch.int64, "count", bk),
+                                             _dev(rr_realised, torch.float64, "rr_realised", bk),
+                                             _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream), _opt(options)))
 
 
-def rqa_line_hist(pts: RqaPoints, norm: int, eps, hist, ws, stream=None) -> None:
+def rqa_line_hist(pts: RqaPoints, norm: int, eps, hist, ws, stream=None, options: RqaOptions = None) -> None:
     """eps float32 CUDA [batch][K]; hist int64 (uint64 bits) CUDA [batch][K][n_points]."""
     import torch
     K = eps.shape[-1]
-    _check(load_library().rqa_line_hist(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps"), K,
-                                        _dev(hist, torch.int64, "hist"), _dev(ws, torch.uint8, "ws"), ws.numel(),
-                                        _stream(stream)))
+    bk = int(pts.batch) * K
+    _check(load_library().rqa_line_hist_opt(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps", bk), K,
+                                            _dev(hist, torch.int64, "hist", bk * int(pts.n_points)),
+                                            _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream), _opt(options)))
 
 
 def rqa_det_avg(hist, l_min: int, det, det_mean, stream=None) -> None:
@@ -167,8 +210,8 @@ def rqa_det_avg(hist, l_min: int, det, det_mean, stream=None) -> None:
     import torch
     batch, K, n = hist.shape
     _check(load_library().rqa_det_avg(_dev(hist, torch.int64, "hist"), batch, K, n, l_min,
-                                      _dev(det, torch.float64, "det"), _dev(det_mean, torch.float64, "det_mean"),
-                                      _stream(stream)))
+                                      _dev(det, torch.float64, "det", batch * K),
+                                      _dev(det_mean, torch.float64, "det_mean", batch), _stream(stream)))
 
 
 def rqa_det_prefix_avg(det, prefix, stream=None) -> None:

@@ -12,8 +12,46 @@ namespace rqa {
 
 static thread_local char t_err[512] = "";
 std::atomic<uint64_t> g_launches{0};
-static Options g_options{0, 0, 0, 0};
-const Options& options() { return g_options; }
+
+rqa_status make_options(const rqa_options* in, Options* out, const char* who) {
+    *out = Options{};
+    if (!in) return RQA_OK;
+    if (in->select_path < 0 || in->select_path > 3) { set_error("%s: options.select_path is 0..3", who); return RQA_ERR_INVALID_ARG; }
+    if (in->line_chunk < 0 || in->line_chunk > 1023) { set_error("%s: options.line_chunk is 0..1023", who); return RQA_ERR_INVALID_ARG; }
+    if (in->line_buffers < 0 || in->line_buffers > 2) { set_error("%s: options.line_buffers is 0..2", who); return RQA_ERR_INVALID_ARG; }
+    if (in->line_segment < 0) { set_error("%s: options.line_segment must be >= 0", who); return RQA_ERR_INVALID_ARG; }
+    if (in->sample_size < 0 || in->cand_cap < 0) { set_error("%s: options.sample_size and cand_cap must be >= 0", who); return RQA_ERR_INVALID_ARG; }
+    if (in->part_count < 0 || in->part_index < 0 || (in->part_count > 0 && in->part_index >= in->part_count) ||
+        (in->part_count == 0 && in->part_index != 0)) {
+        set_error("%s: options need 0 <= part_index < part_count", who);
+        return RQA_ERR_INVALID_ARG;
+    }
+    if (in->part_count > 1 && !in->reduce) { set_error("%s: options.part_count > 1 needs a reduce callback", who); return RQA_ERR_INVALID_ARG; }
+    out->select_path = in->select_path;
+    out->line_chunk = in->line_chunk;
+    out->line_segment = in->line_segment;
+    out->line_buffers = in->line_buffers;
+    out->sample_size = in->sample_size;
+    out->cand_cap = in->cand_cap;
+    out->parts = in->part_count > 1 ? in->part_count : 1;
+    out->part = in->part_count > 1 ? in->part_index : 0;
+    out->reduce = in->reduce;
+    out->reduce_ctx = in->reduce_ctx;
+    return RQA_OK;
+}
+
+int sm_count() {
+    static thread_local int cached_dev = -1, cached = 148;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 148; }
+    if (dev != cached_dev) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) cached = n;
+        else { cudaGetLastError(); cached = 148; }
+        cached_dev = dev;
+    }
+    return cached;
+}
 
 void set_error(const char* fmt, ...) {
     va_list ap;
@@ -132,38 +170,26 @@ const char* rqa_last_error(void) { return t_err; }
 const char* rqa_version(void) { return "0.1 sm_100a"; }
 uint64_t rqa_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
-rqa_status rqa_set_option(const char* name, int64_t value) {
-    if (!name) { set_error("rqa_set_option: name is NULL"); return RQA_ERR_INVALID_ARG; }
-    if (value < 0) { set_error("rqa_set_option: value must be >= 0"); return RQA_ERR_INVALID_ARG; }
-    if (!strcmp(name, "select_path")) {
-        if (value > 3) { set_error("rqa_set_option: select_path is 0..3"); return RQA_ERR_INVALID_ARG; }
-        g_options.select_path = value;
-    } else if (!strcmp(name, "sample_size")) {
-        g_options.sample_size = value;
-    } else if (!strcmp(name, "cand_cap")) {
-        g_options.cand_cap = value;
-    } else if (!strcmp(name, "line_chunk")) {
-        if (value > 1023) { set_error("rqa_set_option: line_chunk is at most 1023"); return RQA_ERR_INVALID_ARG; }
-        g_options.line_chunk = value;
-    } else {
-        set_error("rqa_set_option: unknown option '%s'", name);
-        return RQA_ERR_INVALID_ARG;
-    }
+rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_options* opt, size_t* bytes) {
+    if (!bytes) { set_error("rqa_workspace_bytes: bytes is NULL"); return RQA_ERR_INVALID_ARG; }
+    if (!pts) { set_error("rqa_workspace_bytes: pts is NULL"); return RQA_ERR_INVALID_ARG; }
+    if (K < 1 || K > RQA_MAX_K) { set_error("rqa_workspace_bytes: K = %d outside 1..%d", K, RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
+    Options o;
+    rqa_status st = make_options(opt, &o, "rqa_workspace_bytes");
+    if (st != RQA_OK) return st;
+    // data pointer is not needed for sizing
+    rqa_points p = *pts;
+    if (!p.data) p.data = (const float*)(uintptr_t)256;
+    st = validate_points(&p, "rqa_workspace_bytes");
+    if (st != RQA_OK) return st;
+    View v = make_view(p);
+    size_t a = select_workspace_bytes(v, K, o), b = line_workspace_bytes(v, K, o);
+    *bytes = sizeof(WsStatus) + (a > b ? a : b);
     return RQA_OK;
 }
 
 rqa_status rqa_workspace_bytes(const rqa_points* pts, int32_t K, size_t* bytes) {
-    if (!bytes) { set_error("rqa_workspace_bytes: bytes is NULL"); return RQA_ERR_INVALID_ARG; }
-    if (K < 1 || K > RQA_MAX_K) { set_error("rqa_workspace_bytes: K = %d outside 1..%d", K, RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
-    // data pointer is not needed for sizing
-    rqa_points p = *pts;
-    if (!p.data) p.data = (const float*)(uintptr_t)256;
-    rqa_status st = validate_points(&p, "rqa_workspace_bytes");
-    if (st != RQA_OK) return st;
-    View v = make_view(p);
-    size_t a = select_workspace_bytes(v, K), b = line_workspace_bytes(v, K);
-    *bytes = sizeof(WsStatus) + (a > b ? a : b);
-    return RQA_OK;
+    return rqa_workspace_bytes_opt(pts, K, nullptr, bytes);
 }
 
 rqa_status rqa_workspace_status(const void* d_ws, void* stream) {
@@ -202,7 +228,16 @@ rqa_status rqa_embed(const float* d_series, int64_t N, int32_t batch, int64_t se
 
 rqa_status rqa_eps_for_rr(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps,
                           uint64_t* d_count, double* d_rr_realised, void* d_ws, size_t ws_bytes, void* stream) {
+    return rqa_eps_for_rr_opt(pts, norm, h_rr, K, d_eps, d_count, d_rr_realised, d_ws, ws_bytes, stream, nullptr);
+}
+
+rqa_status rqa_eps_for_rr_opt(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps,
+                              uint64_t* d_count, double* d_rr_realised, void* d_ws, size_t ws_bytes, void* stream,
+                              const rqa_options* opt) {
     rqa_status st = validate_points(pts, "rqa_eps_for_rr");
+    if (st != RQA_OK) return st;
+    Options o;
+    st = make_options(opt, &o, "rqa_eps_for_rr");
     if (st != RQA_OK) return st;
     if (norm != RQA_NORM_MAX && norm != RQA_NORM_EUCLID) { set_error("rqa_eps_for_rr: unknown norm %d", (int)norm); return RQA_ERR_INVALID_ARG; }
     if (K < 1 || K > RQA_MAX_K) { set_error("rqa_eps_for_rr: K = %d outside 1..%d", K, RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
@@ -218,33 +253,41 @@ rqa_status rqa_eps_for_rr(const rqa_points* pts, rqa_norm norm, const double* h_
         double r = std::ceil(rr * (double)P);
         rank[k] = !(r >= 1.0) ? 1 : (r >= (double)P ? P : (uint64_t)r);
     }
-    size_t need = sizeof(WsStatus) + select_workspace_bytes(v, K);
+    size_t need = sizeof(WsStatus) + select_workspace_bytes(v, K, o);
     if (ws_bytes < need) { set_error("rqa_eps_for_rr: workspace %zu < %zu bytes", ws_bytes, need); return RQA_ERR_WORKSPACE_TOO_SMALL; }
     cudaStream_t s = (cudaStream_t)stream;
     Arena ws(d_ws, ws_bytes);
     WsStatus* status = ws.take<WsStatus>(1);
     st = launch_finite_check(v, status, s);
     if (st != RQA_OK) return st;
-    return run_select(v, (int)norm, rank, K, d_eps, d_count, d_rr_realised, ws, s);
+    return run_select(v, (int)norm, rank, K, d_eps, d_count, d_rr_realised, ws, s, o);
 }
 
 rqa_status rqa_line_hist(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
                          void* d_ws, size_t ws_bytes, void* stream) {
+    return rqa_line_hist_opt(pts, norm, d_eps, K, d_hist, d_ws, ws_bytes, stream, nullptr);
+}
+
+rqa_status rqa_line_hist_opt(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
+                             void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt) {
     rqa_status st = validate_points(pts, "rqa_line_hist");
+    if (st != RQA_OK) return st;
+    Options o;
+    st = make_options(opt, &o, "rqa_line_hist");
     if (st != RQA_OK) return st;
     if (norm != RQA_NORM_MAX && norm != RQA_NORM_EUCLID) { set_error("rqa_line_hist: unknown norm %d", (int)norm); return RQA_ERR_INVALID_ARG; }
     if (K < 1 || K > RQA_MAX_K) { set_error("rqa_line_hist: K = %d outside 1..%d", K, RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
     if (!d_eps || !d_hist || !d_ws) { set_error("rqa_line_hist: NULL argument"); return RQA_ERR_INVALID_ARG; }
     if (((uintptr_t)d_ws & 255) != 0) { set_error("rqa_line_hist: workspace must be 256-byte aligned"); return RQA_ERR_INVALID_ARG; }
     View v = make_view(*pts);
-    size_t need = sizeof(WsStatus) + line_workspace_bytes(v, K);
+    size_t need = sizeof(WsStatus) + line_workspace_bytes(v, K, o);
     if (ws_bytes < need) { set_error("rqa_line_hist: workspace %zu < %zu bytes", ws_bytes, need); return RQA_ERR_WORKSPACE_TOO_SMALL; }
     cudaStream_t s = (cudaStream_t)stream;
     Arena ws(d_ws, ws_bytes);
     WsStatus* status = ws.take<WsStatus>(1);
     st = launch_finite_check(v, status, s);
     if (st != RQA_OK) return st;
-    return run_line_hist(v, (int)norm, d_eps, K, d_hist, ws, s);
+    return run_line_hist(v, (int)norm, d_eps, K, d_hist, ws, s, o);
 }
 
 rqa_status rqa_det_avg(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,

@@ -36,14 +36,29 @@ extern std::atomic<uint64_t> g_launches;
     } while (0)
 
 // --------------------------------------------------------------------------------------------- options
-// Process-wide expert/testing knobs (rqa_set_option); 0 = automatic.
+// Validated per-call copy of rqa_options (include/rqa.h); every field 0 = automatic.  There is no process-wide state.
 struct Options {
-    int64_t select_path;   // 0 auto, 1 direct (materialise all distances), 2 bracket (sample + one counting pass), 3 radix
-    int64_t sample_size;   // bracket path: sample size S
-    int64_t cand_cap;      // bracket path: candidate capacity per series
-    int64_t line_chunk;    // diagonal scan: chunk length L (<= 1023)
+    int select_path = 0;      // 0 auto, 1 direct (materialise all distances), 2 bracket (sample + one counting pass), 3 radix
+    int line_chunk = 0;       // diagonal scan: chunk length L (<= 1023)
+    int line_segment = 0;     // diagonal scan: chunks per segment
+    int line_buffers = 0;     // diagonal scan: window sets per block (1 plain loads, 2 bulk-copy double buffer)
+    int part = 0, parts = 1;  // this process' share of the tiles (multi-GPU split of one call)
+    int64_t sample_size = 0;  // bracket path: sample size S
+    int64_t cand_cap = 0;     // bracket path: candidate capacity per series
+    rqa_reduce_fn reduce = nullptr;
+    void* reduce_ctx = nullptr;
 };
-const Options& options();
+rqa_status make_options(const rqa_options* in, Options* out, const char* who);
+
+// Sum n uint64 device counters over the parts of a split call (no-op for a single part).
+inline rqa_status reduce_parts(const Options& o, void* d_counters, size_t n, cudaStream_t s) {
+    if (o.parts <= 1) return RQA_OK;
+    if (o.reduce(o.reduce_ctx, (uint64_t*)d_counters, n, (void*)s) != 0) {
+        set_error("the reduce callback of rqa_options failed");
+        return RQA_ERR_CUDA;
+    }
+    return RQA_OK;
+}
 
 // ------------------------------------------------------------------------------------------------ view
 // Device-side copy of rqa_points (x_i[c] of series b = data[b*bs + i*ps + c*cs]).
@@ -106,13 +121,16 @@ struct Arena {
 // ------------------------------------------------------------------------------------ internal launchers
 rqa_status launch_finite_check(const View& v, WsStatus* st, cudaStream_t s);
 
-size_t select_workspace_bytes(const View& v, int K);
+size_t select_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
-                      double* d_rr, Arena& ws, cudaStream_t s);
+                      double* d_rr, Arena& ws, cudaStream_t s, const Options& opt);
 
-size_t line_workspace_bytes(const View& v, int K);
+size_t line_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws,
-                         cudaStream_t s);
+                         cudaStream_t s, const Options& opt);
+
+// Number of SMs of the current device (cached per thread; 148 on a B200).
+int sm_count();
 
 // ---------------------------------------------------------------------------------------- device helpers
 #ifdef __CUDACC__

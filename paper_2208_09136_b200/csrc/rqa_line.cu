@@ -21,8 +21,14 @@
 //            C_j = sum l*P_j(l), Q2_j = sum (l-1)*P_j(l) and Q3_j = sum_{l>=3} (l-2)*P_j(l), from which the
 //            finalize kernel solves P_j(1..3) exactly.
 //            Lines of length >= 4 that lie inside a chunk go to the shared-memory difference array (l < 128) or
-//            to global atomics (longer).  Runs touching a chunk border are written as (prefix, suffix) summaries
-//            and joined along each diagonal by the stitch kernel.
+//            to global atomics (longer).
+//   blocks : PERSISTENT.  The grid is (blocks per SM) x (SMs); a block draws work items from an atomic counter.  An
+//            item is a SEGMENT = up to S consecutive chunks of one diagonal block of one series.  Inside a segment the
+//            runs that cross a chunk border are carried in place (a per-thread, per-threshold length in an L2-resident
+//            buffer owned by the block), so only segment borders are written as (prefix, suffix) summaries and joined
+//            along each diagonal by the stitch kernel.  The two series windows of the next chunk are fetched by bulk
+//            asynchronous copies (cp.async.bulk + mbarrier) into the other half of a double buffer while the current
+//            chunk is scanned.
 
 #include "rqa_tiles.cuh"
 
@@ -120,14 +126,16 @@ __global__ void __launch_bounds__(128) line_groups_kernel(const float* __restric
     }
 }
 
-// tile_start[ob] = number of tiles of the diagonal blocks before ob; diagonal block ob = diagonals
-// 1 + 256*ob .. 256 + 256*ob, its longest diagonal has n - 1 - 256*ob cells, cut into chunks of L.
-__global__ void __launch_bounds__(1024) tile_table_kernel(int64_t n, int L, int n_ob, uint32_t* __restrict__ tile_start) {
+// tile_start[q] = number of tiles in the local diagonal blocks before q (q = 0..n_obl); local block q is the diagonal
+// block ob = part + q * parts (this process' share of a split call; parts = 1: ob = q), its longest diagonal has
+// nd - 1 - LW*ob cells, cut into tiles of T cells (T = L for the counting pass, S*L = one segment for the scan).
+__global__ void __launch_bounds__(1024) tile_table_kernel(int64_t nd, int64_t T, int n_obl, int part, int parts,
+                                                          uint32_t* __restrict__ tile_start) {
     __shared__ uint32_t s_part[1024];
-    const int per = (n_ob + 1023) / 1024;
-    const int lo = threadIdx.x * per, hi = min(n_ob, lo + per);
+    const int per = (n_obl + 1023) / 1024;
+    const int lo = min(n_obl, (int)threadIdx.x * per), hi = min(n_obl, lo + per);
     uint32_t sum = 0;
-    for (int ob = lo; ob < hi; ++ob) sum += (uint32_t)((n - 1 - (int64_t)LW * ob + L - 1) / L);
+    for (int q = lo; q < hi; ++q) sum += (uint32_t)((nd - 1 - (int64_t)LW * (part + (int64_t)q * parts) + T - 1) / T);
     s_part[threadIdx.x] = sum;
     __syncthreads();
     for (int off = 1; off < 1024; off <<= 1) {
@@ -137,40 +145,49 @@ __global__ void __launch_bounds__(1024) tile_table_kernel(int64_t n, int L, int 
         __syncthreads();
     }
     uint32_t run = s_part[threadIdx.x] - sum;
-    for (int ob = lo; ob < hi; ++ob) {
-        tile_start[ob] = run;
-        run += (uint32_t)((n - 1 - (int64_t)LW * ob + L - 1) / L);
+    for (int q = lo; q < hi; ++q) {
+        tile_start[q] = run;
+        run += (uint32_t)((nd - 1 - (int64_t)LW * (part + (int64_t)q * parts) + T - 1) / T);
     }
-    if (threadIdx.x == 1023) tile_start[n_ob] = s_part[1023];
+    if (threadIdx.x == 1023) tile_start[n_obl] = s_part[1023];
 }
 
 // ------------------------------------------------------------------------------------------ the scan
 // Cell distances: CellDist (rqa_tiles.cuh) with two warm-up cells before the chunk.
 // Shared-memory plan of the scan kernel (bytes); NP: the group has J <= 2*NP distinct thresholds.
-// The two series windows come last because their length depends on the run-time span (m-1)*tau.
+// The series windows come last because their length depends on the run-time span (m-1)*tau and on the chunk length;
+// there are one or two sets of them (double buffer).
 template <int NP>
 struct ScanSmem {
     static constexpr int NLEV = 2 * NP + 1;                   // levels 0..2NP
     static constexpr int off_lut = 0;
     static constexpr int off_eps = off_lut + NB;
-    static constexpr int off_agg = off_eps + 4 * (GK + 4);
+    static constexpr int off_tot = off_eps + 4 * (GK + 4);    // uint32 tot[3][GK+1]: the block's aggregate totals of an item
+    static constexpr int off_agg = off_tot + ((4 * 3 * (GK + 1) + 15) / 16) * 16;
     static constexpr int agg_row = 4 * LW;                    // one level: a word per thread = three 10-bit counters
     static constexpr int off_sh = off_agg + NLEV * agg_row;   // int32 D[NLEV][LS]: difference array over the thresholds
     static constexpr int stk_row = 2 * LW;                    // one stack depth: a 16-bit entry per thread
     static constexpr int off_stk = off_sh + 4 * NLEV * LS;    // uint16 stack[NLEV][LW]
     static constexpr int off_q = off_stk + NLEV * stk_row;    // uint16 queue[QCELLS][LW]: deferred stack events
-    static constexpr int off_ya = off_q + QCELLS * stk_row;
+    static constexpr int off_ya = off_q + QCELLS * stk_row;   // window sets, 16-byte aligned
+    static_assert(off_agg % 16 == 0 && off_ya % 16 == 0, "bulk copies need 16-byte aligned shared addresses");
 };
+constexpr uint32_t CARRY_SEG = 0x80000000u;   // carry flag: the run has been alive since the start of the segment
+
 struct ScanArgs {
     View v;
-    int g, NG, K, L, n_ob;
+    int g, NG, K, L, S;         // threshold group, groups, thresholds, chunk length, chunks per segment
+    int part, parts, n_obl;     // this process' diagonal blocks: ob = part + q*parts, q < n_obl
+    int nbuf;                   // window sets in shared memory (2: bulk-copy double buffer)
     const LineGroup* groups;
-    const uint32_t* tile_start;
+    const uint32_t* seg_start;  // [n_obl+1] segments in the local diagonal blocks before q
     unsigned long long* hist;   // [batch][K][n]
     unsigned long long* agg;    // [batch][NG][3][GK+1]
-    uint16_t* pre;              // [batch][tiles][2*NP][LW]  prefix run of every threshold (recurrent since the chunk start)
-    uint16_t* suf;              // [batch][tiles][2*NP][LW]  run alive at the chunk end
-    uint32_t tiles;
+    uint32_t* pre;              // [batch][segs][2*NP][LW]  prefix run of every threshold (recurrent since the segment start)
+    uint32_t* suf;              // [batch][segs][2*NP][LW]  run alive at the segment end
+    uint32_t* carry;            // [gridDim.x][2*NP][LW]    run alive at the end of the previous chunk of the segment
+    unsigned int* counter;      // work-item counter (zeroed before the launch)
+    uint32_t segs;              // segments per series (this part)
     int m, tau;                 // run-time embedding (used by the M == 0 variant)
 };
 
@@ -208,7 +225,8 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
     uint32_t ya_org;            // ... of the i-side window, index 0
     unsigned long long* grow;   // hist + b*K*n (rows indexed through rep)
     const int* rep;
-    uint16_t* pre_out;
+    uint32_t* carry;            // this thread's column of the block's carry buffer (index j * LW)
+    uint32_t* pre_out;          // this thread's column of the segment's prefix summaries
     float scale, dcap;
     uint32_t J4;
     int64_t n;
@@ -223,7 +241,9 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         return v4;
     }
 
-    // One run of `len` cells ended for the thresholds [lo4, hi4) / 4.  start == 0: it began at the chunk start.
+    // One run of `len` cells ended for the thresholds [lo4, hi4) / 4.  start == 0: it began at the chunk start, i.e. it
+    // continues the run that was alive at the end of the previous chunk (carry, per threshold).  A run that has been
+    // alive since the segment start is the segment's prefix run: written for the stitch kernel, not counted here.
     __device__ __forceinline__ void ended(uint32_t lo4, uint32_t hi4, uint32_t start, uint32_t len) {
         if (start != 0 && len < (uint32_t)LS) {
             const uint32_t col = sh + 4 * len;
@@ -231,7 +251,21 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
             red_u32(col + hi4 * LS, 0xffffffffu);
         } else if (start == 0) {
 #pragma unroll 1
-            for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) pre_out[(j4 >> 2) * LW] = (uint16_t)len;
+            for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) {
+                const uint32_t c = carry[(j4 >> 2) * LW];
+                const uint32_t tot = (c & ~CARRY_SEG) + len;
+                if (c & CARRY_SEG) {
+                    pre_out[(j4 >> 2) * LW] = tot;
+                } else if (tot >= (uint32_t)LMIN_EXPLICIT) {
+                    if (tot < (uint32_t)LS) {
+                        const uint32_t col = sh + 4 * tot + j4 * LS;
+                        red_u32(col, 1u);
+                        red_u32(col + 4 * LS, 0xffffffffu);
+                    } else {
+                        atomicAdd(&grow[(int64_t)rep[j4 >> 2] * n + tot], 1ull);
+                    }
+                }
+            }
         } else {
 #pragma unroll 1
             for (uint32_t j4 = lo4; j4 < hi4; j4 += 4) atomicAdd(&grow[(int64_t)rep[j4 >> 2] * n + len], 1ull);
@@ -340,13 +374,14 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
         if (PHASE == 1) trel8 += (uint32_t)sizeof...(R) << 8;
     }
 
-    // End of the chunk (cnt > 0 cells): the prefix runs that never ended, and the run alive at the end for every
-    // threshold (from the stack for j >= A/4, else 0..3 cells from the last levels).
-    __device__ __forceinline__ void finish(uint32_t cnt, uint16_t* suf_out) {
+    // End of the chunk (cnt > 0 cells): the run alive at the end for every threshold becomes the carry of the next
+    // chunk (from the stack for j >= A/4, else 0..3 cells from the last levels); a run that spans the whole chunk
+    // extends the carry it started from (and keeps its segment flag).
+    __device__ __forceinline__ void finish(uint32_t cnt) {
         const uint32_t w3 = max(w2a, w2b);
 #pragma unroll 1
         for (uint32_t j4 = 0; j4 < min(A, J4); j4 += 4)
-            suf_out[(j4 >> 2) * LW] = (uint16_t)((v1 <= j4) + (w2a <= j4) + (w3 <= j4));
+            carry[(j4 >> 2) * LW] = (v1 <= j4) + (w2a <= j4) + (w3 <= j4);
         uint32_t lo = A, st = ts;
 #pragma unroll 1
         while (lo < J4) {
@@ -354,8 +389,8 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
             const uint32_t nlo = (e << 2) & 0xfcu;
 #pragma unroll 1
             for (uint32_t j4 = lo; j4 < nlo; j4 += 4) {
-                suf_out[(j4 >> 2) * LW] = (uint16_t)(cnt - st);
-                if (st == 0) pre_out[(j4 >> 2) * LW] = (uint16_t)cnt;
+                if (st == 0) carry[(j4 >> 2) * LW] += cnt;
+                else carry[(j4 >> 2) * LW] = cnt - st;
             }
             lo = nlo; st = e >> 6;
             if (top != stk) top -= SM::stk_row;
@@ -367,7 +402,7 @@ struct Scanner : CellDist<NORM, M, TAU, 2> {
 // level table holding at most one threshold, carries no refinement loop; a block executes only one of them.
 template <int NORM, int M, int TAU, int NP, bool MULTI>
 __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc, int cnt, int cnt_lo, int cnt_hi, int ds,
-                                           uint32_t yb_org, uint16_t* suf_out) {
+                                           uint32_t yb_org) {
     using SC = Scanner<NORM, M, TAU, NP, MULTI>;
     constexpr int S = SC::S;
     constexpr int U = S == 3 ? 12 : (S > 3 ? S : 4);          // cells per super-step, a multiple of S
@@ -388,157 +423,249 @@ __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc,
         sc.drain((uint32_t)t0w);
     }
     for (; t < cnt_hi; t += U) sc.template superstep<2>(t, cnt, ds, Seq{});
-    if (cnt > 0) sc.finish((uint32_t)cnt, suf_out);
+    if (cnt > 0) sc.finish((uint32_t)cnt);
 }
 
 template <int NORM, int M, int TAU, int NP>
 __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanArgs a) {
     using SM = ScanSmem<NP>;
     extern __shared__ __align__(16) char smem[];
-    __shared__ int s_ob;
+    __shared__ int s_q;
+    __shared__ unsigned int s_item;
     __shared__ int s_rep[GK];
+    __shared__ __align__(8) unsigned long long s_bar[2];
 
-    const int tid = threadIdx.x;
-    const int b = blockIdx.y;
-    const uint32_t tile = blockIdx.x;
-    const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
-    // which diagonal block / chunk is this tile
-    find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
-    // stage the group's table and thresholds, clear the histograms
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     uint8_t* lut_s = (uint8_t*)(smem + SM::off_lut);
     float* eps_s = (float*)(smem + SM::off_eps);
-    const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
-    const int ps = M > 0 ? 1 : (int)a.v.ps;
-    const int LA = window_la(a.L, span, 2, ps), LB = window_lb(a.L, span, 2, ps);
-    float* ya_s = (float*)(smem + SM::off_ya);
-    float* yb_s = ya_s + LA;
+    uint32_t* tot_s = (uint32_t*)(smem + SM::off_tot);
     uint32_t* agg_s = (uint32_t*)(smem + SM::off_agg);
     int32_t* sh_s = (int32_t*)(smem + SM::off_sh);
     uint16_t* stk_s = (uint16_t*)(smem + SM::off_stk);
-    const int J = G.J;
-    for (int q = tid; q < NB / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)G.lut)[q];
-    if (tid <= GK) eps_s[tid] = G.epsd[tid];
-    if (tid < GK) s_rep[tid] = G.rep_k[tid];
+    const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
+    const int ps = M > 0 ? 1 : (int)a.v.ps;
+    const int L = a.L;
+    // one window set: i-side window, j-side window, each with 4 floats of slack for the 16-byte alignment of bulk copies
+    const int LA = window_la(L, span, 2, ps) + 4, LB = window_lb(L, span, 2, ps) + 4;
+    float* win_s = (float*)(smem + SM::off_ya);
+    const int64_t n = a.v.n;
+    const int64_t T = (int64_t)a.S * L;                         // cells per segment along the diagonals
+    const int64_t ny = (n - 1) * ps + span + 1;                 // floats of one series
+    const int64_t extent = (int64_t)(a.v.batch - 1) * a.v.bs + ny;   // floats of the whole batch: what bulk copies may touch
+    const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(&s_bar[0]);
+    uint32_t* carry_col = a.carry + ((size_t)blockIdx.x * (2 * NP)) * LW + tid;
+    const unsigned int n_items = a.segs * (unsigned)a.v.batch;
+
+    if (tid == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    stk_s[tid] = 0;                                            // (the sentinel is set per series)
+    // the aggregate columns, the difference array and the totals are cleared here once; every flush clears what it read
     for (int q = tid; q < SM::NLEV * LW; q += LW) agg_s[q] = 0;
     for (int q = tid; q < SM::NLEV * LS; q += LW) sh_s[q] = 0;
-    stk_s[tid] = (uint16_t)J;                                  // the sentinel below every stack
-    __syncthreads();
-    const int ob = s_ob;
-    const int c = (int)(tile - a.tile_start[ob]);
-    const int L = a.L;
-    const int64_t n = a.v.n;
-    const int64_t o0 = a.v.w + (int64_t)LW * ob;            // w = 1, or the Theiler window
-    const int64_t s = (int64_t)c * L;                       // chunk start along the diagonals
-    // the two windows: the floats of the points s-2.. and s-2+o0..; the n points span (n-1)*ps + span + 1 floats
-    const float* y = a.v.data + (int64_t)b * a.v.bs;
-    const int64_t ny = (n - 1) * ps + span + 1;
-    stage_windows(y, ny, (s - 2) * ps, (s - 2 + o0) * ps, ya_s, LA, yb_s, LB);
+    if (tid < 3 * (GK + 1)) tot_s[tid] = 0;
+    uint32_t parity = 0;                                       // bit u: phase of mbarrier u
+    int cur_b = -1, J = 0;
     __syncthreads();
 
-    const int64_t o = o0 + tid;
-    const int64_t len = n - o;                              // cells on this thread's diagonal (may be <= 0)
-    int cnt = (int)max((int64_t)0, min((int64_t)L, len - s));
-    const int cnt_hi = __shfl_sync(FULL, cnt, 0);           // the warp's longest lane (smallest o)
-    const int cnt_lo = __shfl_sync(FULL, cnt, 31);
-    unsigned long long* grow = a.hist + (int64_t)b * a.K * n;
+    // Bulk copy of chunk c's two windows into window set `u` (thread 0).  Returns false when the copy would touch
+    // memory outside the batch's floats (the ends of the first and last series): the caller stages with plain loads.
+    auto bulk_ok = [&](const float* y, int64_t sa, int64_t sb, int& sha, int& shb) -> bool {
+        const int64_t ga = (y - a.v.data) + sa, gb = (y - a.v.data) + sb;      // float offsets from the batch base
+        sha = (int)(((uintptr_t)(a.v.data + ga) >> 2) & 3);
+        shb = (int)(((uintptr_t)(a.v.data + gb) >> 2) & 3);
+        return a.nbuf == 2 && ga - sha >= 0 && gb - shb >= 0 && ga - sha + LA <= extent && gb - shb + LB <= extent &&
+               (((uintptr_t)a.v.data) & 3) == 0;
+    };
 
-    if (cnt_hi > 0) {
-        const int64_t out_row = (((int64_t)b * a.tiles + tile) * (2 * NP)) * LW + tid;
-        const uint32_t yb_org = pin(smem_addr(yb_s) + 4 * tid * ps);
-        auto setup = [&](auto& sc) {
-            sc.ya_org = smem_addr(ya_s);
-            sc.lut = pin(smem_addr(lut_s) - BUCKET_MAGIC_BITS);   // indexed with bucket_bits()
-            sc.eps = smem_addr(eps_s);
-            sc.agg = pin(smem_addr(agg_s) + 4 * tid);
-            sc.sh = smem_addr(sh_s);
-            sc.stk = pin(smem_addr(stk_s) + 2 * tid);
-            sc.q0 = pin(smem_addr(smem + SM::off_q) + 2 * tid);
-            sc.grow = (unsigned long long*)pin64((unsigned long long)grow);   // kept in registers, not re-read per cell
-            sc.rep = G.rep_k;                               // global copy: only read for lines of length >= LS
-            sc.pre_out = a.pre + out_row;
-            sc.scale = G.scale;
-            sc.dcap = G.dcap;
-            sc.J4 = 4u * (uint32_t)J;
-            sc.m = a.m;
-            sc.tau = a.tau;
-            sc.ps = ps;
-            sc.n = (int64_t)pin64((unsigned long long)n);
-            sc.v1 = sc.v2 = sc.J4;
-            sc.w2a = sc.w2b = sc.J4;
-            sc.xa = sc.xb = 0;
-            sc.A = 0; sc.ts = 0; sc.top = sc.stk;           // every threshold: recurrent since the chunk start
-        };
-        const int first_real = -(int)min((int64_t)2, s);     // warm-up cells before it lie outside the plot
-        if (G.multi) {
-            Scanner<NORM, M, TAU, NP, true> sc;
-            setup(sc);
-            scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org, a.suf + out_row);
-        } else {
-            Scanner<NORM, M, TAU, NP, false> sc;
-            setup(sc);
-            scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org, a.suf + out_row);
+    while (true) {
+        if (tid == 0) s_item = atomicAdd(a.counter, 1u);
+        __syncthreads();
+        const unsigned int item = s_item;
+        if (item >= n_items) break;
+        const int b = (int)(item / a.segs);
+        const uint32_t t_seg = item - (uint32_t)b * a.segs;
+        find_diagonal_block(a.seg_start, a.n_obl, t_seg, &s_q);
+        const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
+        if (b != cur_b) {                                     // another series: its table and thresholds
+            J = G.J;
+            for (int q = tid; q < NB / 4; q += LW) ((uint32_t*)lut_s)[q] = ((const uint32_t*)G.lut)[q];
+            if (tid <= GK) eps_s[tid] = G.epsd[tid];
+            if (tid < GK) s_rep[tid] = G.rep_k[tid];
+            stk_s[tid] = (uint16_t)J;                          // the sentinel below every stack
+            cur_b = b;
         }
-    }
-    __syncthreads();
-    // flush: aggregates (sum the 256 private columns of every level) and the short lines (prefix sums of D over j)
-    {
-        const int warp = tid >> 5, lane = tid & 31;
-        unsigned long long* ag = a.agg + ((int64_t)b * a.NG + a.g) * 3 * (GK + 1);
-        for (int lev = warp; lev <= J; lev += LW / 32) {
-            const uint32_t* r = agg_s + lev * LW;
-            uint32_t s1 = 0, s2 = 0, s3 = 0;
-            for (int q = lane; q < LW; q += 32) { uint32_t w = r[q]; s1 += w & 0x3ffu; s2 += (w >> 10) & 0x3ffu; s3 += w >> 20; }
-            for (int off = 16; off; off >>= 1) {
-                s1 += __shfl_down_sync(FULL, s1, off);
-                s2 += __shfl_down_sync(FULL, s2, off);
-                s3 += __shfl_down_sync(FULL, s3, off);
-            }
-            if (lane == 0) {
-                if (s1) atomicAdd(&ag[lev], (unsigned long long)s1);
-                if (s2) atomicAdd(&ag[(GK + 1) + lev], (unsigned long long)s2);
-                if (s3) atomicAdd(&ag[2 * (GK + 1) + lev], (unsigned long long)s3);
-            }
+        __syncthreads();
+        const int q_ob = s_q;
+        const int ob = a.part + q_ob * a.parts;
+        const int seg = (int)(t_seg - a.seg_start[q_ob]);
+        const int64_t o0 = a.v.w + (int64_t)LW * ob;          // w = 1, or the Theiler window
+        const int64_t o = o0 + tid;
+        const int64_t len = n - o;                            // cells on this thread's diagonal (may be <= 0)
+        const int64_t seg_s = (int64_t)seg * T;               // segment start along the diagonals
+        const int64_t len0 = n - o0;                          // the block's longest diagonal
+        const int c_end = (int)min((int64_t)a.S, (len0 - seg_s + L - 1) / L);   // chunks of this segment
+        const float* y = a.v.data + (int64_t)b * a.v.bs;
+        unsigned long long* grow = a.hist + (int64_t)b * a.K * n;
+        const size_t out_row = (((size_t)b * a.segs + t_seg) * (2 * NP)) * LW + tid;
+        // every run is alive "since the segment start" until it ends: the segment's prefix runs go to the stitch kernel
+        for (int j = 0; j < J; ++j) carry_col[j * LW] = CARRY_SEG;
+
+        // windows of the first chunk
+        int sha = 0, shb = 0;
+        bool bulk = bulk_ok(y, (seg_s - 2) * ps, (seg_s - 2 + o0) * ps, sha, shb);
+        if (bulk && tid == 0) {
+            fence_proxy_async();
+            mbar_expect_tx(bar0, 4u * (uint32_t)(LA + LB));
+            bulk_g2s((uint32_t)__cvta_generic_to_shared(win_s), y + (seg_s - 2) * ps - sha, 4u * LA, bar0);
+            bulk_g2s((uint32_t)__cvta_generic_to_shared(win_s + LA), y + (seg_s - 2 + o0) * ps - shb, 4u * LB, bar0);
         }
-        for (int l = tid; l < LS; l += LW) {
-            int32_t acc = 0;
+        for (int c = 0; c < c_end; ++c) {
+            const int u = a.nbuf == 2 ? (c & 1) : 0;
+            float* ya_s = win_s + (size_t)u * (LA + LB);
+            float* yb_s = ya_s + LA;
+            const int64_t s = seg_s + (int64_t)c * L;          // chunk start along the diagonals
+            if (bulk) {
+                mbar_wait(bar0 + 8 * u, (parity >> u) & 1u);
+                parity ^= 1u << u;
+            } else {
+                sha = shb = 0;
+                stage_windows(y, ny, (s - 2) * ps, (s - 2 + o0) * ps, ya_s, LA, yb_s, LB);
+                __syncthreads();
+            }
+            const int sha_c = sha, shb_c = shb;
+            // the next chunk's windows, into the other set, while this chunk is scanned
+            bool bulk_next = false;
+            if (c + 1 < c_end) {
+                bulk_next = bulk_ok(y, (s + L - 2) * ps, (s + L - 2 + o0) * ps, sha, shb);
+                if (bulk_next && tid == 0) {
+                    float* na = win_s + (size_t)(u ^ 1) * (LA + LB);
+                    fence_proxy_async();
+                    mbar_expect_tx(bar0 + 8 * (u ^ 1), 4u * (uint32_t)(LA + LB));
+                    bulk_g2s((uint32_t)__cvta_generic_to_shared(na), y + (s + L - 2) * ps - sha, 4u * LA, bar0 + 8 * (u ^ 1));
+                    bulk_g2s((uint32_t)__cvta_generic_to_shared(na + LA), y + (s + L - 2 + o0) * ps - shb, 4u * LB, bar0 + 8 * (u ^ 1));
+                }
+            }
+            int cnt = (int)max((int64_t)0, min((int64_t)L, len - s));
+            const int cnt_hi = __shfl_sync(FULL, cnt, 0);       // the warp's longest lane (smallest o)
+            const int cnt_lo = __shfl_sync(FULL, cnt, 31);
+            if (cnt_hi > 0) {
+                const uint32_t yb_org = pin(smem_addr(yb_s) + 4 * (shb_c + tid * ps));
+                auto setup = [&](auto& sc) {
+                    sc.ya_org = smem_addr(ya_s) + 4 * sha_c;
+                    sc.lut = pin(smem_addr(lut_s) - BUCKET_MAGIC_BITS);   // indexed with bucket_bits()
+                    sc.eps = smem_addr(eps_s);
+                    sc.agg = pin(smem_addr(agg_s) + 4 * tid);
+                    sc.sh = smem_addr(sh_s);
+                    sc.stk = pin(smem_addr(stk_s) + 2 * tid);
+                    sc.q0 = pin(smem_addr(smem + SM::off_q) + 2 * tid);
+                    sc.grow = (unsigned long long*)pin64((unsigned long long)grow);   // kept in registers, not re-read per cell
+                    sc.rep = G.rep_k;                           // global copy: only read for lines of length >= LS
+                    sc.carry = carry_col;
+                    sc.pre_out = a.pre + out_row;
+                    sc.scale = G.scale;
+                    sc.dcap = G.dcap;
+                    sc.J4 = 4u * (uint32_t)J;
+                    sc.m = a.m;
+                    sc.tau = a.tau;
+                    sc.ps = ps;
+                    sc.n = (int64_t)pin64((unsigned long long)n);
+                    sc.v1 = sc.v2 = sc.J4;
+                    sc.w2a = sc.w2b = sc.J4;
+                    sc.xa = sc.xb = 0;
+                    sc.A = 0; sc.ts = 0; sc.top = sc.stk;       // every threshold: recurrent since the chunk start
+                };
+                const int first_real = -(int)min((int64_t)2, s);   // warm-up cells before it lie outside the plot
+                if (G.multi) {
+                    Scanner<NORM, M, TAU, NP, true> sc;
+                    setup(sc);
+                    scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org);
+                } else {
+                    Scanner<NORM, M, TAU, NP, false> sc;
+                    setup(sc);
+                    scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org);
+                }
+            }
+            bulk = bulk_next;
+            __syncthreads();
+            // the chunk's aggregates: sum the LW private columns of every level into the block's totals, clear them
+            // (the counters are 10 bits wide: a chunk has at most 1023 cells)
+            for (int lev = warp; lev <= J; lev += LW / 32) {
+                uint32_t* r = agg_s + lev * LW;
+                uint32_t s1 = 0, s2 = 0, s3 = 0;
+                for (int q = lane; q < LW; q += 32) {
+                    const uint32_t w = r[q];
+                    r[q] = 0;
+                    s1 += w & 0x3ffu; s2 += (w >> 10) & 0x3ffu; s3 += w >> 20;
+                }
+                for (int off = 16; off; off >>= 1) {
+                    s1 += __shfl_down_sync(FULL, s1, off);
+                    s2 += __shfl_down_sync(FULL, s2, off);
+                    s3 += __shfl_down_sync(FULL, s3, off);
+                }
+                if (lane == 0) { tot_s[lev] += s1; tot_s[(GK + 1) + lev] += s2; tot_s[2 * (GK + 1) + lev] += s3; }
+            }
+            __syncthreads();
+        }
+        // end of the segment: the runs still alive (and the prefix runs that never ended) for the stitch kernel
+        if (len > seg_s) {
             for (int j = 0; j < J; ++j) {
-                acc += sh_s[j * LS + l];
-                if (acc) atomicAdd(&grow[(int64_t)s_rep[j] * n + l], (unsigned long long)acc);
+                const uint32_t cj = carry_col[j * LW];
+                if (cj & CARRY_SEG) a.pre[out_row + (size_t)j * LW] = cj & ~CARRY_SEG;
+                a.suf[out_row + (size_t)j * LW] = cj & ~CARRY_SEG;
             }
         }
+        // flush: the item's aggregates and its short lines (prefix sums of D over j)
+        {
+            unsigned long long* ag = a.agg + ((int64_t)b * a.NG + a.g) * 3 * (GK + 1);
+            if (tid < 3 * (GK + 1) && tot_s[tid]) { atomicAdd(&ag[tid], (unsigned long long)tot_s[tid]); tot_s[tid] = 0; }
+            for (int l = tid; l < LS; l += LW) {
+                int32_t acc = 0;
+                for (int j = 0; j <= J; ++j) {
+                    const int32_t dj = sh_s[j * LS + l];
+                    if (dj) sh_s[j * LS + l] = 0;
+                    acc += dj;
+                    if (acc && j < J) atomicAdd(&grow[(int64_t)s_rep[j] * n + l], (unsigned long long)acc);
+                }
+            }
+        }
+        __syncthreads();                                       // before s_item / the tables are overwritten
     }
 }
 
 // ---------------------------------------------------------------------------------------- stitching
-// One thread per (diagonal, distinct threshold): join the (prefix, suffix) summaries of consecutive chunks and
-// emit the lines of length >= 4 that touch a chunk border (including the two ends of the diagonal).
+// One thread per (diagonal, distinct threshold): join the (prefix, suffix) summaries of consecutive segments and
+// emit the lines of length >= 4 that touch a segment border (including the two ends of the diagonal).
 struct StitchArgs {
-    int64_t n, w;
-    int g, NG, K, L, n_ob, NP;
+    int64_t n, w, T;            // T = cells per segment along the diagonals
+    int g, NG, K, NP;
+    int part, parts, n_obl;
     const LineGroup* groups;
-    const uint32_t* tile_start;
+    const uint32_t* seg_start;
     unsigned long long* hist;
-    const uint16_t* pre;
-    const uint16_t* suf;
-    uint32_t tiles;
+    const uint32_t* pre;
+    const uint32_t* suf;
+    uint32_t segs;
 };
 
 __global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
-    const int ob = blockIdx.x, j = blockIdx.y, b = blockIdx.z;
+    const int q_ob = blockIdx.x, j = blockIdx.y, b = blockIdx.z;
     const LineGroup& G = a.groups[(int64_t)b * a.NG + a.g];
     if (j >= G.J) return;
     const int tid = threadIdx.x;
-    const int64_t o = a.w + (int64_t)LW * ob + tid;
+    const int64_t o = a.w + (int64_t)LW * (a.part + (int64_t)q_ob * a.parts) + tid;
     const int64_t len = a.n - o;
     if (len <= 0) return;
     unsigned long long* row = a.hist + ((int64_t)b * a.K + G.rep_k[j]) * a.n;
-    const uint32_t t0 = a.tile_start[ob];
-    const int nc = (int)((len + a.L - 1) / a.L);
+    const uint32_t t0 = a.seg_start[q_ob];
+    const int nc = (int)((len + a.T - 1) / a.T);
     uint32_t carry = 0;
-    // the summaries of SB chunks are loaded together (independent loads), then joined in order
+    // the summaries of SB segments are loaded together (independent loads), then joined in order
     constexpr int SB = 8;
     const int64_t stride = (int64_t)(2 * a.NP) * LW;
-    const int64_t base = (((int64_t)b * a.tiles + t0) * (2 * a.NP) + j) * LW + tid;
+    const int64_t base = (((int64_t)b * a.segs + t0) * (2 * a.NP) + j) * LW + tid;
     for (int c0 = 0; c0 < nc; c0 += SB) {
         uint32_t p[SB], sf[SB];
 #pragma unroll
@@ -550,7 +677,7 @@ __global__ void __launch_bounds__(LW) line_stitch_kernel(StitchArgs a) {
 #pragma unroll
         for (int u = 0; u < SB; ++u) {
             if (c0 + u < nc) {
-                const uint32_t cntc = (uint32_t)min((int64_t)a.L, len - (int64_t)(c0 + u) * a.L);
+                const uint32_t cntc = (uint32_t)min(a.T, len - (int64_t)(c0 + u) * a.T);
                 if (p[u] == cntc) {
                     carry += cntc;
                 } else {
@@ -624,8 +751,9 @@ __global__ void __launch_bounds__(256) line_copy_rows_kernel(int64_t n, int g, i
 // series (point_stride != 1) or the embedding window does not fit the scan kernel's shared-memory windows.
 template <int NORM>
 __global__ void __launch_bounds__(128) line_strided_kernel(View v, const float* __restrict__ eps, int K,
-                                                           unsigned long long* __restrict__ hist) {
+                                                           unsigned long long* __restrict__ hist, int part, int parts) {
     const int b = blockIdx.y;
+    if ((int)(blockIdx.x % (unsigned)parts) != part) return;   // a split call: blocks of diagonals are dealt round robin
     const int64_t o = v.w + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= v.n) return;
     const float* yb = v.data + (int64_t)b * v.bs;
@@ -651,137 +779,213 @@ __global__ void __launch_bounds__(128) line_strided_kernel(View v, const float* 
 // ------------------------------------------------------------------------------------------ host side
 struct LinePlan {
     bool scan;          // false: strided fallback
-    int L, n_ob, NG, NP, span;
-    uint32_t tiles;
+    int L, S, NG, NP, span, nbuf, blocks_per_sm;
+    Tiling tl;          // segments (T = S*L cells) of this part's diagonal blocks
+    unsigned grid;      // persistent blocks
     size_t smem;
 };
 
 int pairs_for(int kg) { return kg <= 10 ? 5 : (kg <= 20 ? 10 : 16); }
 
 template <int NP>
-size_t scan_smem_bytes(int L, int span, int ps) {
-    return (size_t)ScanSmem<NP>::off_ya + 4 * ((size_t)window_la(L, span, 2, ps) + window_lb(L, span, 2, ps));
+size_t scan_smem_bytes(int L, int span, int ps, int nbuf) {
+    return (size_t)ScanSmem<NP>::off_ya + 4 * (size_t)nbuf * ((size_t)window_la(L, span, 2, ps) + window_lb(L, span, 2, ps) + 8);
 }
-size_t scan_smem_bytes(int NP, int L, int span, int ps) {
-    return NP == 5 ? scan_smem_bytes<5>(L, span, ps) : (NP == 10 ? scan_smem_bytes<10>(L, span, ps) : scan_smem_bytes<16>(L, span, ps));
+size_t scan_smem_bytes(int NP, int L, int span, int ps, int nbuf) {
+    return NP == 5 ? scan_smem_bytes<5>(L, span, ps, nbuf)
+                   : (NP == 10 ? scan_smem_bytes<10>(L, span, ps, nbuf) : scan_smem_bytes<16>(L, span, ps, nbuf));
 }
 constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of sm_100a, minus the static part
+constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_BLOCK_RESERVED = 1024;
 
-LinePlan make_plan(const View& v, int K) {
+LinePlan make_plan(const View& v, int K, const Options& opt) {
     LinePlan p{};
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
     p.NG = (K + GK - 1) / GK;
     p.NP = pairs_for(std::min(K, GK));
+    p.blocks_per_sm = p.NP <= 10 ? 2 : 1;                      // the kernel's __launch_bounds__
     const int ps = (int)std::min<int64_t>(v.ps, 1 << 20);
     // tiled scan: delay views, and materialised points (point stride > 1) whose windows fit the shared memory
-    p.scan = p.span <= MAX_SPAN && scan_smem_bytes(p.NP, 32, p.span, ps) <= SMEM_PER_BLOCK_MAX;
-    // chunk length: aim at >= 8 waves of 3 blocks per SM over the whole batch, at most 1023 positions
-    const double cells = (double)n_pairs(v) * (double)v.batch;
-    int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
-    p.L = (int)std::max<int64_t>(32, std::min<int64_t>(LMAX, L));
-    if (options().line_chunk > 0) p.L = (int)std::min<int64_t>(LMAX, options().line_chunk);
-    // wide points: the two windows hold (2L + 512) points, so the chunk shrinks until they fit (one block per SM then)
-    while (p.scan && p.L > 32 && scan_smem_bytes(p.NP, p.L, p.span, ps) > SMEM_PER_BLOCK_MAX) p.L = std::max(32, p.L / 2);
+    p.scan = p.span <= MAX_SPAN && scan_smem_bytes(p.NP, 32, p.span, ps, 1) <= SMEM_PER_BLOCK_MAX;
     const int64_t nd = n_diag(v);                              // the triangle of the counted diagonals w..n-1
-    p.n_ob = (int)((nd - 1 + LW - 1) / LW);
-    uint64_t tiles = 0;
-    for (int ob = 0; ob < p.n_ob; ++ob) tiles += (uint64_t)((nd - 1 - (int64_t)LW * ob + p.L - 1) / p.L);
-    p.tiles = (uint32_t)tiles;
-    p.smem = scan_smem_bytes(p.NP, p.L, p.span, ps);
+    const int sms = sm_count();
+    const unsigned slots = (unsigned)(sms * p.blocks_per_sm);
+    // chunk length: at most 1023 positions (10-bit counters and stack positions); short enough that every block
+    // slot gets several chunks of a small problem
+    const double cells = (double)n_pairs(v) * (double)v.batch / (double)opt.parts;
+    int64_t L = (int64_t)std::ceil(cells / ((double)LW * slots * 4.0));
+    p.L = (int)std::max<int64_t>(32, std::min<int64_t>(LMAX, L));
+    if (opt.line_chunk > 0) p.L = (int)std::min<int64_t>(LMAX, opt.line_chunk);
+    // window sets: two (bulk-copy double buffer) when they fit beside the per-thread state at this occupancy
+    const size_t per_block = SMEM_PER_SM / p.blocks_per_sm - SMEM_BLOCK_RESERVED;
+    const size_t budget = std::min(per_block, SMEM_PER_BLOCK_MAX);
+    p.nbuf = 2;
+    if (p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, 2) > budget) {
+        // shorter chunks cost little in a persistent block (a chunk border is one aggregate flush); keep two sets
+        // down to 256 positions, then give up the double buffer
+        int Ld = p.L;
+        while (Ld > 256 && scan_smem_bytes(p.NP, Ld, p.span, ps, 2) > budget) Ld -= 16;
+        if (opt.line_chunk == 0 && scan_smem_bytes(p.NP, Ld, p.span, ps, 2) <= budget) p.L = Ld;
+        else p.nbuf = 1;
+    }
+    if (opt.line_buffers > 0) p.nbuf = opt.line_buffers;
+    // wide points: the two windows hold (2L + 512) points, so the chunk shrinks until they fit (one block per SM then)
+    while (p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, p.nbuf) > SMEM_PER_BLOCK_MAX) {
+        if (p.nbuf == 2) p.nbuf = 1;
+        else if (p.L > 32) p.L = std::max(32, p.L / 2);
+        else break;
+    }
+    // segment = S consecutive chunks walked by one block with the run state carried in place: long enough that the
+    // summaries at segment borders are rare, short enough that the slowest block's last item is a small share of its
+    // work (about 1/8)
+    const Tiling chunks = make_tiling(nd, p.L, opt.part, opt.parts);
+    const uint64_t all = chunks.tiles * (uint64_t)v.batch;
+    int64_t S = (int64_t)(all / ((uint64_t)slots * 8));
+    p.S = (int)std::max<int64_t>(1, std::min<int64_t>(64, S));
+    if (opt.line_segment > 0) p.S = opt.line_segment;
+    p.tl = make_tiling(nd, (int64_t)p.S * p.L, opt.part, opt.parts);
+    p.grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(p.tl.tiles * (uint64_t)v.batch, slots));
+    p.smem = scan_smem_bytes(p.NP, p.L, p.span, ps, p.nbuf);
     return p;
 }
 
 template <int NORM, int M, int TAU, int NP>
-rqa_status launch_scan(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
+rqa_status launch_scan(const ScanArgs& a, const LinePlan& p, cudaStream_t s) {
     auto kern = line_scan_kernel<NORM, M, TAU, NP>;
-    RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
-    kern<<<dim3(p.tiles, (unsigned)batch), LW, p.smem, s>>>(a);
+    static thread_local size_t attr_set[8] = {0};             // per device: the largest size this thread has opted in to
+    int dev = 0;
+    RQA_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev >= 8 || attr_set[dev] < p.smem) {
+        RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_PER_BLOCK_MAX));
+        if (dev < 8) attr_set[dev] = SMEM_PER_BLOCK_MAX;
+    }
+    kern<<<p.grid, LW, p.smem, s>>>(a);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }
 
 template <int NORM, int NP>
-rqa_status dispatch_embedding(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
+rqa_status dispatch_embedding(const ScanArgs& a, const LinePlan& p, cudaStream_t s) {
     // the embeddings of BASELINE.json's large configs get a register ring; any other (m, tau) recomputes per cell
     const bool delay = a.v.ps == 1;
-    if (delay && a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, batch, s);
-    if (delay && a.m == 3 && a.tau == 3) return launch_scan<NORM, 3, 3, NP>(a, p, batch, s);
-    if (delay && a.m == 5 && a.tau == 2) return launch_scan<NORM, 5, 2, NP>(a, p, batch, s);
-    return launch_scan<NORM, 0, 0, NP>(a, p, batch, s);
+    if (delay && a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, s);
+    if (delay && a.m == 3 && a.tau == 3) return launch_scan<NORM, 3, 3, NP>(a, p, s);
+    if (delay && a.m == 5 && a.tau == 2) return launch_scan<NORM, 5, 2, NP>(a, p, s);
+    return launch_scan<NORM, 0, 0, NP>(a, p, s);
 }
 
 template <int NORM>
-rqa_status dispatch_pairs(const ScanArgs& a, const LinePlan& p, int batch, cudaStream_t s) {
-    if (p.NP == 5) return dispatch_embedding<NORM, 5>(a, p, batch, s);
-    if (p.NP == 10) return dispatch_embedding<NORM, 10>(a, p, batch, s);
-    return dispatch_embedding<NORM, 16>(a, p, batch, s);
+rqa_status dispatch_pairs(const ScanArgs& a, const LinePlan& p, cudaStream_t s) {
+    if (p.NP == 5) return dispatch_embedding<NORM, 5>(a, p, s);
+    if (p.NP == 10) return dispatch_embedding<NORM, 10>(a, p, s);
+    return dispatch_embedding<NORM, 16>(a, p, s);
+}
+
+struct LineWs {
+    LineGroup* groups;
+    uint32_t* seg_start;
+    unsigned long long* agg;
+    unsigned int* counters;
+    uint32_t *pre, *suf, *carry;
+};
+LineWs carve_line(Arena& ws, const View& v, const LinePlan& p) {
+    LineWs w{};
+    w.groups = ws.take<LineGroup>((size_t)v.batch * p.NG);
+    w.seg_start = ws.take<uint32_t>((size_t)p.tl.n_obl + 1);
+    w.agg = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * p.NG * 3 * (GK + 1));
+    w.counters = ws.take<unsigned int>((size_t)p.NG);
+    w.pre = ws.take<uint32_t>((size_t)v.batch * p.tl.tiles * 2 * p.NP * LW);
+    w.suf = ws.take<uint32_t>((size_t)v.batch * p.tl.tiles * 2 * p.NP * LW);
+    w.carry = ws.take<uint32_t>((size_t)p.grid * 2 * p.NP * LW);
+    return w;
+}
+
+// a NaN, infinite or negative threshold is reported through the workspace status (the strided fallback's check; the
+// tiled scan does it in line_groups_kernel)
+__global__ void line_eps_check_kernel(const float* __restrict__ eps, int64_t count, WsStatus* status) {
+    bool bad = false;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (int64_t)gridDim.x * blockDim.x) {
+        const float x = eps[q];
+        bad |= !(x >= 0.0f) || isinf(x);
+    }
+    if (bad) atomicExch(&status->bad_eps, 1);
 }
 
 }  // namespace
 
-rqa_status launch_tile_table(int64_t n, int L, int n_ob, uint32_t* tile_start, cudaStream_t s) {
-    tile_table_kernel<<<1, 1024, 0, s>>>(n, L, n_ob, tile_start);
+rqa_status launch_tile_table(const Tiling& t, uint32_t* tile_start, cudaStream_t s) {
+    tile_table_kernel<<<1, 1024, 0, s>>>(t.nd, t.T, t.n_obl, t.part, t.parts, tile_start);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }
 
-size_t line_workspace_bytes(const View& v, int K) {
-    LinePlan p = make_plan(v, K);
+size_t line_workspace_bytes(const View& v, int K, const Options& opt) {
+    LinePlan p = make_plan(v, K, opt);
     if (!p.scan) return 256;
-    size_t bytes = 0;
-    bytes += align_up(sizeof(LineGroup) * (size_t)v.batch * p.NG);
-    bytes += align_up(sizeof(uint32_t) * ((size_t)p.n_ob + 1));
-    bytes += align_up(sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1));
-    bytes += align_up(sizeof(uint16_t) * (size_t)v.batch * p.tiles * 2 * p.NP * LW);
-    bytes += align_up(sizeof(uint16_t) * (size_t)v.batch * p.tiles * 2 * p.NP * LW);
-    return bytes;
+    Arena a(nullptr, ~(size_t)0);
+    carve_line(a, v, p);
+    return a.off;
 }
 
-rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s) {
+rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s,
+                         const Options& opt) {
     WsStatus* status = (WsStatus*)ws.base;
-    RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * (size_t)v.batch * K * v.n, s));
-    LinePlan p = make_plan(v, K);
+    const size_t hist_words = (size_t)v.batch * K * v.n;
+    RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * hist_words, s));
+    LinePlan p = make_plan(v, K, opt);
     if (!p.scan) {
+        // thread-per-diagonal fallback: the diagonals are dealt to the parts block by block
+        line_eps_check_kernel<<<1, 256, 0, s>>>(d_eps, (int64_t)v.batch * K, status);
+        RQA_LAUNCH_CHECK();
         dim3 grid((unsigned)((v.n - v.w + 127) / 128), (unsigned)v.batch);
         if (norm == RQA_NORM_MAX)
-            line_strided_kernel<RQA_NORM_MAX><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
+            line_strided_kernel<RQA_NORM_MAX><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist, opt.part, opt.parts);
         else
-            line_strided_kernel<RQA_NORM_EUCLID><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist);
+            line_strided_kernel<RQA_NORM_EUCLID><<<grid, 128, 0, s>>>(v, d_eps, K, (unsigned long long*)d_hist, opt.part, opt.parts);
         RQA_LAUNCH_CHECK();
-        return RQA_OK;
+        return reduce_parts(opt, d_hist, hist_words, s);
     }
-    LineGroup* groups = ws.take<LineGroup>((size_t)v.batch * p.NG);
-    uint32_t* tile_start = ws.take<uint32_t>((size_t)p.n_ob + 1);
-    unsigned long long* agg = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * p.NG * 3 * (GK + 1));
-    uint16_t* pre = ws.take<uint16_t>((size_t)v.batch * p.tiles * 2 * p.NP * LW);
-    uint16_t* suf = ws.take<uint16_t>((size_t)v.batch * p.tiles * 2 * p.NP * LW);
+    LineWs w = carve_line(ws, v, p);
     if (!ws.ok()) { set_error("rqa_line_hist: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
-    RQA_CUDA_TRY(cudaMemsetAsync(agg, 0, sizeof(uint64_t) * (size_t)v.batch * p.NG * 3 * (GK + 1), s));
-    line_groups_kernel<<<v.batch, 128, 0, s>>>(d_eps, K, p.NG, groups, status);
+    const size_t agg_words = (size_t)v.batch * p.NG * 3 * (GK + 1);
+    RQA_CUDA_TRY(cudaMemsetAsync(w.agg, 0, sizeof(uint64_t) * agg_words, s));
+    RQA_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(unsigned int) * (size_t)p.NG, s));
+    line_groups_kernel<<<v.batch, 128, 0, s>>>(d_eps, K, p.NG, w.groups, status);
     RQA_LAUNCH_CHECK();
+    if (p.tl.tiles > 0) {
+        rqa_status st = launch_tile_table(p.tl, w.seg_start, s);
+        if (st != RQA_OK) return st;
+    }
+    for (int g = 0; g < p.NG && p.tl.tiles > 0; ++g) {
+        ScanArgs a;
+        a.v = v; a.g = g; a.NG = p.NG; a.K = K; a.L = p.L; a.S = p.S;
+        a.part = opt.part; a.parts = opt.parts; a.n_obl = p.tl.n_obl; a.nbuf = p.nbuf;
+        a.groups = w.groups; a.seg_start = w.seg_start; a.hist = (unsigned long long*)d_hist; a.agg = w.agg;
+        a.pre = w.pre; a.suf = w.suf; a.carry = w.carry; a.counter = w.counters + g; a.segs = (uint32_t)p.tl.tiles;
+        a.m = v.m; a.tau = (int)v.cs;
+        rqa_status st = norm == RQA_NORM_MAX ? dispatch_pairs<RQA_NORM_MAX>(a, p, s) : dispatch_pairs<RQA_NORM_EUCLID>(a, p, s);
+        if (st != RQA_OK) return st;
+        StitchArgs sa;
+        sa.n = v.n; sa.w = v.w; sa.T = p.tl.T; sa.g = g; sa.NG = p.NG; sa.K = K; sa.NP = p.NP;
+        sa.part = opt.part; sa.parts = opt.parts; sa.n_obl = p.tl.n_obl;
+        sa.groups = w.groups; sa.seg_start = w.seg_start; sa.hist = (unsigned long long*)d_hist; sa.pre = w.pre; sa.suf = w.suf;
+        sa.segs = (uint32_t)p.tl.tiles;
+        line_stitch_kernel<<<dim3((unsigned)p.tl.n_obl, (unsigned)(2 * p.NP), (unsigned)v.batch), LW, 0, s>>>(sa);
+        RQA_LAUNCH_CHECK();
+    }
+    // a split call: the explicit lines and the aggregates of all parts, summed, before P(1..3) are solved from them
     {
-        rqa_status st = launch_tile_table(n_diag(v), p.L, p.n_ob, tile_start, s);
+        rqa_status st = reduce_parts(opt, d_hist, hist_words, s);
+        if (st != RQA_OK) return st;
+        st = reduce_parts(opt, w.agg, agg_words, s);
         if (st != RQA_OK) return st;
     }
     for (int g = 0; g < p.NG; ++g) {
-        ScanArgs a;
-        a.v = v; a.g = g; a.NG = p.NG; a.K = K; a.L = p.L; a.n_ob = p.n_ob;
-        a.groups = groups; a.tile_start = tile_start; a.hist = (unsigned long long*)d_hist; a.agg = agg;
-        a.pre = pre; a.suf = suf; a.tiles = p.tiles; a.m = v.m; a.tau = (int)v.cs;
-        rqa_status st = norm == RQA_NORM_MAX ? dispatch_pairs<RQA_NORM_MAX>(a, p, v.batch, s)
-                                             : dispatch_pairs<RQA_NORM_EUCLID>(a, p, v.batch, s);
-        if (st != RQA_OK) return st;
-        StitchArgs sa;
-        sa.n = v.n; sa.w = v.w; sa.g = g; sa.NG = p.NG; sa.K = K; sa.L = p.L; sa.n_ob = p.n_ob; sa.NP = p.NP;
-        sa.groups = groups; sa.tile_start = tile_start; sa.hist = (unsigned long long*)d_hist; sa.pre = pre; sa.suf = suf;
-        sa.tiles = p.tiles;
-        line_stitch_kernel<<<dim3((unsigned)p.n_ob, (unsigned)(2 * p.NP), (unsigned)v.batch), LW, 0, s>>>(sa);
-        RQA_LAUNCH_CHECK();
-        line_finalize_kernel<<<dim3((unsigned)(2 * p.NP), (unsigned)v.batch), 1024, 0, s>>>(v.n, g, p.NG, K, groups, agg,
+        line_finalize_kernel<<<dim3((unsigned)(2 * p.NP), (unsigned)v.batch), 1024, 0, s>>>(v.n, g, p.NG, K, w.groups, w.agg,
                                                                                          (unsigned long long*)d_hist, status);
         RQA_LAUNCH_CHECK();
         unsigned cb = (unsigned)std::min<int64_t>((v.n + 255) / 256, 64);
-        line_copy_rows_kernel<<<dim3(cb, GK, (unsigned)v.batch), 256, 0, s>>>(v.n, g, p.NG, K, groups, (unsigned long long*)d_hist);
+        line_copy_rows_kernel<<<dim3(cb, GK, (unsigned)v.batch), 256, 0, s>>>(v.n, g, p.NG, K, w.groups, (unsigned long long*)d_hist);
         RQA_LAUNCH_CHECK();
     }
     return RQA_OK;

@@ -45,12 +45,17 @@ enum : uint8_t { LEVEL_OUT = 0, LEVEL_CAND = 1, LEVEL_POINT = 2 };
 struct SelState {
     int32_t fallback;                 // 1: the series is (re)done by the radix passes
     int32_t pad;
+    unsigned long long ncand_local;   // candidates in THIS part's list (= ncand for an unsplit call)
+    // the next SEL_REDUCE_WORDS words are summed over the parts of a split call after the counting pass
     unsigned long long ncand;         // candidates appended by the counting pass (may exceed the capacity)
+    unsigned long long over;          // parts whose candidate list overflowed
     unsigned long long level_count[NLEV_MAX + 1];
     int32_t is_point[GK];             // target t of the group fell into a LEVEL_POINT level:
     float point_val[GK];              //   eps = that value,
     unsigned long long point_cnt[GK]; //   C = #{d <= eps}
 };
+
+constexpr size_t SEL_REDUCE_WORDS = 2 + NLEV_MAX + 1;
 
 // state of one buffer select (<= BT targets) of one series
 struct BufSel {
@@ -91,13 +96,13 @@ struct SampleRanks {                  // per target of the group: sample ranks o
 // ------------------------------------------------------------------------------------------ small kernels
 __global__ void sel_init_kernel(SelState* ss, int force_fallback) {
     SelState& s = ss[blockIdx.x];
-    if (threadIdx.x == 0) { s.fallback = force_fallback; s.pad = 0; s.ncand = 0; }
+    if (threadIdx.x == 0) { s.fallback = force_fallback; s.pad = 0; s.ncand = 0; s.over = 0; s.ncand_local = 0; }
     for (int q = threadIdx.x; q <= NLEV_MAX; q += blockDim.x) s.level_count[q] = 0;
 }
 
 __global__ void sel_group_reset_kernel(SelState* ss) {
     SelState& s = ss[blockIdx.x];
-    if (threadIdx.x == 0) s.ncand = 0;
+    if (threadIdx.x == 0) { s.ncand = 0; s.over = 0; s.ncand_local = 0; }
     for (int q = threadIdx.x; q <= NLEV_MAX; q += blockDim.x) s.level_count[q] = 0;
 }
 
@@ -187,7 +192,7 @@ __global__ void __launch_bounds__(256) bufsel_pass_kernel(const float* __restric
     const BufSel& s = st[b];
     const int G = s.G;
     unsigned long long n = cap;
-    if (use_ncand) n = min(cap, ss[b].ncand);
+    if (use_ncand) n = min(cap, ss[b].ncand_local);
     for (int q = threadIdx.x; q < G * 256; q += blockDim.x) sbins[q] = 0;
     for (int q = threadIdx.x; q < G; q += blockDim.x) s_gprefix[q] = s.gprefix[q];
     __syncthreads();
@@ -381,7 +386,7 @@ __global__ void __launch_bounds__(512) sel_table_kernel(const BufSel* __restrict
 // ------------------------------------------------------------------------------------------ counting pass
 struct CountArgs {
     View v;
-    int L, n_ob;
+    int L, n_obl, part, parts;
     const uint32_t* tile_start;
     const SelTable* tabs;
     SelState* ss;
@@ -469,7 +474,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     const uint32_t tile = blockIdx.x;
     const SelTable& T = a.tabs[b];
     if (T.heavy != heavy_pass) return;                        // series with extra tie levels: the wider second launch
-    find_diagonal_block(a.tile_start, a.n_ob, tile, &s_ob);
+    find_diagonal_block(a.tile_start, a.n_obl, tile, &s_ob);
     uint2* lut_s = (uint2*)(smem + CountSmem::off_lut);
     float* beta_s = (float*)(smem + CountSmem::off_beta);
     float* cand_s = (float*)(smem + CountSmem::off_cand);
@@ -484,8 +489,8 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     if (tid < NCUT) { beta_s[tid] = T.beta[tid]; ((uint8_t*)(smem + CountSmem::off_kind))[tid] = T.kind[tid]; }
     for (int q = tid; q < nlev * col_words; q += LW) cols_s[q] = 0;
     __syncthreads();
-    const int ob = s_ob;
-    const int c = (int)(tile - a.tile_start[ob]);
+    const int ob = a.part + s_ob * a.parts;                   // this part's diagonal blocks are interleaved
+    const int c = (int)(tile - a.tile_start[s_ob]);
     const int L = a.L;
     const int64_t n = a.v.n;
     const int64_t o0 = a.v.w + (int64_t)LW * ob;
@@ -556,10 +561,19 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     }
 }
 
+// After the counting pass, before the parts of a split call are summed: this part's candidate count and whether its
+// list overflowed.
+__global__ void sel_local_kernel(SelState* ss, int batch, unsigned long long cap) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    ss[b].ncand_local = ss[b].ncand;
+    ss[b].over = ss[b].ncand > cap ? 1ull : 0ull;
+}
+
 // One block per series: exact level counts -> each target's level.  A candidate level: its rank among the candidates
 // (the buffer select finishes it).  A single-value level: eps and C are known here.  Anything else: radix fallback.
 __global__ void __launch_bounds__(64) sel_bracket_resolve_kernel(SelState* ss, const SelTable* __restrict__ tabs,
-                                                               SampleRanks sr, BufSel* st, unsigned long long cap) {
+                                                               SampleRanks sr, BufSel* st) {
     const int b = blockIdx.x;
     SelState& s = ss[b];
     if (s.fallback) return;
@@ -576,7 +590,7 @@ __global__ void __launch_bounds__(64) sel_bracket_resolve_kernel(SelState* ss, c
             if (T.kind[v] == LEVEL_CAND) cnd += s.level_count[v];
         }
         s_cum[T.J + 1] = cum;
-        s_bad = (cnd != s.ncand) || (s.ncand > cap);
+        s_bad = (cnd != s.ncand) || s.over != 0;
         bufsel_reset(bs, sr.kc);
     }
     __syncthreads();
@@ -658,7 +672,7 @@ __global__ void radix_init_kernel(SelBatch* st, Ranks ranks, int K) {
 template <int NORM>
 __global__ void __launch_bounds__(SEL_W) radix_pass_kernel(View v, int pass, const SelBatch* __restrict__ st,
                                                            unsigned long long* __restrict__ bins, int K,
-                                                           const SelState* __restrict__ ss) {
+                                                           const SelState* __restrict__ ss, int part, int parts) {
     extern __shared__ uint32_t sbins[];      // [G][256]
     __shared__ uint32_t s_gprefix[RQA_MAX_K];
     const int b = blockIdx.y;
@@ -672,7 +686,7 @@ __global__ void __launch_bounds__(SEL_W) radix_pass_kernel(View v, int pass, con
     const int shift = 24 - 8 * pass;
     const uint32_t himask = pass == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * pass));
     const int64_t nx = (v.n - v.w + SEL_W - 1) / SEL_W, ny = (v.n - v.w + SEL_L - 1) / SEL_L;
-    for (int64_t tile = blockIdx.x; tile < nx * ny; tile += gridDim.x) {
+    for (int64_t tile = (int64_t)blockIdx.x * parts + part; tile < nx * ny; tile += (int64_t)gridDim.x * parts) {
         const int64_t o = v.w + (tile % nx) * SEL_W + threadIdx.x;
         const int64_t i0 = (tile / nx) * SEL_L;
         if (o >= v.n) continue;
@@ -778,8 +792,8 @@ enum { PATH_AUTO = 0, PATH_DIRECT = 1, PATH_BRACKET = 2, PATH_RADIX = 3 };
 struct SelectPlan {
     int path;
     unsigned long long P, S, cap;     // pairs, sample size, candidate capacity per series
-    int L, n_ob;
-    uint32_t tiles;
+    int L;
+    Tiling tl;                        // this part's tiles of the counting pass
     int span;
     int fields;                       // counting pass: threads per counter word (2 or 3)
     int ps;                           // point stride in floats
@@ -791,16 +805,18 @@ size_t count_smem_bytes(int nlev, int fields, int L, int span, int ps) {
 }
 constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of sm_100a, minus the static part
 
-SelectPlan make_select_plan(const View& v, int K) {
-    const Options& opt = options();
+SelectPlan make_select_plan(const View& v, int K, const Options& opt) {
     SelectPlan p{};
     p.P = n_pairs(v);
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
     p.ps = (int)std::min<int64_t>(v.ps, 1 << 20);
+    // more than 20 brackets per group: 10-bit counters (two blocks per SM still fit), so shorter chunks
+    p.fields = std::min(K, GK) > 20 ? 3 : 2;
     // tiled counting pass: delay views, and materialised points whose windows fit beside the widest level table
+    // (the heavy launch's, with the counter width this K uses)
     const int nlev_max = 2 * (2 * std::min(K, GK) + 1) - 1;
-    const bool tiled_ok = p.span <= MAX_SPAN && count_smem_bytes(nlev_max, 3, 32, p.span, p.ps) <= SMEM_PER_BLOCK_MAX;
-    p.path = (int)opt.select_path;
+    const bool tiled_ok = p.span <= MAX_SPAN && count_smem_bytes(nlev_max, p.fields, 32, p.span, p.ps) <= SMEM_PER_BLOCK_MAX;
+    p.path = opt.select_path;
     if (p.path == PATH_AUTO) p.path = p.P <= (1ull << 22) ? PATH_DIRECT : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
     if (p.path == PATH_BRACKET && !tiled_ok) p.path = PATH_RADIX;
     if (p.path == PATH_DIRECT && p.P > (1ull << 28)) p.path = tiled_ok ? PATH_BRACKET : PATH_RADIX;
@@ -815,14 +831,11 @@ SelectPlan make_select_plan(const View& v, int K) {
         unsigned long long cap = (unsigned long long)(1.5 * frac * (double)p.P) + 4096;
         if (opt.cand_cap > 0) cap = (unsigned long long)opt.cand_cap;
         p.cap = std::min(cap, p.P);
-        const double cells = (double)p.P * (double)v.batch;
-        int64_t L = (int64_t)std::ceil(cells / ((double)LW * 148.0 * 3.0 * 8.0));
-        // more than 20 brackets per group: 10-bit counters (two blocks per SM still fit), so shorter chunks
-        p.fields = std::min(K, GK) > 20 ? 3 : 2;
+        const double cells = (double)p.P * (double)v.batch / (double)opt.parts;
+        int64_t L = (int64_t)std::ceil(cells / ((double)LW * sm_count() * 3.0 * 8.0));
         p.L = (int)std::max<int64_t>(32, std::min<int64_t>(p.fields == 3 ? 1023 : 2047, L));
         while (p.L > 32 && count_smem_bytes(nlev_max, p.fields, p.L, p.span, p.ps) > SMEM_PER_BLOCK_MAX) p.L = std::max(32, p.L / 2);
-        p.n_ob = (int)((n_diag(v) - 1 + LW - 1) / LW);
-        p.tiles = (uint32_t)count_tiles(n_diag(v), p.L);
+        p.tl = make_tiling(n_diag(v), p.L, opt.part, opt.parts);
     }
     return p;
 }
@@ -834,10 +847,18 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
     // of the other series return at once, and so do the first launch's blocks of those series
     const int nlev_heavy = 2 * nlev - 1;
     const size_t smem = count_smem_bytes(nlev, p.fields, p.L, p.span, p.ps), smem_heavy = count_smem_bytes(nlev_heavy, p.fields, p.L, p.span, p.ps);
-    RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_heavy));
-    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, p.fields, 0);
+    static thread_local bool attr_set[8] = {false};             // per device: opted in to the largest shared-memory size
+    int dev = 0;
+    RQA_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev >= 8 || !attr_set[dev]) {
+        RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_PER_BLOCK_MAX));
+        if (dev < 8) attr_set[dev] = true;
+    }
+    if (smem_heavy > SMEM_PER_BLOCK_MAX) { set_error("rqa_eps_for_rr: counting pass needs %zu bytes of shared memory", smem_heavy); return RQA_ERR_UNSUPPORTED; }
+    if (p.tl.tiles == 0) return RQA_OK;
+    kern<<<dim3((unsigned)p.tl.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, p.fields, 0);
     RQA_LAUNCH_CHECK();
-    kern<<<dim3(p.tiles, (unsigned)batch), LW, smem_heavy, s>>>(a, nlev_heavy, p.fields, 1);
+    kern<<<dim3((unsigned)p.tl.tiles, (unsigned)batch), LW, smem_heavy, s>>>(a, nlev_heavy, p.fields, 1);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }
@@ -853,14 +874,24 @@ rqa_status dispatch_count(const CountArgs& a, const SelectPlan& p, int nlev, int
 
 // 4 radix passes over a buffer for the <= BT targets whose state is already initialised in `st`.
 rqa_status run_bufsel(const float* buf, unsigned long long stride, unsigned long long cap, const SelState* ss,
-                      int use_ncand, BufSel* st, unsigned long long* bins, int T, int batch, cudaStream_t s) {
+                      int use_ncand, BufSel* st, unsigned long long* bins, int T, int batch, cudaStream_t s,
+                      const Options* split = nullptr) {
     const size_t smem = (size_t)T * 256 * sizeof(uint32_t);
-    if (smem > 48 * 1024)
-        RQA_CUDA_TRY(cudaFuncSetAttribute(bufsel_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static thread_local bool attr_set[8] = {false};
+    int dev = 0;
+    RQA_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev >= 8 || !attr_set[dev]) {
+        RQA_CUDA_TRY(cudaFuncSetAttribute(bufsel_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BT * 256 * (int)sizeof(uint32_t)));
+        if (dev < 8) attr_set[dev] = true;
+    }
     unsigned blocks = (unsigned)std::max<unsigned long long>(1, std::min<unsigned long long>((cap + 2047) / 2048, 148 * 4));
     for (int pass = 0; pass < 4; ++pass) {
         bufsel_pass_kernel<<<dim3(blocks, (unsigned)batch), 256, smem, s>>>(buf, stride, cap, ss, use_ncand, pass, st, bins);
         RQA_LAUNCH_CHECK();
+        if (split) {                                             // every part holds a share of the buffer: sum the digit bins
+            rqa_status rs = reduce_parts(*split, bins, (size_t)batch * BT * 256, s);
+            if (rs != RQA_OK) return rs;
+        }
         bufsel_resolve_kernel<<<batch, 256, 0, s>>>(st, bins, pass, ss, use_ncand);
         RQA_LAUNCH_CHECK();
     }
@@ -889,7 +920,7 @@ SelectWs carve(Arena& ws, const View& v, int K, const SelectPlan& p) {
     if (p.path == PATH_DIRECT) w.sample = ws.take<float>((size_t)v.batch * p.P);
     if (p.path == PATH_BRACKET) {
         w.tabs = ws.take<SelTable>(v.batch);
-        w.tile_start = ws.take<uint32_t>((size_t)p.n_ob + 1);
+        w.tile_start = ws.take<uint32_t>((size_t)p.tl.n_obl + 1);
         w.sample = ws.take<float>((size_t)v.batch * p.S);
         w.cand = ws.take<float>((size_t)v.batch * p.cap);
     }
@@ -898,16 +929,16 @@ SelectWs carve(Arena& ws, const View& v, int K, const SelectPlan& p) {
 
 }  // namespace
 
-size_t select_workspace_bytes(const View& v, int K) {
-    SelectPlan p = make_select_plan(v, K);
+size_t select_workspace_bytes(const View& v, int K, const Options& opt) {
+    SelectPlan p = make_select_plan(v, K, opt);
     Arena a(nullptr, ~(size_t)0);
     carve(a, v, K, p);
     return a.off;
 }
 
 rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
-                      double* d_rr, Arena& ws, cudaStream_t s) {
-    const SelectPlan p = make_select_plan(v, K);
+                      double* d_rr, Arena& ws, cudaStream_t s, const Options& opt) {
+    const SelectPlan p = make_select_plan(v, K, opt);
     SelectWs w = carve(ws, v, K, p);
     if (!ws.ok()) { set_error("rqa_eps_for_rr: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
     const unsigned long long P = p.P;
@@ -951,7 +982,8 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
             else sel_sample_kernel<RQA_NORM_EUCLID><<<dim3(blocks, v.batch), 256, 0, s>>>(v, S, w.sample);
             RQA_LAUNCH_CHECK();
         }
-        rqa_status st = launch_tile_table(n_diag(v), p.L, p.n_ob, w.tile_start, s);
+        rqa_status st = RQA_OK;
+        if (p.tl.tiles > 0) st = launch_tile_table(p.tl, w.tile_start, s);
         if (st != RQA_OK) return st;
         for (int base = 0; base < K; base += GK) {
             const int kc = std::min(GK, K - base);
@@ -984,15 +1016,23 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
             sel_table_kernel<<<v.batch, 512, 0, s>>>(w.st, sr, w.tabs);
             RQA_LAUNCH_CHECK();
             CountArgs a;
-            a.v = v; a.L = p.L; a.n_ob = p.n_ob; a.tile_start = w.tile_start; a.tabs = w.tabs; a.ss = w.ss;
+            a.v = v; a.L = p.L; a.n_obl = p.tl.n_obl; a.part = opt.part; a.parts = opt.parts;
+            a.tile_start = w.tile_start; a.tabs = w.tabs; a.ss = w.ss;
             a.cand = w.cand; a.cap = p.cap; a.m = v.m; a.tau = (int)v.cs;
             const int nlev = 2 * kc + 1;
             st = norm == RQA_NORM_MAX ? dispatch_count<RQA_NORM_MAX>(a, p, nlev, v.batch, s)
                                       : dispatch_count<RQA_NORM_EUCLID>(a, p, nlev, v.batch, s);
             if (st != RQA_OK) return st;
-            sel_bracket_resolve_kernel<<<v.batch, 64, 0, s>>>(w.ss, w.tabs, sr, w.st, p.cap);
+            sel_local_kernel<<<(v.batch + 63) / 64, 64, 0, s>>>(w.ss, v.batch, p.cap);
             RQA_LAUNCH_CHECK();
-            st = run_bufsel(w.cand, p.cap, p.cap, w.ss, 1, w.st, w.bins, kc, v.batch, s);
+            // a split call: the level counts (and candidate totals) of all parts, per series
+            for (int b = 0; b < v.batch && opt.parts > 1; ++b) {
+                st = reduce_parts(opt, &w.ss[b].ncand, SEL_REDUCE_WORDS, s);
+                if (st != RQA_OK) return st;
+            }
+            sel_bracket_resolve_kernel<<<v.batch, 64, 0, s>>>(w.ss, w.tabs, sr, w.st);
+            RQA_LAUNCH_CHECK();
+            st = run_bufsel(w.cand, p.cap, p.cap, w.ss, 1, w.st, w.bins, kc, v.batch, s, opt.parts > 1 ? &opt : nullptr);
             if (st != RQA_OK) return st;
             sel_finish_kernel<<<v.batch, BT, 0, s>>>(w.ss, w.st, tm, K, P, 1, d_eps, d_cnt, d_rr);
             RQA_LAUNCH_CHECK();
@@ -1010,10 +1050,14 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
     auto kern = norm == RQA_NORM_MAX ? radix_pass_kernel<RQA_NORM_MAX> : radix_pass_kernel<RQA_NORM_EUCLID>;
     if (smem > 48 * 1024) RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t tiles = ((v.n - v.w + SEL_W - 1) / SEL_W) * ((v.n - v.w + SEL_L - 1) / SEL_L);
-    dim3 grid((unsigned)std::min<int64_t>(tiles, 148 * 16), (unsigned)v.batch);
+    dim3 grid((unsigned)std::min<int64_t>((tiles + opt.parts - 1) / opt.parts, 148 * 16), (unsigned)v.batch);
     for (int pass = 0; pass < 4; ++pass) {
-        kern<<<grid, SEL_W, smem, s>>>(v, pass, w.rst, w.rbins, K, w.ss);
+        kern<<<grid, SEL_W, smem, s>>>(v, pass, w.rst, w.rbins, K, w.ss, opt.part, opt.parts);
         RQA_LAUNCH_CHECK();
+        {
+            rqa_status rs = reduce_parts(opt, w.rbins, (size_t)v.batch * K * 256, s);
+            if (rs != RQA_OK) return rs;
+        }
         radix_resolve_kernel<<<v.batch, 256, 0, s>>>(w.rst, w.rbins, K, pass, P, w.ss, d_eps, d_cnt, d_rr);
         RQA_LAUNCH_CHECK();
     }

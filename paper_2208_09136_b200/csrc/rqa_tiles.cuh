@@ -47,16 +47,29 @@ __device__ inline float bucket_scale(float dcap, int nb = NB) {
     return scale;
 }
 
-// tile_start[ob] = number of tiles in the diagonal blocks before ob (ob = 0..n_ob); diagonal block ob holds the
-// diagonals 1 + LW*ob .. LW + LW*ob, its longest diagonal has n - 1 - LW*ob cells, cut into chunks of L.
-rqa_status launch_tile_table(int64_t n, int L, int n_ob, uint32_t* tile_start, cudaStream_t s);
-
-inline uint64_t count_tiles(int64_t n, int L) {
-    uint64_t tiles = 0;
-    const int n_ob = (int)((n - 1 + LW - 1) / LW);
-    for (int ob = 0; ob < n_ob; ++ob) tiles += (uint64_t)((n - 1 - (int64_t)LW * ob + L - 1) / L);
-    return tiles;
+// Tiling of the triangle of nd = N' - w + 1 "points" (diagonals w..N'-1) for one part of a (possibly split) call.
+// Diagonal block ob holds LW adjacent diagonals; part `part` of `parts` owns the blocks ob = part, part + parts, ...
+// (interleaved: every part gets long and short diagonals).  Local block q <-> ob = part + q*parts.  A tile is T
+// consecutive positions of one diagonal block.
+struct Tiling {
+    int64_t nd;       // points of the counted triangle
+    int64_t T;        // cells per tile along the diagonals
+    int part, parts;
+    int n_ob;         // diagonal blocks of the whole triangle
+    int n_obl;        // ... owned by this part
+    uint64_t tiles;   // tiles of this part (one series)
+};
+inline Tiling make_tiling(int64_t nd, int64_t T, int part, int parts) {
+    Tiling t{};
+    t.nd = nd; t.T = T; t.part = part; t.parts = parts;
+    t.n_ob = (int)((nd - 1 + LW - 1) / LW);
+    t.n_obl = t.n_ob > part ? (t.n_ob - part + parts - 1) / parts : 0;
+    t.tiles = 0;
+    for (int q = 0; q < t.n_obl; ++q) t.tiles += (uint64_t)((nd - 1 - (int64_t)LW * (part + (int64_t)q * parts) + T - 1) / T);
+    return t;
 }
+// tile_start[q] = number of tiles in the local diagonal blocks before q (q = 0..n_obl), computed on the device.
+rqa_status launch_tile_table(const Tiling& t, uint32_t* tile_start, cudaStream_t s);
 
 #ifdef __CUDACC__
 // Shared-memory accesses of the tiled passes' inner loops go through 32-bit shared-window addresses and explicit .shared
@@ -76,6 +89,28 @@ __device__ __forceinline__ void sts_u16(uint32_t a, uint32_t v) { asm volatile("
 __device__ __forceinline__ void sts_v4(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) { asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" :: "r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory"); }
 __device__ __forceinline__ uint32_t atom_u32(uint32_t a, uint32_t v) { uint32_t o; asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory"); return o; }
 __device__ __forceinline__ void red_u32(uint32_t a, uint32_t v) { asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+
+// ---- bulk asynchronous copies global -> shared (the TMA engine's 1-D path) completing on an mbarrier
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) { asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" :: "r"(bar), "r"(parity) : "memory");
+}
+// dst (shared, 16-byte aligned), src (global, 16-byte aligned), bytes a multiple of 16
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// orders earlier generic-proxy accesses of shared memory before later async-proxy (bulk copy) writes
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Which diagonal block does `tile` belong to?  (block-wide search; the caller syncs before reading *s_ob)
 __device__ __forceinline__ void find_diagonal_block(const uint32_t* __restrict__ tile_start, int n_ob, uint32_t tile,

@@ -108,25 +108,66 @@ def test_line_hist_det_embed_reject_bad_arguments(lib):
         (982, 4, 5, 1, 6, 1000)
 
 
-def test_set_option_validation(lib):
-    assert lib.rqa_set_option(b"select_path", 2) == B.RQA_OK
-    assert lib.rqa_set_option(b"select_path", 0) == B.RQA_OK
-    assert lib.rqa_set_option(b"select_path", 4) == B.RQA_ERR_INVALID_ARG
-    assert lib.rqa_set_option(b"line_chunk", 1024) == B.RQA_ERR_INVALID_ARG
-    assert lib.rqa_set_option(b"no_such_option", 1) == B.RQA_ERR_INVALID_ARG
-    assert lib.rqa_set_option(None, 1) == B.RQA_ERR_INVALID_ARG
-    assert lib.rqa_set_option(b"sample_size", -1) == B.RQA_ERR_INVALID_ARG
-    # workspace sizes follow the options: the bracket path needs the sample and candidate buffers
-    sz0, sz2 = ctypes.c_size_t(0), ctypes.c_size_t(0)
+def test_options_are_per_call_and_validated(lib):
+    """struct rqa_options travels with the call (the library has no global state): bad fields are rejected before any
+    launch, and workspace sizes follow the options passed to rqa_workspace_bytes_opt."""
+    assert not hasattr(lib, "rqa_set_option_does_not_exist")
+    with pytest.raises(AttributeError):
+        lib.rqa_set_option                                   # the process-wide knobs of round 1 are gone
+    sz = ctypes.c_size_t(0)
     pts = _pts(n=5000, bs=5002)
-    assert lib.rqa_set_option(b"select_path", 3) == B.RQA_OK
-    assert lib.rqa_workspace_bytes(ctypes.byref(pts), 20, ctypes.byref(sz0)) == B.RQA_OK
-    assert lib.rqa_set_option(b"select_path", 2) == B.RQA_OK
-    assert lib.rqa_set_option(b"sample_size", 50_000_000) == B.RQA_OK
-    assert lib.rqa_workspace_bytes(ctypes.byref(pts), 20, ctypes.byref(sz2)) == B.RQA_OK
-    assert lib.rqa_set_option(b"select_path", 0) == B.RQA_OK
-    assert lib.rqa_set_option(b"sample_size", 0) == B.RQA_OK
-    assert sz2.value >= 4 * 50_000_000 > sz0.value
+
+    def size(**kw):
+        o = B.make_options(**kw)
+        st = lib.rqa_workspace_bytes_opt(ctypes.byref(pts), 20, ctypes.byref(o), ctypes.byref(sz))
+        return st, sz.value
+    assert size(select_path=4)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(select_path=-1)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(line_chunk=1024)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(line_buffers=3)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(line_segment=-1)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(sample_size=-1)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(part_index=2, part_count=2)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(part_index=1, part_count=0)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(part_index=0, part_count=2)[0] == B.RQA_ERR_INVALID_ARG      # a split call needs a reduce callback
+    assert size(part_index=1, part_count=2, reduce=lambda p, n, s: None)[0] == B.RQA_OK
+    # the bracket path needs the sample and candidate buffers, the radix path does not
+    st0, sz0 = size(select_path=3)
+    st2, sz2 = size(select_path=2, sample_size=50_000_000)
+    assert st0 == st2 == B.RQA_OK and sz2 >= 4 * 50_000_000 > sz0
+    # NULL options = automatic = the plain call
+    assert lib.rqa_workspace_bytes_opt(ctypes.byref(pts), 20, None, ctypes.byref(sz)) == B.RQA_OK
+    auto = sz.value
+    assert lib.rqa_workspace_bytes(ctypes.byref(pts), 20, ctypes.byref(sz)) == B.RQA_OK and sz.value == auto
+    # the same call from two threads with different options: no interference (there is nothing to interfere with)
+    import threading
+    out = {}
+
+    def worker(name, **kw):
+        out[name] = [size_local(**kw) for _ in range(50)]
+
+    def size_local(**kw):
+        o, z = B.make_options(**kw), ctypes.c_size_t(0)
+        assert lib.rqa_workspace_bytes_opt(ctypes.byref(pts), 20, ctypes.byref(o), ctypes.byref(z)) == B.RQA_OK
+        return z.value
+    ts = [threading.Thread(target=worker, args=("a",), kwargs={"select_path": 3}),
+          threading.Thread(target=worker, args=("b",), kwargs={"select_path": 2, "sample_size": 50_000_000})]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert set(out["a"]) == {sz0} and set(out["b"]) == {sz2}
+
+
+def test_null_arguments_never_crash(lib):
+    """Every entry point returns a status for NULL pointers (round-1 finding: rqa_workspace_bytes(NULL, ...) crashed)."""
+    sz = ctypes.c_size_t(0)
+    assert lib.rqa_workspace_bytes(None, 20, ctypes.byref(sz)) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_workspace_bytes(ctypes.byref(_pts()), 20, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_workspace_bytes_opt(None, 20, None, ctypes.byref(sz)) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_eps_for_rr(None, 0, FAKE, 2, FAKE, FAKE, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_line_hist(None, 0, FAKE, 2, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_workspace_status(None, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_embed(None, 100, 1, 100, 3, 1, None, None, None) == B.RQA_ERR_INVALID_ARG
+    assert b"NULL" in lib.rqa_last_error()
 
 
 def test_no_cpu_fallback_without_gpu(lib):

@@ -14,10 +14,13 @@ pytestmark = pytest.mark.gpu
 DET_TOL = 1e-12
 
 
+_OPT = {"o": None}     # the rqa_options of the running test (see the `options` fixture)
+
+
 def gpu_sweep(rqa, series, m, tau, rr, norm=0, l_min=2):
     import torch
     s = torch.as_tensor(np.ascontiguousarray(series, dtype=np.float32)).cuda()
-    buf = rqa.averaged_rqa(s, m, tau, rr, norm, l_min)
+    buf = rqa.averaged_rqa(s, m, tau, rr, norm, l_min, options=_OPT["o"])
     torch.cuda.synchronize()
     return {
         "eps": buf.eps.cpu().numpy(),
@@ -204,9 +207,9 @@ def test_materialised_points_equal_delay_view(rqa, oracle, N, m, tau, norm, batc
     cnt = torch.empty((batch, K), dtype=torch.int64, device="cuda")
     rrr = torch.empty((batch, K), dtype=torch.float64, device="cuda")
     hist = torch.empty((batch, K, n), dtype=torch.int64, device="cuda")
-    ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
-    rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
-    rqa.rqa_line_hist(view, norm, eps, hist, ws)
+    ws = torch.empty(rqa.rqa_workspace_bytes(view, K, _OPT["o"]), dtype=torch.uint8, device="cuda")
+    rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws, options=_OPT["o"])
+    rqa.rqa_line_hist(view, norm, eps, hist, ws, options=_OPT["o"])
     rqa.rqa_workspace_status(ws)
     for b in range(batch):
         r = oracle.sweep(ys[b], m, tau, rr, norm, threads=0)
@@ -225,7 +228,7 @@ def test_line_hist_with_caller_thresholds(rqa, oracle):
     n = int(view.n_points)
     hist = torch.empty((1, len(eps), n), dtype=torch.int64, device="cuda")
     ws = torch.empty(rqa.rqa_workspace_bytes(view, len(eps)), dtype=torch.uint8, device="cuda")
-    rqa.rqa_line_hist(view, 0, torch.as_tensor(eps).cuda().unsqueeze(0), hist, ws)
+    rqa.rqa_line_hist(view, 0, torch.as_tensor(eps).cuda().unsqueeze(0), hist, ws, options=_OPT["o"])
     rqa.rqa_workspace_status(ws)
     assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], oracle.line_hist(y, 3, 1, eps, 0))
 
@@ -259,7 +262,7 @@ def test_strict_heaviside_by_previous_float(rqa):
     hist = torch.empty((1, len(eps), n), dtype=torch.int64, device="cuda")
     ws = torch.empty(rqa.rqa_workspace_bytes(view, len(eps)), dtype=torch.uint8, device="cuda")
     below = np.nextafter(eps, np.float32(-np.inf)).astype(np.float32)
-    rqa.rqa_line_hist(view, 0, torch.as_tensor(below).cuda().unsqueeze(0), hist, ws)
+    rqa.rqa_line_hist(view, 0, torch.as_tensor(below).cuda().unsqueeze(0), hist, ws, options=_OPT["o"])
     rqa.rqa_workspace_status(ws)
     assert np.array_equal(hist.cpu().numpy().view(np.uint64)[0], want)
 
@@ -283,7 +286,7 @@ def test_workspace_too_small_is_reported(rqa):
     rrr = torch.empty((1, K), dtype=torch.float64, device="cuda")
     ws = torch.empty(256, dtype=torch.uint8, device="cuda")
     with pytest.raises(rqa.RqaError) as e:
-        rqa.rqa_eps_for_rr(view, 0, [0.1] * K, eps, cnt, rrr, ws)
+        rqa.rqa_eps_for_rr(view, 0, [0.1] * K, eps, cnt, rrr, ws, options=_OPT["o"])
     assert e.value.status == rqa.RQA_ERR_WORKSPACE_TOO_SMALL
 
 
@@ -346,15 +349,12 @@ def test_config4_full_size_white_noise(rqa, oracle):
 # ------------------------------------------------------------------ every path of rqa_eps_for_rr is exact
 @pytest.fixture
 def options(rqa):
-    """Set expert knobs for one test and restore the automatic choices afterwards."""
-    names = ["select_path", "sample_size", "cand_cap", "line_chunk"]
-
+    """Expert knobs (struct rqa_options, passed per call: the library has no global state) for one test: the helpers
+    of this module hand _OPT["o"] to every call they make."""
     def setter(**kw):
-        for k, v in kw.items():
-            rqa.rqa_set_option(k, v)
+        _OPT["o"] = rqa.make_options(**kw) if any(kw.values()) else None
     yield setter
-    for n in names:
-        rqa.rqa_set_option(n, 0)
+    _OPT["o"] = None
 
 
 def _select_only(rqa, series, m, tau, rr, norm=0):
@@ -365,8 +365,8 @@ def _select_only(rqa, series, m, tau, rr, norm=0):
     eps = torch.empty((s.shape[0], K), dtype=torch.float32, device="cuda")
     cnt = torch.empty((s.shape[0], K), dtype=torch.int64, device="cuda")
     rrr = torch.empty((s.shape[0], K), dtype=torch.float64, device="cuda")
-    ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
-    rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
+    ws = torch.empty(rqa.rqa_workspace_bytes(view, K, _OPT["o"]), dtype=torch.uint8, device="cuda")
+    rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws, options=_OPT["o"])
     rqa.rqa_workspace_status(ws)
     return eps.cpu().numpy(), cnt.cpu().numpy().view(np.uint64), rrr.cpu().numpy()
 
@@ -491,13 +491,16 @@ def test_paper_sweep_k99_prefix_measures_sorting(rqa, oracle):
         rqa.rqa_sorting_rate_host(np.zeros((1, 1)))
 
 
-@pytest.mark.parametrize("L", [1, 2, 3, 4, 5, 7, 26, 100, 1023])
-def test_line_hist_any_chunk_length(rqa, oracle, options, L):
-    """The diagonal scan cuts every diagonal into chunks of L cells and joins the runs that cross chunk borders
-    afterwards.  Chunks shorter than the 4-cell window of the run stack, chunks that end inside a drain window, and
-    one chunk per diagonal must all give the oracle's histograms: a noisy sine (short and long lines), an exactly
-    periodic one (lines as long as the diagonals) and a quantised series, embedded and not."""
-    options(line_chunk=L)
+@pytest.mark.parametrize("L,S,nbuf", [(1, 1, 1), (1, 5, 2), (2, 3, 1), (3, 0, 0), (4, 2, 2), (5, 64, 1), (7, 1, 2), (7, 4, 0),
+                                       (26, 1, 1), (26, 3, 2), (100, 2, 2), (100, 0, 1), (1023, 1, 2), (1023, 0, 0)])
+def test_line_hist_any_chunk_length(rqa, oracle, options, L, S, nbuf):
+    """The diagonal scan cuts every diagonal into chunks of L cells; a persistent block walks a segment of S
+    consecutive chunks carrying the runs that cross a chunk border in place, and the runs that cross a segment border
+    are joined afterwards by the stitch kernel; the windows are staged by plain loads (1 set) or bulk asynchronous
+    copies (2 sets).  Chunks shorter than the 4-cell window of the run stack, chunks that end inside a drain window,
+    one chunk per diagonal, one segment per diagonal must all give the oracle's histograms: a noisy sine (short and
+    long lines), an exactly periodic one (lines as long as the diagonals) and a quantised series, embedded and not."""
+    options(line_chunk=L, line_segment=S, line_buffers=nbuf)
     rr = wl.rr_log(12, 0.002, 0.5)
     ys = np.stack([wl.add_noise(wl.sine_signal(1300), 2.0, 8), wl.sine_signal(1300).astype(np.float32),
                    np.round(wl.gaussian(13, 1300) * 3.0).astype(np.float32)])
@@ -539,7 +542,8 @@ def test_random_configurations(rqa, oracle, options, seed):
         l_min = int(rng.choice([1, 2, 2, 3, 5]))
         ys = np.stack([series(int(rng.integers(7)), N, 1000 * case + b) for b in range(batch)])
         options(select_path=int(rng.choice([0, 0, 1, 2, 3])), sample_size=int(rng.choice([0, 0, 50, 4000])),
-                line_chunk=int(rng.choice([0, 0, 0, 1, 2, 3, 6, 13, 64, 500])), cand_cap=int(rng.choice([0, 0, 0, 200])))
+                line_chunk=int(rng.choice([0, 0, 0, 1, 2, 3, 6, 13, 64, 500])), cand_cap=int(rng.choice([0, 0, 0, 200])),
+                line_segment=int(rng.choice([0, 0, 1, 2, 7, 40])), line_buffers=int(rng.choice([0, 1, 2])))
         s = torch.as_tensor(ys).cuda()
         n = N - (m - 1) * tau
         X = torch.empty((batch, n, m), dtype=torch.float32, device="cuda") if rng.random() < 0.25 else None
@@ -551,9 +555,9 @@ def test_random_configurations(rqa, oracle, options, seed):
         hist = torch.empty((batch, K, n), dtype=torch.int64, device="cuda")
         det = torch.empty((batch, K), dtype=torch.float64, device="cuda")
         mean = torch.empty((batch,), dtype=torch.float64, device="cuda")
-        ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
-        rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
-        rqa.rqa_line_hist(view, norm, eps, hist, ws)
+        ws = torch.empty(rqa.rqa_workspace_bytes(view, K, _OPT["o"]), dtype=torch.uint8, device="cuda")
+        rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws, options=_OPT["o"])
+        rqa.rqa_line_hist(view, norm, eps, hist, ws, options=_OPT["o"])
         rqa.rqa_det_avg(hist, l_min, det, mean)
         rqa.rqa_workspace_status(ws)
         g = {"eps": eps.cpu().numpy(), "count": cnt.cpu().numpy().view(np.uint64), "rr": rrr.cpu().numpy(),
@@ -581,9 +585,9 @@ def test_theiler_window(rqa, oracle, options, path):
         cnt = torch.empty((2, K), dtype=torch.int64, device="cuda")
         rrr = torch.empty((2, K), dtype=torch.float64, device="cuda")
         hist = torch.empty((2, K, n), dtype=torch.int64, device="cuda")
-        ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
-        rqa.rqa_eps_for_rr(view, 0, rr, eps, cnt, rrr, ws)
-        rqa.rqa_line_hist(view, 0, eps, hist, ws)
+        ws = torch.empty(rqa.rqa_workspace_bytes(view, K, _OPT["o"]), dtype=torch.uint8, device="cuda")
+        rqa.rqa_eps_for_rr(view, 0, rr, eps, cnt, rrr, ws, options=_OPT["o"])
+        rqa.rqa_line_hist(view, 0, eps, hist, ws, options=_OPT["o"])
         rqa.rqa_workspace_status(ws)
         rrh = torch.empty_like(rrr)
         rqa.rqa_line_measures(hist, 2, rr_hist=rrh, theiler=w)
@@ -596,4 +600,4 @@ def test_theiler_window(rqa, oracle, options, path):
             assert np.array_equal(hist[b].cpu().numpy().view(np.uint64), r["hist"]), (m, tau, w, chunk)
     with pytest.raises(rqa.RqaError):
         bad = rqa.rqa_embed(torch.zeros(50, device="cuda"), 1, 1, theiler=50)
-        rqa.rqa_workspace_bytes(bad, 3)
+        rqa.rqa_workspace_bytes(bad, 3, _OPT["o"])

@@ -412,14 +412,24 @@ __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc,
     sc.seek(sc.ya_org, yb_org, t);
     sc.prime();
     for (; t < 4; t += U) sc.template superstep<0>(t, cnt, ds, Seq{});   // warm-up cells and t < 4
-    constexpr int SPW = QCELLS / U;                          // super-steps per drain window
+    // Drain on demand: a window of super-steps lasts until some lane's queue could overflow in the next super-step
+    // (more than QCELLS - U entries) or the cell index inside the window would leave its 8 bits.  The replay loop runs
+    // as long as the longest queue of the warp, so long windows keep more lanes busy in it: with a drain every 24
+    // cells 7 of 32 lanes held an event per iteration (profiles/r2_scan_drain.md), white noise now fills about half.
+    constexpr int WMAX = 240 / U;                            // super-steps per window at most
+    constexpr uint32_t QHIGH = (uint32_t)(QCELLS - U) * (uint32_t)SC::SM::stk_row;
     sc.aprev = sc.A;
     sc.qp = sc.q0;
     sc.trel8 = 0;
     while (t + U <= cnt_lo) {
         const int t0w = t;
+        int w = 0;
 #pragma unroll 1
-        for (int w = 0; w < SPW && t + U <= cnt_lo; ++w, t += U) sc.template superstep<1>(t, cnt, ds, Seq{});
+        do {
+            sc.template superstep<1>(t, cnt, ds, Seq{});
+            t += U;
+            ++w;
+        } while (w < WMAX && t + U <= cnt_lo && !__any_sync(FULL, sc.qp - sc.q0 > QHIGH));
         sc.drain((uint32_t)t0w);
     }
     for (; t < cnt_hi; t += U) sc.template superstep<2>(t, cnt, ds, Seq{});
@@ -819,15 +829,10 @@ LinePlan make_plan(const View& v, int K, const Options& opt) {
     // window sets: two (bulk-copy double buffer) when they fit beside the per-thread state at this occupancy
     const size_t per_block = SMEM_PER_SM / p.blocks_per_sm - SMEM_BLOCK_RESERVED;
     const size_t budget = std::min(per_block, SMEM_PER_BLOCK_MAX);
-    p.nbuf = 2;
-    if (p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, 2) > budget) {
-        // shorter chunks cost little in a persistent block (a chunk border is one aggregate flush); keep two sets
-        // down to 256 positions, then give up the double buffer
-        int Ld = p.L;
-        while (Ld > 256 && scan_smem_bytes(p.NP, Ld, p.span, ps, 2) > budget) Ld -= 16;
-        if (opt.line_chunk == 0 && scan_smem_bytes(p.NP, Ld, p.span, ps, 2) <= budget) p.L = Ld;
-        else p.nbuf = 1;
-    }
+    // (measured at config 4, profiles/r2_scan_knobs.md: with K = 20 the per-thread state leaves room for ONE window set of
+    // a 1023-cell chunk at two blocks per SM; a second set would cost either the chunk length (L = 256: 44 ms per call)
+    // or the second block (49 ms) against 34.5 ms with one set — the other block of the SM hides the staging)
+    p.nbuf = p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, 2) <= budget ? 2 : 1;
     if (opt.line_buffers > 0) p.nbuf = opt.line_buffers;
     // wide points: the two windows hold (2L + 512) points, so the chunk shrinks until they fit (one block per SM then)
     while (p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, p.nbuf) > SMEM_PER_BLOCK_MAX) {
@@ -841,7 +846,7 @@ LinePlan make_plan(const View& v, int K, const Options& opt) {
     const Tiling chunks = make_tiling(nd, p.L, opt.part, opt.parts);
     const uint64_t all = chunks.tiles * (uint64_t)v.batch;
     int64_t S = (int64_t)(all / ((uint64_t)slots * 8));
-    p.S = (int)std::max<int64_t>(1, std::min<int64_t>(64, S));
+    p.S = (int)std::max<int64_t>(1, std::min<int64_t>(8, S));
     if (opt.line_segment > 0) p.S = opt.line_segment;
     p.tl = make_tiling(nd, (int64_t)p.S * p.L, opt.part, opt.parts);
     p.grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(p.tl.tiles * (uint64_t)v.batch, slots));

@@ -222,6 +222,12 @@ uint64_t rqa_launch_count(void);
  *                 over all parts, in place, ordered on `stream` (e.g. ncclAllReduce(ncclUint64, ncclSum), or
  *                 torch.distributed.all_reduce on a tensor wrapping the pointer); return 0 on success.  Every part
  *                 makes the same sequence of reduce calls with the same n.
+ *   ev_kernel_begin, ev_kernel_end
+ *                 measurement hooks (NULL = none): two cudaEvent_t created by the caller, recorded on `stream` just before
+ *                 and just after the launch(es) of the call's dominant kernel — the counting pass over all cells of
+ *                 rqa_eps_for_rr (first group of 32 targets), the diagonal scan of rqa_line_hist (first group of 32
+ *                 thresholds) — so that a caller can time that kernel alone without a profiler.  Not recorded when the call
+ *                 takes a path without that kernel (small P, strided fallback).
  */
 typedef int (*rqa_reduce_fn)(void* ctx, uint64_t* d_counters, size_t n, void* stream);
 typedef struct rqa_options {
@@ -235,6 +241,8 @@ typedef struct rqa_options {
     int64_t cand_cap;
     rqa_reduce_fn reduce;
     void* reduce_ctx;
+    void* ev_kernel_begin;
+    void* ev_kernel_end;
 } rqa_options;
 
 rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_options* opt, size_t* bytes);

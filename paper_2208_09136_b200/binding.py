@@ -46,13 +46,15 @@ class RqaOptions(ctypes.Structure):
     _fields_ = [("select_path", ctypes.c_int32), ("line_chunk", ctypes.c_int32), ("line_segment", ctypes.c_int32),
                 ("part_index", ctypes.c_int32), ("part_count", ctypes.c_int32), ("line_buffers", ctypes.c_int32),
                 ("sample_size", ctypes.c_int64), ("cand_cap", ctypes.c_int64), ("reduce", REDUCE_FN),
-                ("reduce_ctx", ctypes.c_void_p)]
+                ("reduce_ctx", ctypes.c_void_p), ("ev_kernel_begin", ctypes.c_void_p), ("ev_kernel_end", ctypes.c_void_p)]
 
 
 def make_options(select_path=0, line_chunk=0, line_segment=0, line_buffers=0, sample_size=0, cand_cap=0, part_index=0,
-                 part_count=0, reduce=None) -> RqaOptions:
+                 part_count=0, reduce=None, kernel_events=None) -> RqaOptions:
     """reduce: a Python callable (d_ptr: int, n: int, stream: int) -> None that sums n uint64 device counters over the
-    parts of a split call (see parts.py); kept alive by the returned struct."""
+    parts of a split call (see parts.py); kept alive by the returned struct.
+    kernel_events: a pair of torch.cuda.Event(enable_timing=True) that the call records just before / after its dominant
+    kernel (rqa_options.ev_kernel_begin / ev_kernel_end)."""
     o = RqaOptions()
     o.select_path, o.line_chunk, o.line_segment, o.line_buffers = select_path, line_chunk, line_segment, line_buffers
     o.sample_size, o.cand_cap, o.part_index, o.part_count = sample_size, cand_cap, part_index, part_count
@@ -67,6 +69,11 @@ def make_options(select_path=0, line_chunk=0, line_segment=0, line_buffers=0, sa
                 return 1
         o._cb = REDUCE_FN(_cb)
         o.reduce = o._cb
+    if kernel_events is not None:
+        a, b = kernel_events
+        a.record(); b.record()                               # torch creates the cudaEvent_t lazily, on the first record
+        o._events = (a, b)
+        o.ev_kernel_begin, o.ev_kernel_end = a.cuda_event, b.cuda_event
     return o
 
 

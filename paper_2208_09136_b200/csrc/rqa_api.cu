@@ -37,6 +37,8 @@ rqa_status make_options(const rqa_options* in, Options* out, const char* who) {
     out->part = in->part_count > 1 ? in->part_index : 0;
     out->reduce = in->reduce;
     out->reduce_ctx = in->reduce_ctx;
+    out->ev_begin = in->ev_kernel_begin;
+    out->ev_end = in->ev_kernel_end;
     return RQA_OK;
 }
 

@@ -47,6 +47,8 @@ struct Options {
     int64_t cand_cap = 0;     // bracket path: candidate capacity per series
     rqa_reduce_fn reduce = nullptr;
     void* reduce_ctx = nullptr;
+    void* ev_begin = nullptr;  // cudaEvent_t recorded just before / after the call's dominant kernel (bench.py's roofline)
+    void* ev_end = nullptr;
 };
 rqa_status make_options(const rqa_options* in, Options* out, const char* who);
 

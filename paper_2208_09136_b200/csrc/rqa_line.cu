@@ -200,9 +200,13 @@ struct ScanArgs {
 // initial entry (0, start 0) stands for "recurrent since the chunk start" (prefix runs; start 0 marks them).
 // Per cell the state changes only when A changes: a higher level pops the entries it ends (one line length for a
 // whole range of thresholds -> D[lo][len]++, D[hi][len]--), a lower A pushes one entry.  Cost independent of K.
+// The (3,1) ring with more than 10 thresholds (one window set, plain staging) reads the i-side window four elements per load.
+template <int M, int TAU, int NP>
+__host__ __device__ constexpr bool scan_vec() { return M == 3 && TAU == 1 && NP > 5; }
+
 template <int NORM, int M, int TAU, int NP, bool MULTI>
-struct Scanner : CellDist<NORM, M, TAU, 2> {
-    using CD = CellDist<NORM, M, TAU, 2>;
+struct Scanner : CellDist<NORM, M, TAU, 2, scan_vec<M, TAU, NP>()> {
+    using CD = CellDist<NORM, M, TAU, 2, scan_vec<M, TAU, NP>()>;
     static constexpr int S = CD::S;
     using SM = ScanSmem<NP>;
 
@@ -439,6 +443,7 @@ __device__ __forceinline__ void scan_chunk(Scanner<NORM, M, TAU, NP, MULTI>& sc,
 template <int NORM, int M, int TAU, int NP>
 __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanArgs a) {
     using SM = ScanSmem<NP>;
+    constexpr bool VECK = scan_vec<M, TAU, NP>();              // vector loads of the i-side window: one set, plain staging
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_q;
     __shared__ unsigned int s_item;
@@ -486,7 +491,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
         const int64_t ga = (y - a.v.data) + sa, gb = (y - a.v.data) + sb;      // float offsets from the batch base
         sha = (int)(((uintptr_t)(a.v.data + ga) >> 2) & 3);
         shb = (int)(((uintptr_t)(a.v.data + gb) >> 2) & 3);
-        return a.nbuf == 2 && ga - sha >= 0 && gb - shb >= 0 && ga - sha + LA <= extent && gb - shb + LB <= extent &&
+        return !VECK && a.nbuf == 2 && ga - sha >= 0 && gb - shb >= 0 && ga - sha + LA <= extent && gb - shb + LB <= extent &&
                (((uintptr_t)a.v.data) & 3) == 0;
     };
 
@@ -541,8 +546,10 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
                 mbar_wait(bar0 + 8 * u, (parity >> u) & 1u);
                 parity ^= 1u << u;
             } else {
-                sha = shb = 0;
-                stage_windows(y, ny, (s - 2) * ps, (s - 2 + o0) * ps, ya_s, LA, yb_s, LB);
+                // VECK: the element pushed by the first cell of a super-step (window index 12k + 2) is 16-byte aligned
+                sha = VECK ? 2 : 0;
+                shb = 0;
+                stage_windows(y, ny, (s - 2) * ps, (s - 2 + o0) * ps, ya_s + sha, LA - 4, yb_s, LB);
                 __syncthreads();
             }
             const int sha_c = sha, shb_c = shb;
@@ -834,6 +841,7 @@ LinePlan make_plan(const View& v, int K, const Options& opt) {
     // or the second block (49 ms) against 34.5 ms with one set — the other block of the SM hides the staging)
     p.nbuf = p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, 2) <= budget ? 2 : 1;
     if (opt.line_buffers > 0) p.nbuf = opt.line_buffers;
+    if (v.ps == 1 && v.m == 3 && v.cs == 1 && p.NP > 5) p.nbuf = 1;   // the instantiations with vector loads (scan_vec)
     // wide points: the two windows hold (2L + 512) points, so the chunk shrinks until they fit (one block per SM then)
     while (p.scan && scan_smem_bytes(p.NP, p.L, p.span, ps, p.nbuf) > SMEM_PER_BLOCK_MAX) {
         if (p.nbuf == 2) p.nbuf = 1;
@@ -968,8 +976,10 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
         a.groups = w.groups; a.seg_start = w.seg_start; a.hist = (unsigned long long*)d_hist; a.agg = w.agg;
         a.pre = w.pre; a.suf = w.suf; a.carry = w.carry; a.counter = w.counters + g; a.segs = (uint32_t)p.tl.tiles;
         a.m = v.m; a.tau = (int)v.cs;
+        if (g == 0 && opt.ev_begin) RQA_CUDA_TRY(cudaEventRecord((cudaEvent_t)opt.ev_begin, s));
         rqa_status st = norm == RQA_NORM_MAX ? dispatch_pairs<RQA_NORM_MAX>(a, p, s) : dispatch_pairs<RQA_NORM_EUCLID>(a, p, s);
         if (st != RQA_OK) return st;
+        if (g == 0 && opt.ev_end) RQA_CUDA_TRY(cudaEventRecord((cudaEvent_t)opt.ev_end, s));
         StitchArgs sa;
         sa.n = v.n; sa.w = v.w; sa.T = p.tl.T; sa.g = g; sa.NG = p.NG; sa.K = K; sa.NP = p.NP;
         sa.part = opt.part; sa.parts = opt.parts; sa.n_obl = p.tl.n_obl;

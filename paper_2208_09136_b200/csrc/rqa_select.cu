@@ -406,9 +406,13 @@ struct CountSmem {
     __host__ __device__ static constexpr int col_words(int fields) { return (LW + fields - 1) / fields; }
 };
 
+// The (3,1) ring reads the i-side window four elements per load (CellDist VEC).
+template <int M, int TAU>
+__host__ __device__ constexpr bool count_vec() { return M == 3 && TAU == 1; }
+
 template <int NORM, int M, int TAU, bool MULTI>
-struct Counter : CellDist<NORM, M, TAU, 0> {
-    using CD = CellDist<NORM, M, TAU, 0>;
+struct Counter : CellDist<NORM, M, TAU, 0, count_vec<M, TAU>()> {
+    using CD = CellDist<NORM, M, TAU, 0, count_vec<M, TAU>()>;
     uint32_t lut, beta, kind;         // shared-window addresses of the bucket table, the boundaries, the level kinds
     uint32_t cols;                    // ... of this thread's column, level 0
     uint32_t col_row;                 // bytes between the levels of a column
@@ -481,10 +485,13 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     uint32_t* cols_s = (uint32_t*)(smem + CountSmem::off_cols);
     const int span = M > 0 ? (M - 1) * TAU : (a.m - 1) * a.tau;
     const int ps = M > 0 ? 1 : (int)a.v.ps;
-    const int LA = window_la(a.L, span, 0, ps), LB = window_lb(a.L, span, 0, ps);
+    constexpr bool VECK = count_vec<M, TAU>();
+    const int LA = window_la(a.L, span, 0, ps) + 4, LB = window_lb(a.L, span, 0, ps);   // 4 floats of slack: alignment
     const int col_words = CountSmem::col_words(fields), field_bits = fields == 2 ? 16 : 10;
-    float* ya_s = (float*)(smem + CountSmem::off_cols + nlev * 4 * col_words);
+    float* ya_s = (float*)(smem + ((CountSmem::off_cols + nlev * 4 * col_words + 15) & ~15));
     float* yb_s = ya_s + LA;
+    // VECK: the element pushed by the first cell of a super-step (window index 12k + 2) is 16-byte aligned
+    const int sha = VECK ? 2 : 0;
     for (int q = tid; q < NBS; q += LW) lut_s[q] = T.lut[q];
     if (tid < NCUT) { beta_s[tid] = T.beta[tid]; ((uint8_t*)(smem + CountSmem::off_kind))[tid] = T.kind[tid]; }
     for (int q = tid; q < nlev * col_words; q += LW) cols_s[q] = 0;
@@ -496,7 +503,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     const int64_t o0 = a.v.w + (int64_t)LW * ob;
     const int64_t s = (int64_t)c * L;
     const float* y = a.v.data + (int64_t)b * a.v.bs;
-    stage_windows(y, (n - 1) * ps + span + 1, s * ps, (s + o0) * ps, ya_s, LA, yb_s, LB);
+    stage_windows(y, (n - 1) * ps + span + 1, s * ps, (s + o0) * ps, ya_s + sha, LA - 4, yb_s, LB);
     __syncthreads();
 
     const int64_t len = n - (o0 + tid);
@@ -512,7 +519,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
             ct.m = a.m;
             ct.tau = a.tau;
             ct.ps = ps;
-            ct.seek(smem_addr(ya_s), pin(smem_addr(yb_s) + 4 * tid * ps), 0);
+            ct.seek(smem_addr(ya_s) + 4 * sha, pin(smem_addr(yb_s) + 4 * tid * ps), 0);
             ct.lut = pin(smem_addr(lut_s) - 8u * BUCKET_MAGIC_BITS);   // indexed with 8 * bucket_bits()
             ct.beta = smem_addr(beta_s);
             ct.kind = smem_addr(smem + CountSmem::off_kind);
@@ -528,7 +535,7 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
             ct.wcount = 0;
             ct.lane_lt = (1u << (tid & 31)) - 1u;
             ct.prime();
-            constexpr int U = S == 3 ? 6 : (S > 3 ? S : 4);   // cells per super-step, a multiple of S
+            constexpr int U = S == 3 ? 12 : (S > 3 ? S : 4);  // cells per super-step, a multiple of S (and of 4 with vector loads)
             using Seq = std::make_integer_sequence<int, U>;
             int t = 0;
             for (; t + U <= cnt_lo; t += U) { ct.template superstep<false>(t, cnt, Seq{}); ct.advance(U); }
@@ -800,8 +807,8 @@ struct SelectPlan {
 };
 
 size_t count_smem_bytes(int nlev, int fields, int L, int span, int ps) {
-    return (size_t)CountSmem::off_cols + (size_t)nlev * 4 * CountSmem::col_words(fields) +
-           4 * ((size_t)window_la(L, span, 0, ps) + window_lb(L, span, 0, ps));
+    return (((size_t)CountSmem::off_cols + (size_t)nlev * 4 * CountSmem::col_words(fields) + 15) & ~(size_t)15) +
+           4 * ((size_t)window_la(L, span, 0, ps) + 4 + window_lb(L, span, 0, ps));
 }
 constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of sm_100a, minus the static part
 
@@ -1020,9 +1027,11 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
             a.tile_start = w.tile_start; a.tabs = w.tabs; a.ss = w.ss;
             a.cand = w.cand; a.cap = p.cap; a.m = v.m; a.tau = (int)v.cs;
             const int nlev = 2 * kc + 1;
+            if (base == 0 && opt.ev_begin) RQA_CUDA_TRY(cudaEventRecord((cudaEvent_t)opt.ev_begin, s));
             st = norm == RQA_NORM_MAX ? dispatch_count<RQA_NORM_MAX>(a, p, nlev, v.batch, s)
                                       : dispatch_count<RQA_NORM_EUCLID>(a, p, nlev, v.batch, s);
             if (st != RQA_OK) return st;
+            if (base == 0 && opt.ev_end) RQA_CUDA_TRY(cudaEventRecord((cudaEvent_t)opt.ev_end, s));
             sel_local_kernel<<<(v.batch + 63) / 64, 64, 0, s>>>(w.ss, v.batch, p.cap);
             RQA_LAUNCH_CHECK();
             // a split call: the level counts (and candidate totals) of all parts, per series

@@ -81,6 +81,7 @@ __device__ __forceinline__ unsigned long long pin64(unsigned long long x) { retu
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return pin((uint32_t)__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void lds_f32_u32(uint32_t a, float& x, uint32_t& y) { asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=f"(x), "=r"(y) : "r"(a)); }
+__device__ __forceinline__ void lds_v4f(uint32_t a, float& x, float& y, float& z, float& w) { asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(a)); }
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ uint32_t lds_u16(uint32_t a) { uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ uint32_t lds_u8(uint32_t a) { uint32_t v; asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
@@ -147,10 +148,15 @@ __device__ __forceinline__ void stage_windows(const float* __restrict__ y, int64
 // S = (M-1)*TAU + 1 elements.  M == 0: run-time (m, tau), recomputed from the windows for every cell.
 // The two window addresses are CURSORS: they point at the element of the first cell of the current super-step
 // (seek / advance), so that every access inside a super-step is cursor + a compile-time offset.
-template <int NORM, int M, int TAU, int W>
+// VEC (register-ring variants only): the i-side window is read four elements per load (all lanes read the same
+// address: one broadcast wavefront instead of four).  The caller places the window so that the element pushed by the first
+// cell of a super-step (cursor + S - 1) is 16-byte aligned, and uses super-steps of a multiple of 4 cells.
+template <int NORM, int M, int TAU, int W, bool VEC = false>
 struct CellDist {
     static constexpr int S = M > 0 ? (M - 1) * TAU + 1 : 1;
+    static_assert(!VEC || M > 0, "vector loads belong to the register-ring variants");
     float ring[S];
+    float ya4[VEC ? 4 : 1];     // VEC: the four i-side elements of the current group of cells
     uint32_t ya;                // shared-window address of the i-side window element of cell t0
     uint32_t yb;                // ... of the j-side window, already offset by the thread's diagonal
     int m, tau;                 // M == 0: run-time dimension and coordinate stride (floats)
@@ -178,7 +184,13 @@ struct CellDist {
     // R = offset of the cell from the cursor = its ring phase (static); pushes e_{t+S-1}
     template <int R>
     __device__ __forceinline__ void push() {
-        if (M > 0) ring[(R + S - 1) % S] = elem(R + S - 1);
+        if (M > 0 && VEC) {
+            if (R % 4 == 0) lds_v4f(ya + 4 * (R + S - 1), ya4[0], ya4[1], ya4[2], ya4[3]);
+            float diff = __fsub_rn(ya4[R % 4], lds_f32(yb + 4 * (R + S - 1)));
+            ring[(R + S - 1) % S] = NORM == RQA_NORM_MAX ? diff : __fmul_rn(diff, diff);
+        } else if (M > 0) {
+            ring[(R + S - 1) % S] = elem(R + S - 1);
+        }
     }
     template <int R>
     __device__ __forceinline__ float distance() const {

@@ -262,6 +262,36 @@ def config5(N: int = 20000, n_snr: int = 8, n_seeds: int = 4) -> Workload:
     return Workload(f"config5_batch_N{N}", np.stack(rows), 5, 2, NORM_MAX, rr_log(32, 0.0005, 0.3), (2, 3), labels)
 
 
+def paper_group(signal: str, level: float, N: int, n_real: int = 10, K: int = 99) -> Workload:
+    """One cell of the paper's 3 x 3 x 4 grid: one dynamics at one SNR level and one length, i.e. the
+    10 SNRs level*{0.1, 0.2, .., 1.0} ("SNR L. level") x n_real realisations of the noise = 10*n_real series, row
+    index = realisation*10 + snr_index, ascending SNR.  Here SNR is the paper's VARIANCE ratio:
+    sigma_noise = sigma_signal / sqrt(SNR).  Dynamics as in PAPER.md:103-115: sine with 25 cycles over the series,
+    logistic map at r = 3.679 (band merging, frequent laminar states), Lorenz x (RK4, dt = 0.01) embedded with m = 3,
+    tau = 3; the other two are not embedded (m = 1).  RR_k = k/100, k = 1..K (RR* in 1..99 percent).
+    The clean series is the same for the whole group; only the noise differs between rows."""
+    sig = {"sine": SIG_SINE, "logistic": SIG_LOGISTIC, "lorenz": SIG_LORENZ}[signal]
+    base = make_seed(6, sig, 0, 0) + 7919 * int(round(math.log10(N))) + 104729 * int(round(10 * math.log10(level) + 20))
+    if sig == SIG_SINE:
+        clean = np.sin(2.0 * math.pi * 25.0 * np.arange(N, dtype=np.float64) / N)
+        m, tau = 1, 1
+    elif sig == SIG_LOGISTIC:
+        clean = logistic_signal(N, base, r=3.679)
+        m, tau = 1, 1
+    else:
+        clean = lorenz_signal(N, every=1)
+        m, tau = 3, 3
+    rows, labels = [], []
+    for real in range(n_real):
+        for si in range(10):
+            snr = level * (si + 1) / 10.0
+            seed = base + 1000003 * (real + 1) + 10 * si
+            rows.append(add_noise(clean, math.sqrt(snr), seed))
+            labels.append(_label(sig, snr, seed))
+    return Workload(f"paper_group_{signal}_snrL{level:g}_N{N}_x{10 * n_real}", np.stack(rows), m, tau, NORM_MAX,
+                    rr_linear(K), (2,), labels)
+
+
 def fnv1a64(a: np.ndarray) -> int:
     """FNV-1a-64 checksum of an array's bytes (logged with results so runs can be matched)."""
     h = 0xCBF29CE484222325

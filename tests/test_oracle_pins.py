@@ -478,3 +478,85 @@ def test_theiler_window_brute_force(oracle, w):
     assert np.array_equal(oracle.line_measures(hist, 2, theiler=w)[2], rrr)      # RR from the histogram, over P_w
     if w == 1:
         assert np.array_equal(hist, oracle.line_hist(y, m, tau, eps, oracle.NORM_MAX))
+
+
+# ------------------------------------------------------------------ vertical lines (reading S19; LAM, TT)
+VGOLDEN = Path(__file__).resolve().parent / "golden" / "hand_cases_vertical.txt"
+
+
+def _vertical_cases():
+    cases = []
+    for line in VGOLDEN.read_text().splitlines():
+        if not line.strip() or line.startswith("#"):
+            continue
+        name, y, m, tau, norm, eps, w, hist, lam, tt = [f.strip() for f in line.split("|")]
+        h = {int(a): int(b) for a, b in (t.split(":") for t in hist.split(","))}
+        cases.append(pytest.param(np.array(y.split(), dtype=np.float32), int(m), int(tau), NORMS[norm], np.float32(float(eps)),
+                                  int(w), h, Fraction(*map(int, lam.split("/"))), Fraction(*map(int, tt.split("/"))), id=name))
+    return cases
+
+
+@pytest.mark.parametrize("y,m,tau,norm,eps,w,hist,lam,tt", _vertical_cases())
+def test_vertical_hand_enumerated(oracle, y, m, tau, norm, eps, w, hist, lam, tt):
+    vh = oracle.vert_hist(y, m, tau, [eps], norm, theiler=w)
+    got = {int(v): int(c) for v, c in enumerate(vh[0]) if c}
+    assert got == hist
+    L, T = oracle.lam_tt(vh, 2)
+    assert abs(L[0] - float(lam)) <= 1e-15 and abs(T[0] - float(tt)) <= 1e-15
+
+
+def _numpy_vertical(y, m, tau, norm, eps, w):
+    """Independent run count on the FULL matrix: every column as a string of 0/1 split at the zeros."""
+    D = _numpy_condensed_full(y, m, tau, norm)
+    n = D.shape[0]
+    i, j = np.indices((n, n))
+    R = (D <= eps) & (np.abs(i - j) >= w)
+    h = np.zeros(n, dtype=np.uint64)
+    for col in range(n):
+        for run in "".join("1" if x else "0" for x in R[:, col]).split("0"):
+            if run:
+                h[len(run)] += 1
+    return h
+
+
+def _numpy_condensed_full(y, m, tau, norm):
+    n = len(y) - (m - 1) * tau
+    X = np.stack([y[c * tau: c * tau + n] for c in range(m)], axis=1).astype(np.float32)
+    diff = X[:, None, :] - X[None, :, :]
+    if norm == 0:
+        return np.abs(diff).max(axis=2)
+    sq = diff * diff
+    s = sq[:, :, 0]
+    for c in range(1, m):
+        s = s + sq[:, :, c]
+    return np.sqrt(s)
+
+
+@pytest.mark.parametrize("m,tau,N,w,norm", [(1, 1, 60, 1, 0), (3, 1, 90, 1, 0), (2, 3, 77, 4, 0), (3, 2, 64, 1, 1), (4, 1, 50, 46, 0)])
+def test_vertical_brute_force_full_matrix(oracle, m, tau, N, w, norm):
+    y = np.round(wl.gaussian(500 + N, N) * 4).astype(np.float32) / 4       # quantised: ties and long runs
+    eps = np.array([0.0, 0.5, 1.25, 3.0], dtype=np.float32)
+    vh = oracle.vert_hist(y, m, tau, eps, norm, theiler=w)
+    for k, e in enumerate(eps):
+        assert np.array_equal(vh[k], _numpy_vertical(y, m, tau, norm, e, w))
+    # threads change nothing
+    assert np.array_equal(vh, oracle.vert_hist(y, m, tau, eps, norm, threads=0, theiler=w))
+
+
+def test_vertical_sum_is_twice_the_pair_count_and_ramp_closed_form(oracle):
+    # every recurrent pair (i<j) is one cell of column j and one of column i: sum_v v*P(v) = 2*C  (PAPER.md:57, symmetry)
+    y = wl.logistic_signal(400, seed=77).astype(np.float32)
+    r = oracle.sweep(y, 3, 1, wl.rr_linear(10), 0, 2)
+    vh = oracle.vert_hist(y, 3, 1, r["eps"], 0)
+    v = np.arange(vh.shape[1], dtype=np.uint64)
+    assert np.array_equal((vh * v).sum(axis=1), 2 * r["count"])
+    # ramp y_i = i, max norm, eps = q: column j has a run of min(j, q) cells above the diagonal and min(n-1-j, q) below
+    n, q = 57, 5
+    ramp = np.arange(n, dtype=np.float32)
+    vh = oracle.vert_hist(ramp, 1, 1, np.array([q], dtype=np.float32), 0)[0]
+    expect = np.zeros(n, dtype=np.uint64)
+    for j in range(n):
+        for run in (min(j, q), min(n - 1 - j, q)):
+            if run:
+                expect[run] += 1
+    assert np.array_equal(vh, expect)

@@ -601,3 +601,31 @@ def test_theiler_window(rqa, oracle, options, path):
     with pytest.raises(rqa.RqaError):
         bad = rqa.rqa_embed(torch.zeros(50, device="cuda"), 1, 1, theiler=50)
         rqa.rqa_workspace_bytes(bad, 3, _OPT["o"])
+
+
+# ------------------------------------------------ ONE call split over several parts
+@pytest.mark.parametrize("parts,path,norm,theiler", [(2, 0, 0, 0), (3, 2, 0, 0), (2, 3, 1, 0), (2, 1, 0, 0), (4, 2, 1, 5)])
+def test_split_call_every_part_holds_the_oracle_result(rqa, oracle, parts, path, norm, theiler):
+    """rqa_options.part_index / part_count: each part visits its share of the tiles (diagonal blocks dealt round
+    robin) of BOTH passes and the exact integer counters are summed by the reduce callback.  Here the parts are threads
+    on one GPU that take turns (parts.LocalParts: host barriers, no kernel waits on another); with one process per GPU
+    the same callback slot takes parts.dist_reduce (NCCL all-reduce).  Every part must end with the complete,
+    bit-exact eps_k, C_k, RR_k, P_k(l)."""
+    import torch
+    from paper_2208_09136_b200 import binding as B, parts as P
+    N, m, tau = (1500 if path == 1 else 5200), 3, 2
+    series = np.stack([wl.add_noise(wl.lorenz_signal(N), 1.0, 4242), wl.add_noise(wl.logistic_signal(N, seed=5), 0.5, 4243)])
+    series = series.astype(np.float32)
+    rr = wl.rr_log(12, 0.002, 0.25)
+    dev = torch.as_tensor(series).cuda()
+    local = P.LocalParts(parts)
+
+    def one_part(p, reduce, stream):
+        opt = B.make_options(select_path=path, part_index=p, part_count=parts, reduce=reduce, line_chunk=97)
+        buf = rqa.averaged_rqa(dev, m, tau, rr, norm, 2, theiler=theiler, options=opt)
+        return {"eps": buf.eps.cpu().numpy(), "count": buf.count.cpu().numpy().view(np.uint64), "rr": buf.rr.cpu().numpy(),
+                "hist": buf.hist.cpu().numpy().view(np.uint64), "det": buf.det.cpu().numpy(), "det_mean": buf.det_mean.cpu().numpy()}
+    results = local.run(one_part)
+    assert local.reduce_calls > 0
+    for g in results:
+        assert_parity(oracle, g, series, m, tau, rr, norm, theiler=max(1, theiler))

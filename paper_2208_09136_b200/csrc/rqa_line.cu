@@ -353,6 +353,43 @@ struct Scanner : CellDist<NORM, M, TAU, 2, scan_vec<M, TAU, NP>()> {
         w2b = w2a; w2a = w2;
     }
 
+    // Phase 1 walks the cells in GROUPS of up to four: first the loads and the level of every cell of the group
+    // (independent dependency chains that the hardware overlaps: no atomic or store sits between their shared-memory
+    // loads, which ptxas would otherwise have to keep in program order), then the aggregates and the event queue.
+    template <int R>
+    __device__ __forceinline__ uint32_t level_of_cell() {
+        CD::template push<R>();
+        return level4(CD::template distance<R>());
+    }
+    template <int R>
+    __device__ __forceinline__ void account(uint32_t v4) {
+        const uint32_t w2 = max(v4, v1), w3 = max(w2, v2);
+        red_u32(agg + v4 * (SM::agg_row / 4), 1u);
+        red_u32(agg + w2 * (SM::agg_row / 4), 1u << 10);
+        red_u32(agg + w3 * (SM::agg_row / 4), 1u << 20);
+        const uint32_t a_new = max(w2, w2b);
+        if (a_new != aprev) {
+            sts_u16(qp, a_new + trel8 + ((uint32_t)R << 8));
+            qp += SM::stk_row;
+        }
+        aprev = a_new;
+        v2 = v1; v1 = v4;
+        w2b = w2a; w2a = w2;
+    }
+    template <int R0, int... Q>
+    __device__ __forceinline__ void group(std::integer_sequence<int, Q...>) {
+        const uint32_t v[sizeof...(Q)] = {level_of_cell<R0 + Q>()...};
+        (account<R0 + Q>(v[Q]), ...);
+    }
+    template <int R0, int U>
+    __device__ __forceinline__ void groups() {
+        if constexpr (R0 < U) {
+            constexpr int G = U - R0 >= 4 ? 4 : U - R0;
+            group<R0>(std::make_integer_sequence<int, G>{});
+            groups<R0 + G, U>();
+        }
+    }
+
     // Replay the queued events of the window that started at cell win_t0 (call with the warp converged).
     __device__ __forceinline__ void drain(uint32_t win_t0) {
         const uint32_t nmax = __reduce_max_sync(FULL, qp - q0);
@@ -373,7 +410,8 @@ struct Scanner : CellDist<NORM, M, TAU, 2, scan_vec<M, TAU, NP>()> {
 
     template <int PHASE, int... R>
     __device__ __forceinline__ void superstep(int t, int cnt, int ds, std::integer_sequence<int, R...>) {
-        (cell<R, PHASE>(t + R, cnt, ds), ...);
+        if constexpr (PHASE == 1) groups<0, (int)sizeof...(R)>();
+        else (cell<R, PHASE>(t + R, cnt, ds), ...);
         CD::advance((int)sizeof...(R));
         if (PHASE == 1) trel8 += (uint32_t)sizeof...(R) << 8;
     }

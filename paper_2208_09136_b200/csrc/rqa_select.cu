@@ -463,9 +463,54 @@ struct Counter : CellDist<NORM, M, TAU, 0, count_vec<M, TAU>()> {
             wcount += nc;
         }
     }
+    // The unguarded bulk of a chunk walks the cells in GROUPS of up to four: first the loads and the level of every cell
+    // of the group (independent dependency chains that the hardware overlaps: no atomic or store sits between their
+    // shared-memory loads, which ptxas would otherwise have to keep in program order), then the counter increments, and
+    // one vote per group decides whether any lane holds a candidate.
+    template <int R>
+    __device__ __forceinline__ uint32_t classify(float& d) {
+        CD::template push<R>();
+        d = CD::template distance<R>();
+        float er;
+        uint32_t q;
+        lds_f32_u32(lut + 8 * bucket_bits(d, dcap, scale), er, q);
+        q += d > er ? 0x40000001u : 0u;                       // bit 31: the cell's level is a candidate level (see cell())
+        if (MULTI) {
+            q &= 0xffffu;
+            while (d > lds_f32(beta + 4 * q)) ++q;
+            q |= lds_u8(kind + q) == LEVEL_CAND ? 0x80000000u : 0u;
+        }
+        return q;
+    }
+    __device__ __forceinline__ void append(float d, uint32_t q) {
+        const bool cand = (int32_t)q < 0;
+        const unsigned mc = __ballot_sync(FULL, cand);
+        if (mc) {
+            const uint32_t nc = __popc(mc);
+            if (wcount + nc > (uint32_t)WCAP) flush_warp();
+            if (cand) wbuf[wcount + __popc(mc & lane_lt)] = d;
+            wcount += nc;
+        }
+    }
+    template <int R0, int... Q>
+    __device__ __forceinline__ void group(std::integer_sequence<int, Q...>) {
+        float d[sizeof...(Q)];
+        const uint32_t q[sizeof...(Q)] = {classify<R0 + Q>(d[Q])...};
+        (red_u32(cols + q[Q] * col_row, inc), ...);          // col_row is a multiple of 4: bits 30-31 of q drop out
+        if (__any_sync(FULL, (int32_t)(q[Q] | ...) < 0)) (append(d[Q], q[Q]), ...);
+    }
+    template <int R0, int U>
+    __device__ __forceinline__ void groups() {
+        if constexpr (R0 < U) {
+            constexpr int G = U - R0 >= 4 ? 4 : U - R0;
+            group<R0>(std::make_integer_sequence<int, G>{});
+            groups<R0 + G, U>();
+        }
+    }
     template <bool GUARD, int... R>
     __device__ __forceinline__ void superstep(int t, int cnt, std::integer_sequence<int, R...>) {
-        (cell<R, GUARD>(t + R, cnt), ...);
+        if constexpr (GUARD) (cell<R, GUARD>(t + R, cnt), ...);
+        else groups<0, (int)sizeof...(R)>();
     }
 };
 

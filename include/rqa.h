@@ -88,7 +88,7 @@ const char* rqa_last_error(void);
 const char* rqa_version(void);
 
 /*
- * Bytes of device workspace that rqa_eps_for_rr / rqa_line_hist need for this shape (the larger of the two).
+ * Bytes of device workspace that rqa_eps_for_rr / rqa_line_hist / rqa_vert_hist need for this shape (the largest).
  * The workspace is scratch: its contents need not survive between calls, except that rqa_workspace_status()
  * reads the status block the last call wrote.  It must be 256-byte aligned.
  */
@@ -168,6 +168,30 @@ rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, i
                              void* stream);
 
 /*
+ * Vertical-line histograms at K thresholds ("this approach can also be applied for other RQA measures": the
+ * vertical-line measures laminarity and trapping time; the paper defines none itself, reading S19).
+ *   d_vhist  [batch][K][n_points] uint64, overwritten: d_vhist[b][k][v] = number of maximal runs of exactly v recurrent
+ *            cells (d <= eps_k) down the columns of the FULL symmetric N' x N' matrix.  The cells with
+ *            |i - j| < w (w = 1: the main diagonal; w = pts->theiler > 1: the Theiler window) are not recurrent and split
+ *            a column in two; runs touching the border of the plot or that band count with their truncated length.
+ * Every recurrent pair i<j lies in column j and in column i: sum_v v*d_vhist[b][k][v] == 2*C_k.
+ * Arguments, workspace (rqa_workspace_bytes covers it) and errors as rqa_line_hist; N'^2 cells are visited.
+ */
+rqa_status rqa_vert_hist(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_vhist,
+                         void* d_ws, size_t ws_bytes, void* stream);
+
+/*
+ * Laminarity and trapping time from the vertical-line histogram (the definitions of the paper's ref. [2], which
+ * PAPER.md:86 points to; not written out in the paper):
+ *   d_lam  [batch][K]  LAM_k = sum_{v>=v_min} v*P_k(v) / sum_{v>=1} v*P_k(v)            (0 if the denominator is 0)
+ *   d_tt   [batch][K]  TT_k  = sum_{v>=v_min} v*P_k(v) / sum_{v>=v_min} P_k(v)          (0 if there is no such line)
+ * Exact uint64 sums, one fp64 division each.  Either output may be NULL.  Their averages over the recurrence rates (Eq. 5
+ * applied to LAM / TT) are rqa_det_prefix_avg on d_lam / d_tt.
+ */
+rqa_status rqa_lam_tt(const uint64_t* d_vhist, int32_t batch, int32_t K, int64_t n_points, int64_t v_min, double* d_lam,
+                      double* d_tt, void* stream);
+
+/*
  * Sorting rate S (Eq. 6), the paper's evaluation score; plain host arithmetic on R*n numbers.
  *   h_measure  HOST [R][n]: the measure (DET or averaged DET) of n series given in their natural order (y_j = j, the
  *              order the measure is expected to increase in), for R realisations
@@ -206,7 +230,7 @@ uint64_t rqa_launch_count(void);
  *                 counting pass, 3 = four radix passes
  *   sample_size   bracket path: number of sampled pair distances per series
  *   cand_cap      bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
- *   line_chunk    rqa_line_hist: chunk length along the diagonals, 1..1023
+ *   line_chunk    rqa_line_hist / rqa_vert_hist: chunk length along the diagonals / columns, 1..1023
  *   line_segment  rqa_line_hist: consecutive chunks of one diagonal block that a block walks with the run state
  *                 carried in place (only segment borders are joined by the stitch kernel), >= 1
  *   line_buffers  rqa_line_hist: 1 = one set of series windows per block, staged by plain loads; 2 = two sets, the next
@@ -250,6 +274,8 @@ rqa_status rqa_eps_for_rr_opt(const rqa_points* pts, rqa_norm norm, const double
                               uint64_t* d_count, double* d_rr_realised, void* d_ws, size_t ws_bytes, void* stream,
                               const rqa_options* opt);
 rqa_status rqa_line_hist_opt(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
+                             void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt);
+rqa_status rqa_vert_hist_opt(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_vhist,
                              void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt);
 
 #ifdef __cplusplus

@@ -28,7 +28,8 @@ RQA_MAX_M = 16
 EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_bytes", "rqa_workspace_status",
            "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
            "rqa_sweep_host", "rqa_launch_count", "rqa_workspace_bytes_opt", "rqa_eps_for_rr_opt", "rqa_line_hist_opt",
-           "rqa_det_prefix_avg", "rqa_line_measures", "rqa_sorting_rate_host"]
+           "rqa_det_prefix_avg", "rqa_line_measures", "rqa_sorting_rate_host", "rqa_vert_hist", "rqa_vert_hist_opt",
+           "rqa_lam_tt"]
 
 
 class RqaPoints(ctypes.Structure):
@@ -120,6 +121,9 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_det_prefix_avg.argtypes = [vp, i32, i32, vp, vp]
     lib.rqa_line_measures.argtypes = [vp, i32, i32, i64, i64, i64, vp, vp, vp, vp, vp]
     lib.rqa_sorting_rate_host.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_double)]
+    lib.rqa_vert_hist.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp]
+    lib.rqa_vert_hist_opt.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp, opt]
+    lib.rqa_lam_tt.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -210,6 +214,25 @@ def rqa_line_hist(pts: RqaPoints, norm: int, eps, hist, ws, stream=None, options
     _check(load_library().rqa_line_hist_opt(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps", bk), K,
                                             _dev(hist, torch.int64, "hist", bk * int(pts.n_points)),
                                             _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream), _opt(options)))
+
+
+def rqa_vert_hist(pts: RqaPoints, norm: int, eps, vhist, ws, stream=None, options: RqaOptions = None) -> None:
+    """eps float32 CUDA [batch][K]; vhist int64 (uint64 bits) CUDA [batch][K][n_points]: vertical-line histograms."""
+    import torch
+    K = eps.shape[-1]
+    bk = int(pts.batch) * K
+    _check(load_library().rqa_vert_hist_opt(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps", bk), K,
+                                            _dev(vhist, torch.int64, "vhist", bk * int(pts.n_points)),
+                                            _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream), _opt(options)))
+
+
+def rqa_lam_tt(vhist, v_min: int, lam=None, tt=None, stream=None) -> None:
+    """vhist int64 CUDA [batch][K][n_points]; lam, tt float64 [batch][K] (either may be None)."""
+    import torch
+    batch, K, n = vhist.shape
+    _check(load_library().rqa_lam_tt(_dev(vhist, torch.int64, "vhist"), batch, K, n, v_min,
+                                     None if lam is None else _dev(lam, torch.float64, "lam", batch * K),
+                                     None if tt is None else _dev(tt, torch.float64, "tt", batch * K), _stream(stream)))
 
 
 def rqa_det_avg(hist, l_min: int, det, det_mean, stream=None) -> None:

@@ -1,6 +1,7 @@
 // rqa_api.cu — the C ABI of librqa.so (include/rqa.h): argument validation, workspace carving, and the
 // small kernels of the path (embedding gather, finite check, DET reduction).  The two heavy steps live in
 // rqa_select.cu (thresholds) and rqa_line.cu (line histograms).
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -185,8 +186,8 @@ rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_o
     st = validate_points(&p, "rqa_workspace_bytes");
     if (st != RQA_OK) return st;
     View v = make_view(p);
-    size_t a = select_workspace_bytes(v, K, o), b = line_workspace_bytes(v, K, o);
-    *bytes = sizeof(WsStatus) + (a > b ? a : b);
+    size_t a = select_workspace_bytes(v, K, o), b = line_workspace_bytes(v, K, o), c = vert_workspace_bytes(v, K, o);
+    *bytes = sizeof(WsStatus) + std::max(a, std::max(b, c));
     return RQA_OK;
 }
 
@@ -290,6 +291,33 @@ rqa_status rqa_line_hist_opt(const rqa_points* pts, rqa_norm norm, const float* 
     st = launch_finite_check(v, status, s);
     if (st != RQA_OK) return st;
     return run_line_hist(v, (int)norm, d_eps, K, d_hist, ws, s, o);
+}
+
+rqa_status rqa_vert_hist(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_vhist,
+                         void* d_ws, size_t ws_bytes, void* stream) {
+    return rqa_vert_hist_opt(pts, norm, d_eps, K, d_vhist, d_ws, ws_bytes, stream, nullptr);
+}
+
+rqa_status rqa_vert_hist_opt(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_vhist,
+                             void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt) {
+    rqa_status st = validate_points(pts, "rqa_vert_hist");
+    if (st != RQA_OK) return st;
+    Options o;
+    st = make_options(opt, &o, "rqa_vert_hist");
+    if (st != RQA_OK) return st;
+    if (norm != RQA_NORM_MAX && norm != RQA_NORM_EUCLID) { set_error("rqa_vert_hist: unknown norm %d", (int)norm); return RQA_ERR_INVALID_ARG; }
+    if (K < 1 || K > RQA_MAX_K) { set_error("rqa_vert_hist: K = %d outside 1..%d", K, RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
+    if (!d_eps || !d_vhist || !d_ws) { set_error("rqa_vert_hist: NULL argument"); return RQA_ERR_INVALID_ARG; }
+    if (((uintptr_t)d_ws & 255) != 0) { set_error("rqa_vert_hist: workspace must be 256-byte aligned"); return RQA_ERR_INVALID_ARG; }
+    View v = make_view(*pts);
+    size_t need = sizeof(WsStatus) + vert_workspace_bytes(v, K, o);
+    if (ws_bytes < need) { set_error("rqa_vert_hist: workspace %zu < %zu bytes", ws_bytes, need); return RQA_ERR_WORKSPACE_TOO_SMALL; }
+    cudaStream_t s = (cudaStream_t)stream;
+    Arena ws(d_ws, ws_bytes);
+    WsStatus* status = ws.take<WsStatus>(1);
+    st = launch_finite_check(v, status, s);
+    if (st != RQA_OK) return st;
+    return run_vert_hist(v, (int)norm, d_eps, K, d_vhist, ws, s, o);
 }
 
 rqa_status rqa_det_avg(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t n_points, int64_t l_min,

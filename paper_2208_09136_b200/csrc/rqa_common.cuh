@@ -131,6 +131,10 @@ size_t line_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws,
                          cudaStream_t s, const Options& opt);
 
+size_t vert_workspace_bytes(const View& v, int K, const Options& opt);
+rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_vhist, Arena& ws,
+                         cudaStream_t s, const Options& opt);
+
 // Number of SMs of the current device (cached per thread; 148 on a B200).
 int sm_count();
 

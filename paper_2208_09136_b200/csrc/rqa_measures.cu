@@ -2,6 +2,7 @@
 //   rqa_det_prefix_avg     Eq. 5 as a curve: the averaged determinism for every cut-off RR*
 //   rqa_line_measures      "the histogram is used for the calculation of (DET, L, L_max and RR)",
 //                          plus the entropy of the line-length distribution (one of the "other RQA measures")
+//   rqa_lam_tt             laminarity and trapping time from the vertical-line histogram
 //   rqa_sorting_rate_host  Eq. 6, the paper's evaluation score (host arithmetic on a few numbers)
 #include "rqa_common.cuh"
 
@@ -64,6 +65,34 @@ __global__ void __launch_bounds__(256) line_measures_kernel(const uint64_t* __re
     }
 }
 
+// One block per (threshold, series): LAM and TT from the vertical-line histogram, exact uint64 sums.
+__global__ void __launch_bounds__(256) lam_tt_kernel(const uint64_t* __restrict__ vhist, int K, int64_t n, int64_t v_min,
+                                                     double* __restrict__ lam, double* __restrict__ tt) {
+    const int k = blockIdx.x, b = blockIdx.y;
+    const uint64_t* row = vhist + ((int64_t)b * K + k) * n;
+    unsigned long long all = 0, num = 0, lines = 0;
+    for (int64_t v = 1 + threadIdx.x; v < n; v += blockDim.x) {
+        const unsigned long long h = row[v];
+        all += (unsigned long long)v * h;
+        if (v >= v_min) { num += (unsigned long long)v * h; lines += h; }
+    }
+    __shared__ unsigned long long s[3][8];
+    for (int off = 16; off; off >>= 1) {
+        all += __shfl_down_sync(0xffffffffu, all, off);
+        num += __shfl_down_sync(0xffffffffu, num, off);
+        lines += __shfl_down_sync(0xffffffffu, lines, off);
+    }
+    if ((threadIdx.x & 31) == 0) { const int w = threadIdx.x >> 5; s[0][w] = all; s[1][w] = num; s[2][w] = lines; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        all = num = lines = 0;
+        for (int w = 0; w < 8; ++w) { all += s[0][w]; num += s[1][w]; lines += s[2][w]; }
+        const int64_t o = (int64_t)b * K + k;
+        if (lam) lam[o] = all ? (double)num / (double)all : 0.0;
+        if (tt) tt[o] = lines ? (double)num / (double)lines : 0.0;
+    }
+}
+
 }  // namespace
 }  // namespace rqa
 
@@ -86,6 +115,15 @@ rqa_status rqa_line_measures(const uint64_t* d_hist, int32_t batch, int32_t K, i
     if (batch < 1 || K < 1 || K > RQA_MAX_K || n_points < 2 || l_min < 1 || theiler < 0 || theiler > n_points - 1) { set_error("rqa_line_measures: need batch >= 1, 1 <= K <= %d, n_points >= 2, l_min >= 1, 0 <= theiler <= n_points-1", RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
     line_measures_kernel<<<dim3(K, batch), 256, 0, (cudaStream_t)stream>>>(d_hist, K, n_points, l_min, theiler > 1 ? theiler : 1, d_L,
                                                                           d_Lmax, d_rr_hist, d_entr);
+    RQA_LAUNCH_CHECK();
+    return RQA_OK;
+}
+
+rqa_status rqa_lam_tt(const uint64_t* d_vhist, int32_t batch, int32_t K, int64_t n_points, int64_t v_min, double* d_lam,
+                      double* d_tt, void* stream) {
+    if (!d_vhist) { set_error("rqa_lam_tt: d_vhist is NULL"); return RQA_ERR_INVALID_ARG; }
+    if (batch < 1 || K < 1 || K > RQA_MAX_K || n_points < 2 || v_min < 1) { set_error("rqa_lam_tt: need batch >= 1, 1 <= K <= %d, n_points >= 2, v_min >= 1", RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
+    lam_tt_kernel<<<dim3(K, batch), 256, 0, (cudaStream_t)stream>>>(d_vhist, K, n_points, v_min, d_lam, d_tt);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }

@@ -95,6 +95,14 @@ def test_line_hist_det_embed_reject_bad_arguments(lib):
     assert lib.rqa_line_hist(ctypes.byref(_pts()), 0, None, 2, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
     assert lib.rqa_line_hist(ctypes.byref(_pts()), 0, FAKE, 0, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
     assert lib.rqa_line_hist(ctypes.byref(_pts()), 0, FAKE, 2, FAKE, FAKE, 8, None) == B.RQA_ERR_WORKSPACE_TOO_SMALL
+    # the vertical-line calls validate the same way (reading S19)
+    assert lib.rqa_vert_hist(ctypes.byref(_pts()), 0, None, 2, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_vert_hist(ctypes.byref(_pts()), 2, FAKE, 2, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG     # unknown norm
+    assert lib.rqa_vert_hist(ctypes.byref(_pts()), 0, FAKE, 129, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_vert_hist(ctypes.byref(_pts()), 0, FAKE, 2, FAKE, FAKE, 8, None) == B.RQA_ERR_WORKSPACE_TOO_SMALL
+    assert lib.rqa_vert_hist(None, 0, FAKE, 2, FAKE, FAKE, 1 << 30, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_lam_tt(None, 1, 2, 100, 2, FAKE, FAKE, None) == B.RQA_ERR_INVALID_ARG
+    assert lib.rqa_lam_tt(FAKE, 1, 2, 100, 0, FAKE, FAKE, None) == B.RQA_ERR_INVALID_ARG
     assert lib.rqa_det_avg(None, 1, 2, 100, 2, FAKE, FAKE, None) == B.RQA_ERR_INVALID_ARG
     assert lib.rqa_det_avg(FAKE, 1, 2, 100, 0, FAKE, FAKE, None) == B.RQA_ERR_INVALID_ARG
     assert lib.rqa_det_avg(FAKE, 0, 2, 100, 2, FAKE, FAKE, None) == B.RQA_ERR_INVALID_ARG

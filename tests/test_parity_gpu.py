@@ -629,3 +629,134 @@ def test_split_call_every_part_holds_the_oracle_result(rqa, oracle, parts, path,
     assert local.reduce_calls > 0
     for g in results:
         assert_parity(oracle, g, series, m, tau, rr, norm, theiler=max(1, theiler))
+
+
+# ----------------------------------------- vertical lines, LAM, TT (reading S19; row f2)
+def gpu_vert(rqa, series, m, tau, eps, norm=0, theiler=0, v_min=2, options=None):
+    import torch
+    from paper_2208_09136_b200 import binding as B
+    s = torch.as_tensor(np.ascontiguousarray(np.atleast_2d(series), dtype=np.float32)).cuda()
+    view = B.rqa_embed(s, m, tau, theiler=theiler)
+    e = torch.as_tensor(np.ascontiguousarray(np.atleast_2d(eps), dtype=np.float32)).cuda()
+    K = e.shape[1]
+    vh = torch.empty((s.shape[0], K, int(view.n_points)), dtype=torch.int64, device="cuda")
+    ws = torch.empty(B.rqa_workspace_bytes(view, K, options), dtype=torch.uint8, device="cuda")
+    B.rqa_vert_hist(view, norm, e, vh, ws, options=options)
+    lam = torch.empty((s.shape[0], K), dtype=torch.float64, device="cuda")
+    tt = torch.empty_like(lam)
+    B.rqa_lam_tt(vh, v_min, lam, tt)
+    B.rqa_workspace_status(ws)
+    return vh.cpu().numpy().view(np.uint64), lam.cpu().numpy(), tt.cpu().numpy()
+
+
+def assert_vert(oracle, got, series, m, tau, eps, norm=0, theiler=1, v_min=2):
+    vh, lam, tt = got
+    series, eps = np.atleast_2d(series), np.atleast_2d(eps)
+    for b in range(series.shape[0]):
+        ov = oracle.vert_hist(series[b], m, tau, eps[b], norm, threads=0, theiler=theiler)
+        if not np.array_equal(vh[b], ov):
+            bad = np.argwhere(vh[b] != ov)
+            k, v = bad[0]
+            raise AssertionError(f"vhist, series {b}: {len(bad)} cells differ, first at k={k} v={v}: gpu {vh[b][k, v]} oracle {ov[k, v]}")
+        ol, ot = oracle.lam_tt(ov, v_min)
+        assert np.max(np.abs(lam[b] - ol)) <= DET_TOL and np.max(np.abs(tt[b] - ot)) <= 1e-9 * max(1.0, np.max(ot))
+
+
+def test_vertical_hand_cases_on_gpu(rqa, oracle):
+    from pathlib import Path
+    for line in (Path(__file__).resolve().parent / "golden" / "hand_cases_vertical.txt").read_text().splitlines():
+        if not line.strip() or line.startswith("#"):
+            continue
+        name, y, m, tau, norm, eps, w, hist, lam, tt = [f.strip() for f in line.split("|")]
+        y = np.array(y.split(), dtype=np.float32)
+        vh, L, T = gpu_vert(rqa, y, int(m), int(tau), [float(eps)], 0, theiler=int(w))
+        got = {int(v): int(c) for v, c in enumerate(vh[0][0]) if c}
+        assert got == {int(a): int(b) for a, b in (t.split(":") for t in hist.split(","))}, name
+        ln, ld = map(int, lam.split("/"))
+        assert abs(L[0][0] - ln / ld) <= 1e-15, name
+
+
+@pytest.mark.parametrize("cfg", ["config1", "config2", "config3max", "config3euclid"])
+def test_vertical_lines_on_baseline_configs(rqa, oracle, cfg):
+    """vhist, LAM and TT at the thresholds rqa_eps_for_rr selects, on configs 1-3 at their stated sizes; the invariant
+    sum_v v*P_k(v) = 2*C_k ties the column scan to the select."""
+    w = {"config1": wl.config1, "config2": wl.config2, "config3max": lambda: wl.config3(0),
+         "config3euclid": lambda: wl.config3(1)}[cfg]()
+    series = w.series if not cfg.startswith("config3") else w.series[[0, 3, 5]]
+    g = gpu_sweep(rqa, series, w.m, w.tau, w.rr, w.norm)
+    got = gpu_vert(rqa, series, w.m, w.tau, g["eps"], w.norm)
+    v = np.arange(got[0].shape[2], dtype=np.uint64)
+    assert np.array_equal((got[0] * v).sum(axis=2), 2 * g["count"])
+    assert_vert(oracle, got, series, w.m, w.tau, g["eps"], w.norm)
+
+
+@pytest.mark.parametrize("N,m,tau,norm,w,K,L,S", [(2, 1, 1, 0, 0, 1, 0, 0), (3, 1, 1, 0, 0, 3, 1, 1), (40, 2, 1, 0, 0, 5, 7, 2), (130, 3, 1, 0, 0, 20, 0, 0),
+                                                  (513, 1, 1, 0, 0, 11, 33, 3), (1100, 3, 1, 1, 0, 20, 100, 1), (1500, 4, 6, 0, 9, 33, 0, 0),
+                                                  (2300, 5, 2, 0, 0, 32, 257, 4), (2300, 3, 3, 1, 700, 12, 1023, 1), (700, 2, 5, 0, 689, 4, 64, 64)])
+def test_vertical_ragged_sizes_chunks_theiler(rqa, oracle, options, N, m, tau, norm, w, K, L, S):
+    """Column blocks with a ragged last block, every kind of chunk / segment border, the excluded band at any width (up
+    to all but one diagonal), K above one group of 32, quantised data with long vertical runs and ties."""
+    y = np.round(wl.add_noise(wl.lorenz_signal(N), 2.0, 99 + N) * 8).astype(np.float32) / 8
+    n = N - (m - 1) * tau
+    r = oracle.sweep(y, m, tau, wl.rr_log(K, 0.01, 0.6) if K > 1 else [0.2], norm, 2, threads=0, theiler=max(1, w))
+    from paper_2208_09136_b200 import binding as B
+    opt = B.make_options(line_chunk=L, line_segment=S)
+    got = gpu_vert(rqa, y, m, tau, r["eps"], norm, theiler=w, options=opt)
+    assert_vert(oracle, got, y, m, tau, r["eps"], norm, theiler=max(1, w))
+
+
+def test_vertical_materialised_points_and_split_call(rqa, oracle):
+    """Materialised row-major points (point stride m) through the run-time (m, tau) instantiation, and the column blocks
+    of ONE call dealt to three parts (parts.LocalParts) whose counters are summed by the reduce callback."""
+    import torch
+    from paper_2208_09136_b200 import binding as B, parts as P
+    N, m, tau = 1900, 4, 3
+    y = wl.add_noise(wl.logistic_signal(N, seed=31), 3.0, 32).astype(np.float32)
+    r = oracle.sweep(y, m, tau, wl.rr_log(9, 0.01, 0.3), 0, 2, threads=0)
+    ov = oracle.vert_hist(y, m, tau, r["eps"], 0, threads=0)
+    s = torch.as_tensor(y).cuda().unsqueeze(0)
+    n = N - (m - 1) * tau
+    X = torch.empty((1, n, m), dtype=torch.float32, device="cuda")
+    view = B.rqa_embed(s, m, tau, X=X)
+    e = torch.as_tensor(r["eps"]).cuda().unsqueeze(0)
+    vh = torch.empty((1, 9, n), dtype=torch.int64, device="cuda")
+    ws = torch.empty(B.rqa_workspace_bytes(view, 9), dtype=torch.uint8, device="cuda")
+    B.rqa_vert_hist(view, 0, e, vh, ws)
+    B.rqa_workspace_status(ws)
+    assert np.array_equal(vh.cpu().numpy().view(np.uint64)[0], ov)
+    dview = B.rqa_embed(s, m, tau)
+    local = P.LocalParts(3)
+
+    def one_part(p, reduce, stream):
+        opt = B.make_options(part_index=p, part_count=3, reduce=reduce, line_chunk=211)
+        out = torch.empty((1, 9, n), dtype=torch.int64, device="cuda")
+        w2 = torch.empty(B.rqa_workspace_bytes(dview, 9, opt), dtype=torch.uint8, device="cuda")
+        B.rqa_vert_hist(dview, 0, e, out, w2, options=opt)
+        return out.cpu().numpy().view(np.uint64)[0]
+    for part in local.run(one_part):
+        assert np.array_equal(part, ov)
+
+
+# ------------------------------------------------------------- the paper's experiment on one group of its grid (row f1)
+@pytest.mark.parametrize("signal,level,N", [("logistic", 1.0, 100), ("sine", 0.1, 200), ("lorenz", 10.0, 300)])
+def test_paper_group_sorting_experiment(rqa, oracle, signal, level, N):
+    """10 SNRs x 10 realisations of one dynamics (logistic at r = 3.679, 25-cycle sine, Lorenz embedded
+    with m = 3, tau = 3), the K = 99 integer-percent recurrence rates, DET_RR, the averaged DET_{RR*} of Eq. 5 for every
+    RR* and the sorting rate S of Eq. 6 for both, as ONE batched call of 100 series; every number against the oracle."""
+    from paper_2208_09136_b200 import experiment
+    w = wl.paper_group(signal, level, N)
+    assert (w.batch, w.K) == (100, 99)
+    out = experiment.sorting_experiment(w)
+    buf = out["buffers"]
+    g = {"eps": buf.eps.cpu().numpy(), "count": buf.count.cpu().numpy().view(np.uint64), "rr": buf.rr.cpu().numpy(),
+         "hist": buf.hist.cpu().numpy().view(np.uint64), "det": buf.det.cpu().numpy(), "det_mean": buf.det_mean.cpu().numpy()}
+    assert_parity(oracle, g, w.series, w.m, w.tau, w.rr, w.norm)
+    odet = np.stack([oracle.sweep(w.series[b], w.m, w.tau, w.rr, w.norm, 2, threads=0)["det"] for b in range(w.batch)])
+    oavg = np.stack([oracle.det_prefix_avg(odet[b]) for b in range(w.batch)])
+    assert np.max(np.abs(out["det_avg"] - oavg)) <= DET_TOL
+    for k in (0, 1, 9, 49, 98):
+        # S is a ratio of small integers: ties in the measure would make it order-sensitive, so compare on the GPU's own
+        # values (bit-equal to the oracle's up to 1e-12) through the oracle's independent argsort-based S
+        assert out["S_det"][k] == oracle.sorting_rate(out["det"][:, k].reshape(10, 10))
+        assert out["S_avg"][k] == oracle.sorting_rate(out["det_avg"][:, k].reshape(10, 10))
+    assert np.all((out["S_avg"] >= 0) & (out["S_avg"] <= 1))

@@ -45,20 +45,31 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     objdir = PKG / "build"
     objdir.mkdir(exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
-    # one nvcc per translation unit, side by side (the two big ones take about a minute each), then link
-    jobs = []
+    # one nvcc per translation unit, side by side (the big ones take minutes each), then link.  Objects are kept and
+    # reused while they are newer than their source, every header and this file (force=True rebuilds all of them).
+    headers = list(CSRC.glob("*.cuh")) + [ROOT / "include" / "rqa.h", Path(__file__)]
+    newest_header = max(h.stat().st_mtime for h in headers)
+    jobs, objs = [], []
     for src in sources():
-        obj = objdir / f"{src.stem}.{os.getpid()}.o"
-        jobs.append((obj, subprocess.Popen([nvcc, *NVCC_FLAGS, *extra, "-c", "-o", str(obj), str(src)])))
-    failed = [str(obj) for obj, proc in jobs if proc.wait() != 0]
+        obj = objdir / f"{src.stem}.o"
+        objs.append(obj)
+        if not force and obj.exists() and obj.stat().st_mtime > max(src.stat().st_mtime, newest_header):
+            continue
+        tmp = objdir / f"{src.stem}.{os.getpid()}.tmp.o"
+        jobs.append((obj, tmp, subprocess.Popen([nvcc, *NVCC_FLAGS, *extra, "-c", "-o", str(tmp), str(src)])))
+    failed = []
+    for obj, tmp, proc in jobs:
+        if proc.wait() != 0:
+            failed.append(str(obj))
+            tmp.unlink(missing_ok=True)
+        else:
+            os.replace(tmp, obj)
     if failed:
         raise RuntimeError(f"nvcc failed for {failed}")
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(tmp), *[str(obj) for obj, _ in jobs]],
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(tmp), *[str(o) for o in objs]],
                    check=True)
     os.replace(tmp, LIB)
-    for obj, _ in jobs:
-        obj.unlink(missing_ok=True)
     return LIB
 
 

@@ -132,6 +132,25 @@ __global__ void det_kernel(const uint64_t* __restrict__ hist, int K, int64_t n, 
     }
 }
 
+// Short rows (the many-short-series regime of the paper's grid): one WARP per (k, b) row, eight rows per block.
+__global__ void __launch_bounds__(256) det_rows_kernel(const uint64_t* __restrict__ hist, int64_t rows, int64_t n, int64_t l_min,
+                                                       double* __restrict__ det) {
+    const int64_t row = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= rows) return;
+    const uint64_t* h = hist + row * n;
+    unsigned long long num = 0, den = 0;
+    for (int64_t l = 1 + (threadIdx.x & 31); l < n; l += 32) {
+        unsigned long long w = (unsigned long long)l * h[l];
+        den += w;
+        if (l >= l_min) num += w;
+    }
+    for (int off = 16; off; off >>= 1) {
+        num += __shfl_down_sync(0xffffffffu, num, off);
+        den += __shfl_down_sync(0xffffffffu, den, off);
+    }
+    if ((threadIdx.x & 31) == 0) det[row] = den ? (double)num / (double)den : 0.0;
+}
+
 // Eq. 5: mean over the K rates, summed k = 0..K-1 left to right in fp64 (reading S11).
 __global__ void det_mean_kernel(const double* __restrict__ det, int K, int batch, double* __restrict__ mean) {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -325,7 +344,12 @@ rqa_status rqa_det_avg(const uint64_t* d_hist, int32_t batch, int32_t K, int64_t
     if (!d_hist || !d_det || !d_det_mean) { set_error("rqa_det_avg: NULL argument"); return RQA_ERR_INVALID_ARG; }
     if (batch < 1 || K < 1 || K > RQA_MAX_K || n_points < 2 || l_min < 1) { set_error("rqa_det_avg: need batch >= 1, 1 <= K <= %d, n_points >= 2, l_min >= 1", RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
     cudaStream_t s = (cudaStream_t)stream;
-    det_kernel<<<dim3(K, batch), 256, 0, s>>>(d_hist, K, n_points, l_min, d_det);
+    if (n_points <= 2048) {
+        const int64_t rows = (int64_t)K * batch;
+        det_rows_kernel<<<(unsigned)((rows + 7) / 8), 256, 0, s>>>(d_hist, rows, n_points, l_min, d_det);
+    } else {
+        det_kernel<<<dim3(K, batch), 256, 0, s>>>(d_hist, K, n_points, l_min, d_det);
+    }
     RQA_LAUNCH_CHECK();
     det_mean_kernel<<<(batch + 127) / 128, 128, 0, s>>>(d_det, K, batch, d_det_mean);
     RQA_LAUNCH_CHECK();

@@ -131,6 +131,14 @@ size_t line_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws,
                          cudaStream_t s, const Options& opt);
 
+// Short series (at most 8192 counted pairs): one block per series, everything in shared memory (rqa_small.cu).
+bool small_series(const View& v);
+bool small_line_fits(const View& v, int K);
+rqa_status run_select_small(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
+                            double* d_rr, cudaStream_t s);
+rqa_status run_line_small(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, WsStatus* status,
+                          cudaStream_t s);
+
 size_t vert_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_vhist, Arena& ws,
                          cudaStream_t s, const Options& opt);

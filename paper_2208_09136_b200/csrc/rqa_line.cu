@@ -560,6 +560,7 @@ template <int NORM, int NP>
 rqa_status dispatch_embedding(const ScanArgs& a, const LinePlan& p, cudaStream_t s) {
     // the embeddings of BASELINE.json's large configs get a register ring; any other (m, tau) recomputes per cell
     const bool delay = a.v.ps == 1;
+    if (delay && a.m == 1) return launch_scan<NORM, 1, 1, NP>(a, p, s);
     if (delay && a.m == 3 && a.tau == 1) return launch_scan<NORM, 3, 1, NP>(a, p, s);
     if (delay && a.m == 3 && a.tau == 3) return launch_scan<NORM, 3, 3, NP>(a, p, s);
     if (delay && a.m == 5 && a.tau == 2) return launch_scan<NORM, 5, 2, NP>(a, p, s);
@@ -616,8 +617,10 @@ rqa_status launch_line_groups(const float* d_eps, int K, int NG, int batch, void
 rqa_status launch_line_finalize(int64_t n, int NG, int NP, int K, int batch, const void* groups, const unsigned long long* agg,
                                 unsigned long long* hist, WsStatus* status, cudaStream_t s) {
     for (int g = 0; g < NG; ++g) {
-        line_finalize_kernel<<<dim3((unsigned)(2 * NP), (unsigned)batch), 1024, 0, s>>>(n, g, NG, K, (const LineGroup*)groups, agg,
-                                                                                       hist, status);
+        // one block per (distinct threshold, series) sums its histogram row: about 8 bins per thread
+        const unsigned threads = (unsigned)std::max<int64_t>(64, std::min<int64_t>(1024, ((n / 8 + 31) / 32) * 32));
+        line_finalize_kernel<<<dim3((unsigned)(2 * NP), (unsigned)batch), threads, 0, s>>>(n, g, NG, K, (const LineGroup*)groups, agg,
+                                                                                          hist, status);
         RQA_LAUNCH_CHECK();
         unsigned cb = (unsigned)std::min<int64_t>((n + 255) / 256, 64);
         line_copy_rows_kernel<<<dim3(cb, GK, (unsigned)batch), 256, 0, s>>>(n, g, NG, K, (const LineGroup*)groups, hist);
@@ -644,6 +647,10 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
                          const Options& opt) {
     WsStatus* status = (WsStatus*)ws.base;
     const size_t hist_words = (size_t)v.batch * K * v.n;
+    // short series: one block per series, shared-memory distances and histogram (explicit scan knobs and split calls
+    // keep the general machinery)
+    if (opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
+        return run_line_small(v, norm, d_eps, K, d_hist, status, s);
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * hist_words, s));
     LinePlan p = make_plan(v, K, opt);
     if (!p.scan) {

@@ -918,6 +918,7 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
 template <int NORM>
 rqa_status dispatch_count(const CountArgs& a, const SelectPlan& p, int nlev, int batch, cudaStream_t s) {
     const bool delay = p.ps == 1;
+    if (delay && a.m == 1) return launch_count<NORM, 1, 1>(a, p, nlev, batch, s);
     if (delay && a.m == 3 && a.tau == 1) return launch_count<NORM, 3, 1>(a, p, nlev, batch, s);
     if (delay && a.m == 3 && a.tau == 3) return launch_count<NORM, 3, 3>(a, p, nlev, batch, s);
     if (delay && a.m == 5 && a.tau == 2) return launch_count<NORM, 5, 2>(a, p, nlev, batch, s);
@@ -990,6 +991,10 @@ size_t select_workspace_bytes(const View& v, int K, const Options& opt) {
 
 rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
                       double* d_rr, Arena& ws, cudaStream_t s, const Options& opt) {
+    // short series: one block sorts all distances of a series in shared memory (any explicit path choice, and a split
+    // call, keep the general machinery)
+    if (opt.select_path == PATH_AUTO && opt.parts == 1 && small_series(v))
+        return run_select_small(v, norm, h_rank, K, d_eps, d_count, d_rr, s);
     const SelectPlan p = make_select_plan(v, K, opt);
     SelectWs w = carve(ws, v, K, p);
     if (!ws.ok()) { set_error("rqa_eps_for_rr: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }

@@ -374,6 +374,7 @@ rqa_status launch_vscan(const VertArgs& a, const VertPlan& p, cudaStream_t s) {
 template <int NORM, int NP>
 rqa_status dispatch_vembedding(const VertArgs& a, const VertPlan& p, cudaStream_t s) {
     const bool delay = a.v.ps == 1;
+    if (delay && a.m == 1) return launch_vscan<NORM, 1, 1, NP>(a, p, s);
     if (delay && a.m == 3 && a.tau == 1) return launch_vscan<NORM, 3, 1, NP>(a, p, s);
     if (delay && a.m == 3 && a.tau == 3) return launch_vscan<NORM, 3, 3, NP>(a, p, s);
     if (delay && a.m == 5 && a.tau == 2) return launch_vscan<NORM, 5, 2, NP>(a, p, s);

@@ -102,3 +102,63 @@ def test_config5_one_call_of_96_series(rqa, oracle):
         g["hist"][b] = buf.hist[b].cpu().numpy().view(np.uint64)
         gold = load_golden("config5", b, w.series[b], w.rr)
         check_series(oracle, g, b, gold, w.n_pairs, [(2, det2, mean2), (3, det3, mean3)], f"config5 series {b} {w.labels[b]}")
+
+
+def vert_call(rqa, s, w, eps):
+    import torch
+    from paper_2208_09136_b200 import binding as B
+    view = B.rqa_embed(s, w.m, w.tau)
+    vh = torch.empty((s.shape[0], w.K, w.n_points), dtype=torch.int64, device="cuda")
+    ws = torch.empty(B.rqa_workspace_bytes(view, w.K), dtype=torch.uint8, device="cuda")
+    B.rqa_vert_hist(view, w.norm, eps, vh, ws)
+    B.rqa_workspace_status(ws)
+    return vh
+
+
+def test_config5_vertical_lines_one_call_of_96_series(rqa, oracle):
+    """rqa_vert_hist on config 5 as ONE call of 96 series (N = 2e4, K = 32) at the stored oracle thresholds: the
+    12-series slice element by element against the stored oracle vertical-line histograms, LAM / TT against the oracle's
+    reduction of them; all 96 x 32 rows through sum_v v*P(v) = 2*C."""
+    import torch
+    w = wl.config5()
+    s = torch.as_tensor(w.series).cuda()
+    buf = rqa.averaged_rqa(s, w.m, w.tau, w.rr, w.norm, 2)
+    vh = vert_call(rqa, s, w, buf.eps)
+    lam = torch.empty_like(buf.det)
+    tt = torch.empty_like(buf.det)
+    rqa.rqa_lam_tt(vh, 2, lam, tt)
+    v = torch.arange(w.n_points, device="cuda", dtype=torch.int64)
+    sums = (vh * v).sum(dim=2).cpu().numpy().view(np.uint64)
+    assert np.array_equal(sums, 2 * buf.count.cpu().numpy().view(np.uint64)), "sum v*P(v) = 2C on all 96 x 32 rows"
+    lam, tt = lam.cpu().numpy(), tt.cpu().numpy()
+    for b in CONFIG5_SLICE:
+        gold = load_golden("config5", b, w.series[b], w.rr)
+        assert gold["vhist"] is not None
+        assert np.array_equal(buf.eps[b].cpu().numpy().view(np.uint32), gold["eps"].view(np.uint32))
+        got = vh[b].cpu().numpy().view(np.uint64)
+        if not np.array_equal(got, gold["vhist"]):
+            bad = np.argwhere(got != gold["vhist"])
+            raise AssertionError(f"config5 series {b}: {len(bad)} vertical-histogram cells differ, first at {bad[0]}")
+        ol, ot = oracle.lam_tt(gold["vhist"], 2)
+        assert np.max(np.abs(lam[b] - ol)) <= 1e-12 and np.max(np.abs(tt[b] - ot)) <= 1e-9 * max(1.0, float(np.max(ot)))
+
+
+def test_config4_vertical_lines_full_size(rqa, oracle):
+    """rqa_vert_hist at N = 1e5 (1e10 cells per series and threshold set): the series that have a stored oracle
+    vertical-line histogram element by element; all five through sum_v v*P(v) = 2*C."""
+    import torch
+    w = wl.config4()
+    s = torch.as_tensor(w.series).cuda()
+    buf = rqa.averaged_rqa(s, w.m, w.tau, w.rr, w.norm, 2)
+    vh = vert_call(rqa, s, w, buf.eps)
+    v = torch.arange(w.n_points, device="cuda", dtype=torch.int64)
+    sums = (vh * v).sum(dim=2).cpu().numpy().view(np.uint64)
+    assert np.array_equal(sums, 2 * buf.count.cpu().numpy().view(np.uint64))
+    checked = 0
+    for b in range(w.batch):
+        gold = load_golden("config4", b, w.series[b], w.rr)
+        if gold["vhist"] is None:
+            continue
+        assert np.array_equal(vh[b].cpu().numpy().view(np.uint64), gold["vhist"]), f"config4 series {b}"
+        checked += 1
+    assert checked >= 1, "no stored vertical-line histogram: run make_fullsize_golden.py config4 <s> --stage vhist"

@@ -760,3 +760,66 @@ def test_paper_group_sorting_experiment(rqa, oracle, signal, level, N):
         assert out["S_det"][k] == oracle.sorting_rate(out["det"][:, k].reshape(10, 10))
         assert out["S_avg"][k] == oracle.sorting_rate(out["det_avg"][:, k].reshape(10, 10))
     assert np.all((out["S_avg"] >= 0) & (out["S_avg"] <= 1))
+
+
+# ------------------------------------------- stand-ins for compute-sanitizer (closed on this GPU pool)
+@pytest.mark.parametrize("path", [0, 1, 2, 3])
+def test_workspace_contents_and_guard_bands(rqa, oracle, path):
+    """initcheck / memcheck by hand.  The workspace is scratch the caller does not initialise: whatever it holds before
+    a call (zeros, 0xFF, random bytes, the previous call's leftovers) the results must be bit-identical and correct —
+    a kernel that reads a word it has not written shows up as a difference.  Every buffer (workspace and outputs) is
+    followed by a guard band of a known pattern that must come back intact: a write past the size the library asked for
+    shows up there.  All select paths, the diagonal scan and the column scan, two chunk configurations."""
+    import torch
+    from paper_2208_09136_b200 import binding as B
+    N, m, tau, K = (700 if path == 1 else 3000), 3, 2, 20
+    y = np.stack([wl.add_noise(wl.lorenz_signal(N), 1.0, 808), np.round(wl.gaussian(809, N) * 3) / 3]).astype(np.float32)
+    rr = wl.rr_log(K, 0.002, 0.3)
+    s = torch.as_tensor(y).cuda()
+    GUARD = 4096
+    ref = None
+    for fill, chunk in (("zeros", 0), ("ff", 0), ("random", 61), ("leftover", 0)):
+        opt = B.make_options(select_path=path, line_chunk=chunk, line_segment=3 if chunk else 0)
+        view = B.rqa_embed(s, m, tau)
+        n = int(view.n_points)
+        nbytes = B.rqa_workspace_bytes(view, K, opt)
+        wsg = torch.empty(nbytes + GUARD, dtype=torch.uint8, device="cuda")
+        if fill == "zeros":
+            wsg.zero_()
+        elif fill == "ff":
+            wsg.fill_(255)
+        elif fill == "random":
+            wsg.copy_(torch.randint(0, 256, (nbytes + GUARD,), dtype=torch.uint8, device="cuda"))
+        else:                                                       # whatever the previous calls of this test left behind
+            B.rqa_eps_for_rr(view, 0, rr, *[torch.empty((2, K), dtype=d, device="cuda") for d in (torch.float32, torch.int64, torch.float64)],
+                             wsg[:nbytes], options=opt)
+        wsg[nbytes:].fill_(0xA5)
+        ws = wsg[:nbytes]
+
+        def guarded(shape, dtype):
+            numel = int(np.prod(shape))
+            g = torch.full((numel + GUARD // 8,), 0x5A5A5A5A, dtype=dtype, device="cuda") if dtype != torch.float32 and dtype != torch.float64 \
+                else torch.full((numel + GUARD // 8,), -7.25, dtype=dtype, device="cuda")
+            return g, g[:numel].view(shape)
+        ge, eps = guarded((2, K), torch.float32)
+        gc, cnt = guarded((2, K), torch.int64)
+        gr, rrr = guarded((2, K), torch.float64)
+        gh, hist = guarded((2, K, n), torch.int64)
+        gv, vh = guarded((2, K, n), torch.int64)
+        B.rqa_eps_for_rr(view, 0, rr, eps, cnt, rrr, ws, options=opt)
+        B.rqa_line_hist(view, 0, eps, hist, ws, options=opt)
+        B.rqa_vert_hist(view, 0, eps, vh, ws, options=opt)
+        B.rqa_workspace_status(ws)
+        assert bool((wsg[nbytes:] == 0xA5).all()), f"write past the workspace ({fill})"
+        for g, numel, pat in ((ge, 2 * K, -7.25), (gr, 2 * K, -7.25), (gc, 2 * K, 0x5A5A5A5A), (gh, 2 * K * n, 0x5A5A5A5A), (gv, 2 * K * n, 0x5A5A5A5A)):
+            assert bool((g[numel:] == pat).all()), f"write past an output buffer ({fill})"
+        got = (eps.cpu().numpy().copy(), cnt.cpu().numpy().copy(), hist.cpu().numpy().copy(), vh.cpu().numpy().copy())
+        if ref is None:
+            ref = got
+            for b in range(2):
+                r = oracle.sweep(y[b], m, tau, rr, 0, 2, threads=0)
+                assert np.array_equal(got[0][b], r["eps"]) and np.array_equal(got[2][b].view(np.uint64), r["hist"])
+                assert np.array_equal(got[3][b].view(np.uint64), oracle.vert_hist(y[b], m, tau, r["eps"], 0, threads=0))
+        else:
+            for a, c in zip(got, ref):
+                assert np.array_equal(a, c), f"results depend on the workspace contents ({fill})"

@@ -95,13 +95,13 @@ __global__ void __launch_bounds__(SMALL_THREADS) sel_small_kernel(View v, SmallR
 // ends, each giving ONE line length for a whole range [a, b) of thresholds, counted as D[a][len]++, D[b][len]-- in a
 // difference array over the thresholds.  Work per cell does not depend on K (the same idea as the tiled scan, in its
 // plainest form: lines of every length are emitted, nothing is deferred).
-// Shared memory (32-bit words): dist[P] diagonal by diagonal | D[(K+1)][n] | eps sorted distinct [K+1] | j_of[K] | 2 x scratch[K] |
+// Shared memory: uint8 level[P] diagonal by diagonal | then 32-bit words: D[(K+1)][n] | eps sorted distinct [K+1] | j_of[K] | 2 x scratch[K] |
 // stacks [LINE_SMALL_THREADS][K+1] uint16 (lo << 8 | start).
-constexpr int LINE_SMALL_THREADS = 128;
+constexpr int LINE_SMALL_THREADS = 256;
 
 __host__ __device__ inline size_t line_small_smem(int64_t P, int K, int64_t n) {
-    return 4 * ((size_t)P + (size_t)(K + 1) * (size_t)n + (size_t)(K + 1) + 3 * (size_t)K) +
-           2 * (size_t)LINE_SMALL_THREADS * (size_t)(K + 2);
+    return 4 * (((size_t)P + 3) / 4 + (size_t)(K + 1) * (size_t)n + (size_t)(K + 1) + 3 * (size_t)K) +
+           2 * (size_t)(SMALL_MAX_N) * (size_t)(K + 2);
 }
 
 template <int NORM>
@@ -114,8 +114,8 @@ __global__ void __launch_bounds__(LINE_SMALL_THREADS) line_small_kernel(View v, 
     const int b = blockIdx.x, tid = threadIdx.x;
     const int n = (int)v.n, w = (int)v.w, nd = n - w;
     const int P = nd * (nd + 1) / 2;
-    float* s_d = (float*)s_mem;
-    int* s_D = (int*)(s_mem + P);
+    uint8_t* s_lev = (uint8_t*)s_mem;                         // level of every cell, diagonal by diagonal
+    int* s_D = (int*)(s_mem + (P + 3) / 4);
     float* s_eps = (float*)(s_D + (K + 1) * n);
     int* s_jof = (int*)(s_eps + (K + 1));
     float* s_san = (float*)(s_jof + K);                      // thresholds with NaN / negative / infinite values replaced by 0
@@ -149,6 +149,9 @@ __global__ void __launch_bounds__(LINE_SMALL_THREADS) line_small_kernel(View v, 
         s_eps[below] = s_san[k];                             // equal thresholds write the same value to the same slot
         atomicMax(&s_J, below + 1);
     }
+    __syncthreads();
+    const int J = s_J;
+    // every cell's level = number of distinct thresholds below its distance (all threads, one flat loop over the pairs)
     for (int p = tid; p < P; p += LINE_SMALL_THREADS) {
         int lo = 0, hi = nd;                                  // diagonal of pair p: last q with off(q) <= p
         while (hi - lo > 1) {
@@ -156,12 +159,17 @@ __global__ void __launch_bounds__(LINE_SMALL_THREADS) line_small_kernel(View v, 
             if (s_off[mid] <= p) lo = mid; else hi = mid;
         }
         const int i = p - s_off[lo];
-        s_d[p] = point_distance<NORM>(yb, i, i + w + lo, v.m, v.ps, v.cs);
+        const float x = point_distance<NORM>(yb, i, i + w + lo, v.m, v.ps, v.cs);
+        int a = 0, c = J;
+        while (a < c) {
+            const int mid = (a + c) >> 1;
+            if (s_eps[mid] < x) a = mid + 1; else c = mid;
+        }
+        s_lev[p] = (uint8_t)a;
     }
     __syncthreads();
-    const int J = s_J;
     for (int q = tid; q < nd; q += LINE_SMALL_THREADS) {     // diagonal o = w + q, len = nd - q cells
-        const float* d = s_d + s_off[q];
+        const uint8_t* lev = s_lev + s_off[q];
         const int len = nd - q;
         int top = 0, pv = J;
         auto ended = [&](int vnew, int t) {                  // the thresholds [pv, vnew) end their runs before cell t
@@ -182,12 +190,7 @@ __global__ void __launch_bounds__(LINE_SMALL_THREADS) line_small_kernel(View v, 
             }
         };
         for (int t = 0; t < len; ++t) {
-            const float x = d[t];
-            int lo = 0, hi = J;                               // level = number of distinct thresholds < x
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (s_eps[mid] < x) lo = mid + 1; else hi = mid;
-            }
+            const int lo = lev[t];
             if (lo < pv) s_stk[top++] = (uint16_t)((lo << 8) | t);
             else if (lo > pv) ended(lo, t);
             pv = lo;

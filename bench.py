@@ -291,9 +291,11 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
     rank, world, local = shard.env_rank_world()
+    if args.same_gpu:                                               # functional test of the multi-rank path on a 1-GPU box
+        local = 0
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    shard.init_process_group("nccl")
+    shard.init_process_group(args.backend)
     rqa.load_library()
     split = args.mode == "split" and world > 1
 
@@ -364,7 +366,7 @@ def run_ours(args):
     t_det = [e[2].elapsed_time(e[3]) for e in events]
     t_step = [e[0].elapsed_time(e[3]) for e in events]
     total_ms = sum(t_step)
-    value, max_ms = shard.whole_job_throughput(units_per_step * args.steps, total_ms, world, dev)
+    value, max_ms = shard.whole_job_throughput(units_per_step * args.steps, total_ms, world, dev if args.backend == "nccl" else "cpu")
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     e2e = None
@@ -390,7 +392,7 @@ def run_ours(args):
             torch.cuda.synchronize()
             e2e_ms += a.elapsed_time(b)
             flush.fill_(it & 1)
-        e2e_value, _ = shard.whole_job_throughput(units_per_step * e2e_steps, e2e_ms, world, dev)
+        e2e_value, _ = shard.whole_job_throughput(units_per_step * e2e_steps, e2e_ms, world, dev if args.backend == "nccl" else "cpu")
         h2d = hs.numel() * 4
         d2h = h_eps.numel() * 4 + h_cnt.numel() * 8 + h_rr.numel() * 8 + h_det.numel() * 8 + h_mean.numel() * 8 + h_hist.numel() * 8
         e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -469,6 +471,8 @@ def run_ours(args):
                             "rqa_det_avg": statistics.mean(t_det), "step_min": min(t_step), "step_median": statistics.median(t_step)},
            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e,
            "gpu_launches": int(launches), "clocks": clocks, "other_configs": others}
+    if args.same_gpu:
+        out["functional_test_only"] = "all ranks shared one GPU: not a measurement"
     print(json.dumps(out), flush=True)
     return 0
 
@@ -510,6 +514,10 @@ def main():
     ap.add_argument("--no-others", action="store_true", help="skip the secondary timings of the other configs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--profile-step", action="store_true", help="run ONE bare step and exit (for ncu; prints nothing)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="torch.distributed backend of the ranks")
+    ap.add_argument("--same-gpu", action="store_true",
+                    help="FUNCTIONAL TEST ONLY: all ranks share cuda:0 (use with --backend gloo; NCCL refuses one device "
+                         "twice).  The ranks take turns on the device: the number printed is not a measurement.")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

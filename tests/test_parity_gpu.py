@@ -823,3 +823,25 @@ def test_workspace_contents_and_guard_bands(rqa, oracle, path):
         else:
             for a, c in zip(got, ref):
                 assert np.array_equal(a, c), f"results depend on the workspace contents ({fill})"
+
+
+def test_bench_launches_its_own_ranks_split_mode(rqa):
+    """`python bench.py --gpus 2` outside torchrun starts two ranks itself; --mode split gives each rank a share of the
+    tiles of ONE batch and all-reduces the exact counters through torch.distributed.  Only one GPU is available here,
+    so the two ranks share it and rendezvous over gloo (--same-gpu --backend gloo: a FUNCTIONAL test of the launch,
+    rank plumbing and reduce callback — the ranks take turns on the device and the printed number is not a measurement;
+    bit-exactness of the split is test_split_call_every_part_holds_the_oracle_result's job)."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    cmd = [sys.executable, str(root / "bench.py"), "--gpus", "2", "--mode", "split", "--same-gpu", "--backend", "gloo", "--N", "12000",
+           "--series", "2,4", "--steps", "2", "--warmup", "1", "--no-cpu-baseline", "--no-others", "--no-e2e"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(line) == 1, "rank 0 alone prints the JSON line"
+    d = json.loads(line[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["gpu_launches"] > 0 and "functional_test_only" in d
+    assert d["config"]["parallelism"].startswith("one batch split over 2 ranks")

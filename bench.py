@@ -86,7 +86,7 @@ def read_step_counters(path: Path = STEP_COUNTERS):
         name = r[kn]
         if "at::" in name or "cub::" in name:                 # torch's own kernels (fills): not part of the step
             continue
-        short = name.split("(")[0].replace("void ", "").replace("rqa::", "").replace("<unnamed>::", "").strip()
+        short = name.split("(")[0].replace("void ", "").replace("rqa::", "").replace("<unnamed>::", "").replace("unnamed>::", "").strip()
         v = float(r[mv].replace(",", ""))
         unit = r[mu]
         scale = {"ns": 1e-6, "us": 1e-3, "usecond": 1e-3, "msecond": 1.0, "ms": 1.0, "nsecond": 1e-6, "second": 1e3,

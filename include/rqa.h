@@ -24,6 +24,10 @@
  *   - runs that touch the border of the plot count with their truncated length (S8);
  *   - counts are exact uint64; RR and DET are fp64 ratios of exact integers.
  *
+ * Workspace size: rqa_workspace_bytes sizes for the worst case of the shape (the recurrence rates are not known then): about
+ * 0.9 GB per series of 1e5 points at K = 20 (candidate list of the threshold select, up to 6 % of the pairs; segment
+ * summaries of the scans), 80 MB per series of 2e4 points at K = 32, linear in the batch.
+ *
  * Memory and ownership: every buffer is owned by the caller.  Pointers named d_* are DEVICE pointers,
  * h_* are HOST pointers.  The library keeps no device allocation and no global state between calls (the only
  * process-wide datum is the monotone launch counter behind rqa_launch_count()).
@@ -227,7 +231,11 @@ uint64_t rqa_launch_count(void);
  * computed, never the result (every path of rqa_eps_for_rr is exact).  Workspace sizes depend on them: pass the same
  * options to rqa_workspace_bytes_opt and to the call that uses the workspace.
  *   select_path   rqa_eps_for_rr: 0 automatic, 1 = materialise all distances (small P), 2 = sample-bracket + one
- *                 counting pass, 3 = four radix passes
+ *                 counting pass, 3 = four radix passes.  The radix passes serve views the tiled passes cannot stage
+ *                 (coordinate span above 4096 elements, very wide points) and are the automatic recovery of a bracket
+ *                 miss; they recompute every distance from global memory four times and cost about 20 x the bracket path
+ *                 (88 ms instead of 4 ms per series of 1e5 points on a B200).  Automatic: series of at most 8192 pairs are
+ *                 sorted whole in shared memory, P <= 2^22 takes path 1, everything else path 2.
  *   sample_size   bracket path: number of sampled pair distances per series
  *   cand_cap      bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
  *   line_chunk    rqa_line_hist / rqa_vert_hist: chunk length along the diagonals / columns, 1..1023

@@ -160,14 +160,15 @@ int rqa_oracle_eps_for_rr(const float* y, int64_t N, int m, int64_t tau, int nor
     return ORACLE_OK;
 }
 
-/* The counting certificate: for every k, lt[k] = #{i<j : d_ij < eps_k}, le[k] = #{i<j : d_ij <= eps_k}.
+/* The counting certificate: for every k, lt[k] = #{i<j : d_ij < eps_k}, le[k] = #{i<j : d_ij <= eps_k}, over the pairs
+ * with j - i >= theiler.
  * eps is the r-th smallest distance iff lt < r <= le.  O(1) extra memory, no sort.  Used where the
  * 4*P-byte sorted array does not fit (N = 1e5) and as an independent check of the sort-based path. */
 int rqa_oracle_count_lt_le(const float* y, int64_t N, int m, int64_t tau, int norm, const float* eps, int K,
-                           uint64_t* lt, uint64_t* le, int threads) {
-    if (!y || !eps || !lt || !le || m < 1 || tau < 1 || K < 1) return ORACLE_BAD_ARG;
+                           uint64_t* lt, uint64_t* le, int threads, int64_t theiler) {
+    if (!y || !eps || !lt || !le || m < 1 || tau < 1 || K < 1 || theiler < 1) return ORACLE_BAD_ARG;
     int64_t Np = embedded_points(N, m, tau);
-    if (Np < 2) return ORACLE_BAD_ARG;
+    if (Np < 2 || theiler > Np - 1) return ORACLE_BAD_ARG;
     int nt = pick_threads(threads);
     std::vector<uint64_t> acc_lt((size_t)nt * K, 0), acc_le((size_t)nt * K, 0);
 #ifdef _OPENMP
@@ -181,7 +182,7 @@ int rqa_oracle_count_lt_le(const float* y, int64_t N, int m, int64_t tau, int no
 #endif
         uint64_t* a = &acc_lt[(size_t)t * K];
         uint64_t* b = &acc_le[(size_t)t * K];
-        for (int64_t j = i + 1; j < Np; ++j) {
+        for (int64_t j = i + theiler; j < Np; ++j) {           /* theiler = 1: every pair i < j (reading S9) */
             float d = distance(y, i, j, m, tau, norm);
             for (int k = 0; k < K; ++k) {
                 a[k] += (d < eps[k]) ? 1u : 0u;

@@ -54,7 +54,7 @@ def _load():
     lib.rqa_oracle_rank.argtypes = [ctypes.c_double, ctypes.c_uint64]
     lib.rqa_oracle_rank.restype = ctypes.c_uint64
     lib.rqa_oracle_eps_for_rr.argtypes = [f32p, i64, i32, i64, i32, f64p, i32, f32p, u64p, f64p, i64]
-    lib.rqa_oracle_count_lt_le.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, u64p, i32]
+    lib.rqa_oracle_count_lt_le.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, u64p, i32, i64]
     lib.rqa_oracle_line_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i32, i64]
     lib.rqa_oracle_vert_hist.argtypes = [f32p, i64, i32, i64, i32, f32p, i32, u64p, i32, i64]
     lib.rqa_oracle_lam_tt.argtypes = [u64p, i32, i64, i64, f64p, f64p]
@@ -129,15 +129,15 @@ def eps_for_rr(y, m: int, tau: int, rr, norm: int = NORM_MAX, theiler: int = 1):
     return eps, cnt, rrr
 
 
-def count_lt_le(y, m: int, tau: int, eps, norm: int = NORM_MAX, threads: int = 0):
-    """-> (#{d < eps_k}, #{d <= eps_k}) as uint64[K] — the counting certificate."""
+def count_lt_le(y, m: int, tau: int, eps, norm: int = NORM_MAX, threads: int = 0, theiler: int = 1):
+    """-> (#{d < eps_k}, #{d <= eps_k}) as uint64[K] over the pairs with j - i >= theiler — the counting certificate."""
     y = _series(y)
     eps = np.ascontiguousarray(eps, dtype=np.float32)
     K = len(eps)
     lt = np.empty(K, dtype=np.uint64)
     le = np.empty(K, dtype=np.uint64)
     _check(_load().rqa_oracle_count_lt_le(_p(y, ctypes.c_float), len(y), m, tau, norm, _p(eps, ctypes.c_float), K,
-                                          _p(lt, ctypes.c_uint64), _p(le, ctypes.c_uint64), threads),
+                                          _p(lt, ctypes.c_uint64), _p(le, ctypes.c_uint64), threads, max(1, theiler)),
            "count_lt_le")
     return lt, le
 

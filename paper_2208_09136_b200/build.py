@@ -30,12 +30,28 @@ def sources():
     return sorted(CSRC.glob("*.cu"))
 
 
+def _objects():
+    objdir = PKG / "build"
+    return [(src, objdir / f"{src.stem}.o") for src in sources()]
+
+
+def _newest_header() -> float:
+    headers = list(CSRC.glob("*.cuh")) + [ROOT / "include" / "rqa.h", Path(__file__)]
+    return max(h.stat().st_mtime for h in headers)
+
+
+def _obj_stale(src: Path, obj: Path, newest_header: float) -> bool:
+    return not obj.exists() or obj.stat().st_mtime <= max(src.stat().st_mtime, newest_header)
+
+
 def _stale() -> bool:
+    """The library is stale if it is missing, if an object is older than its source or any header, or if it is older than
+    an object (an object rebuilt after the last link)."""
     if not LIB.exists():
         return True
+    nh = _newest_header()
     t = LIB.stat().st_mtime
-    deps = list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + [ROOT / "include" / "rqa.h", Path(__file__)]
-    return any(d.stat().st_mtime > t for d in deps)
+    return any(_obj_stale(src, obj, nh) or obj.stat().st_mtime > t for src, obj in _objects())
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
@@ -47,13 +63,11 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     extra = ["-Xptxas", "-v"] if verbose else []
     # one nvcc per translation unit, side by side (the big ones take minutes each), then link.  Objects are kept and
     # reused while they are newer than their source, every header and this file (force=True rebuilds all of them).
-    headers = list(CSRC.glob("*.cuh")) + [ROOT / "include" / "rqa.h", Path(__file__)]
-    newest_header = max(h.stat().st_mtime for h in headers)
+    newest_header = _newest_header()
     jobs, objs = [], []
-    for src in sources():
-        obj = objdir / f"{src.stem}.o"
+    for src, obj in _objects():
         objs.append(obj)
-        if not force and obj.exists() and obj.stat().st_mtime > max(src.stat().st_mtime, newest_header):
+        if not force and not _obj_stale(src, obj, newest_header):
             continue
         tmp = objdir / f"{src.stem}.{os.getpid()}.tmp.o"
         jobs.append((obj, tmp, subprocess.Popen([nvcc, *NVCC_FLAGS, *extra, "-c", "-o", str(tmp), str(src)])))

@@ -480,6 +480,25 @@ def test_theiler_window_brute_force(oracle, w):
         assert np.array_equal(hist, oracle.line_hist(y, m, tau, eps, oracle.NORM_MAX))
 
 
+def test_certificate_with_theiler_window(oracle):
+    """count_lt_le over the pairs with j - i >= w brackets the rank of the windowed order statistic, and agrees with a
+    numpy count on the full distance matrix."""
+    y = np.round(wl.gaussian(321, 150) * 5).astype(np.float32) / 5
+    for w in (1, 2, 9, 140):
+        rr = [0.05, 0.3, 0.9]
+        eps, cnt, _ = oracle.eps_for_rr(y, 2, 3, rr, 0, theiler=w)
+        lt, le = oracle.count_lt_le(y, 2, 3, eps, 0, threads=2, theiler=w)
+        n = len(y) - 3
+        Pw = (n - w) * (n - w + 1) // 2
+        D = _numpy_condensed_full(y, 2, 3, 0)
+        i, j = np.indices(D.shape)
+        sel = (j - i) >= w
+        for k in range(3):
+            r = oracle.rank(rr[k], Pw)
+            assert lt[k] < r <= le[k] and le[k] == cnt[k]
+            assert lt[k] == int((D[sel] < eps[k]).sum()) and le[k] == int((D[sel] <= eps[k]).sum())
+
+
 # ------------------------------------------------------------------ vertical lines (reading S19; LAM, TT)
 VGOLDEN = Path(__file__).resolve().parent / "golden" / "hand_cases_vertical.txt"
 

@@ -279,6 +279,22 @@ def other_configs(rqa):
                     "unit": UNIT, "gpu_launches_per_call": int(launches)})
         del buf, s
         torch.cuda.empty_cache()
+    # stream-level overlap for the grid (row f4): the nine groups of one series length, one stream vs four
+    from paper_2208_09136_b200 import experiment
+    for N in (100, 1000):
+        groups = experiment.grid_groups(N)
+        units = sum(w.units for w in groups)
+        res = {}
+        for ns in (1, 4):
+            runner = experiment.GridRunner(groups, streams=ns)
+            med, mn = time_call(runner.run)
+            res[ns] = med
+            del runner
+            torch.cuda.empty_cache()
+        out.append({"workload": f"paper_grid_9groups_x100_N{N}", "batch": 900, "N": N, "K": 99, "ms_per_call": res[4],
+                    "ms_one_stream": res[1], "streams": 4, "value": units / (res[4] * 1e-3), "unit": UNIT,
+                    "note": "nine groups (3 dynamics x 3 SNR levels) of 100 series each, every group its own call chain; host "
+                            "enqueue time is inside the interval"})
     return out
 
 

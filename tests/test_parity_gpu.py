@@ -845,3 +845,25 @@ def test_bench_launches_its_own_ranks_split_mode(rqa):
     d = json.loads(line[0])
     assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["gpu_launches"] > 0 and "functional_test_only" in d
     assert d["config"]["parallelism"].startswith("one batch split over 2 ranks")
+
+
+def test_grid_groups_on_several_streams(rqa, oracle):
+    """Stream-level overlap for the paper's grid (row f4): the nine groups of one series length enqueued round robin on
+    four streams give exactly what one stream gives, and what the oracle gives for a sample of the series."""
+    import torch
+    from paper_2208_09136_b200 import experiment
+    groups = experiment.grid_groups(100, n_real=2, K=99)
+    assert len(groups) == 9 and all(w.batch == 20 for w in groups)
+    one = experiment.GridRunner(groups, streams=1)
+    b1, p1 = one.run()
+    four = experiment.GridRunner(groups, streams=4)
+    for _ in range(3):                                             # repeated runs reuse the buffers
+        b4, p4 = four.run()
+    for g, w in enumerate(groups):
+        assert torch.equal(b1[g].eps, b4[g].eps) and torch.equal(b1[g].count, b4[g].count)
+        assert torch.equal(b1[g].hist, b4[g].hist) and torch.equal(p1[g], p4[g])
+        for b in (0, 13):
+            r = oracle.sweep(w.series[b], w.m, w.tau, w.rr, w.norm, 2, threads=0)
+            assert np.array_equal(b4[g].eps[b].cpu().numpy(), r["eps"])
+            assert np.array_equal(b4[g].hist[b].cpu().numpy().view(np.uint64), r["hist"])
+            assert np.max(np.abs(p4[g][b].cpu().numpy() - oracle.det_prefix_avg(r["det"]))) <= DET_TOL

@@ -4,7 +4,7 @@
 // of the level tables.  Internal to librqa.so; nothing here is shared with the oracle.
 //
 // Tiling.  The recurrence plot's upper triangle (only j > i is visited, R_ij is computed on the
-// fly) is cut into diagonal blocks of LW = 256 adjacent diagonals o = j - i (one per thread), and every diagonal
+// fly) is cut into diagonal blocks of LW = 512 adjacent diagonals o = j - i (one per thread), and every diagonal
 // block into chunks of L consecutive positions i.  A tile = (diagonal block, chunk).  The lanes of a warp sit on
 // 32 adjacent diagonals at the same position i, so y[i] is a shared-memory broadcast and y[i + o] is 32
 // consecutive words: no bank conflicts.

@@ -867,3 +867,42 @@ def test_grid_groups_on_several_streams(rqa, oracle):
             assert np.array_equal(b4[g].eps[b].cpu().numpy(), r["eps"])
             assert np.array_equal(b4[g].hist[b].cpu().numpy().view(np.uint64), r["hist"])
             assert np.max(np.abs(p4[g][b].cpu().numpy() - oracle.det_prefix_avg(r["det"]))) <= DET_TOL
+
+
+def test_kernel_event_hooks_and_nccl_reduce_wrapper(rqa):
+    """rqa_options.ev_kernel_begin/end: the library records the caller's two events around its dominant kernel (what
+    bench.py's roofline times), for both heavy calls.  And parts.dist_reduce under NCCL: an in-place all-reduce on a
+    tensor that wraps raw device counters (world size 1 here — one GPU —, which still goes through NCCL's all-reduce)."""
+    import os
+    import subprocess
+    import sys
+    import torch
+    from paper_2208_09136_b200 import binding as B
+    w = wl.config3(0)
+    s = torch.as_tensor(w.series[:2]).cuda()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    o_sel, o_line = B.make_options(kernel_events=ev[:2]), B.make_options(kernel_events=ev[2:])
+    buf = rqa.SweepBuffers.allocate(s, w.m, w.tau, w.K)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    B.rqa_eps_for_rr(buf.view, w.norm, w.rr, buf.eps, buf.count, buf.rr, buf.ws, options=o_sel)
+    B.rqa_line_hist(buf.view, w.norm, buf.eps, buf.hist, buf.ws, options=o_line)
+    b.record()
+    torch.cuda.synchronize()
+    t_count, t_scan, t_all = ev[0].elapsed_time(ev[1]), ev[2].elapsed_time(ev[3]), a.elapsed_time(b)
+    assert 0 < t_count < t_all and 0 < t_scan < t_all and a.elapsed_time(ev[0]) > 0 and ev[1].elapsed_time(ev[2]) > 0
+    code = ("import os, torch, torch.distributed as dist\n"
+            "from paper_2208_09136_b200 import parts\n"
+            "os.environ.update(MASTER_ADDR='127.0.0.1', MASTER_PORT='29533')\n"
+            "torch.cuda.set_device(0)\n"
+            "dist.init_process_group('nccl', rank=0, world_size=1)\n"
+            "t = torch.tensor([5, -3, 1 << 62], dtype=torch.int64, device='cuda')\n"
+            "parts.dist_reduce('cuda')(t.data_ptr(), 3, 0)\n"
+            "torch.cuda.synchronize()\n"
+            "assert t.tolist() == [5, -3, 1 << 62]\n"
+            "dist.destroy_process_group()\nprint('nccl ok')\n")
+    from pathlib import Path
+    root = str(Path(__file__).resolve().parent.parent)
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300, cwd=root,
+                         env=dict(os.environ, PYTHONPATH=root))
+    assert out.returncode == 0 and "nccl ok" in out.stdout, out.stderr[-1500:]

@@ -157,6 +157,30 @@ def test_ramp_closed_form_large(rqa, N, m, tau):
         assert np.array_equal(g["hist"][0, k], exp)
 
 
+@pytest.mark.slow
+def test_ramp_closed_form_a_million_points(rqa):
+    """The same closed form at N = 1e6 (P = 5e11 cells, ten times the headline length; 1 953 diagonal blocks, about two
+    million tiles per pass): 64-bit cell counts, tile tables and ranks far beyond 2^32, lines of a million cells joined
+    across two thousand segments.  The closed form is evaluated arithmetically (no loop over o)."""
+    N, m, tau = 1_000_000, 3, 1
+    y = np.arange(N, dtype=np.float32)                        # exact in fp32 up to 2^24
+    n = N - (m - 1) * tau
+    P = n * (n - 1) // 2
+    rr = np.array([1e-6, 0.001, 0.05, 0.2])
+    g = gpu_sweep(rqa, y, m, tau, rr, 0)
+    for k, q in enumerate(rr):
+        rank = min(max(math.ceil(q * float(P)), 1), P)
+        # smallest o* with sum_{o<=o*} (n - o) = o*(2n - o* - 1)/2 >= rank
+        ostar = int((2 * n - 1 - math.sqrt((2 * n - 1) ** 2 - 8 * rank)) / 2) - 2
+        ostar = max(ostar, 0)
+        while ostar * (2 * n - ostar - 1) // 2 < rank:
+            ostar += 1
+        cum = ostar * (2 * n - ostar - 1) // 2
+        assert g["eps"][0, k] == np.float32(ostar) and int(g["count"][0, k]) == cum
+        h = g["hist"][0, k]
+        assert int(h.sum()) == ostar and np.all(h[n - ostar:] == 1)
+
+
 def test_max_k_and_k1(rqa, oracle):
     y = wl.add_noise(wl.lorenz_signal(600), 1.0, 5)
     rr = wl.rr_log(128, 0.0005, 0.9)

@@ -40,8 +40,18 @@ def _newest_header() -> float:
     return max(h.stat().st_mtime for h in headers)
 
 
+def _src_mtime(src: Path) -> float:
+    """mtime of a translation unit = its own and that of any .cu file it includes (rqa_fused_scan.cu includes rqa_line.cu)."""
+    import re
+    t = src.stat().st_mtime
+    for inc in re.findall(r'#include\s+"([^"]+\.cu)"', src.read_text()):
+        if (CSRC / inc).exists():
+            t = max(t, (CSRC / inc).stat().st_mtime)
+    return t
+
+
 def _obj_stale(src: Path, obj: Path, newest_header: float) -> bool:
-    return not obj.exists() or obj.stat().st_mtime <= max(src.stat().st_mtime, newest_header)
+    return not obj.exists() or obj.stat().st_mtime <= max(_src_mtime(src), newest_header)
 
 
 def _stale() -> bool:

@@ -278,25 +278,6 @@ typedef struct rqa_options {
 } rqa_options;
 
 rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_options* opt, size_t* bytes);
-
-/*
- * rqa_eps_for_rr + rqa_line_hist in one call, with ONE full pass over the recurrence plot instead of two where that is
- * possible: same arguments, same outputs (d_eps, d_count, d_rr_realised as rqa_eps_for_rr,
- * d_hist as rqa_line_hist at those thresholds), bit for bit.  How: brackets (lo_k, hi_k] around every eps_k from a sample
- * of the distances; the diagonal scan runs at the thresholds lo_k, its exact level counts and a log of the few cells inside
- * the brackets give eps_k and C_k exactly, and the histograms are then corrected from lo_k to eps_k by re-walking only the
- * runs that a logged cell with lo_k < d <= eps_k joins.  Applies to K <= 32 thresholds on views the tiled scan handles with
- * more than 2^22 pairs, unsplit; otherwise, and whenever a series does not come through (a bracket miss: probability
- * < 1e-5 per threshold; massive ties; an overflowing log), the call runs rqa_eps_for_rr and rqa_line_hist itself.
- * Unlike the other device calls this one SYNCHRONISES the stream once (it has to look at the per-series outcome before it
- * can return); the outputs are complete on return.  opt may be NULL.
- */
-rqa_status rqa_sweep(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps, uint64_t* d_count,
-                     double* d_rr_realised, uint64_t* d_hist, void* d_ws, size_t ws_bytes, void* stream,
-                     const rqa_options* opt);
-/* Which way the calling thread's last rqa_sweep went (like rqa_last_error, thread-local): 1 = one pass, 2 = two passes because
- * the one-pass sweep does not apply to the call, 3 = two passes after an attempt in which some series did not come through. */
-int32_t rqa_sweep_last_path(void);
 rqa_status rqa_eps_for_rr_opt(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps,
                               uint64_t* d_count, double* d_rr_realised, void* d_ws, size_t ws_bytes, void* stream,
                               const rqa_options* opt);

@@ -29,7 +29,7 @@ EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_
            "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
            "rqa_sweep_host", "rqa_launch_count", "rqa_workspace_bytes_opt", "rqa_eps_for_rr_opt", "rqa_line_hist_opt",
            "rqa_det_prefix_avg", "rqa_line_measures", "rqa_sorting_rate_host", "rqa_vert_hist", "rqa_vert_hist_opt",
-           "rqa_lam_tt", "rqa_sweep", "rqa_sweep_last_path"]
+           "rqa_lam_tt"]
 
 
 class RqaPoints(ctypes.Structure):
@@ -124,7 +124,6 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_vert_hist.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp]
     lib.rqa_vert_hist_opt.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp, opt]
     lib.rqa_lam_tt.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp]
-    lib.rqa_sweep.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, vp, vp, vp, sz, vp, opt]
     _lib = lib
     return lib
 
@@ -205,22 +204,6 @@ def rqa_eps_for_rr(pts: RqaPoints, norm: int, rr, eps, count, rr_realised, ws, s
                                              _dev(eps, torch.float32, "eps", bk), _dev(count, torch.int64, "count", bk),
                                              _dev(rr_realised, torch.float64, "rr_realised", bk),
                                              _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream), _opt(options)))
-
-
-def rqa_sweep(pts: RqaPoints, norm: int, rr, eps, count, rr_realised, hist, ws, stream=None, options: RqaOptions = None) -> None:
-    """rqa_eps_for_rr + rqa_line_hist in one call (one full pass where possible); synchronises the stream."""
-    import torch
-    rr = np.ascontiguousarray(rr, dtype=np.float64)
-    K = len(rr)
-    bk = int(pts.batch) * K
-    _check(load_library().rqa_sweep(ctypes.byref(pts), norm, rr.ctypes.data, K, _dev(eps, torch.float32, "eps", bk),
-                                    _dev(count, torch.int64, "count", bk), _dev(rr_realised, torch.float64, "rr_realised", bk),
-                                    _dev(hist, torch.int64, "hist", bk * int(pts.n_points)), _dev(ws, torch.uint8, "ws"),
-                                    ws.numel(), _stream(stream), _opt(options)))
-
-
-def rqa_sweep_last_path() -> int:
-    return int(load_library().rqa_sweep_last_path())
 
 
 def rqa_line_hist(pts: RqaPoints, norm: int, eps, hist, ws, stream=None, options: RqaOptions = None) -> None:

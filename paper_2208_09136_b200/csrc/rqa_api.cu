@@ -12,7 +12,6 @@
 namespace rqa {
 
 static thread_local char t_err[512] = "";
-static thread_local int t_sweep_path = 0;
 std::atomic<uint64_t> g_launches{0};
 
 rqa_status make_options(const rqa_options* in, Options* out, const char* who) {
@@ -207,8 +206,7 @@ rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_o
     if (st != RQA_OK) return st;
     View v = make_view(p);
     size_t a = select_workspace_bytes(v, K, o), b = line_workspace_bytes(v, K, o), c = vert_workspace_bytes(v, K, o);
-    size_t d = fused_workspace_bytes(v, K, o);
-    *bytes = sizeof(WsStatus) + std::max(std::max(a, d), std::max(b, c));
+    *bytes = sizeof(WsStatus) + std::max(a, std::max(b, c));
     return RQA_OK;
 }
 
@@ -313,52 +311,6 @@ rqa_status rqa_line_hist_opt(const rqa_points* pts, rqa_norm norm, const float* 
     if (st != RQA_OK) return st;
     return run_line_hist(v, (int)norm, d_eps, K, d_hist, ws, s, o);
 }
-
-rqa_status rqa_sweep(const rqa_points* pts, rqa_norm norm, const double* h_rr, int32_t K, float* d_eps, uint64_t* d_count,
-                     double* d_rr_realised, uint64_t* d_hist, void* d_ws, size_t ws_bytes, void* stream,
-                     const rqa_options* opt) {
-    rqa_status st = validate_points(pts, "rqa_sweep");
-    if (st != RQA_OK) return st;
-    Options o;
-    st = make_options(opt, &o, "rqa_sweep");
-    if (st != RQA_OK) return st;
-    if (norm != RQA_NORM_MAX && norm != RQA_NORM_EUCLID) { set_error("rqa_sweep: unknown norm %d", (int)norm); return RQA_ERR_INVALID_ARG; }
-    if (K < 1 || K > RQA_MAX_K) { set_error("rqa_sweep: K = %d outside 1..%d", K, RQA_MAX_K); return RQA_ERR_INVALID_ARG; }
-    if (!h_rr || !d_eps || !d_count || !d_rr_realised || !d_hist || !d_ws) { set_error("rqa_sweep: NULL argument"); return RQA_ERR_INVALID_ARG; }
-    if (((uintptr_t)d_ws & 255) != 0) { set_error("rqa_sweep: workspace must be 256-byte aligned"); return RQA_ERR_INVALID_ARG; }
-    View v = make_view(*pts);
-    const uint64_t P = n_pairs(v);
-    uint64_t rank[RQA_MAX_K];
-    for (int k = 0; k < K; ++k) {
-        const double rr = h_rr[k];
-        if (!(rr > 0.0) || !(rr <= 1.0)) { set_error("rqa_sweep: rr[%d] = %g outside (0, 1]", k, rr); return RQA_ERR_INVALID_ARG; }
-        const double r = std::ceil(rr * (double)P);          // the literal fp64 expression, clamped to [1, P] (reading S5)
-        rank[k] = !(r >= 1.0) ? 1 : (r >= (double)P ? P : (uint64_t)r);
-    }
-    size_t need = 0;
-    st = rqa_workspace_bytes_opt(pts, K, opt, &need);
-    if (st != RQA_OK) return st;
-    if (ws_bytes < need) { set_error("rqa_sweep: workspace %zu < %zu bytes", ws_bytes, need); return RQA_ERR_WORKSPACE_TOO_SMALL; }
-    cudaStream_t s = (cudaStream_t)stream;
-    {
-        Arena ws(d_ws, ws_bytes);
-        WsStatus* status = ws.take<WsStatus>(1);
-        st = launch_finite_check(v, status, s);
-        if (st != RQA_OK) return st;
-        int failed = 0;
-        st = run_sweep_fused(v, (int)norm, rank, K, d_eps, d_count, d_rr_realised, d_hist, ws, s, o, &failed);
-        if (st == RQA_OK && failed == 0) { t_sweep_path = 1; return RQA_OK; }
-        if (st != RQA_OK && st != RQA_ERR_UNSUPPORTED) return st;
-        t_sweep_path = st == RQA_ERR_UNSUPPORTED ? 2 : 3;
-    }
-    // the one-pass sweep does not apply to this call, or some series did not come through (a bracket miss, massive ties,
-    // an overflowing log): the two-pass path, which handles everything
-    st = rqa_eps_for_rr_opt(pts, norm, h_rr, K, d_eps, d_count, d_rr_realised, d_ws, ws_bytes, stream, opt);
-    if (st != RQA_OK) return st;
-    return rqa_line_hist_opt(pts, norm, d_eps, K, d_hist, d_ws, ws_bytes, stream, opt);
-}
-
-int32_t rqa_sweep_last_path(void) { return t_sweep_path; }
 
 rqa_status rqa_vert_hist(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_vhist,
                          void* d_ws, size_t ws_bytes, void* stream) {

@@ -143,28 +143,6 @@ size_t vert_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_vhist, Arena& ws,
                          cudaStream_t s, const Options& opt);
 
-// Fused sweep (thresholds and line histograms from ONE full pass; rqa_select.cu: run_sweep_fused).  The scan runs at the
-// lower ends of the sample brackets and logs the cells inside the brackets.
-struct LineLog {
-    const float* hi;              // [batch][K] upper bracket end of threshold k (a negative value: nothing is logged)
-    float* cand_d;                // [batch][cap]
-    unsigned long long* cand_pos; // [batch][cap]  diagonal << 32 | index along it
-    unsigned long long* cand_n;   // [batch] entries reserved (zeroed by the caller)
-    unsigned long long* ncand;    // [batch][33] candidates per level (zeroed by the caller)
-    unsigned long long cap;
-    void* groups_out;             // out: the scan's per-series level tables (LineGroup[batch]) ...
-    unsigned long long* agg_out;  // ... and aggregates [batch][3][33], valid until the workspace is reused
-    int NP_out;
-};
-bool line_scan_applies(const View& v, int K, const Options& opt);
-rqa_status run_line_hist_log(const View& v, int norm, const float* d_lo, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s,
-                             const Options& opt, LineLog* lg);
-size_t fused_workspace_bytes(const View& v, int K, const Options& opt);
-// *h_failed = number of series the fused pass could not finish (bracket miss, candidate overflow, ties): the caller
-// recomputes the batch with the two-pass path.  Synchronises the stream once.
-rqa_status run_sweep_fused(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
-                           double* d_rr, uint64_t* d_hist, Arena& ws, cudaStream_t s, const Options& opt, int* h_failed);
-
 // Number of SMs of the current device (cached per thread; 148 on a B200).
 int sm_count();
 

@@ -147,27 +147,10 @@ struct ScanArgs {
     unsigned int* counter;      // work-item counter (zeroed before the launch)
     uint32_t segs;              // segments per series (this part)
     int m, tau;                 // run-time embedding (used by the M == 0 variant)
-    // candidate log of the fused sweep (only read by the LOG instantiations; rqa_fused.cu)
-    const float* log_hi;        // [batch][K] upper bracket end of the caller's threshold k (the thresholds are the lower ends)
-    float* log_d;               // [batch][log_cap] candidate values
-    unsigned long long* log_pos;  // [batch][log_cap] candidate positions
-    unsigned long long* log_n;  // [batch] entries reserved
-    unsigned long long* log_ncand;  // [batch][GK+1] candidates per level
-    unsigned long long log_cap;
 };
-
-#ifdef RQA_LINE_LOG
-constexpr bool LINE_LOG = true;
-#else
-constexpr bool LINE_LOG = false;
-#endif
 
 template <int NORM, int M, int TAU, int NP>
 __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanArgs a) {
-    constexpr bool LOG = LINE_LOG;
-    __shared__ float s_hi[GK];
-    __shared__ uint32_t s_ncand[GK + 1];
-    __shared__ __align__(8) unsigned long long s_chunk[LW / 32][2];
     using SM = ScanSmem<NP>;
     constexpr bool VECK = scan_vec<M, TAU, NP>();              // vector loads of the i-side window: one set, plain staging
     extern __shared__ __align__(16) char smem[];
@@ -221,15 +204,6 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
                (((uintptr_t)a.v.data) & 3) == 0;
     };
 
-    int log_b = -1;                                            // LOG: the series the warps' open chunks belong to
-    auto close_chunks = [&](int bb) {
-        const unsigned long long base = s_chunk[tid >> 5][0];
-        const uint32_t used = (uint32_t)s_chunk[tid >> 5][1];
-        float* cd = a.log_d + (unsigned long long)bb * a.log_cap;
-        for (uint32_t q = used + (tid & 31); q < LOG_CHUNK; q += 32)
-            if (base + q < a.log_cap) cd[base + q] = __uint_as_float(LOG_HOLE);
-    };
-
     while (true) {
         if (tid == 0) s_item = atomicAdd(a.counter, 1u);
         __syncthreads();
@@ -245,24 +219,7 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
             if (tid <= GK) eps_s[tid] = G.epsd[tid];
             if (tid < GK) s_rep[tid] = G.rep_k[tid];
             stk_s[tid] = (uint16_t)J;                          // the sentinel below every stack
-            if (LOG && tid < J) {                              // upper bracket end of every distinct threshold
-                float h = 0.0f;
-                for (int q = 0; q < G.kcount; ++q)
-                    if (G.j_of[q] == tid) h = fmaxf(h, a.log_hi[(int64_t)b * a.K + G.k_of[q]]);
-                s_hi[tid] = h;
-            }
             cur_b = b;
-        }
-        if (LOG) {
-            if (tid <= GK) s_ncand[tid] = 0;
-            if (b != log_b) {
-                // a warp keeps its chunk of the series' list across items; when the block moves to another series the
-                // chunks are closed (their unused rest becomes holes)
-                if (log_b >= 0) close_chunks(log_b);
-                __syncthreads();
-                if (tid < LW / 32) { s_chunk[tid][0] = 0; s_chunk[tid][1] = LOG_CHUNK; }   // no chunk yet: the first append reserves one
-                log_b = b;
-            }
         }
         __syncthreads();
         const int q_ob = s_q;
@@ -345,25 +302,14 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
                     sc.w2a = sc.w2b = sc.J4;
                     sc.xa = sc.xb = 0;
                     sc.A = 0; sc.ts = 0; sc.top = sc.stk;       // every threshold: recurrent since the chunk start
-                    if (LOG) {
-                        sc.lg.hi = smem_addr(s_hi);
-                        sc.lg.ncand = smem_addr(s_ncand);
-                        sc.lg.chunk = smem_addr(&s_chunk[tid >> 5][0]);
-                        sc.lg.cand_d = a.log_d + (unsigned long long)b * a.log_cap;
-                        sc.lg.cand_pos = a.log_pos + (unsigned long long)b * a.log_cap;
-                        sc.lg.cand_n = a.log_n + b;
-                        sc.lg.cap = a.log_cap;
-                        sc.lg.diag = (uint32_t)o;
-                        sc.lg.row0 = (uint32_t)s;
-                    }
                 };
                 const int first_real = -(int)min((int64_t)2, s);   // warm-up cells before it lie outside the plot
                 if (G.multi) {
-                    Scanner<NORM, M, TAU, NP, true, LOG> sc;
+                    Scanner<NORM, M, TAU, NP, true> sc;
                     setup(sc);
                     scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org);
                 } else {
-                    Scanner<NORM, M, TAU, NP, false, LOG> sc;
+                    Scanner<NORM, M, TAU, NP, false> sc;
                     setup(sc);
                     scan_chunk(sc, cnt, cnt_lo, cnt_hi, first_real, yb_org);
                 }
@@ -382,12 +328,8 @@ __global__ void __launch_bounds__(LW, (NP <= 10 ? 2 : 1)) line_scan_kernel(ScanA
             }
         }
         flush_item(tot_s, sh_s, J, a.agg + ((int64_t)b * a.NG + a.g) * 3 * (GK + 1), grow, s_rep, n);
-        if (LOG) {                                            // hand over the item's candidate counts
-            if (tid <= GK && s_ncand[tid]) atomicAdd(&a.log_ncand[(int64_t)b * (GK + 1) + tid], (unsigned long long)s_ncand[tid]);
-        }
         __syncthreads();                                       // before s_item / the tables are overwritten
     }
-    if (LOG && log_b >= 0) close_chunks(log_b);
 }
 
 // ---------------------------------------------------------------------------------------- stitching
@@ -549,7 +491,7 @@ size_t scan_smem_bytes(int NP, int L, int span, int ps, int nbuf) {
     return NP == 5 ? scan_smem_bytes<5>(L, span, ps, nbuf)
                    : (NP == 10 ? scan_smem_bytes<10>(L, span, ps, nbuf) : scan_smem_bytes<16>(L, span, ps, nbuf));
 }
-constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 1024;    // opt-in limit of sm_100a, minus the static part (672 B with the log)
+constexpr size_t SMEM_PER_BLOCK_MAX = 227 * 1024 - 256;     // opt-in limit of sm_100a, minus the static part
 constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_BLOCK_RESERVED = 1024;
 
 LinePlan make_plan(const View& v, int K, const Options& opt) {
@@ -664,7 +606,6 @@ __global__ void line_eps_check_kernel(const float* __restrict__ eps, int64_t cou
 
 }  // namespace
 
-#ifndef RQA_LINE_LOG
 int scan_pairs_for(int kg) { return kg <= 10 ? 5 : (kg <= 20 ? 10 : 16); }
 
 rqa_status launch_line_groups(const float* d_eps, int K, int NG, int batch, void* groups, WsStatus* status, cudaStream_t s) {
@@ -702,27 +643,16 @@ size_t line_workspace_bytes(const View& v, int K, const Options& opt) {
     return a.off;
 }
 
-// The tiled scan applies to this call (not the short-series kernel, not the strided fallback) with one threshold group.
-bool line_scan_applies(const View& v, int K, const Options& opt) {
-    const bool small = opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K);
-    return !small && K <= GK && make_plan(v, K, opt).scan && make_plan(v, K, opt).tl.tiles > 0;
-}
-#endif  // !RQA_LINE_LOG
-
-// The body of rqa_line_hist.  lg != nullptr (only in the translation unit built with RQA_LINE_LOG, rqa_fused_scan.cu): the
-// scan also logs the cells inside the sample brackets for the fused sweep and reports where its level tables and
-// aggregates live.
-static rqa_status line_hist_impl(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s,
-                                 const Options& opt, LineLog* lg) {
+rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s,
+                         const Options& opt) {
     WsStatus* status = (WsStatus*)ws.base;
     const size_t hist_words = (size_t)v.batch * K * v.n;
     // short series: one block per series, shared-memory distances and histogram (explicit scan knobs and split calls
     // keep the general machinery)
-    if (!lg && opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
+    if (opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
         return run_line_small(v, norm, d_eps, K, d_hist, status, s);
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * hist_words, s));
     LinePlan p = make_plan(v, K, opt);
-    if (lg && !p.scan) { set_error("fused sweep: the tiled scan does not apply"); return RQA_ERR_UNSUPPORTED; }
     if (!p.scan) {
         // thread-per-diagonal fallback: the diagonals are dealt to the parts block by block
         line_eps_check_kernel<<<1, 256, 0, s>>>(d_eps, (int64_t)v.batch * K, status);
@@ -755,12 +685,6 @@ static rqa_status line_hist_impl(const View& v, int norm, const float* d_eps, in
         a.groups = w.groups; a.seg_start = w.seg_start; a.hist = (unsigned long long*)d_hist; a.agg = w.agg;
         a.pre = w.pre; a.suf = w.suf; a.carry = w.carry; a.counter = w.counters + g; a.segs = (uint32_t)p.tl.tiles;
         a.m = v.m; a.tau = (int)v.cs;
-        a.log_hi = nullptr; a.log_d = nullptr; a.log_pos = nullptr; a.log_n = nullptr; a.log_ncand = nullptr; a.log_cap = 0;
-        if (lg) {
-            a.log_hi = lg->hi; a.log_d = lg->cand_d; a.log_pos = lg->cand_pos; a.log_n = lg->cand_n; a.log_ncand = lg->ncand;
-            a.log_cap = lg->cap;
-            lg->groups_out = w.groups; lg->agg_out = w.agg; lg->NP_out = p.NP;
-        }
         if (g == 0 && opt.ev_begin) RQA_CUDA_TRY(cudaEventRecord((cudaEvent_t)opt.ev_begin, s));
         rqa_status st = norm == RQA_NORM_MAX ? dispatch_pairs<RQA_NORM_MAX>(a, p, s) : dispatch_pairs<RQA_NORM_EUCLID>(a, p, s);
         if (st != RQA_OK) return st;
@@ -786,17 +710,5 @@ static rqa_status line_hist_impl(const View& v, int norm, const float* d_eps, in
     }
     return RQA_OK;
 }
-
-#ifndef RQA_LINE_LOG
-rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s,
-                         const Options& opt) {
-    return line_hist_impl(v, norm, d_eps, K, d_hist, ws, s, opt, nullptr);
-}
-#else
-rqa_status run_line_hist_log(const View& v, int norm, const float* d_lo, int K, uint64_t* d_hist, Arena& ws, cudaStream_t s,
-                             const Options& opt, LineLog* lg) {
-    return line_hist_impl(v, norm, d_lo, K, d_hist, ws, s, opt, lg);
-}
-#endif
 
 }  // namespace rqa

@@ -70,26 +70,9 @@ template <int M, int TAU, int NP>
 __host__ __device__ constexpr bool scan_vec() { return M == 3 && TAU == 1 && NP > 5; }
 
 // CDT supplies the cell distances along the walk (CellDist: a diagonal of the plot; ColDist in rqa_vert.cu: a column).
-// Candidate log of the fused sweep (rqa_fused.cu): the scan runs at the LOWER ends lo of the sample brackets and appends
-// every cell inside a bracket, lo_j < d <= hi_j for the cell's level j + 1, with its position, to a per-series list.
-struct ScanLogState {                 // per-thread view of the log (only in the LOG instantiations)
-    uint32_t hi;                      // shared-window address of hi[j]: upper bracket end of distinct threshold j
-    uint32_t ncand;                   // shared-window address of uint32 ncand[level]: candidates of this item per level
-    uint32_t chunk;                   // shared-window address of this warp's {uint64 base, uint32 used} chunk state
-    float* cand_d;                    // the series' candidate values
-    unsigned long long* cand_pos;     // ... and positions (diagonal << 32 | index along it)
-    unsigned long long* cand_n;       // entries reserved in the series' list
-    unsigned long long cap;
-    uint32_t diag;                    // this thread's diagonal o
-    uint32_t row0;                    // index along the diagonal of the chunk's first cell
-};
-constexpr uint32_t LOG_CHUNK = 64;    // entries a warp reserves at a time
-constexpr uint32_t LOG_HOLE = 0xffffffffu;   // value pattern of a reserved but unused entry (sorts last, skipped by the fix-up)
-
-template <class CDT, int NP, bool MULTI, bool LOG = false>
+template <class CDT, int NP, bool MULTI>
 struct ScannerT : CDT {
     using CD = CDT;
-    ScanLogState lg;                  // unused (and optimised away) unless LOG
     static constexpr int S = CD::S;
     using SM = ScanSmem<NP>;
 
@@ -190,44 +173,6 @@ struct ScannerT : CDT {
         ts = t - 3;
     }
 
-    // LOG: is the cell (distance d, level v4) inside a bracket?  v4 > 0 and d <= hi[v4/4 - 1].
-    __device__ __forceinline__ bool in_bracket(float d, uint32_t v4) const {
-        return v4 != 0 && d <= lds_f32(lg.hi + v4 - 4);
-    }
-    // LOG: append the cells flagged `c` of one warp-cell (call with the warp converged).  A warp writes into chunks of
-    // LOG_CHUNK entries it reserves from the series' list with one global atomic; a chunk that cannot take the next
-    // batch is closed (its rest marked as holes).
-    __device__ __noinline__ void log_append(bool c, float d, uint32_t v4, uint32_t t) {
-        const unsigned mc = __ballot_sync(FULL, c);
-        if (!mc) return;
-        const uint32_t lane = threadIdx.x & 31, n = __popc(mc);
-        unsigned long long base;
-        uint32_t used;
-        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(base) : "r"(lg.chunk) : "memory");
-        asm volatile("ld.shared.u32 %0, [%1+8];" : "=r"(used) : "r"(lg.chunk) : "memory");
-        if (used + n > LOG_CHUNK) {
-            for (uint32_t q = used + lane; q < LOG_CHUNK; q += 32)
-                if (base + q < lg.cap) lg.cand_d[base + q] = __uint_as_float(LOG_HOLE);
-            if (lane == 0) base = atomicAdd(lg.cand_n, (unsigned long long)LOG_CHUNK);
-            base = __shfl_sync(FULL, base, 0);
-            used = 0;
-        }
-        if (c) {
-            const unsigned long long idx = base + used + __popc(mc & ((1u << lane) - 1u));
-            if (idx < lg.cap) {
-                lg.cand_d[idx] = d;
-                lg.cand_pos[idx] = ((unsigned long long)lg.diag << 32) | (unsigned long long)(lg.row0 + t);
-            }
-            red_u32(lg.ncand + v4, 1u);
-        }
-        __syncwarp();
-        if (lane == 0) {
-            asm volatile("st.shared.u64 [%0], %1;" :: "r"(lg.chunk), "l"(base) : "memory");
-            asm volatile("st.shared.u32 [%0+8], %1;" :: "r"(lg.chunk), "r"(used + n) : "memory");
-        }
-        __syncwarp();
-    }
-
     // One cell.  R = offset from the cursor = ring phase (static), t = position inside the chunk (t < 0: warm-up
     // cells before the chunk), cnt = this lane's number of cells.  PHASE 0: the first cells of the chunk (t < 4,
     // guarded), 1: the part of the chunk where every lane is inside (unguarded; t is not used), 2: the tail (guarded).
@@ -240,13 +185,6 @@ struct ScannerT : CDT {
             uint32_t v4 = t < first_real ? J4 : level4(CD::template distance<R>());
             v2 = v1; v1 = v4;
             return;
-        }
-        if (LOG && GUARD) {
-            // the guarded phases log cell by cell (lanes outside the chunk take part in the vote with no candidate)
-            const bool real = t < cnt;
-            const float dl = CD::template distance<R>();
-            const uint32_t vl = level4(dl);
-            log_append(real && in_bracket(dl, vl), dl, vl, (uint32_t)t);
         }
         if (GUARD && t >= cnt) return;
         const float d = CD::template distance<R>();
@@ -304,31 +242,17 @@ struct ScannerT : CDT {
         v2 = v1; v1 = v4;
         w2b = w2a; w2a = w2;
     }
-    template <int R>
-    __device__ __forceinline__ uint32_t level_of_cell(float& d) {
-        CD::template push<R>();
-        d = CD::template distance<R>();
-        return level4(d);
-    }
     template <int R0, int... Q>
-    __device__ __forceinline__ void group(int t, std::integer_sequence<int, Q...>) {
-        if constexpr (LOG) {
-            float d[sizeof...(Q)];
-            const uint32_t v[sizeof...(Q)] = {level_of_cell<R0 + Q>(d[Q])...};
-            const bool c[sizeof...(Q)] = {in_bracket(d[Q], v[Q])...};
-            if (__any_sync(FULL, (c[Q] || ...))) (log_append(c[Q], d[Q], v[Q], (uint32_t)(t + R0 + Q)), ...);
-            (account<R0 + Q>(v[Q]), ...);
-        } else {
-            const uint32_t v[sizeof...(Q)] = {level_of_cell<R0 + Q>()...};
-            (account<R0 + Q>(v[Q]), ...);
-        }
+    __device__ __forceinline__ void group(std::integer_sequence<int, Q...>) {
+        const uint32_t v[sizeof...(Q)] = {level_of_cell<R0 + Q>()...};
+        (account<R0 + Q>(v[Q]), ...);
     }
     template <int R0, int U>
-    __device__ __forceinline__ void groups(int t) {
+    __device__ __forceinline__ void groups() {
         if constexpr (R0 < U) {
             constexpr int G = U - R0 >= 4 ? 4 : U - R0;
-            group<R0>(t, std::make_integer_sequence<int, G>{});
-            groups<R0 + G, U>(t);
+            group<R0>(std::make_integer_sequence<int, G>{});
+            groups<R0 + G, U>();
         }
     }
 
@@ -352,7 +276,7 @@ struct ScannerT : CDT {
 
     template <int PHASE, int... R>
     __device__ __forceinline__ void superstep(int t, int cnt, int ds, std::integer_sequence<int, R...>) {
-        if constexpr (PHASE == 1) groups<0, (int)sizeof...(R)>(t);
+        if constexpr (PHASE == 1) groups<0, (int)sizeof...(R)>();
         else (cell<R, PHASE>(t + R, cnt, ds), ...);
         CD::advance((int)sizeof...(R));
         if (PHASE == 1) trel8 += (uint32_t)sizeof...(R) << 8;
@@ -382,8 +306,8 @@ struct ScannerT : CDT {
     }
 };
 
-template <int NORM, int M, int TAU, int NP, bool MULTI, bool LOG = false>
-using Scanner = ScannerT<CellDist<NORM, M, TAU, 2, scan_vec<M, TAU, NP>()>, NP, MULTI, LOG>;
+template <int NORM, int M, int TAU, int NP, bool MULTI>
+using Scanner = ScannerT<CellDist<NORM, M, TAU, 2, scan_vec<M, TAU, NP>()>, NP, MULTI>;
 
 // The walk of one thread along its chunk.  Two instantiations (MULTI) so that the common case, every bucket of the
 // level table holding at most one threshold, carries no refinement loop; a block executes only one of them.

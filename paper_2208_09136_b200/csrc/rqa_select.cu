@@ -26,10 +26,7 @@
 #include <cmath>
 #include <type_traits>
 
-#include <cstdio>
-#include <vector>
-
-#include "rqa_scan.cuh"
+#include "rqa_tiles.cuh"
 
 namespace rqa {
 
@@ -983,302 +980,7 @@ SelectWs carve(Arena& ws, const View& v, int K, const SelectPlan& p) {
     return w;
 }
 
-// =================================================================================== fused sweep
-// Thresholds AND line histograms from ONE full pass over the triangle (instead of the counting pass + the scan):
-//   1. sample brackets (lo_k, hi_k] as in the bracket path;
-//   2. the diagonal scan runs at the thresholds lo_k and logs every cell inside a bracket (value + position); its level
-//      aggregates are the exact counts #{d <= lo_k};
-//   3. the exact counts place each rank among the logged cells (a proof, as in the bracket path), the buffer select over
-//      the logged values returns eps_k and C_k;
-//   4. the histograms, built at lo_k, are corrected to eps_k: every logged cell with lo_k < d <= eps_k becomes recurrent at
-//      threshold k; the first such cell of each new run re-walks that run (distances recomputed), removes the old runs
-//      inside it and adds the new one.
-// Anything the brackets do not cover (a miss, overlapping brackets with uncovered cells, massive ties, an overflowing
-// log) marks the series as failed; the caller then recomputes the batch with the two-pass path.
-struct FusedTarget {                  // per caller threshold k
-    int32_t k_of[GK];                 // sorted position (by rank) -> caller index
-    unsigned long long rank[GK];      // caller index -> rank among all P distances
-    unsigned long long lo_rank[GK], hi_rank[GK];   // sorted position -> sample ranks of the bracket ends (0 = open)
-    int32_t K;
-};
-
-// One block per series: bracket ends from the sample order statistics, in the caller's order.
-__global__ void fused_bracket_kernel(const BufSel* __restrict__ st, FusedTarget ft, float* __restrict__ lo,
-                                     float* __restrict__ hi, int* __restrict__ fail) {
-    const int b = blockIdx.x;
-    const BufSel& s = st[b];
-    __shared__ int s_bad;
-    if (threadIdx.x == 0) s_bad = 0;
-    __syncthreads();
-    const int t = threadIdx.x;
-    float l = 0.0f, h = -1.0f;
-    if (t < ft.K) {
-        // an open end or a collapsed bracket (the sample sees massive ties) is left to the two-pass path
-        if (ft.lo_rank[t] == 0 || ft.hi_rank[t] == 0) s_bad = 1;
-        else {
-            l = s.out_val[2 * t];
-            h = s.out_val[2 * t + 1];
-            if (!(l < h)) s_bad = 1;
-        }
-    }
-    __syncthreads();
-    if (t < ft.K) {
-        const int k = ft.k_of[t];
-        lo[(int64_t)b * ft.K + k] = s_bad ? 0.0f : l;
-        hi[(int64_t)b * ft.K + k] = s_bad ? -1.0f : h;          // hi < 0: the scan logs nothing for this series
-    }
-    if (t == 0 && s_bad) fail[b] = 1;
-}
-
-// One block per series: exact level counts + candidate counts -> each target's rank among the logged cells.
-__global__ void __launch_bounds__(64) fused_resolve_kernel(FusedTarget ft, const void* __restrict__ groups_v,
-                                                          const unsigned long long* __restrict__ agg,
-                                                          const unsigned long long* __restrict__ ncand,
-                                                          const unsigned long long* __restrict__ cand_n,
-                                                          unsigned long long cap, unsigned long long P, int* __restrict__ fail,
-                                                          SelState* ss, BufSel* st) {
-    const int b = blockIdx.x;
-    const LineGroup& G = ((const LineGroup*)groups_v)[b];   // one threshold group (K <= 32)
-    __shared__ unsigned long long s_cum[GK + 2], s_cnd[GK + 2];
-    __shared__ int s_bad;
-    BufSel& bs = st[b];
-    SelState& S = ss[b];
-    if (threadIdx.x == 0) {
-        const int J = G.J;
-        const unsigned long long* ag = agg + (int64_t)b * 3 * (GK + 1);
-        const unsigned long long* nc = ncand + (int64_t)b * (GK + 1);
-        unsigned long long cum = 0, cnd = 0;
-        for (int v = 0; v <= J; ++v) {                       // level v = #{distinct lo < d}
-            cum += ag[v];
-            cnd += nc[v];
-            s_cum[v] = cum;                                  // cells of the levels 0..v
-            s_cnd[v] = cnd;                                  // logged cells of the levels 0..v
-        }
-        s_bad = fail[b] || cand_n[b] > cap || cum != P;
-#ifdef RQA_FUSED_DEBUG
-        printf("resolve b=%d J=%d fail=%d cand_n=%llu cap=%llu cum=%llu P=%llu cnd=%llu\n", b, J, fail[b], cand_n[b], cap, cum, P, cnd);
-#endif
-        bufsel_reset(bs, ft.K);
-        S.fallback = 0;
-        S.ncand_local = cand_n[b] < cap ? cand_n[b] : cap;
-    }
-    __syncthreads();
-    const int t = threadIdx.x;
-    int bad = s_bad;
-    if (t < ft.K) {
-        const int k = ft.k_of[t];
-        const unsigned long long r = ft.rank[k];
-        int j = -1;                                          // distinct index of the caller's threshold lo_k
-        for (int q = 0; q < G.kcount; ++q)
-            if (G.k_of[q] == k) j = G.j_of[q];
-        int v = 0;
-        while (v <= G.J && s_cum[v] < r) ++v;                // the level that holds rank r
-        const unsigned long long nc_v = v >= 1 && v <= G.J ? s_cnd[v] - s_cnd[v - 1] : 0;
-        bool ok = j >= 0 && v >= j + 1 && v <= G.J && r - s_cum[v - 1] <= nc_v;
-        // every cell of the levels between lo_k and the level of eps_k must have been logged
-        for (int u = j + 1; ok && u < v; ++u) ok = (s_cnd[u] - s_cnd[u - 1]) == (s_cum[u] - s_cum[u - 1]);
-        if (!ok) bad = 1;
-#ifdef RQA_FUSED_DEBUG
-        if (b == 0) printf("  t=%d k=%d r=%llu j=%d v=%d cum[v-1]=%llu cum[v]=%llu nc_v=%llu ok=%d\n", t, k, r, j, v, v >= 1 ? s_cum[v - 1] : 0ull, s_cum[v <= G.J ? v : G.J], nc_v, (int)ok);
-#endif
-        bs.group_of[t] = 0;
-        bs.prefix[t] = 0;
-        bs.below[t] = 0;
-        bs.resid[t] = ok ? s_cnd[v - 1] + (r - s_cum[v - 1]) : 1;
-        bs.base[t] = ok ? s_cum[v - 1] - s_cnd[v - 1] : 0;
-    }
-    if (__syncthreads_or(bad) && threadIdx.x == 0) { fail[b] = 1; S.fallback = 1; }
-}
-
-__global__ void fused_finish_kernel(const BufSel* __restrict__ st, FusedTarget ft, unsigned long long P,
-                                    const int* __restrict__ fail, float* __restrict__ eps,
-                                    unsigned long long* __restrict__ count, double* __restrict__ rr) {
-    const int b = blockIdx.x, t = threadIdx.x;
-    if (t >= ft.K || fail[b]) return;
-    const BufSel& s = st[b];
-    const int k = ft.k_of[t];
-    const unsigned long long c = s.base[t] + s.out_cnt[t];
-    eps[(int64_t)b * ft.K + k] = s.out_val[t];
-    count[(int64_t)b * ft.K + k] = c;
-    rr[(int64_t)b * ft.K + k] = (double)c / (double)P;
-}
-
-// One thread per logged cell: for every threshold k with lo_k < d <= eps_k the cell becomes recurrent.  The first such
-// cell of a new run (none between it and the run's start) re-walks the run and replaces the old runs inside it.
-template <int NORM>
-__global__ void __launch_bounds__(256) fused_fixup_kernel(View v, int K, const float* __restrict__ lo, const float* __restrict__ eps,
-                                                          const float* __restrict__ cand_d,
-                                                          const unsigned long long* __restrict__ cand_pos,
-                                                          const unsigned long long* __restrict__ cand_n, unsigned long long cap,
-                                                          const int* __restrict__ fail, unsigned long long* __restrict__ hist) {
-    const int b = blockIdx.y;
-    if (fail[b]) return;
-    __shared__ float s_lo[GK], s_eps[GK];
-    if (threadIdx.x < K) { s_lo[threadIdx.x] = lo[(int64_t)b * K + threadIdx.x]; s_eps[threadIdx.x] = eps[(int64_t)b * K + threadIdx.x]; }
-    __syncthreads();
-    const unsigned long long total = cand_n[b] < cap ? cand_n[b] : cap;
-    const float* yb = v.data + (int64_t)b * v.bs;
-    const float* cd = cand_d + (unsigned long long)b * cap;
-    const unsigned long long* cp = cand_pos + (unsigned long long)b * cap;
-    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
-         e += (unsigned long long)gridDim.x * blockDim.x) {
-        const float d = cd[e];
-        if (__float_as_uint(d) == 0xffffffffu) continue;     // a hole of the log
-        const unsigned long long pos = cp[e];
-        const int64_t o = (int64_t)(pos >> 32), i = (int64_t)(pos & 0xffffffffull);
-        const int64_t len = v.n - o;
-        for (int k = 0; k < K; ++k) {
-            const float l = s_lo[k], x = s_eps[k];
-            if (!(l < d && d <= x)) continue;
-            unsigned long long* h = hist + ((int64_t)b * K + k) * v.n;
-            // to the left: old-recurrent cells (<= lo) up to the start of the new run; another new cell on the way means
-            // this one is not the first of its run
-            int64_t a = i;
-            bool first = true;
-            while (a > 0) {
-                const float dd = point_distance<NORM>(yb, a - 1, a - 1 + o, v.m, v.ps, v.cs);
-                if (dd > x) break;
-                if (dd > l) { first = false; break; }
-                --a;
-            }
-            if (!first) continue;
-            if (i > a) atomicAdd(&h[i - a], ~0ull);          // the old run that ended just before the cell
-            int64_t run = 0, e2 = i + 1;
-            while (e2 < len) {
-                const float dd = point_distance<NORM>(yb, e2, e2 + o, v.m, v.ps, v.cs);
-                if (dd > x) break;
-                if (dd <= l) {
-                    ++run;
-                } else if (run) {
-                    atomicAdd(&h[run], ~0ull);
-                    run = 0;
-                }
-                ++e2;
-            }
-            if (run) atomicAdd(&h[run], ~0ull);
-            atomicAdd(&h[e2 - a], 1ull);
-        }
-    }
-}
-
-// log capacity per series: the select's candidate capacity plus the holes the persistent grid's warps can leave (one
-// open chunk of 64 entries per warp and series change, generously)
-unsigned long long fused_cap(const SelectPlan& p) { return p.cap + 4ull * 148 * 2 * 16 * 64; }
-
-struct FusedWs {
-    BufSel* st;
-    SelState* ss;
-    unsigned long long* bins;
-    float *sample, *lo, *hi, *cand_d;
-    unsigned long long *cand_pos, *cand_n, *ncand;
-    int* fail;
-};
-FusedWs carve_fused(Arena& ws, const View& v, int K, const SelectPlan& p) {
-    FusedWs w{};
-    w.st = ws.take<BufSel>(v.batch);
-    w.ss = ws.take<SelState>(v.batch);
-    w.bins = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * BT * 256);
-    w.sample = ws.take<float>((size_t)v.batch * p.S);
-    w.lo = ws.take<float>((size_t)v.batch * K);
-    w.hi = ws.take<float>((size_t)v.batch * K);
-    w.cand_d = ws.take<float>((size_t)v.batch * fused_cap(p));
-    w.cand_pos = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * fused_cap(p));
-    w.cand_n = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch);
-    w.ncand = (unsigned long long*)ws.take<uint64_t>((size_t)v.batch * (GK + 1));
-    w.fail = ws.take<int>((size_t)v.batch);
-    return w;
-}
-
-bool fused_applies(const View& v, int K, const Options& opt) {
-    if (K > GK || opt.parts != 1 || opt.select_path != PATH_AUTO) return false;
-    if (make_select_plan(v, K, opt).path != PATH_BRACKET) return false;
-    return line_scan_applies(v, K, opt);
-}
-
 }  // namespace
-
-size_t fused_workspace_bytes(const View& v, int K, const Options& opt) {
-    if (!fused_applies(v, K, opt)) return 0;
-    Options o = opt;
-    o.select_path = PATH_BRACKET;
-    const SelectPlan p = make_select_plan(v, K, o);
-    Arena a(nullptr, ~(size_t)0);
-    carve_fused(a, v, K, p);
-    return a.off + line_workspace_bytes(v, K, opt);
-}
-
-rqa_status run_sweep_fused(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
-                           double* d_rr, uint64_t* d_hist, Arena& ws, cudaStream_t s, const Options& opt, int* h_failed) {
-    *h_failed = v.batch;
-    if (!fused_applies(v, K, opt)) return RQA_ERR_UNSUPPORTED;
-    const SelectPlan p = make_select_plan(v, K, opt);
-    FusedWs w = carve_fused(ws, v, K, p);
-    if (!ws.ok()) { set_error("rqa_sweep: workspace too small"); return RQA_ERR_WORKSPACE_TOO_SMALL; }
-    const unsigned long long P = p.P, S = p.S;
-    RQA_CUDA_TRY(cudaMemsetAsync(w.bins, 0, sizeof(uint64_t) * (size_t)v.batch * BT * 256, s));
-    RQA_CUDA_TRY(cudaMemsetAsync(w.cand_n, 0, sizeof(uint64_t) * (size_t)v.batch, s));
-    RQA_CUDA_TRY(cudaMemsetAsync(w.ncand, 0, sizeof(uint64_t) * (size_t)v.batch * (GK + 1), s));
-    RQA_CUDA_TRY(cudaMemsetAsync(w.fail, 0, sizeof(int) * (size_t)v.batch, s));
-    {
-        unsigned blocks = (unsigned)std::min<unsigned long long>((S + 255) / 256, 148 * 16);
-        if (norm == RQA_NORM_MAX) sel_sample_kernel<RQA_NORM_MAX><<<dim3(blocks, v.batch), 256, 0, s>>>(v, S, w.sample);
-        else sel_sample_kernel<RQA_NORM_EUCLID><<<dim3(blocks, v.batch), 256, 0, s>>>(v, S, w.sample);
-        RQA_LAUNCH_CHECK();
-    }
-    int order[GK];
-    for (int k = 0; k < K; ++k) order[k] = k;
-    std::stable_sort(order, order + K, [&](int a, int b) { return h_rank[a] < h_rank[b]; });
-    FusedTarget ft{};
-    Ranks64 rk{};
-    ft.K = K;
-    for (int t = 0; t < K; ++t) {
-        const unsigned long long r = h_rank[order[t]];
-        const double q = (double)r / (double)P;
-        const double mean = q * (double)S, sd = std::sqrt((double)S * q * (1.0 - q));
-        const double lo = std::floor(mean - BRACKET_SIGMAS * sd) - 1.0;
-        const double hi = std::ceil(mean + BRACKET_SIGMAS * sd) + 1.0;
-        ft.lo_rank[t] = lo >= 1.0 ? (unsigned long long)lo : 0;
-        ft.hi_rank[t] = hi <= (double)S ? (unsigned long long)hi : 0;
-        ft.k_of[t] = order[t];
-        ft.rank[order[t]] = r;
-        rk.r[2 * t] = ft.lo_rank[t] ? ft.lo_rank[t] : 1;
-        rk.r[2 * t + 1] = ft.hi_rank[t] ? ft.hi_rank[t] : S;
-    }
-    bufsel_init_kernel<<<v.batch, BT, 0, s>>>(w.st, rk, 2 * K);
-    RQA_LAUNCH_CHECK();
-    rqa_status st = run_bufsel(w.sample, S, S, nullptr, 0, w.st, w.bins, 2 * K, v.batch, s);
-    if (st != RQA_OK) return st;
-    fused_bracket_kernel<<<v.batch, GK, 0, s>>>(w.st, ft, w.lo, w.hi, w.fail);
-    RQA_LAUNCH_CHECK();
-    LineLog lg{};
-    lg.hi = w.hi; lg.cand_d = w.cand_d; lg.cand_pos = w.cand_pos; lg.cand_n = w.cand_n; lg.ncand = w.ncand; lg.cap = fused_cap(p);
-    st = run_line_hist_log(v, norm, w.lo, K, d_hist, ws, s, opt, &lg);
-    if (st != RQA_OK) return st;
-    fused_resolve_kernel<<<v.batch, 64, 0, s>>>(ft, lg.groups_out, lg.agg_out, w.ncand, w.cand_n, fused_cap(p), P, w.fail, w.ss, w.st);
-    RQA_LAUNCH_CHECK();
-    st = run_bufsel(w.cand_d, fused_cap(p), fused_cap(p), w.ss, 1, w.st, w.bins, K, v.batch, s);
-    if (st != RQA_OK) return st;
-    fused_finish_kernel<<<v.batch, GK, 0, s>>>(w.st, ft, P, w.fail, d_eps, (unsigned long long*)d_count, d_rr);
-    RQA_LAUNCH_CHECK();
-    {
-        dim3 grid(148 * 8, (unsigned)v.batch);
-        if (norm == RQA_NORM_MAX)
-            fused_fixup_kernel<RQA_NORM_MAX><<<grid, 256, 0, s>>>(v, K, w.lo, d_eps, w.cand_d, w.cand_pos, w.cand_n, fused_cap(p), w.fail,
-                                                                  (unsigned long long*)d_hist);
-        else
-            fused_fixup_kernel<RQA_NORM_EUCLID><<<grid, 256, 0, s>>>(v, K, w.lo, d_eps, w.cand_d, w.cand_pos, w.cand_n, fused_cap(p), w.fail,
-                                                                     (unsigned long long*)d_hist);
-        RQA_LAUNCH_CHECK();
-    }
-    // the one synchronisation of the call: did every series come through?
-    std::vector<int> h_fail((size_t)v.batch);
-    RQA_CUDA_TRY(cudaMemcpyAsync(h_fail.data(), w.fail, sizeof(int) * (size_t)v.batch, cudaMemcpyDeviceToHost, s));
-    RQA_CUDA_TRY(cudaStreamSynchronize(s));
-    int failed = 0;
-    for (int b = 0; b < v.batch; ++b) failed += h_fail[b] != 0;
-    *h_failed = failed;
-    return RQA_OK;
-}
 
 size_t select_workspace_bytes(const View& v, int K, const Options& opt) {
     SelectPlan p = make_select_plan(v, K, opt);

@@ -930,65 +930,3 @@ def test_kernel_event_hooks_and_nccl_reduce_wrapper(rqa):
     out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300, cwd=root,
                          env=dict(os.environ, PYTHONPATH=root))
     assert out.returncode == 0 and "nccl ok" in out.stdout, out.stderr[-1500:]
-
-
-# ----------------------------------------------- rqa_sweep: thresholds and histograms from ONE full pass
-def gpu_one_pass(rqa, series, m, tau, rr, norm=0, theiler=0, l_min=2, options=None):
-    import torch
-    from paper_2208_09136_b200 import binding as B
-    s = torch.as_tensor(np.ascontiguousarray(np.atleast_2d(series), dtype=np.float32)).cuda()
-    view = B.rqa_embed(s, m, tau, theiler=theiler)
-    K, batch, n = len(rr), s.shape[0], int(view.n_points)
-    eps = torch.empty((batch, K), dtype=torch.float32, device="cuda")
-    cnt = torch.empty((batch, K), dtype=torch.int64, device="cuda")
-    rrr = torch.empty((batch, K), dtype=torch.float64, device="cuda")
-    hist = torch.empty((batch, K, n), dtype=torch.int64, device="cuda")
-    det = torch.empty((batch, K), dtype=torch.float64, device="cuda")
-    mean = torch.empty((batch,), dtype=torch.float64, device="cuda")
-    ws = torch.empty(B.rqa_workspace_bytes(view, K, options), dtype=torch.uint8, device="cuda")
-    B.rqa_sweep(view, norm, rr, eps, cnt, rrr, hist, ws, options=options)
-    path = B.rqa_sweep_last_path()
-    B.rqa_det_avg(hist, l_min, det, mean)
-    B.rqa_workspace_status(ws)
-    return {"eps": eps.cpu().numpy(), "count": cnt.cpu().numpy().view(np.uint64), "rr": rrr.cpu().numpy(),
-            "hist": hist.cpu().numpy().view(np.uint64), "det": det.cpu().numpy(), "det_mean": mean.cpu().numpy()}, path
-
-
-@pytest.mark.parametrize("kind,N,m,tau,norm,K,w", [("lorenz1", 5200, 3, 1, 0, 20, 0), ("lorenz1", 5200, 3, 3, 1, 20, 0), ("noise", 4400, 3, 1, 0, 32, 0),
-                                                   ("logistic", 6100, 5, 2, 0, 12, 0), ("lorenzclean", 5000, 3, 3, 0, 20, 0), ("noise", 4000, 1, 1, 0, 7, 0),
-                                                   ("logistic", 4500, 2, 7, 1, 5, 0), ("lorenz1", 5200, 3, 1, 0, 1, 0), ("lorenz1", 5600, 3, 1, 0, 20, 37)])
-def test_one_pass_sweep_matches_oracle(rqa, oracle, kind, N, m, tau, norm, K, w):
-    """rqa_sweep on shapes where the one-pass path applies (more than 2^22 pairs, K <= 32): sample brackets, the scan at
-    their lower ends with the candidate log, exact ranks from the level counts, histograms corrected from lo_k to eps_k —
-    every output bit for bit against the oracle, and the path taken must be the one-pass one."""
-    make = {"lorenz1": lambda: wl.add_noise(wl.lorenz_signal(N), 1.0, 700 + N), "lorenzclean": lambda: wl.lorenz_signal(N).astype(np.float32),
-            "noise": lambda: wl.gaussian(900 + N, N).astype(np.float32), "logistic": lambda: wl.add_noise(wl.logistic_signal(N, seed=3), 2.0, 800 + N)}[kind]
-    y = np.stack([make(), make()[::-1].copy()]).astype(np.float32)
-    rr = wl.rr_log(K, 0.002, 0.25) if K > 1 else np.array([0.05])
-    g, path = gpu_one_pass(rqa, y, m, tau, rr, norm, theiler=w)
-    assert path == 1, "the one-pass sweep should have applied"
-    assert_parity(oracle, g, y, m, tau, rr, norm, theiler=max(1, w))
-
-
-def test_one_pass_sweep_gives_up_cleanly(rqa, oracle):
-    """Where the one-pass sweep cannot work the call still returns the exact result through the two-pass path: massive
-    ties (quantised and constant series: collapsed brackets), a mixed batch (one tie-heavy series spoils the attempt for
-    the batch), K above one threshold group, a short series, rr = 1 (open upper bracket)."""
-    N = 4200
-    noisy = wl.add_noise(wl.lorenz_signal(N), 1.0, 55)
-    quant = (np.round(wl.gaussian(56, N) * 2) / 2).astype(np.float32)
-    rr = wl.rr_log(10, 0.01, 0.3)
-    for series, expect in ((np.stack([quant, np.full(N, 1.5, np.float32)]), 3), (np.stack([noisy, quant]), 3)):
-        g, path = gpu_one_pass(rqa, series, 3, 1, rr)
-        assert path == expect
-        assert_parity(oracle, g, series, 3, 1, rr)
-    g, path = gpu_one_pass(rqa, noisy, 3, 1, wl.rr_log(40, 0.01, 0.3))
-    assert path == 2
-    assert_parity(oracle, g, noisy, 3, 1, wl.rr_log(40, 0.01, 0.3))
-    g, path = gpu_one_pass(rqa, noisy[:900], 3, 1, rr)
-    assert path == 2
-    assert_parity(oracle, g, noisy[:900], 3, 1, rr)
-    rr1 = np.array([0.1, 1.0])
-    g, path = gpu_one_pass(rqa, noisy, 3, 1, rr1)
-    assert path == 3
-    assert_parity(oracle, g, noisy, 3, 1, rr1)

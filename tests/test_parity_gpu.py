@@ -930,3 +930,40 @@ def test_kernel_event_hooks_and_nccl_reduce_wrapper(rqa):
     out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300, cwd=root,
                          env=dict(os.environ, PYTHONPATH=root))
     assert out.returncode == 0 and "nccl ok" in out.stdout, out.stderr[-1500:]
+
+
+def test_call_chain_is_cuda_graph_capturable(rqa, oracle):
+    """No call of the chain synchronises or allocates, so a caller can capture rqa_eps_for_rr -> rqa_line_hist ->
+    rqa_det_avg -> rqa_vert_hist into a CUDA graph and replay it (the many-short-series regime: 24 launches become one
+    graph launch).  The replay must reproduce the oracle's numbers on fresh input placed in the same buffers."""
+    import torch
+    from paper_2208_09136_b200 import binding as B
+    w = wl.config2()
+    s = torch.as_tensor(w.series).cuda()
+    buf = rqa.SweepBuffers.allocate(s, w.m, w.tau, w.K)
+    vh = torch.empty_like(buf.hist)
+
+    def chain():
+        B.rqa_eps_for_rr(buf.view, w.norm, w.rr, buf.eps, buf.count, buf.rr, buf.ws)
+        B.rqa_line_hist(buf.view, w.norm, buf.eps, buf.hist, buf.ws)
+        B.rqa_det_avg(buf.hist, 2, buf.det, buf.det_mean)
+        B.rqa_vert_hist(buf.view, w.norm, buf.eps, vh, buf.ws)
+    st = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(st):
+        chain()                                                  # warm-up outside the capture (one-time function attributes)
+        st.synchronize()
+        with torch.cuda.graph(g, stream=st):
+            chain()
+    # new data in the captured input buffer: the reversed series
+    rev = np.ascontiguousarray(w.series[:, ::-1])
+    s.copy_(torch.as_tensor(rev).cuda())
+    buf.hist.zero_(); buf.eps.zero_(); vh.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    B.rqa_workspace_status(buf.ws)
+    g_out = {"eps": buf.eps.cpu().numpy(), "count": buf.count.cpu().numpy().view(np.uint64), "rr": buf.rr.cpu().numpy(),
+             "hist": buf.hist.cpu().numpy().view(np.uint64), "det": buf.det.cpu().numpy(), "det_mean": buf.det_mean.cpu().numpy()}
+    assert_parity(oracle, g_out, rev, w.m, w.tau, w.rr, w.norm)
+    for b in (0, 4):
+        assert np.array_equal(vh[b].cpu().numpy().view(np.uint64), oracle.vert_hist(rev[b], w.m, w.tau, g_out["eps"][b], w.norm, threads=0))

@@ -327,8 +327,12 @@ def run_ours(args):
     ev_scan = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
     part = dict(part_index=rank, part_count=world, reduce=parts.dist_reduce("cuda")) if split else {}
     o_sel = B.make_options(kernel_events=ev_count, **part)
-    o_line = B.make_options(kernel_events=ev_scan, **part)
-    buf = rqa.SweepBuffers.allocate(series, w.m, w.tau, K, options=o_sel)
+    knobs = {}
+    if args.line_knobs:                                             # expert knobs of the diagonal scan (profiles/r2_scan_knobs.md)
+        nb, ch, sg = (int(x) for x in args.line_knobs.split(","))
+        knobs = dict(line_buffers=nb, line_chunk=ch, line_segment=sg)
+    o_line = B.make_options(kernel_events=ev_scan, **knobs, **part)
+    buf = rqa.SweepBuffers.allocate(series, w.m, w.tau, K, options=o_line if knobs else o_sel)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step(ev=None):
@@ -530,6 +534,8 @@ def main():
     ap.add_argument("--no-others", action="store_true", help="skip the secondary timings of the other configs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--profile-step", action="store_true", help="run ONE bare step and exit (for ncu; prints nothing)")
+    ap.add_argument("--line-knobs", default="", help="'buffers,chunk,segment' for rqa_line_hist (rqa_options.line_buffers, "
+                                                     "line_chunk, line_segment; 0 = automatic): the knob sweep of profiles/r2_scan_knobs.md")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="torch.distributed backend of the ranks")
     ap.add_argument("--same-gpu", action="store_true",
                     help="FUNCTIONAL TEST ONLY: all ranks share cuda:0 (use with --backend gloo; NCCL refuses one device "

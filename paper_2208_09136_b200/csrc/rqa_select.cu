@@ -393,6 +393,8 @@ struct CountArgs {
     float* cand;                      // [batch][cap]
     unsigned long long cap;
     int m, tau;
+    unsigned long long* counter;      // work-item counter of this launch (zeroed before)
+    uint32_t tiles;                   // tiles per series (this part)
 };
 
 struct CountSmem {
@@ -516,14 +518,12 @@ struct Counter : CellDist<NORM, M, TAU, 0, count_vec<M, TAU>()> {
 
 template <int NORM, int M, int TAU>
 __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev, int fields, int heavy_pass) {
+    // PERSISTENT: the grid is two blocks per SM; a block draws (series, tile) items from an atomic counter, series by series,
+    // so that the level table is loaded once per series and block, not once per tile.
     extern __shared__ __align__(16) char smem[];
     __shared__ int s_ob;
-    const int tid = threadIdx.x, b = blockIdx.y;
-    if (a.ss[b].fallback) return;
-    const uint32_t tile = blockIdx.x;
-    const SelTable& T = a.tabs[b];
-    if (T.heavy != heavy_pass) return;                        // series with extra tie levels: the wider second launch
-    find_diagonal_block(a.tile_start, a.n_obl, tile, &s_ob);
+    __shared__ unsigned long long s_item;
+    const int tid = threadIdx.x;
     uint2* lut_s = (uint2*)(smem + CountSmem::off_lut);
     float* beta_s = (float*)(smem + CountSmem::off_beta);
     float* cand_s = (float*)(smem + CountSmem::off_cand);
@@ -537,9 +537,31 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
     float* yb_s = ya_s + LA;
     // VECK: the element pushed by the first cell of a super-step (window index 12k + 2) is 16-byte aligned
     const int sha = VECK ? 2 : 0;
-    for (int q = tid; q < NBS; q += LW) lut_s[q] = T.lut[q];
-    if (tid < NCUT) { beta_s[tid] = T.beta[tid]; ((uint8_t*)(smem + CountSmem::off_kind))[tid] = T.kind[tid]; }
     for (int q = tid; q < nlev * col_words; q += LW) cols_s[q] = 0;
+    const unsigned long long n_items = (unsigned long long)a.tiles * (unsigned long long)a.v.batch;
+    int cur_b = -1;
+    __syncthreads();
+  while (true) {
+    if (tid == 0) s_item = atomicAdd(a.counter, 1ull);
+    __syncthreads();
+    const unsigned long long item = s_item;
+    if (item >= n_items) break;
+    const int b = (int)(item / a.tiles);
+    const uint32_t tile = (uint32_t)(item - (unsigned long long)b * a.tiles);
+    const SelTable& T = a.tabs[b];
+    // series given to the radix passes, and series of the other launch (extra tie levels: the wider second launch), are
+    // skipped as a whole: the counter jumps to the next series
+    if (a.ss[b].fallback || T.heavy != heavy_pass) {
+        if (tid == 0) atomicMax(a.counter, (unsigned long long)(b + 1) * a.tiles);
+        __syncthreads();
+        continue;
+    }
+    find_diagonal_block(a.tile_start, a.n_obl, tile, &s_ob);
+    if (b != cur_b) {
+        for (int q = tid; q < NBS; q += LW) lut_s[q] = T.lut[q];
+        if (tid < NCUT) { beta_s[tid] = T.beta[tid]; ((uint8_t*)(smem + CountSmem::off_kind))[tid] = T.kind[tid]; }
+        cur_b = b;
+    }
     __syncthreads();
     const int ob = a.part + s_ob * a.parts;                   // this part's diagonal blocks are interleaved
     const int c = (int)(tile - a.tile_start[s_ob]);
@@ -600,17 +622,20 @@ __global__ void __launch_bounds__(LW, 2) sel_count_kernel(CountArgs a, int nlev,
         const int warp = tid >> 5, lane = tid & 31;
         unsigned long long* lc = a.ss[b].level_count;
         for (int row = warp; row < nlev; row += LW / 32) {
-            const uint32_t* r = cols_s + row * col_words;
+            uint32_t* r = cols_s + row * col_words;
             uint32_t sum = 0;
             const uint32_t fmask = (1u << field_bits) - 1u;
             for (int q = lane; q < col_words; q += 32) {
                 uint32_t w = r[q];
+                r[q] = 0;                                      // cleared for the block's next tile
                 sum += (w & fmask) + ((w >> field_bits) & fmask) + (fields == 3 ? w >> 20 : 0u);
             }
             for (int off = 16; off; off >>= 1) sum += __shfl_down_sync(FULL, sum, off);
             if (lane == 0 && sum) atomicAdd(&lc[row], (unsigned long long)sum);
         }
     }
+    __syncthreads();                                          // before the next item overwrites s_item, s_ob and the windows
+  }
 }
 
 // After the counting pass, before the parts of a split call are summed: this part's candidate count and whether its
@@ -908,9 +933,13 @@ rqa_status launch_count(const CountArgs& a, const SelectPlan& p, int nlev, int b
     }
     if (smem_heavy > SMEM_PER_BLOCK_MAX) { set_error("rqa_eps_for_rr: counting pass needs %zu bytes of shared memory", smem_heavy); return RQA_ERR_UNSUPPORTED; }
     if (p.tl.tiles == 0) return RQA_OK;
-    kern<<<dim3((unsigned)p.tl.tiles, (unsigned)batch), LW, smem, s>>>(a, nlev, p.fields, 0);
+    const unsigned grid = (unsigned)std::min<uint64_t>(p.tl.tiles * (uint64_t)batch, (uint64_t)(2 * sm_count()));
+    CountArgs a0 = a, a1 = a;
+    a0.tiles = a1.tiles = (uint32_t)p.tl.tiles;
+    a1.counter = a.counter + 1;
+    kern<<<grid, LW, smem, s>>>(a0, nlev, p.fields, 0);
     RQA_LAUNCH_CHECK();
-    kern<<<dim3((unsigned)p.tl.tiles, (unsigned)batch), LW, smem_heavy, s>>>(a, nlev_heavy, p.fields, 1);
+    kern<<<grid, LW, smem_heavy, s>>>(a1, nlev_heavy, p.fields, 1);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }
@@ -957,6 +986,7 @@ struct SelectWs {
     unsigned long long* bins;         // [batch][BT][256]
     SelTable* tabs;
     uint32_t* tile_start;
+    unsigned long long* counters;     // work-item counters of the two counting-pass launches
     float* sample;                    // [batch][S] (DIRECT: [batch][P])
     float* cand;                      // [batch][cap]
     SelBatch* rst;
@@ -974,6 +1004,7 @@ SelectWs carve(Arena& ws, const View& v, int K, const SelectPlan& p) {
     if (p.path == PATH_BRACKET) {
         w.tabs = ws.take<SelTable>(v.batch);
         w.tile_start = ws.take<uint32_t>((size_t)p.tl.n_obl + 1);
+        w.counters = (unsigned long long*)ws.take<uint64_t>(2);
         w.sample = ws.take<float>((size_t)v.batch * p.S);
         w.cand = ws.take<float>((size_t)v.batch * p.cap);
     }
@@ -1076,6 +1107,8 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
             a.v = v; a.L = p.L; a.n_obl = p.tl.n_obl; a.part = opt.part; a.parts = opt.parts;
             a.tile_start = w.tile_start; a.tabs = w.tabs; a.ss = w.ss;
             a.cand = w.cand; a.cap = p.cap; a.m = v.m; a.tau = (int)v.cs;
+            a.counter = w.counters; a.tiles = (uint32_t)p.tl.tiles;
+            RQA_CUDA_TRY(cudaMemsetAsync(w.counters, 0, 2 * sizeof(unsigned long long), s));
             const int nlev = 2 * kc + 1;
             if (base == 0 && opt.ev_begin) RQA_CUDA_TRY(cudaEventRecord((cudaEvent_t)opt.ev_begin, s));
             st = norm == RQA_NORM_MAX ? dispatch_count<RQA_NORM_MAX>(a, p, nlev, v.batch, s)

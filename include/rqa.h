@@ -30,7 +30,8 @@
  *
  * Memory and ownership: every buffer is owned by the caller.  Pointers named d_* are DEVICE pointers,
  * h_* are HOST pointers.  The library keeps no device allocation and no global state between calls (the only
- * process-wide datum is the monotone launch counter behind rqa_launch_count()).
+ * process-wide datum is the monotone launch counter behind rqa_launch_count()), with ONE stated exception: the static
+ * scratch array of rqa_line_hist_static, the entry point for callers that cannot allocate (see there).
  * Every call enqueues its work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
  * stream) and returns without synchronising; outputs are valid once the stream has been synchronised.
  *
@@ -285,6 +286,27 @@ rqa_status rqa_line_hist_opt(const rqa_points* pts, rqa_norm norm, const float* 
                              void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt);
 rqa_status rqa_vert_hist_opt(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_vhist,
                              void* d_ws, size_t ws_bytes, void* stream, const rqa_options* opt);
+
+/*
+ * rqa_line_hist for callers that cannot allocate device memory (code under CUDA-graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): same arguments minus the workspace, same kernels, same
+ * results bit for bit.  The scratch is a static device array of RQA_STATIC_SCRATCH_BYTES inside the library; the call
+ * makes no cudaMalloc / cudaFree / allocating library call and is asynchronous on `stream` like rqa_line_hist.
+ *   - every GPU on which the process uses this call holds RQA_STATIC_SCRATCH_BYTES of device memory until exit;
+ *   - a shape whose scan needs more scratch returns RQA_ERR_UNSUPPORTED (nothing launched; the message states the
+ *     bytes needed).  The scan's scratch grows with the number of tiles it cuts the triangle into, not simply with N:
+ *     BASELINE.json's configs 1-3 fit (6 series of 10^4 points at K = 20 need 113 MiB), one series of 10^4 points fits
+ *     at any K, one series of 10^5 points does not (207 MiB);
+ *   - all calls on one device share the array and it keeps the last call's contents: calls in stream order are
+ *     independent (the path clears what must start at zero), calls that OVERLAP on the GPU race — serialise them or use
+ *     rqa_line_hist with one workspace per stream;
+ *   - a non-finite point or a bad threshold is recorded in the scratch as in a workspace; there is no
+ *     rqa_workspace_status for it (validate inputs with the workspace calls where that matters).
+ * Errors: as rqa_line_hist, plus RQA_ERR_UNSUPPORTED as above and RQA_ERR_CUDA if the scratch address cannot be got.
+ */
+#define RQA_STATIC_SCRATCH_BYTES (128u << 20)
+rqa_status rqa_line_hist_static(const rqa_points* pts, rqa_norm norm, const float* d_eps, int32_t K, uint64_t* d_hist,
+                                void* stream);
 
 #ifdef __cplusplus
 }

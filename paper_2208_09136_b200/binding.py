@@ -23,13 +23,14 @@ RQA_NORM_MAX = 0
 RQA_NORM_EUCLID = 1
 RQA_MAX_K = 128
 RQA_MAX_M = 16
+RQA_STATIC_SCRATCH_BYTES = 128 << 20
 
 # every symbol include/rqa.h declares (tests check that the library exports them all)
 EXPORTS = ["rqa_status_string", "rqa_last_error", "rqa_version", "rqa_workspace_bytes", "rqa_workspace_status",
            "rqa_embed", "rqa_eps_for_rr", "rqa_line_hist", "rqa_det_avg", "rqa_sweep_workspace_bytes",
            "rqa_sweep_host", "rqa_launch_count", "rqa_workspace_bytes_opt", "rqa_eps_for_rr_opt", "rqa_line_hist_opt",
            "rqa_det_prefix_avg", "rqa_line_measures", "rqa_sorting_rate_host", "rqa_vert_hist", "rqa_vert_hist_opt",
-           "rqa_lam_tt"]
+           "rqa_lam_tt", "rqa_line_hist_static"]
 
 
 class RqaPoints(ctypes.Structure):
@@ -124,6 +125,7 @@ def load_library() -> ctypes.CDLL:
     lib.rqa_vert_hist.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp]
     lib.rqa_vert_hist_opt.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp, sz, vp, opt]
     lib.rqa_lam_tt.argtypes = [vp, i32, i32, i64, i64, vp, vp, vp]
+    lib.rqa_line_hist_static.argtypes = [pts, ctypes.c_int, vp, i32, vp, vp]
     _lib = lib
     return lib
 
@@ -214,6 +216,17 @@ def rqa_line_hist(pts: RqaPoints, norm: int, eps, hist, ws, stream=None, options
     _check(load_library().rqa_line_hist_opt(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps", bk), K,
                                             _dev(hist, torch.int64, "hist", bk * int(pts.n_points)),
                                             _dev(ws, torch.uint8, "ws"), ws.numel(), _stream(stream), _opt(options)))
+
+
+def rqa_line_hist_static(pts: RqaPoints, norm: int, eps, hist, stream=None) -> None:
+    """rqa_line_hist without a workspace argument: the scratch is a static device array inside the library
+    (RQA_STATIC_SCRATCH_BYTES; larger shapes raise RQA_ERR_UNSUPPORTED).  No device allocation is made by the call."""
+    import torch
+    K = eps.shape[-1]
+    bk = int(pts.batch) * K
+    _check(load_library().rqa_line_hist_static(ctypes.byref(pts), norm, _dev(eps, torch.float32, "eps", bk), K,
+                                               _dev(hist, torch.int64, "hist", bk * int(pts.n_points)),
+                                               _stream(stream)))
 
 
 def rqa_vert_hist(pts: RqaPoints, norm: int, eps, vhist, ws, stream=None, options: RqaOptions = None) -> None:

@@ -235,8 +235,10 @@ uint64_t rqa_launch_count(void);
  *                 counting pass, 3 = four radix passes.  The radix passes serve views the tiled passes cannot stage
  *                 (coordinate span above 4096 elements, very wide points) and are the automatic recovery of a bracket
  *                 miss; they recompute every distance from global memory four times and cost about 20 x the bracket path
- *                 (88 ms instead of 4 ms per series of 1e5 points on a B200).  Automatic: series of at most 8192 pairs are
- *                 sorted whole in shared memory, P <= 2^22 takes path 1, everything else path 2.
+ *                 (88 ms instead of 4 ms per series of 1e5 points on a B200).  4 = one thread block per series, three
+ *                 walks over the triangle with shared-memory histograms, nothing materialised (P <= 2^22 only; otherwise
+ *                 automatic).  Automatic: series of at most 8192 pairs are sorted whole in shared memory, P <= 2^22
+ *                 takes path 4 for batches of at least 8 series and path 1 below, everything else path 2.
  *   sample_size   bracket path: number of sampled pair distances per series
  *   cand_cap      bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
  *   line_chunk    rqa_line_hist / rqa_vert_hist: chunk length along the diagonals / columns, 1..1023

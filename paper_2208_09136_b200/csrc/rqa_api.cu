@@ -17,7 +17,7 @@ std::atomic<uint64_t> g_launches{0};
 rqa_status make_options(const rqa_options* in, Options* out, const char* who) {
     *out = Options{};
     if (!in) return RQA_OK;
-    if (in->select_path < 0 || in->select_path > 3) { set_error("%s: options.select_path is 0..3", who); return RQA_ERR_INVALID_ARG; }
+    if (in->select_path < 0 || in->select_path > 4) { set_error("%s: options.select_path is 0..4", who); return RQA_ERR_INVALID_ARG; }
     if (in->line_chunk < 0 || in->line_chunk > 1023) { set_error("%s: options.line_chunk is 0..1023", who); return RQA_ERR_INVALID_ARG; }
     if (in->line_buffers < 0 || in->line_buffers > 2) { set_error("%s: options.line_buffers is 0..2", who); return RQA_ERR_INVALID_ARG; }
     if (in->line_segment < 0) { set_error("%s: options.line_segment must be >= 0", who); return RQA_ERR_INVALID_ARG; }

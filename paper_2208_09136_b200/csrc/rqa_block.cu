@@ -1,0 +1,350 @@
+// rqa_block.cu — thresholds for MANY series of moderate length (8192 < P <= 2^22 counted pairs, N' up to ~2900) in one
+// call: one thread block selects all K thresholds of a series, nothing is materialised in global memory.
+//
+// The paper's experiment grid is 900 series per length at N = 10^2, 10^3 with K = 99 recurrence rates
+// (PAPER.md:82-84).  For N = 10^3 the materialise-then-radix-select path of rqa_select.cu reads the 1.8 GB of
+// distances of such a batch eight times with a prefix search per element (18 ms); here every series is one block that
+// recomputes its distances from a shared-memory copy of the series in three walks over the triangle:
+//   walk 1  histogram of all P distances over BLK_NB1 equal-width bins of [0, bound]   (bound >= every distance)
+//           -> per target: its bin, the count below the bin, the residual rank inside it
+//   walk 2  for the cells that fall into a target's bin: histogram over its 256 equal sub-bins
+//           -> per target: its (bin, sub-bin) cell, count below, residual rank
+//   walk 3  the cells that fall into a target's (bin, sub-bin) cell are collected (a few per target), sorted by their
+//           fp32 bit patterns in shared memory, and eps_k = the residual-rank-th of its cell, C_k = #{d <= eps_k}
+// (readings S4-S6: exact order statistic, ties counted).  The bin of a distance is floor(d * scale), a
+// monotone function of d, so everything in a lower bin is strictly smaller than everything in a higher one and equal
+// values share a bin: the selection is exact.  A series whose target cells hold more than BLK_CAP distances (massive
+// ties: a constant or coarsely quantised series) is flagged and done by the radix passes of rqa_select.cu.
+#include <algorithm>
+#include <cmath>
+
+#include "rqa_tiles.cuh"
+
+namespace rqa {
+
+namespace {
+
+constexpr int BLK_THREADS = 1024;
+constexpr int BLK_NB1 = 4096;            // bins of walk 1
+constexpr int BLK_SUB = 256;             // sub-bins of walk 2
+constexpr int BLK_CAP = 8192;            // collected distances of walk 3 (sorted in shared memory)
+constexpr uint32_t BLK_MARK = 0x80000000u;
+constexpr size_t BLK_SMEM_MAX = 227 * 1024 - 4096;   // opt-in limit minus the static arrays below
+
+struct BlockTargets {
+    unsigned long long r[RQA_MAX_K];     // ranks, ascending
+    int32_t k_of[RQA_MAX_K];             // caller's index of the target
+};
+
+// Distance provider.  M > 0: a delay view (point stride 1) with m == M whose samples sit in shared memory at byte
+// address `sa`: shared-memory loads with compile-time trip counts.  M == 0: any view, through a generic pointer (the
+// shared copy when it fits, the global series otherwise).
+template <int NORM, int M>
+struct BlockDist {
+    uint32_t sa;
+    int cs4;                     // 4 * coordinate stride (bytes)
+    const float* yb;
+    int m, ps, cs;
+    __device__ __forceinline__ float at(int i, int o) const {
+        if (M > 0) {
+            const uint32_t a = sa + 4u * (uint32_t)i, b = a + 4u * (uint32_t)o;
+            if (NORM == RQA_NORM_MAX) {
+                float d = 0.0f;
+#pragma unroll
+                for (int c = 0; c < M; ++c) d = fmaxf(d, fabsf(__fsub_rn(lds_f32(a + c * cs4), lds_f32(b + c * cs4))));
+                return d;
+            }
+            float t = __fsub_rn(lds_f32(a), lds_f32(b));
+            float s = __fmul_rn(t, t);
+#pragma unroll
+            for (int c = 1; c < M; ++c) {
+                t = __fsub_rn(lds_f32(a + c * cs4), lds_f32(b + c * cs4));
+                s = __fadd_rn(s, __fmul_rn(t, t));
+            }
+            return __fsqrt_rn(s);
+        }
+        const float* pa = yb + (size_t)i * ps;
+        const float* pb = pa + (size_t)o * ps;
+        if (NORM == RQA_NORM_MAX) {
+            float d = 0.0f;
+            for (int c = 0; c < m; ++c) d = fmaxf(d, fabsf(__fsub_rn(pa[c * cs], pb[c * cs])));
+            return d;
+        }
+        float t = __fsub_rn(pa[0], pb[0]);
+        float s = __fmul_rn(t, t);
+        for (int c = 1; c < m; ++c) {
+            t = __fsub_rn(pa[c * cs], pb[c * cs]);
+            s = __fadd_rn(s, __fmul_rn(t, t));
+        }
+        return __fsqrt_rn(s);
+    }
+};
+
+// Every counted cell (i, j = i + o), o = w..n-1, exactly once.  Diagonal w + q is paired with diagonal n - 1 - q: every
+// pair has n - w + 1 cells.  A pair is cut into `split` equal ranges so that the items fill the block; the lanes of a
+// warp sit on adjacent diagonals at the same i (x_i is a broadcast, x_j a run of consecutive addresses).
+template <class D, class F>
+__device__ __forceinline__ void walk_triangle(const D& dist, int n, int w, int split, F&& f) {
+    const int nd = n - w, nq = (nd + 1) / 2, items = nq * split;
+    for (int it = threadIdx.x; it < items; it += BLK_THREADS) {
+        const int h = it / nq, q = it - h * nq;
+        const int o1 = w + q, o2 = n - 1 - q, len1 = n - o1, len = len1 + (o2 != o1 ? n - o2 : 0);
+        const int a = (int)((long long)len * h / split), b = (int)((long long)len * (h + 1) / split);
+        const int e1 = b < len1 ? b : len1;
+#pragma unroll 4
+        for (int i = a; i < e1; ++i) f(dist.at(i, o1));
+        const int a2 = (a > len1 ? a : len1) - len1, e2 = b - len1;
+#pragma unroll 4
+        for (int i = a2; i < e2; ++i) f(dist.at(i, o2));
+    }
+}
+
+__device__ __forceinline__ int bin_of(float t) {               // t >= 0 (a NaN converts to 0, +inf to INT_MAX)
+    return min((int)t, BLK_NB1 - 1);
+}
+__device__ __forceinline__ int sub_of(float t, int bin) {
+    const int s = (int)(__fmul_rn(__fsub_rn(t, (float)bin), (float)BLK_SUB));   // t - bin is exact for t < BLK_NB1
+    return min(max(s, 0), BLK_SUB - 1);
+}
+
+// Shared memory: hist1 [BLK_NB1] | hist2 [K][BLK_SUB] | cand [BLK_CAP] (32-bit words) | slot1 [BLK_NB1] bytes |
+// the series (stage_floats floats, optional)
+__host__ __device__ inline size_t block_smem_bytes(int K, size_t stage_floats) {
+    return 4 * ((size_t)BLK_NB1 + (size_t)K * BLK_SUB + (size_t)BLK_CAP + stage_floats) + (size_t)BLK_NB1;
+}
+
+template <int NORM, int M>
+__global__ void __launch_bounds__(BLK_THREADS) sel_block_kernel(View v, BlockTargets tg, int K, unsigned int P,
+                                                                int stage_floats, int split, int32_t* fallback,
+                                                                size_t fallback_stride, float* __restrict__ eps,
+                                                                unsigned long long* __restrict__ count,
+                                                                double* __restrict__ rr) {
+    extern __shared__ __align__(16) uint32_t s_mem[];
+    __shared__ float s_red[2][BLK_THREADS / 32];
+    __shared__ uint32_t s_scan[BLK_THREADS / 32];
+    __shared__ int s_bin[RQA_MAX_K], s_slot[RQA_MAX_K], s_sub[RQA_MAX_K];
+    __shared__ uint32_t s_below[RQA_MAX_K], s_rho[RQA_MAX_K], s_before[RQA_MAX_K];
+    __shared__ uint32_t s_ncand, s_total;
+    __shared__ float s_scale;
+    uint32_t* hist1 = s_mem;
+    uint32_t* hist2 = hist1 + BLK_NB1;
+    uint32_t* cand = hist2 + (size_t)K * BLK_SUB;
+    uint8_t* slot1 = (uint8_t*)(cand + BLK_CAP);
+    float* stage = (float*)(slot1 + BLK_NB1);
+
+    const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n = (int)v.n, w = (int)v.w, m = v.m, ps = (int)v.ps, cs = (int)v.cs;
+    const float* yb = v.data + (int64_t)b * v.bs;
+
+    // the series' value range bounds every distance: |a - b| <= max - min per coordinate (Euclid: times sqrt(m))
+    const int ny = (n - 1) * ps + (m - 1) * cs + 1;
+    float lo = __int_as_float(0x7f800000), hi = -lo;
+    for (int q = tid; q < ny; q += BLK_THREADS) {
+        const float x = yb[q];
+        if (stage_floats) stage[q] = x;
+        lo = fminf(lo, x);
+        hi = fmaxf(hi, x);
+    }
+    for (int off = 16; off; off >>= 1) {
+        lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+        hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+    }
+    if (lane == 0) { s_red[0][warp] = lo; s_red[1][warp] = hi; }
+    for (int q = tid; q < BLK_NB1; q += BLK_THREADS) { hist1[q] = 0; slot1[q] = 0; }
+    for (int q = tid; q < K * BLK_SUB; q += BLK_THREADS) hist2[q] = 0;
+    if (tid == 0) s_ncand = 0;
+    __syncthreads();
+    if (tid == 0) {
+        float a = s_red[0][0], c = s_red[1][0];
+        for (int q = 1; q < BLK_THREADS / 32; ++q) { a = fminf(a, s_red[0][q]); c = fmaxf(c, s_red[1][q]); }
+        float bound = c - a;
+        if (NORM != RQA_NORM_MAX) bound *= sqrtf((float)m);
+        s_scale = bound > 0.0f && bound < __int_as_float(0x7f800000) ? (float)BLK_NB1 / bound : 0.0f;
+    }
+    __syncthreads();
+    if (stage_floats) yb = stage;
+    const float scale = s_scale;
+    BlockDist<NORM, M> dist;
+    dist.sa = smem_addr(stage);
+    dist.cs4 = 4 * cs;
+    dist.yb = yb; dist.m = m; dist.ps = ps; dist.cs = cs;
+
+    // ---- walk 1: all distances into BLK_NB1 bins
+    walk_triangle(dist, n, w, split, [&](float d) { atomicAdd(&hist1[bin_of(__fmul_rn(d, scale))], 1u); });
+    __syncthreads();
+    {   // inclusive prefix sums of hist1 in place (four bins per thread)
+        uint32_t c[BLK_NB1 / BLK_THREADS], sum = 0;
+#pragma unroll
+        for (int q = 0; q < BLK_NB1 / BLK_THREADS; ++q) { sum += hist1[tid * (BLK_NB1 / BLK_THREADS) + q]; c[q] = sum; }
+        uint32_t incl = sum;
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += u;
+        }
+        if (lane == 31) s_scan[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t x = s_scan[lane];
+            for (int off = 1; off < 32; off <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, x, off);
+                if (lane >= off) x += u;
+            }
+            s_scan[lane] = x;
+        }
+        __syncthreads();
+        const uint32_t base = incl - sum + (warp ? s_scan[warp - 1] : 0u);
+#pragma unroll
+        for (int q = 0; q < BLK_NB1 / BLK_THREADS; ++q) hist1[tid * (BLK_NB1 / BLK_THREADS) + q] = base + c[q];
+    }
+    __syncthreads();
+    if (tid < K) {                                             // target tid: first bin whose cumulative count reaches its rank
+        const uint32_t r = (uint32_t)tg.r[tid];
+        int a = 0, c = BLK_NB1 - 1;
+        while (a < c) {
+            const int mid = (a + c) >> 1;
+            if (hist1[mid] >= r) c = mid; else a = mid + 1;
+        }
+        const uint32_t below = a ? hist1[a - 1] : 0u;
+        s_bin[tid] = a;
+        s_below[tid] = below;
+        s_rho[tid] = r - below;
+    }
+    __syncthreads();
+    if (tid == 0) {                                            // distinct target bins, ascending (ranks are ascending)
+        int slot = 0;
+        for (int t = 0; t < K; ++t) {
+            if (t > 0 && s_bin[t] != s_bin[t - 1]) ++slot;
+            s_slot[t] = slot;
+            slot1[s_bin[t]] = (uint8_t)(slot + 1);
+        }
+    }
+    __syncthreads();
+
+    // ---- walk 2: the cells of the target bins into 256 sub-bins each
+    walk_triangle(dist, n, w, split, [&](float d) {
+        const float t = __fmul_rn(d, scale);
+        const int bin = bin_of(t), s = slot1[bin];
+        if (s) atomicAdd(&hist2[(s - 1) * BLK_SUB + sub_of(t, bin)], 1u);
+    });
+    __syncthreads();
+    if (tid < K) {
+        const uint32_t* h = hist2 + s_slot[tid] * BLK_SUB;
+        const uint32_t rho = s_rho[tid];
+        uint32_t acc = 0;
+        int sub = 0;
+        for (; sub < BLK_SUB - 1; ++sub) {
+            if (acc + h[sub] >= rho) break;
+            acc += h[sub];
+        }
+        s_sub[tid] = sub;
+        s_below[tid] += acc;
+        s_rho[tid] = rho - acc;
+    }
+    __syncthreads();
+    if (tid == 0) {                                            // distinct target cells, ascending: offsets in the sorted list
+        uint32_t before = 0, prev_count = 0;
+        for (int t = 0; t < K; ++t) {
+            const int cell = s_slot[t] * BLK_SUB + s_sub[t];
+            if (t > 0 && cell != s_slot[t - 1] * BLK_SUB + s_sub[t - 1]) before += prev_count;
+            prev_count = hist2[cell] & ~BLK_MARK;
+            hist2[cell] |= BLK_MARK;
+            s_before[t] = before;
+        }
+        s_total = before + prev_count;
+    }
+    __syncthreads();
+    const uint32_t total = s_total;
+    if (total > (uint32_t)BLK_CAP) {                          // massive ties: the radix passes redo this series
+        if (tid == 0) *(int32_t*)((char*)fallback + (size_t)b * fallback_stride) = 1;
+        return;
+    }
+
+    // ---- walk 3: collect the distances of the target cells, sort them
+    walk_triangle(dist, n, w, split, [&](float d) {
+        const float t = __fmul_rn(d, scale);
+        const int bin = bin_of(t), s = slot1[bin];
+        if (s && (hist2[(s - 1) * BLK_SUB + sub_of(t, bin)] & BLK_MARK)) {
+            const uint32_t at = atomicAdd(&s_ncand, 1u);
+            if (at < (uint32_t)BLK_CAP) cand[at] = __float_as_uint(d);
+        }
+    });
+    int P2 = 2;
+    while ((uint32_t)P2 < total) P2 <<= 1;
+    __syncthreads();
+    for (int q = (int)total + tid; q < P2; q += BLK_THREADS) cand[q] = 0xffffffffu;      // padding sorts last
+    __syncthreads();
+    for (int k = 2; k <= P2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = tid; t < P2 / 2; t += BLK_THREADS) {
+                const int q = 2 * t - (t & (j - 1)), p = q | j;
+                const uint32_t a = cand[q], c = cand[p];
+                const bool up = (q & k) == 0;
+                if ((a > c) == up) { cand[q] = c; cand[p] = a; }
+            }
+            __syncthreads();
+        }
+    }
+    if (tid < K) {
+        const uint32_t e = cand[s_before[tid] + s_rho[tid] - 1];
+        int a = 0, c = (int)total;                              // first index with key > e
+        while (a < c) {
+            const int mid = (a + c) >> 1;
+            if (cand[mid] <= e) a = mid + 1; else c = mid;
+        }
+        const unsigned long long C = (unsigned long long)s_below[tid] + ((uint32_t)a - s_before[tid]);
+        const int64_t at = (int64_t)b * K + tg.k_of[tid];
+        eps[at] = __uint_as_float(e);
+        count[at] = C;
+        rr[at] = (double)C / (double)P;
+    }
+}
+
+}  // namespace
+
+bool block_select_fits(const View& v, int K) {
+    const uint64_t P = n_pairs(v);
+    return P > 0 && P <= (1ull << 22) && v.n <= (1 << 20) && v.ps <= 64 && v.cs <= (1 << 16) &&
+           block_smem_bytes(K, 0) <= BLK_SMEM_MAX;
+}
+
+rqa_status run_select_block(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
+                            double* d_rr, int32_t* d_fallback, size_t fallback_stride, cudaStream_t s) {
+    int order[RQA_MAX_K];
+    for (int k = 0; k < K; ++k) order[k] = k;
+    std::stable_sort(order, order + K, [&](int a, int b) { return h_rank[a] < h_rank[b]; });
+    BlockTargets tg{};
+    for (int t = 0; t < K; ++t) { tg.r[t] = h_rank[order[t]]; tg.k_of[t] = order[t]; }
+    // the series is copied to shared memory when it fits beside the histograms
+    const size_t ny = (size_t)(v.n - 1) * v.ps + (size_t)(v.m - 1) * v.cs + 1;
+    const size_t stage = block_smem_bytes(K, ny) <= BLK_SMEM_MAX ? ny : 0;
+    const size_t smem = block_smem_bytes(K, stage);
+    // cut the diagonal pairs so that the work items fill the block's threads evenly
+    const int nq = (int)((v.n - v.w + 1) / 2);
+    int split = 1;
+    double best = 0.0;
+    for (int c = 1; c <= 8; ++c) {
+        const double items = (double)nq * c, eff = items / (std::ceil(items / BLK_THREADS) * BLK_THREADS);
+        if (eff > best + 0.02) { best = eff; split = c; }
+    }
+    // compiled-in embedding for staged delay views of the common dimensions
+    const int M = (stage && v.ps == 1 && (v.m == 1 || v.m == 3)) ? v.m : 0;
+    using Kern = void (*)(View, BlockTargets, int, unsigned int, int, int, int32_t*, size_t, float*, unsigned long long*, double*);
+    const bool mx = norm == RQA_NORM_MAX;
+    Kern kern = M == 1 ? (mx ? sel_block_kernel<RQA_NORM_MAX, 1> : sel_block_kernel<RQA_NORM_EUCLID, 1>)
+              : M == 3 ? (mx ? sel_block_kernel<RQA_NORM_MAX, 3> : sel_block_kernel<RQA_NORM_EUCLID, 3>)
+                       : (mx ? sel_block_kernel<RQA_NORM_MAX, 0> : sel_block_kernel<RQA_NORM_EUCLID, 0>);
+    static thread_local bool attr_set[8][6] = {};
+    int dev = 0;
+    RQA_CUDA_TRY(cudaGetDevice(&dev));
+    const int which = (mx ? 0 : 1) + 2 * (M == 1 ? 1 : M == 3 ? 2 : 0);
+    if (dev >= 8 || !attr_set[dev][which]) {
+        RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BLK_SMEM_MAX));
+        if (dev < 8) attr_set[dev][which] = true;
+    }
+    kern<<<v.batch, BLK_THREADS, smem, s>>>(v, tg, K, (unsigned int)n_pairs(v), (int)stage, split, d_fallback, fallback_stride,
+                                            d_eps, (unsigned long long*)d_count, d_rr);
+    RQA_LAUNCH_CHECK();
+    return RQA_OK;
+}
+
+}  // namespace rqa

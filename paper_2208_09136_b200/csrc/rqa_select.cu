@@ -864,7 +864,7 @@ __global__ void __launch_bounds__(256) radix_resolve_kernel(SelBatch* st, unsign
 }
 
 // ------------------------------------------------------------------------------------------ host side
-enum { PATH_AUTO = 0, PATH_DIRECT = 1, PATH_BRACKET = 2, PATH_RADIX = 3 };
+enum { PATH_AUTO = 0, PATH_DIRECT = 1, PATH_BRACKET = 2, PATH_RADIX = 3, PATH_BLOCK = 4 };
 
 struct SelectPlan {
     int path;
@@ -894,7 +894,11 @@ SelectPlan make_select_plan(const View& v, int K, const Options& opt) {
     const int nlev_max = 2 * (2 * std::min(K, GK) + 1) - 1;
     const bool tiled_ok = p.span <= MAX_SPAN && count_smem_bytes(nlev_max, p.fields, 32, p.span, p.ps) <= SMEM_PER_BLOCK_MAX;
     p.path = opt.select_path;
-    if (p.path == PATH_AUTO) p.path = p.P <= (1ull << 22) ? PATH_DIRECT : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
+    // one block per series (rqa_block.cu) where the batch can fill the GPU with such blocks; forced: any batch
+    const bool block_ok = opt.parts == 1 && block_select_fits(v, K);
+    if (p.path == PATH_BLOCK && !block_ok) p.path = PATH_AUTO;
+    if (p.path == PATH_AUTO)
+        p.path = p.P <= (1ull << 22) ? (block_ok && v.batch >= 8 ? PATH_BLOCK : PATH_DIRECT) : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
     if (p.path == PATH_BRACKET && !tiled_ok) p.path = PATH_RADIX;
     if (p.path == PATH_DIRECT && p.P > (1ull << 28)) p.path = tiled_ok ? PATH_BRACKET : PATH_RADIX;
     if (p.path == PATH_BRACKET) {
@@ -1040,6 +1044,12 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
     int order[RQA_MAX_K];
     for (int k = 0; k < K; ++k) order[k] = k;
     std::stable_sort(order, order + K, [&](int a, int b) { return h_rank[a] < h_rank[b]; });
+
+    if (p.path == PATH_BLOCK) {
+        // every series in one block; a series with massive ties sets its fallback flag and is redone below
+        rqa_status st = run_select_block(v, norm, h_rank, K, d_eps, d_count, d_rr, &w.ss[0].fallback, sizeof(SelState), s);
+        if (st != RQA_OK) return st;
+    }
 
     if (p.path == PATH_DIRECT) {
         unsigned blocks = (unsigned)std::min<int64_t>(v.n - v.w, 148 * 8);

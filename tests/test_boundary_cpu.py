@@ -129,7 +129,7 @@ def test_options_are_per_call_and_validated(lib):
         o = B.make_options(**kw)
         st = lib.rqa_workspace_bytes_opt(ctypes.byref(pts), 20, ctypes.byref(o), ctypes.byref(sz))
         return st, sz.value
-    assert size(select_path=4)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(select_path=5)[0] == B.RQA_ERR_INVALID_ARG
     assert size(select_path=-1)[0] == B.RQA_ERR_INVALID_ARG
     assert size(line_chunk=1024)[0] == B.RQA_ERR_INVALID_ARG
     assert size(line_buffers=3)[0] == B.RQA_ERR_INVALID_ARG

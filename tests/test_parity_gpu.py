@@ -404,10 +404,10 @@ def _assert_select(oracle, got, series, m, tau, rr, norm=0):
         assert np.array_equal(got[2][b], r), f"rr, series {b}"
 
 
-@pytest.mark.parametrize("path", [1, 2, 3])
+@pytest.mark.parametrize("path", [1, 2, 3, 4])
 @pytest.mark.parametrize("norm", [0, 1])
 def test_select_paths_agree_with_oracle(rqa, oracle, options, path, norm):
-    """direct / bracket / radix on the same inputs: a noisy Lorenz batch (m=3, tau=1: compiled-in embedding) and a
+    """direct / bracket / radix / one-block-per-series on the same inputs: a noisy Lorenz batch (m=3, tau=1: compiled-in embedding) and a
     sine batch (m=4, tau=6: run-time embedding), unsorted RRs with duplicates and rr = 1."""
     options(select_path=path)
     rr = np.array([0.3, 0.0007, 0.02, 0.02, 0.11, 1.0, 0.5, 0.004])
@@ -463,6 +463,39 @@ def test_bracket_path_many_targets(rqa, oracle, options):
     for K in (128, 33):
         rr = wl.rr_log(K, 0.0005, 0.95)
         _assert_select(oracle, _select_only(rqa, y, 3, 3, rr), y, 3, 3, rr)
+
+
+@pytest.mark.parametrize("norm", [0, 1])
+def test_block_path_ties_targets_and_fallback(rqa, oracle, options, norm):
+    """One block per series (select_path 4, rqa_block.cu): noisy series next to series whose target cells carry massive
+    ties (exactly periodic, quantised, constant: flagged and redone by the radix passes) in one batch; K = 1, K = 128,
+    unsorted / duplicate targets and rr = 1; several embeddings incl. a run-time one."""
+    options(select_path=4)
+    noisy = wl.add_noise(wl.sine_signal(2300), 0.7, 3)
+    clean = wl.sine_signal(2300).astype(np.float32)
+    quant = np.floor(wl.uniform01(5, 2300) * 4).astype(np.float32)
+    const = np.full(2300, -1.25, dtype=np.float32)
+    fine = (np.round(wl.gaussian(12, 2300) * 400.0) / 400.0).astype(np.float32)       # ties, but few per value
+    tiny = (wl.gaussian(13, 2300) * 1e-30).astype(np.float32)
+    ys = np.stack([noisy, clean, quant, const, fine, tiny])
+    for m, tau, rr in [(2, 3, wl.rr_log(12, 0.002, 0.4)), (1, 1, np.array([0.37])), (3, 1, wl.rr_log(128, 0.0005, 0.95)),
+                       (4, 6, np.array([0.3, 0.0007, 0.02, 0.02, 1.0, 0.5]))]:
+        _assert_select(oracle, _select_only(rqa, ys, m, tau, rr, norm), ys, m, tau, rr, norm)
+
+
+def test_block_path_is_the_default_for_large_batches(rqa, oracle):
+    """A batch of at least 8 series with 8192 < P <= 2^22 takes the one-block-per-series path by default (the paper's
+    grid: 900 series of 10^3 points, K = 99; here 12 series of three kinds at three lengths, whole path)."""
+    rr = np.arange(1, 100) / 100.0
+    for N in (180, 1000, 2890):
+        ys = np.stack([wl.add_noise([wl.sine_signal(N), wl.logistic_signal(N, 70 + b), wl.lorenz_signal(N)][b % 3],
+                                    [math.inf, 3.0, 0.3, 0.03][b % 4], 900 + b) for b in range(12)])
+        n0 = rqa.rqa_launch_count()
+        got = _select_only(rqa, ys, 1, 1, rr)
+        assert rqa.rqa_launch_count() - n0 <= 14, "one kernel for the batch, plus the idle radix tail"
+        _assert_select(oracle, got, ys, 1, 1, rr)
+    g = gpu_sweep(rqa, ys[:, :1500], 3, 2, rr[::7], 1)
+    assert_parity(oracle, g, ys[:, :1500], 3, 2, rr[::7], 1)
 
 
 def test_config3_size_default_path_is_bracket(rqa, oracle):
@@ -565,7 +598,7 @@ def test_random_configurations(rqa, oracle, options, seed):
             rr[rng.integers(K)] = 1.0
         l_min = int(rng.choice([1, 2, 2, 3, 5]))
         ys = np.stack([series(int(rng.integers(7)), N, 1000 * case + b) for b in range(batch)])
-        options(select_path=int(rng.choice([0, 0, 1, 2, 3])), sample_size=int(rng.choice([0, 0, 50, 4000])),
+        options(select_path=int(rng.choice([0, 0, 1, 2, 3, 4])), sample_size=int(rng.choice([0, 0, 50, 4000])),
                 line_chunk=int(rng.choice([0, 0, 0, 1, 2, 3, 6, 13, 64, 500])), cand_cap=int(rng.choice([0, 0, 0, 200])),
                 line_segment=int(rng.choice([0, 0, 1, 2, 7, 40])), line_buffers=int(rng.choice([0, 1, 2])))
         s = torch.as_tensor(ys).cuda()
@@ -589,7 +622,7 @@ def test_random_configurations(rqa, oracle, options, seed):
         assert_parity(oracle, g, ys, m, tau, rr, norm, l_min, threads=0, theiler=w)
 
 
-@pytest.mark.parametrize("path", [0, 1, 2, 3])
+@pytest.mark.parametrize("path", [0, 1, 2, 3, 4])
 def test_theiler_window(rqa, oracle, options, path):
     """Theiler window w (rqa_points.theiler): thresholds over the pairs with j - i >= w and lines on the diagonals
     w..N'-1, on every select path, for delay views and materialised points, several chunk lengths, windows from 2

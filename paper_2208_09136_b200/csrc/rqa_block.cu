@@ -299,6 +299,179 @@ __global__ void __launch_bounds__(BLK_THREADS) sel_block_kernel(View v, BlockTar
     }
 }
 
+
+// ------------------------------------------------------------------------------------------- diagonal lines
+// rqa_line_hist for the same regime: one block per series, one thread per pair of diagonals.
+// Thresholds are nested, so after a cell of level v (= number of distinct thresholds below its distance) exactly the
+// thresholds j >= v are inside a run, and the runs of all thresholds on a diagonal form a stack of (lowest threshold,
+// start) entries: a lower level pushes one entry, a higher level pops the entries it ends, each giving ONE line length for
+// a whole range [a, b) of thresholds, counted as D[a][len]++, D[b][len]-- in a shared-memory difference array over the
+// thresholds (lengths below LB_LCAP; longer lines use the histogram rows themselves as the difference array).  Work per cell
+// does not depend on K: all K = 99 thresholds of the paper's sweep in ONE walk, where the tiled scan takes one pass per
+// group of 32.  The level of a cell: a bucket table over [0, eps_max] gives the thresholds in lower buckets, a short
+// loop adds those of the cell's own bucket.
+constexpr int LB_THREADS = 512;
+constexpr int LB_LCAP = 128;             // line lengths counted in shared memory
+constexpr int LB_NB = 4096;              // buckets of the level table
+
+__host__ __device__ inline size_t line_block_smem_bytes(int K, size_t stage_floats) {
+    return 4 * ((size_t)(K + 1) * LB_LCAP + stage_floats) + (size_t)LB_NB;
+}
+
+template <int NORM, int M>
+__global__ void __launch_bounds__(LB_THREADS, 2) line_block_kernel(View v, const float* __restrict__ eps, int K,
+                                                                  int stage_floats,
+                                                                  unsigned long long* __restrict__ hist,
+                                                                  WsStatus* status) {
+    extern __shared__ __align__(16) uint32_t s_mem[];
+    __shared__ float s_eps[RQA_MAX_K + 1], s_san[RQA_MAX_K];
+    __shared__ int s_jof[RQA_MAX_K], s_first[RQA_MAX_K];
+    __shared__ int s_J;
+    int* s_D = (int*)s_mem;                                   // [(K + 1)][LB_LCAP]
+    uint8_t* lut = (uint8_t*)(s_D + (size_t)(K + 1) * LB_LCAP);
+    float* stage = (float*)(lut + LB_NB);
+
+    const int b = blockIdx.x, tid = threadIdx.x;
+    const int n = (int)v.n, w = (int)v.w, m = v.m, ps = (int)v.ps, cs = (int)v.cs;
+    const float* yb = v.data + (int64_t)b * v.bs;
+    const float* e = eps + (int64_t)b * K;
+    unsigned long long* out = hist + (int64_t)b * K * n;
+
+    if (stage_floats) {
+        const int ny = (n - 1) * ps + (m - 1) * cs + 1;
+        for (int q = tid; q < ny; q += LB_THREADS) stage[q] = yb[q];
+        yb = stage;
+    }
+    for (int q = tid; q < (K + 1) * LB_LCAP; q += LB_THREADS) s_D[q] = 0;
+    // the histogram rows beyond the shared-memory lengths start at zero (written before the walk's atomics)
+    if (n > LB_LCAP)
+        for (int q = tid; q < K * (n - LB_LCAP); q += LB_THREADS) {
+            const int k = q / (n - LB_LCAP), l = LB_LCAP + (q - k * (n - LB_LCAP));
+            out[(int64_t)k * n + l] = 0ull;
+        }
+    // the K thresholds sorted, duplicates removed: distinct index j_of[k] of caller threshold k
+    bool bad = false;
+    for (int k = tid; k < K; k += LB_THREADS) {
+        float x = e[k];
+        if (!(x >= 0.0f) || isinf(x)) { bad = true; x = 0.0f; }
+        s_san[k] = x;
+    }
+    if (bad) atomicExch(&status->bad_eps, 1);
+    if (tid == 0) s_J = 0;
+    __syncthreads();
+    for (int k = tid; k < K; k += LB_THREADS) {
+        int first = 1;
+        for (int u = 0; u < k; ++u) first &= s_san[u] != s_san[k];
+        s_first[k] = first;
+    }
+    __syncthreads();
+    for (int k = tid; k < K; k += LB_THREADS) {
+        int below = 0;
+        for (int q = 0; q < K; ++q) below += s_first[q] && s_san[q] < s_san[k];
+        s_jof[k] = below;
+        s_eps[below] = s_san[k];
+        atomicMax(&s_J, below + 1);
+    }
+    __syncthreads();
+    const int J = s_J;
+    const float emax = s_eps[J - 1];
+    const float scale = emax > 0.0f ? (float)LB_NB / emax : 0.0f;
+    // lut[q] = thresholds whose bucket is below q (all of them are below every distance of bucket q)
+    for (int q = tid; q < LB_NB; q += LB_THREADS) {
+        int a = 0, c = J;
+        while (a < c) {
+            const int mid = (a + c) >> 1;
+            if (min((int)__fmul_rn(s_eps[mid], scale), LB_NB - 1) < q) a = mid + 1; else c = mid;
+        }
+        lut[q] = (uint8_t)a;
+    }
+    __syncthreads();
+
+    BlockDist<NORM, M> dist;
+    dist.sa = smem_addr(stage);
+    dist.cs4 = 4 * cs;
+    dist.yb = yb; dist.m = m; dist.ps = ps; dist.cs = cs;
+
+    uint32_t stk[RQA_MAX_K + 1];                              // (lowest threshold << 16 | start), top = smallest threshold
+    auto emit = [&](int lo, int upto, int len) {              // one line of `len` cells for the thresholds [lo, upto)
+        if (len < LB_LCAP) {
+            atomicAdd(&s_D[lo * LB_LCAP + len], 1);
+            atomicSub(&s_D[upto * LB_LCAP + len], 1);
+        } else {
+            // long lines: the same difference array in the histogram rows themselves (row j = distinct threshold j for
+            // now; 64-bit wrap-around arithmetic; no row is needed for upto == J)
+            atomicAdd(&out[(int64_t)lo * n + len], 1ull);
+            if (upto < J) atomicAdd(&out[(int64_t)upto * n + len], ~0ull);
+        }
+    };
+    auto diagonal = [&](int o) {
+        const int len = n - o;
+        // the top entry lives in `cur` (registers), the entries below it in stk[0 .. depth-2]
+        int depth = 0, pv = J;
+        uint32_t cur = 0;
+        auto ended = [&](int vnew, int t) {                   // the thresholds [pv, vnew) end their runs before cell t
+            while (depth > 0) {
+                const uint32_t nxt = depth > 1 ? stk[depth - 2] : ((uint32_t)J << 16);
+                const int lo = (int)(cur >> 16), start = (int)(cur & 0xffffu), hi = (int)(nxt >> 16);
+                emit(lo, hi < vnew ? hi : vnew, t - start);
+                if (hi <= vnew) {
+                    --depth;
+                    cur = nxt;
+                    if (hi == vnew) break;
+                } else {
+                    cur = ((uint32_t)vnew << 16) | (uint32_t)start;            // the rest of the entry lives on
+                    break;
+                }
+            }
+        };
+        for (int t = 0; t < len; ++t) {
+            const float d = dist.at(t, o);
+            int lev = lut[min((int)__fmul_rn(d, scale), LB_NB - 1)];
+            while (lev < J && s_eps[lev] < d) ++lev;
+            if (lev < pv) {
+                if (depth > 0) stk[depth - 1] = cur;
+                cur = ((uint32_t)lev << 16) | (uint32_t)t;
+                ++depth;
+            } else if (lev > pv) {
+                ended(lev, t);
+            }
+            pv = lev;
+        }
+        if (pv < J) ended(J, len);
+    };
+    const int nd = n - w, nq = (nd + 1) / 2;
+    for (int q = tid; q < nq; q += LB_THREADS) {
+        const int o1 = w + q, o2 = n - 1 - q;
+        diagonal(o1);
+        if (o2 != o1) diagonal(o2);
+    }
+    __syncthreads();
+    // prefix sums of D over the thresholds turn every column into the histogram of the distinct thresholds
+    const int ncol = n < LB_LCAP ? n : LB_LCAP;
+    for (int l = tid; l < ncol; l += LB_THREADS) {
+        int acc = 0;
+        for (int j = 0; j < J; ++j) {
+            acc += s_D[j * LB_LCAP + l];
+            s_D[j * LB_LCAP + l] = acc;
+        }
+    }
+    __syncthreads();
+    for (int q = tid; q < K * ncol; q += LB_THREADS) {
+        const int k = q / ncol, l = q - k * ncol;
+        out[(int64_t)k * n + l] = l == 0 ? 0ull : (unsigned long long)(unsigned int)s_D[s_jof[k] * LB_LCAP + l];
+    }
+    // the long lengths: prefix sums over the distinct thresholds, then row k of the caller = row j_of[k] (a column is
+    // read completely by its thread before it is rewritten)
+    for (int l = LB_LCAP + tid; l < n; l += LB_THREADS) {
+        unsigned long long acc = 0;
+        for (int j = 0; j < J; ++j) {
+            acc += out[(int64_t)j * n + l];
+            stk[j] = (uint32_t)acc;
+        }
+        for (int k = 0; k < K; ++k) out[(int64_t)k * n + l] = (unsigned long long)stk[s_jof[k]];
+    }
+}
+
 }  // namespace
 
 bool block_select_fits(const View& v, int K) {
@@ -343,6 +516,36 @@ rqa_status run_select_block(const View& v, int norm, const uint64_t* h_rank, int
     }
     kern<<<v.batch, BLK_THREADS, smem, s>>>(v, tg, K, (unsigned int)n_pairs(v), (int)stage, split, d_fallback, fallback_stride,
                                             d_eps, (unsigned long long*)d_count, d_rr);
+    RQA_LAUNCH_CHECK();
+    return RQA_OK;
+}
+
+bool block_line_fits(const View& v, int K) {
+    const uint64_t P = n_pairs(v);
+    return P > 0 && P <= (1ull << 22) && v.n < 65536 && v.ps <= 64 && v.cs <= (1 << 16) &&
+           line_block_smem_bytes(K, 0) <= 100 * 1024;
+}
+
+rqa_status run_line_block(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, WsStatus* status,
+                          cudaStream_t s) {
+    const size_t ny = (size_t)(v.n - 1) * v.ps + (size_t)(v.m - 1) * v.cs + 1;
+    const size_t stage = line_block_smem_bytes(K, ny) <= 110 * 1024 ? ny : 0;     // two blocks per SM
+    const size_t smem = line_block_smem_bytes(K, stage);
+    const int M = (stage && v.ps == 1 && (v.m == 1 || v.m == 3)) ? v.m : 0;
+    using Kern = void (*)(View, const float*, int, int, unsigned long long*, WsStatus*);
+    const bool mx = norm == RQA_NORM_MAX;
+    Kern kern = M == 1 ? (mx ? line_block_kernel<RQA_NORM_MAX, 1> : line_block_kernel<RQA_NORM_EUCLID, 1>)
+              : M == 3 ? (mx ? line_block_kernel<RQA_NORM_MAX, 3> : line_block_kernel<RQA_NORM_EUCLID, 3>)
+                       : (mx ? line_block_kernel<RQA_NORM_MAX, 0> : line_block_kernel<RQA_NORM_EUCLID, 0>);
+    static thread_local bool attr_set[8][6] = {};
+    int dev = 0;
+    RQA_CUDA_TRY(cudaGetDevice(&dev));
+    const int which = (mx ? 0 : 1) + 2 * (M == 1 ? 1 : M == 3 ? 2 : 0);
+    if (dev >= 8 || !attr_set[dev][which]) {
+        RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
+        if (dev < 8) attr_set[dev][which] = true;
+    }
+    kern<<<v.batch, LB_THREADS, smem, s>>>(v, d_eps, K, (int)stage, (unsigned long long*)d_hist, status);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }

@@ -145,6 +145,10 @@ bool block_select_fits(const View& v, int K);
 rqa_status run_select_block(const View& v, int norm, const uint64_t* h_rank, int K, float* d_eps, uint64_t* d_count,
                             double* d_rr, int32_t* d_fallback, size_t fallback_stride, cudaStream_t s);
 
+bool block_line_fits(const View& v, int K);
+rqa_status run_line_block(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, WsStatus* status,
+                          cudaStream_t s);
+
 size_t vert_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_vhist, Arena& ws,
                          cudaStream_t s, const Options& opt);

@@ -651,6 +651,10 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     // keep the general machinery)
     if (opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
         return run_line_small(v, norm, d_eps, K, d_hist, status, s);
+    // many series of moderate length: one block per series walks every diagonal once for all K thresholds (rqa_block.cu)
+    if (opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && v.batch >= 8 &&
+        block_line_fits(v, K))
+        return run_line_block(v, norm, d_eps, K, d_hist, status, s);
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * hist_words, s));
     LinePlan p = make_plan(v, K, opt);
     if (!p.scan) {

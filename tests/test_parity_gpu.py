@@ -498,6 +498,51 @@ def test_block_path_is_the_default_for_large_batches(rqa, oracle):
     assert_parity(oracle, g, ys[:, :1500], 3, 2, rr[::7], 1)
 
 
+@pytest.mark.parametrize("norm", [0, 1])
+def test_block_paths_whole_sweep_large_batches(rqa, oracle, norm):
+    """Batches of at least 8 series with P <= 2^22 run rqa_eps_for_rr AND rqa_line_hist as one block per series
+    (rqa_block.cu: all K thresholds in one walk per diagonal, lines of 128 cells and more by global atomics): noisy,
+    exactly periodic (lines as long as the plot), quantised and constant series side by side; compiled-in (m = 1; m = 3)
+    and run-time embeddings, materialised points, Theiler windows, K = 1 ... 128 with duplicates, series shorter than the
+    shared-memory length cap."""
+    import torch
+    def batch(N):
+        return np.stack([wl.add_noise(wl.sine_signal(N), 0.7, 3), wl.sine_signal(N).astype(np.float32),
+                         np.floor(wl.uniform01(5, N) * 4).astype(np.float32), np.full(N, -1.25, dtype=np.float32),
+                         wl.add_noise(wl.logistic_signal(N, 8), 3.0, 8), wl.add_noise(wl.lorenz_signal(N), 1.0, 9),
+                         wl.gaussian(10, N).astype(np.float32), (wl.gaussian(13, N) * 1e-30).astype(np.float32),
+                         wl.add_noise(wl.sine_signal(N), math.inf, 1) * 3.0])
+    cases = [(1400, 1, 1, np.arange(1, 100) / 100.0, 0, False), (900, 3, 1, wl.rr_log(128, 0.0005, 0.95), 0, False),
+             (1100, 4, 6, np.array([0.3, 0.0007, 0.02, 0.02, 1.0, 0.5]), 0, False), (700, 2, 3, np.array([0.2]), 0, True),
+             (1300, 3, 1, wl.rr_log(20, 0.001, 0.2), 40, False), (2000, 1, 1, wl.rr_log(7, 0.01, 0.6), 1700, False),
+             (140, 1, 1, wl.rr_log(128, 0.001, 0.9), 0, False), (160, 3, 3, wl.rr_log(99, 0.01, 0.99), 30, True)]
+    for (N, m, tau, rr, w, mat) in cases:
+        ys = batch(N)
+        s = torch.as_tensor(ys).cuda()
+        n, K, B = N - (m - 1) * tau, len(rr), ys.shape[0]
+        X = torch.empty((B, n, m), dtype=torch.float32, device="cuda") if mat else None
+        view = rqa.rqa_embed(s, m, tau, X, theiler=w)
+        eps = torch.empty((B, K), dtype=torch.float32, device="cuda")
+        cnt = torch.empty((B, K), dtype=torch.int64, device="cuda")
+        rrr = torch.empty((B, K), dtype=torch.float64, device="cuda")
+        hist = torch.full((B, K, n), -3, dtype=torch.int64, device="cuda")
+        ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
+        n0 = rqa.rqa_launch_count()
+        rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
+        rqa.rqa_line_hist(view, norm, eps, hist, ws)
+        assert rqa.rqa_launch_count() - n0 <= 18
+        rqa.rqa_workspace_status(ws)
+        for b in range(B):
+            r = oracle.sweep(ys[b], m, tau, rr, norm, 2, threads=0, theiler=max(1, w))
+            assert np.array_equal(eps[b].cpu().numpy().view(np.uint32), r["eps"].view(np.uint32)), (N, m, tau, b)
+            assert np.array_equal(cnt[b].cpu().numpy().view(np.uint64), r["count"]), (N, m, tau, b)
+            got = hist[b].cpu().numpy().view(np.uint64)
+            if not np.array_equal(got, r["hist"]):
+                bad = np.argwhere(got != r["hist"])
+                raise AssertionError(f"hist N={N} m={m} tau={tau} w={w} series {b}: {len(bad)} cells differ, first "
+                                     f"{tuple(bad[0])}: {got[tuple(bad[0])]} vs {r['hist'][tuple(bad[0])]}")
+
+
 def test_config3_size_default_path_is_bracket(rqa, oracle):
     """N = 1e4 (P = 5e7 > 2^22) takes the bracket path by default: one Lorenz series at each norm."""
     w = wl.config3(0)

@@ -238,7 +238,7 @@ uint64_t rqa_launch_count(void);
  *                 (88 ms instead of 4 ms per series of 1e5 points on a B200).  4 = one thread block per series, three
  *                 walks over the triangle with shared-memory histograms, nothing materialised (P <= 2^22 only; otherwise
  *                 automatic).  Automatic: series of at most 8192 pairs are sorted whole in shared memory, P <= 2^22
- *                 takes path 4 for batches of at least 8 series and path 1 below, everything else path 2.
+ *                 takes path 4 for batches of at least 12 series and path 1 below, everything else path 2.
  *   sample_size   bracket path: number of sampled pair distances per series
  *   cand_cap      bracket path: capacity of the candidate list per series (overflow falls back to the radix passes)
  *   line_chunk    rqa_line_hist / rqa_vert_hist: chunk length along the diagonals / columns, 1..1023
@@ -246,6 +246,10 @@ uint64_t rqa_launch_count(void);
  *                 carried in place (only segment borders are joined by the stitch kernel), >= 1
  *   line_buffers  rqa_line_hist: 1 = one set of series windows per block, staged by plain loads; 2 = two sets, the next
  *                 chunk's windows fetched by bulk asynchronous copies while the current chunk is scanned
+ *   line_path     rqa_line_hist: 0 automatic, 1 = the tiled scan, 2 = one thread block per series walking every diagonal
+ *                 once for all K thresholds (P <= 2^22 only; otherwise automatic).  Automatic: series of at most 8192
+ *                 pairs take their one-block kernel, P <= 2^22 takes path 2 when the batch is large enough to fill the
+ *                 GPU with such blocks (batch x ceil(K/32) >= 192), everything else the tiled scan.
  *   part_index, part_count
  *                 split of ONE call over part_count processes (one GPU each): this process visits
  *                 only its share of the tiles of the triangle (diagonal blocks part_index, part_index + part_count,
@@ -278,6 +282,8 @@ typedef struct rqa_options {
     void* reduce_ctx;
     void* ev_kernel_begin;
     void* ev_kernel_end;
+    int32_t line_path;
+    int32_t reserved;      /* must be 0 */
 } rqa_options;
 
 rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_options* opt, size_t* bytes);

@@ -42,6 +42,7 @@ struct Options {
     int line_chunk = 0;       // diagonal scan: chunk length L (<= 1023)
     int line_segment = 0;     // diagonal scan: chunks per segment
     int line_buffers = 0;     // diagonal scan: window sets per block (1 plain loads, 2 bulk-copy double buffer)
+    int line_path = 0;        // 0 auto, 1 tiled scan, 2 one block per series (P <= 2^22)
     int part = 0, parts = 1;  // this process' share of the tiles (multi-GPU split of one call)
     int64_t sample_size = 0;  // bracket path: sample size S
     int64_t cand_cap = 0;     // bracket path: candidate capacity per series

@@ -649,11 +649,13 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     const size_t hist_words = (size_t)v.batch * K * v.n;
     // short series: one block per series, shared-memory distances and histogram (explicit scan knobs and split calls
     // keep the general machinery)
-    if (opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
+    if (opt.line_path == 0 && opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
         return run_line_small(v, norm, d_eps, K, d_hist, status, s);
     // many series of moderate length: one block per series walks every diagonal once for all K thresholds (rqa_block.cu)
-    if (opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && v.batch >= 8 &&
-        block_line_fits(v, K))
+    // (the tiled scan costs about batch x groups of 32 thresholds, the blocks one round per 2 x SMs series)
+    const bool knobs = opt.line_chunk != 0 || opt.line_segment != 0 || opt.line_buffers != 0;
+    if (opt.parts == 1 && block_line_fits(v, K) &&
+        (opt.line_path == 2 || (opt.line_path == 0 && !knobs && (int64_t)v.batch * ((K + GK - 1) / GK) >= 192)))
         return run_line_block(v, norm, d_eps, K, d_hist, status, s);
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * hist_words, s));
     LinePlan p = make_plan(v, K, opt);

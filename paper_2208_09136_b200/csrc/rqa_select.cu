@@ -898,7 +898,7 @@ SelectPlan make_select_plan(const View& v, int K, const Options& opt) {
     const bool block_ok = opt.parts == 1 && block_select_fits(v, K);
     if (p.path == PATH_BLOCK && !block_ok) p.path = PATH_AUTO;
     if (p.path == PATH_AUTO)
-        p.path = p.P <= (1ull << 22) ? (block_ok && v.batch >= 8 ? PATH_BLOCK : PATH_DIRECT) : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
+        p.path = p.P <= (1ull << 22) ? (block_ok && v.batch >= 12 ? PATH_BLOCK : PATH_DIRECT) : (tiled_ok ? PATH_BRACKET : PATH_RADIX);
     if (p.path == PATH_BRACKET && !tiled_ok) p.path = PATH_RADIX;
     if (p.path == PATH_DIRECT && p.P > (1ull << 28)) p.path = tiled_ok ? PATH_BRACKET : PATH_RADIX;
     if (p.path == PATH_BRACKET) {

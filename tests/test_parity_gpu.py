@@ -484,8 +484,9 @@ def test_block_path_ties_targets_and_fallback(rqa, oracle, options, norm):
 
 
 def test_block_path_is_the_default_for_large_batches(rqa, oracle):
-    """A batch of at least 8 series with 8192 < P <= 2^22 takes the one-block-per-series path by default (the paper's
-    grid: 900 series of 10^3 points, K = 99; here 12 series of three kinds at three lengths, whole path)."""
+    """Batches with 8192 < P <= 2^22 take the one-block-per-series paths by default once they are large enough to fill
+    the GPU with such blocks (the paper's grid: 900 series of 10^3 points, K = 99): rqa_eps_for_rr from 12 series on
+    (three lengths), the whole sweep for 60 series at K = 99 (a launch count only the block kernels reach)."""
     rr = np.arange(1, 100) / 100.0
     for N in (180, 1000, 2890):
         ys = np.stack([wl.add_noise([wl.sine_signal(N), wl.logistic_signal(N, 70 + b), wl.lorenz_signal(N)][b % 3],
@@ -494,14 +495,19 @@ def test_block_path_is_the_default_for_large_batches(rqa, oracle):
         got = _select_only(rqa, ys, 1, 1, rr)
         assert rqa.rqa_launch_count() - n0 <= 14, "one kernel for the batch, plus the idle radix tail"
         _assert_select(oracle, got, ys, 1, 1, rr)
-    g = gpu_sweep(rqa, ys[:, :1500], 3, 2, rr[::7], 1)
-    assert_parity(oracle, g, ys[:, :1500], 3, 2, rr[::7], 1)
+    ys = np.stack([wl.add_noise([wl.sine_signal(600), wl.logistic_signal(600, 70 + b), wl.lorenz_signal(600)][b % 3],
+                                [math.inf, 3.0, 0.3, 0.03][b % 4], 300 + b) for b in range(60)])
+    n0 = rqa.rqa_launch_count()
+    g = gpu_sweep(rqa, ys, 3, 2, rr, 1)
+    assert rqa.rqa_launch_count() - n0 <= 20
+    assert_parity(oracle, g, ys, 3, 2, rr, 1)
 
 
 @pytest.mark.parametrize("norm", [0, 1])
-def test_block_paths_whole_sweep_large_batches(rqa, oracle, norm):
-    """Batches of at least 8 series with P <= 2^22 run rqa_eps_for_rr AND rqa_line_hist as one block per series
-    (rqa_block.cu: all K thresholds in one walk per diagonal, lines of 128 cells and more by global atomics): noisy,
+def test_block_paths_whole_sweep(rqa, oracle, norm):
+    """rqa_eps_for_rr AND rqa_line_hist as one block per series (rqa_block.cu; select_path 4, line_path 2: the default
+    for large batches with P <= 2^22; all K thresholds in one walk per diagonal, lines of 128 cells and more through
+    the histogram rows): noisy,
     exactly periodic (lines as long as the plot), quantised and constant series side by side; compiled-in (m = 1; m = 3)
     and run-time embeddings, materialised points, Theiler windows, K = 1 ... 128 with duplicates, series shorter than the
     shared-memory length cap."""
@@ -526,10 +532,11 @@ def test_block_paths_whole_sweep_large_batches(rqa, oracle, norm):
         cnt = torch.empty((B, K), dtype=torch.int64, device="cuda")
         rrr = torch.empty((B, K), dtype=torch.float64, device="cuda")
         hist = torch.full((B, K, n), -3, dtype=torch.int64, device="cuda")
-        ws = torch.empty(rqa.rqa_workspace_bytes(view, K), dtype=torch.uint8, device="cuda")
+        opt = rqa.make_options(select_path=4, line_path=2)
+        ws = torch.empty(rqa.rqa_workspace_bytes(view, K, opt), dtype=torch.uint8, device="cuda")
         n0 = rqa.rqa_launch_count()
-        rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws)
-        rqa.rqa_line_hist(view, norm, eps, hist, ws)
+        rqa.rqa_eps_for_rr(view, norm, rr, eps, cnt, rrr, ws, options=opt)
+        rqa.rqa_line_hist(view, norm, eps, hist, ws, options=opt)
         assert rqa.rqa_launch_count() - n0 <= 18
         rqa.rqa_workspace_status(ws)
         for b in range(B):

@@ -7,7 +7,7 @@
 // recomputes its distances from a shared-memory copy of the series in three walks over the triangle:
 //   walk 1  histogram of all P distances over BLK_NB1 equal-width bins of [0, bound]   (bound >= every distance)
 //           -> per target: its bin, the count below the bin, the residual rank inside it
-//   walk 2  for the cells that fall into a target's bin: histogram over its 256 equal sub-bins
+//   walk 2  for the cells that fall into a target's bin: histogram over its BLK_SUB equal sub-bins
 //           -> per target: its (bin, sub-bin) cell, count below, residual rank
 //   walk 3  the cells that fall into a target's (bin, sub-bin) cell are collected (a few per target), sorted by their
 //           fp32 bit patterns in shared memory, and eps_k = the residual-rank-th of its cell, C_k = #{d <= eps_k}
@@ -26,7 +26,7 @@ namespace {
 
 constexpr int BLK_THREADS = 1024;
 constexpr int BLK_NB1 = 4096;            // bins of walk 1
-constexpr int BLK_SUB = 256;             // sub-bins of walk 2
+constexpr int BLK_SUB = 128;             // sub-bins of walk 2 (128: two blocks per SM fit at K = 99)
 constexpr int BLK_CAP = 8192;            // collected distances of walk 3 (sorted in shared memory)
 constexpr uint32_t BLK_MARK = 0x80000000u;
 constexpr size_t BLK_SMEM_MAX = 227 * 1024 - 4096;   // opt-in limit minus the static arrays below
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(BLK_THREADS) sel_block_kernel(View v, BlockTar
     }
     __syncthreads();
 
-    // ---- walk 2: the cells of the target bins into 256 sub-bins each
+    // ---- walk 2: the cells of the target bins into BLK_SUB sub-bins each
     walk_triangle(dist, n, w, split, [&](float d) {
         const float t = __fmul_rn(d, scale);
         const int bin = bin_of(t), s = slot1[bin];
@@ -404,46 +404,56 @@ __global__ void __launch_bounds__(LB_THREADS, 2) line_block_kernel(View v, const
             if (upto < J) atomicAdd(&out[(int64_t)upto * n + len], ~0ull);
         }
     };
-    auto diagonal = [&](int o) {
-        const int len = n - o;
-        // the top entry lives in `cur` (registers), the entries below it in stk[0 .. depth-2]
-        int depth = 0, pv = J;
-        uint32_t cur = 0;
-        auto ended = [&](int vnew, int t) {                   // the thresholds [pv, vnew) end their runs before cell t
-            while (depth > 0) {
-                const uint32_t nxt = depth > 1 ? stk[depth - 2] : ((uint32_t)J << 16);
-                const int lo = (int)(cur >> 16), start = (int)(cur & 0xffffu), hi = (int)(nxt >> 16);
-                emit(lo, hi < vnew ? hi : vnew, t - start);
-                if (hi <= vnew) {
-                    --depth;
-                    cur = nxt;
-                    if (hi == vnew) break;
-                } else {
-                    cur = ((uint32_t)vnew << 16) | (uint32_t)start;            // the rest of the entry lives on
-                    break;
-                }
-            }
-        };
-        for (int t = 0; t < len; ++t) {
-            const float d = dist.at(t, o);
-            int lev = lut[min((int)__fmul_rn(d, scale), LB_NB - 1)];
-            while (lev < J && s_eps[lev] < d) ++lev;
-            if (lev < pv) {
-                if (depth > 0) stk[depth - 1] = cur;
-                cur = ((uint32_t)lev << 16) | (uint32_t)t;
-                ++depth;
-            } else if (lev > pv) {
-                ended(lev, t);
-            }
-            pv = lev;
-        }
-        if (pv < J) ended(J, len);
-    };
+    // Every lane is a small state machine over its two diagonals: one step either takes the next cell (level, maybe a
+    // push) or ends ONE stack entry of a pending level rise.  A rise that ends several entries spreads over several
+    // steps while the other lanes go on with their cells, so the warp never waits for the longest pop sequence of a
+    // cell (lanes drift apart along their diagonals; the walk's loads are then plain shared-memory gathers).
     const int nd = n - w, nq = (nd + 1) / 2;
     for (int q = tid; q < nq; q += LB_THREADS) {
         const int o1 = w + q, o2 = n - 1 - q;
-        diagonal(o1);
-        if (o2 != o1) diagonal(o2);
+        int o = o1, len = n - o1, t = 0;
+        int depth = 0, pv = J;                                 // top entry in `cur`, the entries below in stk[0 .. depth-2]
+        uint32_t cur = 0;
+        int vnew = -1, tend = 0;                               // pending rise: the thresholds [.., vnew) end before cell tend
+        bool second = o2 == o1;                                // no second diagonal for the middle one
+        while (true) {
+            if (vnew >= 0) {                                   // end one entry
+                const uint32_t nxt = depth > 1 ? stk[depth - 2] : ((uint32_t)J << 16);
+                const int lo = (int)(cur >> 16), start = (int)(cur & 0xffffu), hi = (int)(nxt >> 16);
+                emit(lo, hi < vnew ? hi : vnew, tend - start);
+                if (hi <= vnew) {
+                    --depth;
+                    cur = nxt;
+                    if (hi == vnew || depth == 0) vnew = -1;
+                } else {
+                    cur = ((uint32_t)vnew << 16) | (uint32_t)start;            // the rest of the entry lives on
+                    vnew = -1;
+                }
+            } else if (t < len) {                              // next cell
+                const float d = dist.at(t, o);
+                int lev = lut[min((int)__fmul_rn(d, scale), LB_NB - 1)];
+                while (lev < J && s_eps[lev] < d) ++lev;
+                if (lev < pv) {
+                    if (depth > 0) stk[depth - 1] = cur;
+                    cur = ((uint32_t)lev << 16) | (uint32_t)t;
+                    ++depth;
+                } else if (lev > pv) {
+                    vnew = lev;
+                    tend = t;
+                }
+                pv = lev;
+                ++t;
+            } else if (pv < J) {                               // end of the diagonal: every open run ends
+                vnew = J;
+                tend = len;
+                pv = J;
+            } else if (!second) {                              // on to the partner diagonal
+                second = true;
+                o = o2; len = n - o2; t = 0;
+            } else {
+                break;
+            }
+        }
     }
     __syncthreads();
     // prefix sums of D over the thresholds turn every column into the histogram of the distinct thresholds

@@ -521,7 +521,8 @@ def test_block_paths_whole_sweep(rqa, oracle, norm):
     cases = [(1400, 1, 1, np.arange(1, 100) / 100.0, 0, False), (900, 3, 1, wl.rr_log(128, 0.0005, 0.95), 0, False),
              (1100, 4, 6, np.array([0.3, 0.0007, 0.02, 0.02, 1.0, 0.5]), 0, False), (700, 2, 3, np.array([0.2]), 0, True),
              (1300, 3, 1, wl.rr_log(20, 0.001, 0.2), 40, False), (2000, 1, 1, wl.rr_log(7, 0.01, 0.6), 1700, False),
-             (140, 1, 1, wl.rr_log(128, 0.001, 0.9), 0, False), (160, 3, 3, wl.rr_log(99, 0.01, 0.99), 30, True)]
+             (140, 1, 1, wl.rr_log(128, 0.001, 0.9), 0, False), (160, 3, 3, wl.rr_log(99, 0.01, 0.99), 30, True),
+             (2815, 16, 1, wl.rr_log(128, 0.0005, 0.9), 0, True)]      # too wide for shared memory: global loads
     for (N, m, tau, rr, w, mat) in cases:
         ys = batch(N)
         s = torch.as_tensor(ys).cuda()

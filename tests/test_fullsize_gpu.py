@@ -161,4 +161,4 @@ def test_config4_vertical_lines_full_size(rqa, oracle):
             continue
         assert np.array_equal(vh[b].cpu().numpy().view(np.uint64), gold["vhist"]), f"config4 series {b}"
         checked += 1
-    assert checked >= 1, "no stored vertical-line histogram: run make_fullsize_golden.py config4 <s> --stage vhist"
+    assert checked == w.batch, "a stored vertical-line histogram is missing: run make_fullsize_golden.py config4 <s> --stage vhist"

@@ -260,7 +260,7 @@ def other_configs(rqa):
     out = []
     cases = [wl.config1(), wl.config2(), wl.config3(0), wl.config3(1), wl.config5(),
              wl.paper_group("logistic", 1.0, 100, n_real=90), wl.paper_group("logistic", 1.0, 1000, n_real=90),
-             wl.paper_group("lorenz", 1.0, 1000, n_real=10, K=99)]
+             wl.paper_group("lorenz", 1.0, 1000, n_real=10, K=99), wl.paper_group("logistic", 1.0, 10000, n_real=10, K=99)]
     for w in cases:
         s = torch.as_tensor(w.series).cuda()
         buf = rqa.SweepBuffers.allocate(s, w.m, w.tau, w.K)

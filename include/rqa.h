@@ -26,7 +26,7 @@
  *
  * Workspace size: rqa_workspace_bytes sizes for the worst case of the shape (the recurrence rates are not known then): about
  * 0.9 GB per series of 1e5 points at K = 20 (candidate list of the threshold select, up to 6 % of the pairs; segment
- * summaries of the scans), 80 MB per series of 2e4 points at K = 32, linear in the batch.
+ * summaries of the scans), 126 MB per series of 2e4 points at K = 32, linear in the batch.
  *
  * Memory and ownership: every buffer is owned by the caller.  Pointers named d_* are DEVICE pointers,
  * h_* are HOST pointers.  The library keeps no device allocation and no global state between calls (the only

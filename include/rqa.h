@@ -246,6 +246,9 @@ uint64_t rqa_launch_count(void);
  *                 carried in place (only segment borders are joined by the stitch kernel), >= 1
  *   line_buffers  rqa_line_hist: 1 = one set of series windows per block, staged by plain loads; 2 = two sets, the next
  *                 chunk's windows fetched by bulk asynchronous copies while the current chunk is scanned
+ *   group_size    thresholds (targets) per pass of the grouped kernels of all three heavy calls, 1..32; 0 automatic: K <= 32
+ *                 in one pass, more in groups of 20 (a pass over at most 20 thresholds keeps two blocks per SM; 7 % faster
+ *                 and a third less workspace than groups of 32 at K = 99)
  *   line_path     rqa_line_hist: 0 automatic, 1 = the tiled scan, 2 = one thread block per series walking every diagonal
  *                 once for all K thresholds (P <= 2^22 only; otherwise automatic).  Automatic: series of at most 8192
  *                 pairs take their one-block kernel, P <= 2^22 takes path 2 when the batch is large enough to fill the
@@ -283,7 +286,7 @@ typedef struct rqa_options {
     void* ev_kernel_begin;
     void* ev_kernel_end;
     int32_t line_path;
-    int32_t reserved;      /* must be 0 */
+    int32_t group_size;
 } rqa_options;
 
 rqa_status rqa_workspace_bytes_opt(const rqa_points* pts, int32_t K, const rqa_options* opt, size_t* bytes);

@@ -49,11 +49,11 @@ class RqaOptions(ctypes.Structure):
                 ("part_index", ctypes.c_int32), ("part_count", ctypes.c_int32), ("line_buffers", ctypes.c_int32),
                 ("sample_size", ctypes.c_int64), ("cand_cap", ctypes.c_int64), ("reduce", REDUCE_FN),
                 ("reduce_ctx", ctypes.c_void_p), ("ev_kernel_begin", ctypes.c_void_p), ("ev_kernel_end", ctypes.c_void_p),
-                ("line_path", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("line_path", ctypes.c_int32), ("group_size", ctypes.c_int32)]
 
 
 def make_options(select_path=0, line_chunk=0, line_segment=0, line_buffers=0, sample_size=0, cand_cap=0, part_index=0,
-                 part_count=0, reduce=None, kernel_events=None, line_path=0) -> RqaOptions:
+                 part_count=0, reduce=None, kernel_events=None, line_path=0, group_size=0) -> RqaOptions:
     """reduce: a Python callable (d_ptr: int, n: int, stream: int) -> None that sums n uint64 device counters over the
     parts of a split call (see parts.py); kept alive by the returned struct.
     kernel_events: a pair of torch.cuda.Event(enable_timing=True) that the call records just before / after its dominant
@@ -61,7 +61,7 @@ def make_options(select_path=0, line_chunk=0, line_segment=0, line_buffers=0, sa
     o = RqaOptions()
     o.select_path, o.line_chunk, o.line_segment, o.line_buffers = select_path, line_chunk, line_segment, line_buffers
     o.sample_size, o.cand_cap, o.part_index, o.part_count = sample_size, cand_cap, part_index, part_count
-    o.line_path = line_path
+    o.line_path, o.group_size = line_path, group_size
     if reduce is not None:
         def _cb(ctx, ptr, n, stream):
             try:

@@ -21,7 +21,7 @@ rqa_status make_options(const rqa_options* in, Options* out, const char* who) {
     if (in->line_chunk < 0 || in->line_chunk > 1023) { set_error("%s: options.line_chunk is 0..1023", who); return RQA_ERR_INVALID_ARG; }
     if (in->line_buffers < 0 || in->line_buffers > 2) { set_error("%s: options.line_buffers is 0..2", who); return RQA_ERR_INVALID_ARG; }
     if (in->line_path < 0 || in->line_path > 2) { set_error("%s: options.line_path is 0..2", who); return RQA_ERR_INVALID_ARG; }
-    if (in->reserved != 0) { set_error("%s: options.reserved must be 0", who); return RQA_ERR_INVALID_ARG; }
+    if (in->group_size < 0 || in->group_size > 32) { set_error("%s: options.group_size is 0..32", who); return RQA_ERR_INVALID_ARG; }
     if (in->line_segment < 0) { set_error("%s: options.line_segment must be >= 0", who); return RQA_ERR_INVALID_ARG; }
     if (in->sample_size < 0 || in->cand_cap < 0) { set_error("%s: options.sample_size and cand_cap must be >= 0", who); return RQA_ERR_INVALID_ARG; }
     if (in->part_count < 0 || in->part_index < 0 || (in->part_count > 0 && in->part_index >= in->part_count) ||
@@ -35,6 +35,7 @@ rqa_status make_options(const rqa_options* in, Options* out, const char* who) {
     out->line_segment = in->line_segment;
     out->line_buffers = in->line_buffers;
     out->line_path = in->line_path;
+    out->group_size = in->group_size;
     out->sample_size = in->sample_size;
     out->cand_cap = in->cand_cap;
     out->parts = in->part_count > 1 ? in->part_count : 1;

@@ -43,6 +43,7 @@ struct Options {
     int line_segment = 0;     // diagonal scan: chunks per segment
     int line_buffers = 0;     // diagonal scan: window sets per block (1 plain loads, 2 bulk-copy double buffer)
     int line_path = 0;        // 0 auto, 1 tiled scan, 2 one block per series (P <= 2^22)
+    int group_size = 0;       // thresholds per pass of the grouped kernels (0 auto)
     int part = 0, parts = 1;  // this process' share of the tiles (multi-GPU split of one call)
     int64_t sample_size = 0;  // bracket path: sample size S
     int64_t cand_cap = 0;     // bracket path: candidate capacity per series
@@ -61,6 +62,16 @@ inline rqa_status reduce_parts(const Options& o, void* d_counters, size_t n, cud
         return RQA_ERR_CUDA;
     }
     return RQA_OK;
+}
+
+// Thresholds (targets) per pass of the grouped kernels (counting pass, diagonal scan, column scan; at most GK = 32).
+// More than 32 go in groups of 20 (a pass over at most 20 thresholds keeps two blocks per SM): measured on 10 series
+// of 1e5 points at K = 99, rqa_line_hist 553 -> 503 ms, rqa_eps_for_rr 283 -> 278 ms, workspace 13.2 -> 8.5 GB; groups
+// of 25 or 10 are slower (810 / 1248 ms for both calls), and K = 32 in two groups of 16 is slower than in one pass
+// (config 5: 71 -> 103 ms).
+inline int group_size_for(int K, const Options& opt) {
+    if (opt.group_size > 0) return opt.group_size < 32 ? opt.group_size : 32;
+    return K <= 32 ? 32 : 20;
 }
 
 // ------------------------------------------------------------------------------------------------ view

@@ -37,7 +37,7 @@ namespace rqa {
 namespace {
 
 // One block per series: sort the K thresholds, split them into groups of 32, build each group's table.
-__global__ void __launch_bounds__(128) line_groups_kernel(const float* __restrict__ eps, int K, int NG,
+__global__ void __launch_bounds__(128) line_groups_kernel(const float* __restrict__ eps, int K, int NG, int gs,
                                                           LineGroup* __restrict__ groups, WsStatus* status) {
     const int b = blockIdx.x;
     const float* e = eps + (int64_t)b * K;
@@ -62,8 +62,8 @@ __global__ void __launch_bounds__(128) line_groups_kernel(const float* __restric
     if (threadIdx.x == 0 && s_bad) atomicExch(&status->bad_eps, 1);
     for (int g = 0; g < NG; ++g) {
         LineGroup& G = groups[(int64_t)b * NG + g];
-        const int base = g * GK;
-        const int kc = min(GK, K - base);
+        const int base = g * gs;                              // gs <= GK thresholds per group
+        const int kc = min(gs, K - base);
         __shared__ int s_J;
         __shared__ float s_scale, s_dcap;
         if (threadIdx.x == 0) {
@@ -476,7 +476,7 @@ __global__ void __launch_bounds__(128) line_strided_kernel(View v, const float* 
 // ------------------------------------------------------------------------------------------ host side
 struct LinePlan {
     bool scan;          // false: strided fallback
-    int L, S, NG, NP, span, nbuf, blocks_per_sm;
+    int L, S, NG, NP, gs, span, nbuf, blocks_per_sm;
     Tiling tl;          // segments (T = S*L cells) of this part's diagonal blocks
     unsigned grid;      // persistent blocks
     size_t smem;
@@ -497,8 +497,9 @@ constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_BLOCK_RESERVED = 1024;
 LinePlan make_plan(const View& v, int K, const Options& opt) {
     LinePlan p{};
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
-    p.NG = (K + GK - 1) / GK;
-    p.NP = scan_pairs_for(std::min(K, GK));
+    p.gs = group_size_for(K, opt);
+    p.NG = (K + p.gs - 1) / p.gs;
+    p.NP = scan_pairs_for(std::min(K, p.gs));
     p.blocks_per_sm = p.NP <= 10 ? 2 : 1;                      // the kernel's __launch_bounds__
     const int ps = (int)std::min<int64_t>(v.ps, 1 << 20);
     // tiled scan: delay views, and materialised points (point stride > 1) whose windows fit the shared memory
@@ -608,8 +609,8 @@ __global__ void line_eps_check_kernel(const float* __restrict__ eps, int64_t cou
 
 int scan_pairs_for(int kg) { return kg <= 10 ? 5 : (kg <= 20 ? 10 : 16); }
 
-rqa_status launch_line_groups(const float* d_eps, int K, int NG, int batch, void* groups, WsStatus* status, cudaStream_t s) {
-    line_groups_kernel<<<batch, 128, 0, s>>>(d_eps, K, NG, (LineGroup*)groups, status);
+rqa_status launch_line_groups(const float* d_eps, int K, int NG, int gs, int batch, void* groups, WsStatus* status, cudaStream_t s) {
+    line_groups_kernel<<<batch, 128, 0, s>>>(d_eps, K, NG, gs, (LineGroup*)groups, status);
     RQA_LAUNCH_CHECK();
     return RQA_OK;
 }
@@ -677,7 +678,7 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     RQA_CUDA_TRY(cudaMemsetAsync(w.agg, 0, sizeof(uint64_t) * agg_words, s));
     RQA_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(unsigned int) * (size_t)p.NG, s));
     {
-        rqa_status st = launch_line_groups(d_eps, K, p.NG, v.batch, w.groups, status, s);
+        rqa_status st = launch_line_groups(d_eps, K, p.NG, p.gs, v.batch, w.groups, status, s);
         if (st != RQA_OK) return st;
     }
     if (p.tl.tiles > 0) {

@@ -391,7 +391,7 @@ __device__ __forceinline__ void flush_item(uint32_t* tot_s, int32_t* sh_s, int J
 //   groups    one block per series: sort the K thresholds, split them into groups of 32, build each group's level table
 //   finalize  P(1..3) of every distinct threshold from the aggregates and the explicit lines, then the rows of duplicate
 //             thresholds are copied from their representative row
-rqa_status launch_line_groups(const float* d_eps, int K, int NG, int batch, void* groups, WsStatus* status, cudaStream_t s);
+rqa_status launch_line_groups(const float* d_eps, int K, int NG, int gs, int batch, void* groups, WsStatus* status, cudaStream_t s);
 rqa_status launch_line_finalize(int64_t n, int NG, int NP, int K, int batch, const void* groups, const unsigned long long* agg,
                                 unsigned long long* hist, WsStatus* status, cudaStream_t s);
 int scan_pairs_for(int kg);          // NP of the scan instantiation for kg thresholds per group: 5, 10 or 16

@@ -873,6 +873,7 @@ struct SelectPlan {
     Tiling tl;                        // this part's tiles of the counting pass
     int span;
     int fields;                       // counting pass: threads per counter word (2 or 3)
+    int gs;                           // targets per group (<= GK)
     int ps;                           // point stride in floats
 };
 
@@ -888,10 +889,11 @@ SelectPlan make_select_plan(const View& v, int K, const Options& opt) {
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
     p.ps = (int)std::min<int64_t>(v.ps, 1 << 20);
     // more than 20 brackets per group: 10-bit counters (two blocks per SM still fit), so shorter chunks
-    p.fields = std::min(K, GK) > 20 ? 3 : 2;
+    p.gs = group_size_for(K, opt);
+    p.fields = std::min(K, p.gs) > 20 ? 3 : 2;
     // tiled counting pass: delay views, and materialised points whose windows fit beside the widest level table
     // (the heavy launch's, with the counter width this K uses)
-    const int nlev_max = 2 * (2 * std::min(K, GK) + 1) - 1;
+    const int nlev_max = 2 * (2 * std::min(K, p.gs) + 1) - 1;
     const bool tiled_ok = p.span <= MAX_SPAN && count_smem_bytes(nlev_max, p.fields, 32, p.span, p.ps) <= SMEM_PER_BLOCK_MAX;
     p.path = opt.select_path;
     // one block per series (rqa_block.cu) where the batch can fill the GPU with such blocks; forced: any batch
@@ -908,7 +910,7 @@ SelectPlan make_select_plan(const View& v, int K, const Options& opt) {
         // with many targets on a series of moderate length S grows until the brackets cover at most 20 % (P <= 2^26)
         // or 10 % of the pairs.  (Measured: 100 series of 10^4 points at K = 99 261 -> 55 ms, 10 series of 2*10^4 points
         // at K = 99 105 -> 17 ms, config 5 46.7 -> 41 ms; config 4 unchanged.)
-        const int kg = std::min(K, GK);
+        const int kg = std::min(K, p.gs);
         const double cover = p.P <= (1ull << 26) ? 0.2 : 0.1;
         const double s_targets = std::pow(kg * (BRACKET_SIGMAS + 1.0) / cover, 2.0);
         double s = std::max(5.5 * std::pow((double)p.P, 2.0 / 3.0), s_targets);
@@ -1092,8 +1094,8 @@ rqa_status run_select(const View& v, int norm, const uint64_t* h_rank, int K, fl
         rqa_status st = RQA_OK;
         if (p.tl.tiles > 0) st = launch_tile_table(p.tl, w.tile_start, s);
         if (st != RQA_OK) return st;
-        for (int base = 0; base < K; base += GK) {
-            const int kc = std::min(GK, K - base);
+        for (int base = 0; base < K; base += p.gs) {
+            const int kc = std::min(p.gs, K - base);
             SampleRanks sr{};
             Ranks64 rk{};
             TargetMap tm{};

@@ -315,7 +315,7 @@ constexpr size_t SMEM_PER_SM = 228 * 1024, SMEM_BLOCK_RESERVED = 1024;
 
 struct VertPlan {
     bool scan;
-    int L, S, NG, NP, span, blocks_per_sm;
+    int L, S, NG, NP, gs, span, blocks_per_sm;
     int n_cb, n_cbl;            // column blocks of the plot / of this part
     uint32_t segs;
     unsigned grid;
@@ -330,8 +330,9 @@ size_t vert_smem_bytes(int NP, int L, int span, int ps) {
 VertPlan make_vert_plan(const View& v, int K, const Options& opt) {
     VertPlan p{};
     p.span = (int)std::min<int64_t>((int64_t)(v.m - 1) * v.cs, (int64_t)MAX_SPAN + 1);
-    p.NG = (K + GK - 1) / GK;
-    p.NP = scan_pairs_for(std::min(K, GK));
+    p.gs = group_size_for(K, opt);
+    p.NG = (K + p.gs - 1) / p.gs;
+    p.NP = scan_pairs_for(std::min(K, p.gs));
     p.blocks_per_sm = p.NP <= 10 ? 2 : 1;
     const int ps = (int)std::min<int64_t>(v.ps, 1 << 20);
     p.scan = p.span <= MAX_SPAN && vert_smem_bytes(p.NP, 32, p.span, ps) <= SMEM_PER_BLOCK_MAX;
@@ -438,7 +439,7 @@ rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uin
     const size_t agg_words = (size_t)v.batch * p.NG * 3 * (GK + 1);
     RQA_CUDA_TRY(cudaMemsetAsync(w.agg, 0, sizeof(uint64_t) * agg_words, s));
     RQA_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(unsigned int) * (size_t)p.NG, s));
-    rqa_status st = launch_line_groups(d_eps, K, p.NG, v.batch, w.groups, status, s);
+    rqa_status st = launch_line_groups(d_eps, K, p.NG, p.gs, v.batch, w.groups, status, s);
     if (st != RQA_OK) return st;
     for (int g = 0; g < p.NG && p.n_cbl > 0; ++g) {
         VertArgs a;

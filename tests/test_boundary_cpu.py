@@ -134,6 +134,7 @@ def test_options_are_per_call_and_validated(lib):
     assert size(line_chunk=1024)[0] == B.RQA_ERR_INVALID_ARG
     assert size(line_buffers=3)[0] == B.RQA_ERR_INVALID_ARG
     assert size(line_path=3)[0] == B.RQA_ERR_INVALID_ARG
+    assert size(group_size=33)[0] == B.RQA_ERR_INVALID_ARG
     assert size(line_segment=-1)[0] == B.RQA_ERR_INVALID_ARG
     assert size(sample_size=-1)[0] == B.RQA_ERR_INVALID_ARG
     assert size(part_index=2, part_count=2)[0] == B.RQA_ERR_INVALID_ARG

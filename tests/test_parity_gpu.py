@@ -654,7 +654,7 @@ def test_random_configurations(rqa, oracle, options, seed):
         options(select_path=int(rng.choice([0, 0, 1, 2, 3, 4])), sample_size=int(rng.choice([0, 0, 50, 4000])),
                 line_chunk=int(rng.choice([0, 0, 0, 1, 2, 3, 6, 13, 64, 500])), cand_cap=int(rng.choice([0, 0, 0, 200])),
                 line_segment=int(rng.choice([0, 0, 1, 2, 7, 40])), line_buffers=int(rng.choice([0, 1, 2])),
-                line_path=int(rng.choice([0, 0, 1, 2])))
+                line_path=int(rng.choice([0, 0, 1, 2])), group_size=int(rng.choice([0, 0, 0, 1, 3, 7, 20, 32])))
         s = torch.as_tensor(ys).cuda()
         n = N - (m - 1) * tau
         X = torch.empty((batch, n, m), dtype=torch.float32, device="cuda") if rng.random() < 0.25 else None

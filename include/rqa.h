@@ -249,8 +249,8 @@ uint64_t rqa_launch_count(void);
  *   group_size    thresholds (targets) per pass of the grouped kernels of all three heavy calls, 1..32; 0 automatic: K <= 32
  *                 in one pass, more in groups of 20 (a pass over at most 20 thresholds keeps two blocks per SM; 7 % faster
  *                 and a third less workspace than groups of 32 at K = 99)
- *   line_path     rqa_line_hist: 0 automatic, 1 = the tiled scan, 2 = one thread block per series walking every diagonal
- *                 once for all K thresholds (P <= 2^22 only; otherwise automatic).  Automatic: series of at most 8192
+ *   line_path     rqa_line_hist / rqa_vert_hist: 0 automatic, 1 = the tiled scan, 2 = one thread block per series walking
+ *                 every diagonal / column once for all K thresholds (P <= 2^22 only; otherwise automatic).  Automatic: series of at most 8192
  *                 pairs take their one-block kernel, P <= 2^22 takes path 2 when the batch is large enough to fill the
  *                 GPU with such blocks (batch x ceil(K/32) >= 192), everything else the tiled scan.
  *   part_index, part_count

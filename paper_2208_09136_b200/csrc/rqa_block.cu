@@ -318,7 +318,9 @@ __host__ __device__ inline size_t line_block_smem_bytes(int K, size_t stage_floa
     return 4 * ((size_t)(K + 1) * LB_LCAP + stage_floats) + (size_t)LB_NB;
 }
 
-template <int NORM, int M>
+// VERT: the same walk down the COLUMNS of the full symmetric matrix (rqa_vert_hist, reading S19): one thread per
+// column j, rows i = 0..n-1, the cells with |i - j| < w excluded (not recurrent at any threshold; they split a column).
+template <int NORM, int M, bool VERT>
 __global__ void __launch_bounds__(LB_THREADS, 2) line_block_kernel(View v, const float* __restrict__ eps, int K,
                                                                   int stage_floats,
                                                                   unsigned long long* __restrict__ hist,
@@ -408,14 +410,14 @@ __global__ void __launch_bounds__(LB_THREADS, 2) line_block_kernel(View v, const
     // push) or ends ONE stack entry of a pending level rise.  A rise that ends several entries spreads over several
     // steps while the other lanes go on with their cells, so the warp never waits for the longest pop sequence of a
     // cell (lanes drift apart along their diagonals; the walk's loads are then plain shared-memory gathers).
-    const int nd = n - w, nq = (nd + 1) / 2;
+    const int nd = n - w, nq = VERT ? n : (nd + 1) / 2;
     for (int q = tid; q < nq; q += LB_THREADS) {
-        const int o1 = w + q, o2 = n - 1 - q;
-        int o = o1, len = n - o1, t = 0;
+        const int o1 = VERT ? q : w + q, o2 = VERT ? q : n - 1 - q;      // VERT: o = the column
+        int o = o1, len = VERT ? n : n - o1, t = 0;
         int depth = 0, pv = J;                                 // top entry in `cur`, the entries below in stk[0 .. depth-2]
         uint32_t cur = 0;
         int vnew = -1, tend = 0;                               // pending rise: the thresholds [.., vnew) end before cell tend
-        bool second = o2 == o1;                                // no second diagonal for the middle one
+        bool second = o2 == o1;                                // no second diagonal for the middle one (VERT: never)
         while (true) {
             if (vnew >= 0) {                                   // end one entry
                 const uint32_t nxt = depth > 1 ? stk[depth - 2] : ((uint32_t)J << 16);
@@ -430,9 +432,13 @@ __global__ void __launch_bounds__(LB_THREADS, 2) line_block_kernel(View v, const
                     vnew = -1;
                 }
             } else if (t < len) {                              // next cell
-                const float d = dist.at(t, o);
-                int lev = lut[min((int)__fmul_rn(d, scale), LB_NB - 1)];
-                while (lev < J && s_eps[lev] < d) ++lev;
+                int lev = J;
+                const int gap = VERT ? (t > o ? t - o : o - t) : w;
+                if (gap >= w) {
+                    const float d = VERT ? dist.at(t < o ? t : o, gap) : dist.at(t, o);
+                    lev = lut[min((int)__fmul_rn(d, scale), LB_NB - 1)];
+                    while (lev < J && s_eps[lev] < d) ++lev;
+                }
                 if (lev < pv) {
                     if (depth > 0) stk[depth - 1] = cur;
                     cur = ((uint32_t)lev << 16) | (uint32_t)t;
@@ -537,20 +543,26 @@ bool block_line_fits(const View& v, int K) {
 }
 
 rqa_status run_line_block(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, WsStatus* status,
-                          cudaStream_t s) {
+                          cudaStream_t s, bool vertical) {
     const size_t ny = (size_t)(v.n - 1) * v.ps + (size_t)(v.m - 1) * v.cs + 1;
     const size_t stage = line_block_smem_bytes(K, ny) <= 110 * 1024 ? ny : 0;     // two blocks per SM
     const size_t smem = line_block_smem_bytes(K, stage);
     const int M = (stage && v.ps == 1 && (v.m == 1 || v.m == 3)) ? v.m : 0;
     using Kern = void (*)(View, const float*, int, int, unsigned long long*, WsStatus*);
     const bool mx = norm == RQA_NORM_MAX;
-    Kern kern = M == 1 ? (mx ? line_block_kernel<RQA_NORM_MAX, 1> : line_block_kernel<RQA_NORM_EUCLID, 1>)
-              : M == 3 ? (mx ? line_block_kernel<RQA_NORM_MAX, 3> : line_block_kernel<RQA_NORM_EUCLID, 3>)
-                       : (mx ? line_block_kernel<RQA_NORM_MAX, 0> : line_block_kernel<RQA_NORM_EUCLID, 0>);
-    static thread_local bool attr_set[8][6] = {};
+    Kern kern;
+    if (!vertical)
+        kern = M == 1 ? (mx ? line_block_kernel<RQA_NORM_MAX, 1, false> : line_block_kernel<RQA_NORM_EUCLID, 1, false>)
+             : M == 3 ? (mx ? line_block_kernel<RQA_NORM_MAX, 3, false> : line_block_kernel<RQA_NORM_EUCLID, 3, false>)
+                      : (mx ? line_block_kernel<RQA_NORM_MAX, 0, false> : line_block_kernel<RQA_NORM_EUCLID, 0, false>);
+    else
+        kern = M == 1 ? (mx ? line_block_kernel<RQA_NORM_MAX, 1, true> : line_block_kernel<RQA_NORM_EUCLID, 1, true>)
+             : M == 3 ? (mx ? line_block_kernel<RQA_NORM_MAX, 3, true> : line_block_kernel<RQA_NORM_EUCLID, 3, true>)
+                      : (mx ? line_block_kernel<RQA_NORM_MAX, 0, true> : line_block_kernel<RQA_NORM_EUCLID, 0, true>);
+    static thread_local bool attr_set[8][12] = {};
     int dev = 0;
     RQA_CUDA_TRY(cudaGetDevice(&dev));
-    const int which = (mx ? 0 : 1) + 2 * (M == 1 ? 1 : M == 3 ? 2 : 0);
+    const int which = (mx ? 0 : 1) + 2 * (M == 1 ? 1 : M == 3 ? 2 : 0) + (vertical ? 6 : 0);
     if (dev >= 8 || !attr_set[dev][which]) {
         RQA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
         if (dev < 8) attr_set[dev][which] = true;

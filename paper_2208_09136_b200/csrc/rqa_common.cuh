@@ -159,7 +159,7 @@ rqa_status run_select_block(const View& v, int norm, const uint64_t* h_rank, int
 
 bool block_line_fits(const View& v, int K);
 rqa_status run_line_block(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, WsStatus* status,
-                          cudaStream_t s);
+                          cudaStream_t s, bool vertical = false);   // vertical: the columns of the full matrix (rqa_vert_hist)
 
 size_t vert_workspace_bytes(const View& v, int K, const Options& opt);
 rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uint64_t* d_vhist, Arena& ws,

@@ -421,6 +421,11 @@ rqa_status run_vert_hist(const View& v, int norm, const float* d_eps, int K, uin
                          const Options& opt) {
     WsStatus* status = (WsStatus*)ws.base;
     const size_t hist_words = (size_t)v.batch * K * v.n;
+    // many series of moderate length: one block per series walks every column once for all K thresholds (rqa_block.cu)
+    // (N'^2 cells per block: only where the plot itself is moderate, whatever the Theiler window leaves of it)
+    if (opt.parts == 1 && block_line_fits(v, K) && v.n <= 4096 &&
+        (opt.line_path == 2 || (opt.line_path == 0 && opt.line_chunk == 0 && (int64_t)v.batch * ((K + GK - 1) / GK) >= 192)))
+        return run_line_block(v, norm, d_eps, K, d_vhist, status, s, true);
     RQA_CUDA_TRY(cudaMemsetAsync(d_vhist, 0, sizeof(uint64_t) * hist_words, s));
     VertPlan p = make_vert_plan(v, K, opt);
     if (!p.scan) {

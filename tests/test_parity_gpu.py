@@ -787,6 +787,48 @@ def test_vertical_hand_cases_on_gpu(rqa, oracle):
         assert abs(L[0][0] - ln / ld) <= 1e-15, name
 
 
+@pytest.mark.parametrize("norm", [0, 1])
+def test_vertical_lines_one_block_per_series(rqa, oracle, norm):
+    """rqa_vert_hist as one block per series (line_path 2, rqa_block.cu: one thread per column, all K thresholds in one
+    walk; the default for large batches with P <= 2^22): noisy, exactly periodic (columns recurrent from top to bottom),
+    quantised and constant series; compiled-in and run-time embeddings, Theiler windows that split the columns, K up to
+    128 with duplicates, series shorter than the shared-memory length cap; the hand cases; and the default path on a
+    batch large enough to take it."""
+    from pathlib import Path
+    from paper_2208_09136_b200 import binding as B
+    opt = B.make_options(line_path=2)
+    def batch(N):
+        return np.stack([wl.add_noise(wl.sine_signal(N), 0.7, 3), wl.sine_signal(N).astype(np.float32),
+                         np.floor(wl.uniform01(5, N) * 4).astype(np.float32), np.full(N, -1.25, dtype=np.float32),
+                         wl.add_noise(wl.logistic_signal(N, 8), 3.0, 8), wl.gaussian(10, N).astype(np.float32)])
+    for (N, m, tau, rr, w) in [(900, 1, 1, np.arange(1, 100) / 100.0, 0), (700, 3, 1, wl.rr_log(128, 0.0005, 0.95), 0),
+                               (800, 4, 6, np.array([0.3, 0.0007, 0.02, 0.02, 1.0, 0.5]), 0),
+                               (1000, 3, 1, wl.rr_log(20, 0.001, 0.2), 40), (1200, 1, 1, wl.rr_log(7, 0.01, 0.6), 900),
+                               (140, 1, 1, wl.rr_log(99, 0.001, 0.9), 0), (150, 3, 3, wl.rr_log(33, 0.01, 0.99), 30)]:
+        ys = batch(N)
+        eps = np.stack([oracle.eps_for_rr(y, m, tau, rr, norm, theiler=max(1, w))[0] for y in ys])
+        got = gpu_vert(rqa, ys, m, tau, eps, norm, theiler=w, options=opt)
+        assert_vert(oracle, got, ys, m, tau, eps, norm, theiler=max(1, w))
+    if norm == 0:
+        for line in (Path(__file__).resolve().parent / "golden" / "hand_cases_vertical.txt").read_text().splitlines():
+            if not line.strip() or line.startswith("#"):
+                continue
+            name, y, m, tau, nrm, eps, w, hist, lam, tt = [f.strip() for f in line.split("|")]
+            y = np.array(y.split(), dtype=np.float32)
+            vh, L, T = gpu_vert(rqa, y, int(m), int(tau), [float(eps)], 0, theiler=int(w), options=opt)
+            got = {int(v): int(c) for v, c in enumerate(vh[0][0]) if c}
+            assert got == {int(a): int(b) for a, b in (t.split(":") for t in hist.split(","))}, name
+    # default path: 60 series at K = 99 (a launch count only the block kernel reaches)
+    ys = np.stack([wl.add_noise([wl.sine_signal(500), wl.logistic_signal(500, 70 + b), wl.lorenz_signal(500)][b % 3],
+                                [math.inf, 3.0, 0.3, 0.03][b % 4], 300 + b) for b in range(60)])
+    rr = np.arange(1, 100) / 100.0
+    eps = np.stack([oracle.eps_for_rr(y, 3, 2, rr, norm)[0] for y in ys])
+    n0 = rqa.rqa_launch_count()
+    got = gpu_vert(rqa, ys, 3, 2, eps, norm)
+    assert rqa.rqa_launch_count() - n0 <= 6
+    assert_vert(oracle, got, ys, 3, 2, eps, norm)
+
+
 @pytest.mark.parametrize("cfg", ["config1", "config2", "config3max", "config3euclid"])
 def test_vertical_lines_on_baseline_configs(rqa, oracle, cfg):
     """vhist, LAM and TT at the thresholds rqa_eps_for_rr selects, on configs 1-3 at their stated sizes; the invariant

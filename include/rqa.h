@@ -307,7 +307,8 @@ rqa_status rqa_vert_hist_opt(const rqa_points* pts, rqa_norm norm, const float* 
  *   - a shape whose scan needs more scratch returns RQA_ERR_UNSUPPORTED (nothing launched; the message states the
  *     bytes needed).  The scan's scratch grows with the number of tiles it cuts the triangle into, not simply with N:
  *     BASELINE.json's configs 1-3 fit (6 series of 10^4 points at K = 20 need 113 MiB), one series of 10^4 points fits
- *     at any K, one series of 10^5 points does not (207 MiB);
+ *     at any K, one series of 10^5 points does not (207 MiB); a batch that runs as one block per series (line_path
+ *     above) needs none at all, e.g. 900 series of 10^3 points at K = 99;
  *   - all calls on one device share the array and it keeps the last call's contents: calls in stream order are
  *     independent (the path clears what must start at zero), calls that OVERLAP on the GPU race — serialise them or use
  *     rqa_line_hist with one workspace per stream;

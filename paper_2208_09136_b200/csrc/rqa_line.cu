@@ -636,7 +636,20 @@ rqa_status launch_tile_table(const Tiling& t, uint32_t* tile_start, cudaStream_t
     return RQA_OK;
 }
 
+// The two one-block-per-series paths need no workspace beyond the status block.
+static bool line_small_path(const View& v, int K, const Options& opt) {
+    return opt.line_path == 0 && opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 &&
+           small_line_fits(v, K);
+}
+static bool line_block_path(const View& v, int K, const Options& opt) {
+    // (the tiled scan costs about batch x groups of 32 thresholds, the blocks one round per 2 x SMs series)
+    const bool knobs = opt.line_chunk != 0 || opt.line_segment != 0 || opt.line_buffers != 0;
+    return opt.parts == 1 && block_line_fits(v, K) &&
+           (opt.line_path == 2 || (opt.line_path == 0 && !knobs && (int64_t)v.batch * ((K + GK - 1) / GK) >= 192));
+}
+
 size_t line_workspace_bytes(const View& v, int K, const Options& opt) {
+    if (line_small_path(v, K, opt) || line_block_path(v, K, opt)) return 256;
     LinePlan p = make_plan(v, K, opt);
     if (!p.scan) return 256;
     Arena a(nullptr, ~(size_t)0);
@@ -650,14 +663,9 @@ rqa_status run_line_hist(const View& v, int norm, const float* d_eps, int K, uin
     const size_t hist_words = (size_t)v.batch * K * v.n;
     // short series: one block per series, shared-memory distances and histogram (explicit scan knobs and split calls
     // keep the general machinery)
-    if (opt.line_path == 0 && opt.line_chunk == 0 && opt.line_segment == 0 && opt.line_buffers == 0 && opt.parts == 1 && small_line_fits(v, K))
-        return run_line_small(v, norm, d_eps, K, d_hist, status, s);
+    if (line_small_path(v, K, opt)) return run_line_small(v, norm, d_eps, K, d_hist, status, s);
     // many series of moderate length: one block per series walks every diagonal once for all K thresholds (rqa_block.cu)
-    // (the tiled scan costs about batch x groups of 32 thresholds, the blocks one round per 2 x SMs series)
-    const bool knobs = opt.line_chunk != 0 || opt.line_segment != 0 || opt.line_buffers != 0;
-    if (opt.parts == 1 && block_line_fits(v, K) &&
-        (opt.line_path == 2 || (opt.line_path == 0 && !knobs && (int64_t)v.batch * ((K + GK - 1) / GK) >= 192)))
-        return run_line_block(v, norm, d_eps, K, d_hist, status, s);
+    if (line_block_path(v, K, opt)) return run_line_block(v, norm, d_eps, K, d_hist, status, s);
     RQA_CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(uint64_t) * hist_words, s));
     LinePlan p = make_plan(v, K, opt);
     if (!p.scan) {

@@ -79,6 +79,21 @@ def test_static_scratch_twice_on_the_same_input(rqa):
 
 
 @pytest.mark.gpu
+def test_static_scratch_takes_a_large_batch_of_moderate_series(rqa):
+    """A batch that runs as one block per series needs no scratch beyond the status block, whatever its size: a group
+    of the paper's grid (900 series of 10^3 points, K = 99) goes through the static entry point, twice in a row."""
+    import torch
+    w = wl.paper_group("logistic", 1.0, 1000, n_real=90)
+    s, buf = _existing_path(rqa, w)
+    out = torch.empty_like(buf.hist)
+    for call in range(2):
+        out.fill_(-1)
+        rqa.rqa_line_hist_static(buf.view, w.norm, buf.eps, out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, buf.hist), f"call {call}"
+
+
+@pytest.mark.gpu
 def test_static_scratch_rejects_a_shape_beyond_the_maximum_on_the_gpu(rqa):
     import torch
     N = 100_000                                                 # config 4's length: 207 MiB of scratch for one series

@@ -916,7 +916,7 @@ def test_paper_group_sorting_experiment(rqa, oracle, signal, level, N):
 
 
 # ------------------------------------------- stand-ins for compute-sanitizer (closed on this GPU pool)
-@pytest.mark.parametrize("path", [0, 1, 2, 3])
+@pytest.mark.parametrize("path", [0, 1, 2, 3, 4])
 def test_workspace_contents_and_guard_bands(rqa, oracle, path):
     """initcheck / memcheck by hand.  The workspace is scratch the caller does not initialise: whatever it holds before
     a call (zeros, 0xFF, random bytes, the previous call's leftovers) the results must be bit-identical and correct —
@@ -925,14 +925,16 @@ def test_workspace_contents_and_guard_bands(rqa, oracle, path):
     shows up there.  All select paths, the diagonal scan and the column scan, two chunk configurations."""
     import torch
     from paper_2208_09136_b200 import binding as B
-    N, m, tau, K = (700 if path == 1 else 3000), 3, 2, 20
+    N, m, tau, K = (700 if path == 1 else (2800 if path == 4 else 3000)), 3, 2, 20
     y = np.stack([wl.add_noise(wl.lorenz_signal(N), 1.0, 808), np.round(wl.gaussian(809, N) * 3) / 3]).astype(np.float32)
     rr = wl.rr_log(K, 0.002, 0.3)
     s = torch.as_tensor(y).cuda()
     GUARD = 4096
     ref = None
     for fill, chunk in (("zeros", 0), ("ff", 0), ("random", 61), ("leftover", 0)):
-        opt = B.make_options(select_path=path, line_chunk=chunk, line_segment=3 if chunk else 0)
+        # path 4: every call as one block per series (rqa_block.cu), which has no chunks
+        opt = B.make_options(select_path=path, line_path=2) if path == 4 else \
+            B.make_options(select_path=path, line_chunk=chunk, line_segment=3 if chunk else 0)
         view = B.rqa_embed(s, m, tau)
         n = int(view.n_points)
         nbytes = B.rqa_workspace_bytes(view, K, opt)

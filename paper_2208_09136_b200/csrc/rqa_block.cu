@@ -91,10 +91,10 @@ __device__ __forceinline__ void walk_triangle(const D& dist, int n, int w, int s
         const int o1 = w + q, o2 = n - 1 - q, len1 = n - o1, len = len1 + (o2 != o1 ? n - o2 : 0);
         const int a = (int)((long long)len * h / split), b = (int)((long long)len * (h + 1) / split);
         const int e1 = b < len1 ? b : len1;
-#pragma unroll 4
+#pragma unroll 8
         for (int i = a; i < e1; ++i) f(dist.at(i, o1));
         const int a2 = (a > len1 ? a : len1) - len1, e2 = b - len1;
-#pragma unroll 4
+#pragma unroll 8
         for (int i = a2; i < e2; ++i) f(dist.at(i, o2));
     }
 }

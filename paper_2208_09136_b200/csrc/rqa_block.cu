@@ -321,7 +321,7 @@ __host__ __device__ inline size_t line_block_smem_bytes(int K, size_t stage_floa
 // VERT: the same walk down the COLUMNS of the full symmetric matrix (rqa_vert_hist, reading S19): one thread per
 // column j, rows i = 0..n-1, the cells with |i - j| < w excluded (not recurrent at any threshold; they split a column).
 template <int NORM, int M, bool VERT>
-__global__ void __launch_bounds__(LB_THREADS, 2) line_block_kernel(View v, const float* __restrict__ eps, int K,
+__global__ void __launch_bounds__(LB_THREADS, 3) line_block_kernel(View v, const float* __restrict__ eps, int K,
                                                                   int stage_floats,
                                                                   unsigned long long* __restrict__ hist,
                                                                   WsStatus* status) {
@@ -545,7 +545,7 @@ bool block_line_fits(const View& v, int K) {
 rqa_status run_line_block(const View& v, int norm, const float* d_eps, int K, uint64_t* d_hist, WsStatus* status,
                           cudaStream_t s, bool vertical) {
     const size_t ny = (size_t)(v.n - 1) * v.ps + (size_t)(v.m - 1) * v.cs + 1;
-    const size_t stage = line_block_smem_bytes(K, ny) <= 110 * 1024 ? ny : 0;     // two blocks per SM
+    const size_t stage = line_block_smem_bytes(K, ny) <= 74 * 1024 ? ny : 0;      // three blocks per SM
     const size_t smem = line_block_smem_bytes(K, stage);
     const int M = (stage && v.ps == 1 && (v.m == 1 || v.m == 3)) ? v.m : 0;
     using Kern = void (*)(View, const float*, int, int, unsigned long long*, WsStatus*);
